@@ -1,0 +1,275 @@
+/*
+ * vrc_oracle.c -- CPU ORACLE for the VRC (volumetric-ray-casting) fluence estimator.
+ *
+ * TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may build, load or call this file.
+ * It shares no code, header, table or helper with the CUDA library under
+ * paper_1706_07476_b200/csrc/ and neither includes the other.
+ *
+ * What it computes (PAPER.md = /root/reference/PAPER.md at build time of this repo):
+ *   Eq. (1)  PAPER.md:23-25   F = W/S * (1 - exp(-S l))          expected path length in a cell
+ *   Eq. (2)  PAPER.md:45-51   W_i = W exp(-int_0^{|r'-r|} S_t ds) attenuation to the cell entrance
+ *   Eq. (3)  PAPER.md:53-56   product of the two
+ *   Eq. (4)  PAPER.md:58-65   the same per ray j with weight W/N (the caller passes W/N, reading Q15)
+ *   PAPER.md:85               "first calculating all cross-sections, then ray casting the particle
+ *                              [through the entire geometry storing the path length travelled in each
+ *                              cell], and finally calculating the VRC estimator"; cross sections are
+ *                              "linearly interpolated between table values".
+ * Everything is IEEE double, round-to-nearest; build with -O2 -ffp-contract=off (no FMA
+ * contraction, no fast-math).  Steps O1..O6 below follow SURVEY.md §8(c) / DESIGN.md §3 in
+ * that order and notation; there is no blocking, fusion or reordering.
+ *
+ * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"): numpy.interp for O2; the textbook slab
+ * method for the exit parameter; brute-force sorted plane crossings for the trace; the
+ * homogeneous closed form W/S(1-exp(-S L)); the collision-probability invariant; the S->0
+ * track-length limit; the two-slab closed form; fine-step quadrature of the plain
+ * definition; linearity, additivity and mirror symmetry; published FNV-1a test vectors.
+ * Nothing in this file is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct {
+    int32_t nx, ny, nz;        /* cells per axis */
+    const double *xe, *ye, *ze; /* n+1 strictly increasing plane positions per axis (cm) */
+    int32_t M;                 /* materials */
+    const double *density;     /* [M] g/cc */
+    int32_t K;                 /* material slots per cell */
+    const int32_t *cell_mat;   /* [ncell*K], -1 = empty slot; cell c = ix + nx*(iy + ny*iz) (Q17) */
+    const double *cell_frac;   /* [ncell*K] volume fractions */
+    const int64_t *xs_off;     /* [M+1] offsets of each material's table in xs_E / xs_sig */
+    const double *xs_E;        /* energies, MeV, strictly increasing per table */
+    const double *xs_sig;      /* total cross sections, cm^2/g */
+} vrc_problem;
+
+typedef struct {
+    int64_t rays_accepted, rays_rejected, segments;
+} vrc_counts;
+
+/* Optional per-ray outputs (O6); any pointer may be NULL. */
+typedef struct {
+    uint32_t *nseg;       /* [n] segments of the ray (0 if rejected) */
+    uint64_t *hash;       /* [n] FNV-1a 64 over the little-endian bytes of the uint32 cell indices, in order */
+    double *sum_l;        /* [n] sum of segment lengths */
+    double *t_exit;       /* [n] crossing parameter at which the ray left the mesh */
+    double *tau_exit;     /* [n] optical thickness to the mesh exit */
+    double *sum_score;    /* [n] sum_i score_i */
+    double *sum_sig_score;/* [n] sum_i Sigma_i * score_i */
+    int32_t *cells;       /* [n*cap] cell index per segment, first min(nseg,cap) filled */
+    double *lens;         /* [n*cap] segment lengths */
+    double *scores;       /* [n*cap] segment scores */
+    int64_t cap;
+} vrc_diag;
+
+#define FNV_BASIS 0xcbf29ce484222325ULL
+#define FNV_PRIME 0x100000001b3ULL
+
+uint64_t vrc_fnv1a_cells(const uint32_t *cells, int64_t n)
+{
+    uint64_t h = FNV_BASIS;
+    for (int64_t i = 0; i < n; ++i)
+        for (int b = 0; b < 4; ++b) {
+            h ^= (uint64_t)((cells[i] >> (8 * b)) & 0xffu);
+            h *= FNV_PRIME;
+        }
+    return h;
+}
+
+/* number of elements of a[0..n) that are <= v  (std::upper_bound as an index) */
+static int64_t upper_bound(const double *a, int64_t n, double v)
+{
+    int64_t lo = 0, hi = n;
+    while (lo < hi) {
+        int64_t mid = lo + (hi - lo) / 2;
+        if (a[mid] <= v) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+/* O2: lin-lin interpolated sigma_m(E), clamped to the end values (reading Q5). */
+double vrc_sigma(const vrc_problem *p, int32_t m, double E)
+{
+    const double *Eg = p->xs_E + p->xs_off[m];
+    const double *Sg = p->xs_sig + p->xs_off[m];
+    int64_t n = p->xs_off[m + 1] - p->xs_off[m];
+    if (n == 1 || E < Eg[0]) return Sg[0];
+    if (E >= Eg[n - 1]) return Sg[n - 1];
+    int64_t k = upper_bound(Eg, n, E) - 1;
+    if (k < 0) k = 0;
+    if (k > n - 2) k = n - 2;
+    double t = (E - Eg[k]) / (Eg[k + 1] - Eg[k]);
+    return Sg[k] + t * (Sg[k + 1] - Sg[k]);
+}
+
+/* One ray, steps O1..O6.  Returns 1 if accepted, 0 if rejected.  tally may be NULL (trace only). */
+static int cast_one(const vrc_problem *p, const double *ray, double *tally, int atomic,
+                    const vrc_diag *dg, int64_t r, int64_t *segments_out)
+{
+    const double o[3] = {ray[0], ray[1], ray[2]};
+    const double d[3] = {ray[3], ray[4], ray[5]};
+    const double E = ray[6], W = ray[7];
+    const int32_t n[3] = {p->nx, p->ny, p->nz};
+    const double *edges[3] = {p->xe, p->ye, p->ze};
+
+    uint32_t nseg = 0;
+    uint64_t hash = FNV_BASIS;
+    double sum_l = 0.0, tau = 0.0, sum_score = 0.0, sum_sig_score = 0.0, t_cur = 0.0;
+    int accepted = 1;
+
+    /* O1 validate */
+    for (int f = 0; f < 8; ++f) if (!isfinite(ray[f])) accepted = 0;
+    if (!(E > 0.0)) accepted = 0;
+    if (d[0] == 0.0 && d[1] == 0.0 && d[2] == 0.0) accepted = 0;
+    for (int a = 0; a < 3 && accepted; ++a)
+        if (!(o[a] >= edges[a][0] && o[a] < edges[a][n[a]])) accepted = 0;
+
+    if (accepted) {
+        /* O2 cross sections of every material at the ray's energy */
+        double sig[64];
+        for (int32_t m = 0; m < p->M; ++m) sig[m] = vrc_sigma(p, m, E);
+
+        /* O3 start cell: pure comparisons */
+        int32_t i[3], step[3], plane[3];
+        double inv[3], t[3];
+        for (int a = 0; a < 3; ++a)
+            i[a] = (int32_t)(upper_bound(edges[a], n[a] + 1, o[a]) - 1);
+
+        /* O4 crossing sequences: t_a(p) = (edges_a[p] - o_a) * inv_a, one subtract then one multiply */
+        for (int a = 0; a < 3; ++a) {
+            inv[a] = (d[a] != 0.0) ? 1.0 / d[a] : 0.0;
+            if (d[a] == 0.0 || !isfinite(inv[a])) { /* Q10: the axis never steps */
+                step[a] = 0; plane[a] = 0; t[a] = INFINITY;
+            } else {
+                step[a] = d[a] > 0.0 ? 1 : -1;
+                plane[a] = d[a] > 0.0 ? i[a] + 1 : i[a];
+                t[a] = (edges[a][plane[a]] - o[a]) * inv[a];
+            }
+        }
+
+        /* O5 the walk */
+        for (;;) {
+            int a = 0;                       /* argmin, ties x < y < z */
+            if (t[1] < t[a]) a = 1;
+            if (t[2] < t[a]) a = 2;
+            double l = t[a] - t_cur;
+            int64_t c = (int64_t)i[0] + (int64_t)n[0] * ((int64_t)i[1] + (int64_t)n[1] * (int64_t)i[2]);
+            double S = 0.0;
+            for (int32_t k = 0; k < p->K; ++k) {
+                int32_t m = p->cell_mat[c * p->K + k];
+                if (m >= 0) S += (p->cell_frac[c * p->K + k] * p->density[m]) * sig[m];
+            }
+            double x = S * l;
+            double score = W * exp(-tau) * (x > 0.0 ? -expm1(-x) / S : l);
+            if (tally) {
+                if (atomic) {
+#ifdef _OPENMP
+#pragma omp atomic
+#endif
+                    tally[c] += score;
+                } else
+                    tally[c] += score;
+            }
+            if (dg && dg->cap > 0 && (int64_t)nseg < dg->cap) {
+                if (dg->cells) dg->cells[r * dg->cap + nseg] = (int32_t)c;
+                if (dg->lens) dg->lens[r * dg->cap + nseg] = l;
+                if (dg->scores) dg->scores[r * dg->cap + nseg] = score;
+            }
+            for (int b = 0; b < 4; ++b) {
+                hash ^= (uint64_t)(((uint32_t)c >> (8 * b)) & 0xffu);
+                hash *= FNV_PRIME;
+            }
+            nseg += 1;
+            sum_l += l;
+            sum_score += score;
+            sum_sig_score += S * score;
+            tau += x;
+            t_cur = t[a];
+            i[a] += step[a];
+            if (i[a] < 0 || i[a] >= n[a]) break;
+            plane[a] += step[a];
+            t[a] = (edges[a][plane[a]] - o[a]) * inv[a];
+        }
+    }
+
+    /* O6 diagnostics */
+    if (dg) {
+        if (dg->nseg) dg->nseg[r] = nseg;
+        if (dg->hash) dg->hash[r] = accepted ? hash : 0;
+        if (dg->sum_l) dg->sum_l[r] = sum_l;
+        if (dg->t_exit) dg->t_exit[r] = t_cur;
+        if (dg->tau_exit) dg->tau_exit[r] = tau;
+        if (dg->sum_score) dg->sum_score[r] = sum_score;
+        if (dg->sum_sig_score) dg->sum_sig_score[r] = sum_sig_score;
+    }
+    *segments_out += nseg;
+    return accepted;
+}
+
+/* Cast n rays (double AoS x,y,z,u,v,w,E,W) one after another; tally[c] += score.  Single thread. */
+int vrc_cast(const vrc_problem *p, int64_t n, const double *rays, double *tally,
+             const vrc_diag *dg, vrc_counts *counts)
+{
+    if (p->M > 64) return -1;
+    vrc_counts cnt = {0, 0, 0};
+    for (int64_t r = 0; r < n; ++r) {
+        if (cast_one(p, rays + 8 * r, tally, 0, dg, r, &cnt.segments)) cnt.rays_accepted++;
+        else cnt.rays_rejected++;
+    }
+    if (counts) *counts = cnt;
+    return 0;
+}
+
+/* The same loop over contiguous chunks of rays on `threads` OpenMP threads.  Each thread adds into a
+ * private tally when threads*ncell doubles fit in `private_bytes_max`, else all add atomically into
+ * `tally`.  Private tallies are summed in thread order.  Returns the number of threads used (<0 error). */
+int vrc_cast_mt(const vrc_problem *p, int64_t n, const double *rays, double *tally,
+                const vrc_diag *dg, vrc_counts *counts, int threads, int64_t private_bytes_max)
+{
+    if (p->M > 64) return -1;
+#ifndef _OPENMP
+    threads = 1;
+#endif
+    if (threads < 1) threads = 1;
+    if (threads == 1) { vrc_cast(p, n, rays, tally, dg, counts); return 1; }
+    int64_t ncell = (int64_t)p->nx * p->ny * p->nz;
+    int use_private = tally && (int64_t)threads * ncell * 8 <= private_bytes_max;
+    double *priv = NULL;
+    if (use_private) {
+        priv = (double *)calloc((size_t)threads * (size_t)ncell, sizeof(double));
+        if (!priv) use_private = 0;
+    }
+    int64_t acc = 0, rej = 0, seg = 0;
+#ifdef _OPENMP
+#pragma omp parallel num_threads(threads) reduction(+ : acc, rej, seg)
+    {
+        int tid = omp_get_thread_num();
+        int nt = omp_get_num_threads();
+        int64_t lo = n * tid / nt, hi = n * (tid + 1) / nt;
+        double *mine = use_private ? priv + (size_t)tid * (size_t)ncell : tally;
+        for (int64_t r = lo; r < hi; ++r) {
+            if (cast_one(p, rays + 8 * r, mine, !use_private, dg, r, &seg)) acc++; else rej++;
+        }
+    }
+#endif
+    if (use_private) {
+        for (int t = 0; t < threads; ++t)
+            for (int64_t c = 0; c < ncell; ++c) tally[c] += priv[(size_t)t * (size_t)ncell + c];
+        free(priv);
+    }
+    if (counts) { counts->rays_accepted = acc; counts->rays_rejected = rej; counts->segments = seg; }
+    return threads;
+}
+
+int vrc_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,176 @@
+"""ctypes loader for the CPU oracle (oracle/vrc_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this module.  It does not
+import, and is not imported by, anything under paper_1706_07476_b200/.
+
+The shared object is built on first use with
+    gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC vrc_oracle.c -lm
+(no fast-math, no FMA contraction -- see the header of vrc_oracle.c).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "vrc_oracle.c")
+_LIB = os.path.join(_HERE, "libvrc_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".{os.getpid()}.tmp"
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+                               "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Problem(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("xe", C.c_void_p), ("ye", C.c_void_p), ("ze", C.c_void_p),
+                ("M", C.c_int32), ("density", C.c_void_p), ("K", C.c_int32),
+                ("cell_mat", C.c_void_p), ("cell_frac", C.c_void_p),
+                ("xs_off", C.c_void_p), ("xs_E", C.c_void_p), ("xs_sig", C.c_void_p)]
+
+
+class _Counts(C.Structure):
+    _fields_ = [("rays_accepted", C.c_int64), ("rays_rejected", C.c_int64), ("segments", C.c_int64)]
+
+
+class _Diag(C.Structure):
+    _fields_ = [("nseg", C.c_void_p), ("hash", C.c_void_p), ("sum_l", C.c_void_p), ("t_exit", C.c_void_p),
+                ("tau_exit", C.c_void_p), ("sum_score", C.c_void_p), ("sum_sig_score", C.c_void_p),
+                ("cells", C.c_void_p), ("lens", C.c_void_p), ("scores", C.c_void_p), ("cap", C.c_int64)]
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.vrc_sigma.restype = C.c_double
+        _lib.vrc_sigma.argtypes = [C.POINTER(_Problem), C.c_int32, C.c_double]
+        _lib.vrc_cast.restype = C.c_int
+        _lib.vrc_cast.argtypes = [C.POINTER(_Problem), C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        _lib.vrc_cast_mt.restype = C.c_int
+        _lib.vrc_cast_mt.argtypes = [C.POINTER(_Problem), C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                     C.c_int, C.c_int64]
+        _lib.vrc_fnv1a_cells.restype = C.c_uint64
+        _lib.vrc_fnv1a_cells.argtypes = [C.c_void_p, C.c_int64]
+        _lib.vrc_max_threads.restype = C.c_int
+    return _lib
+
+
+def fnv1a_cells(cells) -> int:
+    a = np.ascontiguousarray(cells, dtype=np.uint32)
+    return int(_load().vrc_fnv1a_cells(a.ctypes.data, a.size))
+
+
+def max_threads() -> int:
+    return int(_load().vrc_max_threads())
+
+
+@dataclass
+class CastResult:
+    tally: Optional[np.ndarray]
+    rays_accepted: int
+    rays_rejected: int
+    segments: int
+    threads: int
+    nseg: Optional[np.ndarray] = None
+    hash: Optional[np.ndarray] = None
+    sum_l: Optional[np.ndarray] = None
+    t_exit: Optional[np.ndarray] = None
+    tau_exit: Optional[np.ndarray] = None
+    sum_score: Optional[np.ndarray] = None
+    sum_sig_score: Optional[np.ndarray] = None
+    cells: Optional[np.ndarray] = None
+    lens: Optional[np.ndarray] = None
+    scores: Optional[np.ndarray] = None
+
+
+class Oracle:
+    """The oracle bound to one problem (mesh + materials + tables).
+
+    `prob` is any object with nx, ny, nz, xe, ye, ze, density, K, cell_mat, cell_frac, xs
+    (e.g. workloads.Problem).  Arrays are taken as float64 / int32 views, never modified.
+    """
+
+    def __init__(self, prob):
+        self.lib = _load()
+        self.nx, self.ny, self.nz = int(prob.nx), int(prob.ny), int(prob.nz)
+        self.ncell = self.nx * self.ny * self.nz
+        self._xe = np.ascontiguousarray(prob.xe, dtype=np.float64)
+        self._ye = np.ascontiguousarray(prob.ye, dtype=np.float64)
+        self._ze = np.ascontiguousarray(prob.ze, dtype=np.float64)
+        self._den = np.ascontiguousarray(prob.density, dtype=np.float64)
+        self.M = len(self._den)
+        self.K = int(prob.K)
+        self._mat = np.ascontiguousarray(prob.cell_mat, dtype=np.int32).reshape(-1)
+        self._frac = np.ascontiguousarray(prob.cell_frac, dtype=np.float64).reshape(-1)
+        assert self._mat.size == self.ncell * self.K and self._frac.size == self.ncell * self.K
+        assert len(prob.xs) == self.M and self.M <= 64
+        off = np.zeros(self.M + 1, dtype=np.int64)
+        for m, (e, s) in enumerate(prob.xs):
+            assert len(e) == len(s) and len(e) >= 1
+            off[m + 1] = off[m] + len(e)
+        self._off = off
+        self._E = np.ascontiguousarray(np.concatenate([np.asarray(e, dtype=np.float64) for e, _ in prob.xs]))
+        self._S = np.ascontiguousarray(np.concatenate([np.asarray(s, dtype=np.float64) for _, s in prob.xs]))
+        self._p = _Problem(self.nx, self.ny, self.nz, self._xe.ctypes.data, self._ye.ctypes.data,
+                           self._ze.ctypes.data, self.M, self._den.ctypes.data, self.K, self._mat.ctypes.data,
+                           self._frac.ctypes.data, self._off.ctypes.data, self._E.ctypes.data, self._S.ctypes.data)
+
+    def sigma(self, m: int, E: float) -> float:
+        return float(self.lib.vrc_sigma(C.byref(self._p), int(m), float(E)))
+
+    def cast(self, rays, tally: Optional[np.ndarray] = None, *, score: bool = True, per_ray: bool = False,
+             cap: int = 0, threads: int = 1, private_bytes_max: int = 8 << 30) -> CastResult:
+        """Cast `rays` ([n,8], any float dtype; promoted exactly to double).
+
+        score=False walks without touching a tally (trace only).  per_ray=True returns the O6
+        per-ray diagnostics; cap>0 also returns the first `cap` (cell, length, score) of each ray.
+        """
+        r = np.ascontiguousarray(np.asarray(rays, dtype=np.float64).reshape(-1, 8))
+        n = r.shape[0]
+        if score and tally is None:
+            tally = np.zeros(self.ncell, dtype=np.float64)
+        if tally is not None:
+            assert tally.dtype == np.float64 and tally.size == self.ncell and tally.flags.c_contiguous
+        res = CastResult(tally if score else None, 0, 0, 0, 1)
+        dg = None
+        if per_ray or cap > 0:
+            res.nseg = np.zeros(n, dtype=np.uint32)
+            res.hash = np.zeros(n, dtype=np.uint64)
+            for nm in ("sum_l", "t_exit", "tau_exit", "sum_score", "sum_sig_score"):
+                setattr(res, nm, np.zeros(n, dtype=np.float64))
+            dg = _Diag(res.nseg.ctypes.data, res.hash.ctypes.data, res.sum_l.ctypes.data, res.t_exit.ctypes.data,
+                       res.tau_exit.ctypes.data, res.sum_score.ctypes.data, res.sum_sig_score.ctypes.data,
+                       None, None, None, 0)
+            if cap > 0:
+                res.cells = np.full((n, cap), -1, dtype=np.int32)
+                res.lens = np.zeros((n, cap), dtype=np.float64)
+                res.scores = np.zeros((n, cap), dtype=np.float64)
+                dg.cells, dg.lens, dg.scores, dg.cap = res.cells.ctypes.data, res.lens.ctypes.data, res.scores.ctypes.data, cap
+        cnt = _Counts()
+        tptr = tally.ctypes.data if (score and tally is not None) else None
+        dptr = C.cast(C.byref(dg), C.c_void_p) if dg is not None else None
+        if threads <= 1:
+            rc = self.lib.vrc_cast(C.byref(self._p), n, r.ctypes.data, tptr, dptr, C.cast(C.byref(cnt), C.c_void_p))
+            used = 1
+        else:
+            rc = self.lib.vrc_cast_mt(C.byref(self._p), n, r.ctypes.data, tptr, dptr,
+                                      C.cast(C.byref(cnt), C.c_void_p), int(threads), int(private_bytes_max))
+            used = rc
+        if rc < 0:
+            raise RuntimeError(f"oracle error {rc}")
+        res.rays_accepted, res.rays_rejected, res.segments, res.threads = (
+            int(cnt.rays_accepted), int(cnt.rays_rejected), int(cnt.segments), int(used))
+        return res

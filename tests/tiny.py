@@ -1,0 +1,62 @@
+"""Tiny random problems for pins and property tests (input generation only; no method arithmetic)."""
+from __future__ import annotations
+
+from types import SimpleNamespace
+
+import numpy as np
+
+
+def f32r(a):
+    return np.asarray(a, dtype=np.float64).astype(np.float32).astype(np.float64)
+
+
+def tiny_problem(seed, nx=4, ny=3, nz=5, M=3, K=2, n_e=17, uniform=False, void=False, homogeneous=False,
+                 fp32_values=True):
+    g = np.random.default_rng(seed)
+    rnd = f32r if fp32_values else (lambda a: np.asarray(a, dtype=np.float64))
+
+    def edges(n):
+        if uniform:
+            return -1.0 + 0.75 * np.arange(n + 1)
+        return np.concatenate([[-1.0], -1.0 + np.cumsum(0.2 + g.random(n))])
+
+    xe, ye, ze = edges(nx), edges(ny), edges(nz)
+    ncell = nx * ny * nz
+    density = rnd(0.5 + 3.0 * g.random(M))
+    if void:
+        density = np.zeros(M)
+    cell_mat = g.integers(-1, M, size=(ncell, K)).astype(np.int32)
+    cell_frac = rnd(g.random((ncell, K)))
+    cell_frac[cell_mat < 0] = 0.0
+    if homogeneous:
+        cell_mat[:] = -1
+        cell_mat[:, 0] = 0
+        cell_frac[:] = 0.0
+        cell_frac[:, 0] = 1.0
+    xs = []
+    for m in range(M):
+        e = rnd(np.sort(1e-3 * 1e4 ** g.random(n_e)))
+        e = np.unique(e)
+        s = rnd(0.05 + g.random(len(e)))
+        xs.append((e, s))
+    return SimpleNamespace(config=0, name=f"tiny{seed}", nx=nx, ny=ny, nz=nz, xe=xe, ye=ye, ze=ze,
+                           density=density, K=K, cell_mat=cell_mat, cell_frac=cell_frac, xs=xs,
+                           M=M, ncell=ncell)
+
+
+def tiny_rays(prob, seed, n, axis_aligned_share=0.0, e_lo=5e-4, e_hi=20.0, dtype=np.float32):
+    g = np.random.default_rng(seed)
+    lo = np.array([prob.xe[0], prob.ye[0], prob.ze[0]])
+    hi = np.array([prob.xe[-1], prob.ye[-1], prob.ze[-1]])
+    pos = lo + (0.001 + 0.998 * g.random((n, 3))) * (hi - lo)
+    d = g.normal(size=(n, 3))
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    k = int(axis_aligned_share * n)
+    for r in range(k):  # zero out one or two components (exercises Q10, including -0.0)
+        z = g.permutation(3)[: 1 + (r % 2)]
+        d[r, z] = 0.0 if r % 3 else -0.0
+        d[r] /= np.linalg.norm(d[r])
+    e = e_lo * (e_hi / e_lo) ** g.random(n)
+    w = 0.5 + g.random(n)
+    rays = np.concatenate([pos, d, e[:, None], w[:, None]], axis=1)
+    return np.ascontiguousarray(rays.astype(dtype))
