@@ -1,0 +1,191 @@
+/*
+ * monteray.h -- C ABI of the B200-native VRC (volumetric-ray-casting) fluence-tally library.
+ *
+ * The library is the GPU side of the method of arXiv:1706.07476 (PAPER.md = the paper's text):
+ * a host Monte Carlo random walk fills a buffer with rays (one per sampled outgoing
+ * direction/energy at a collision or source event) and hands the full buffer to
+ * the library (Fig. 4); for every ray the GPU evaluates all cross sections at
+ * the ray's energy, casts the ray through the whole 3-D Cartesian mesh and scores Eq. (4)
+ * into every crossed cell (Fig. 5); the tally stays on the GPU until it is read
+ * back at the end.
+ *
+ * Conventions that hold for every call:
+ *   - plain C, no exceptions cross the boundary; every function returns an mr_status;
+ *     mr_last_error(ctx) gives a human-readable message owned by the context.
+ *   - "host" pointers are ordinary CPU memory (pageable or pinned); "device" pointers are
+ *     CUDA device memory on the context's device.  The caller owns every array it passes.
+ *     The library has copied (or consumed) a HOST input before the call returns, so the
+ *     caller may free or overwrite it at once -- the paper's "the CPU cleared the buffer and
+ *     resumed".  A DEVICE input of mr_cast_rays / mr_trace_rays is read by
+ *     work queued on the context's stream: keep it alive and unmodified until that work
+ *     has finished (stream order, or mr_sync).
+ *   - outputs are caller-allocated host arrays.
+ *   - one context is used by one host thread at a time.  All device work of a context is
+ *     queued on ONE CUDA stream (mr_set_stream; default: the legacy default stream).
+ *   - cell linear index c = ix + nx*(iy + ny*iz), x fastest.
+ *   - units: cm, MeV, g/cc, cm^2/g; the tally is raw weight*cm sums (no volume or source
+ *     normalisation: that is host-side bookkeeping, off the hot path).
+ * Readings of the paper where it is silent (Q1..Q20) are listed in DESIGN.md §3.
+ */
+#ifndef MONTERAY_H
+#define MONTERAY_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define MR_API __attribute__((visibility("default")))
+#else
+#define MR_API
+#endif
+
+typedef struct mr_ctx mr_ctx;
+
+typedef enum {
+    MR_OK = 0,
+    MR_ERR_INVALID_ARG = 1, /* bad pointer/size/value; the context is unchanged */
+    MR_ERR_STATE = 2,       /* wrong call order (e.g. cast before all tables are loaded) */
+    MR_ERR_CUDA = 3,        /* a CUDA call failed; sticky errors keep being reported */
+    MR_ERR_OOM = 4,         /* device or pinned-host allocation failed */
+    MR_ERR_UNSUPPORTED = 5  /* a size beyond MR_MAX_* */
+} mr_status;
+
+/* Precision mode ("double-precision operations ... but using single precision
+ * cross-sections and distances"; reading Q1):
+ *   MIXED : fp32 energy grids, sigma tables, ray records and cell coefficients; fp64 mesh
+ *           traversal, Eq. (4) evaluation and tally.  Ray record = 8 floats (32 B).
+ *   DOUBLE: everything fp64.  Ray record = 8 doubles (64 B). */
+enum { MR_PRECISION_MIXED = 0, MR_PRECISION_DOUBLE = 1 };
+
+/* Where a ray buffer lives. */
+enum { MR_WHERE_HOST = 0, MR_WHERE_DEVICE = 1 };
+
+#define MR_MAX_MATERIALS 64
+#define MR_MAX_SLOTS 16
+
+/* Optional device-memory allocator supplied by the caller (the Python binding passes one that
+ * hands out torch caching-allocator blocks).  alloc returns a device pointer aligned to 256 B
+ * or NULL; both are called on the thread that calls into the library. */
+typedef void *(*mr_alloc_fn)(void *user, size_t bytes, int device);
+typedef void (*mr_free_fn)(void *user, void *ptr, int device);
+typedef struct {
+    mr_alloc_fn alloc;
+    mr_free_fn free;
+    void *user;
+} mr_allocator;
+
+typedef struct {
+    int64_t rays_accepted;  /* rays cast since creation or the last mr_clear_tally */
+    int64_t rays_rejected;  /* rays refused by the validation rule below */
+    int64_t segments;       /* ray-cell segments scored (zero-length ones included) */
+    int64_t kernel_launches;/* kernels this context has launched since creation */
+    double last_cast_ms;    /* device time of the most recent mr_cast_rays work (all its kernels) */
+    int64_t reserved[4];
+} mr_stats;
+
+/* ---- life cycle -------------------------------------------------------------------------- */
+
+/* Creates a context on CUDA device `device`.  `alloc` may be NULL (cudaMalloc is used).
+ * Errors: INVALID_ARG (out NULL, unknown precision, bad device), CUDA. */
+MR_API int mr_create(mr_ctx **out, int device, int precision);
+MR_API int mr_create_ex(mr_ctx **out, int device, int precision, const mr_allocator *alloc);
+
+/* Synchronises the stream, frees every device and pinned buffer.  NULL is accepted. */
+MR_API int mr_destroy(mr_ctx *ctx);
+
+/* Makes `cuda_stream` (a cudaStream_t passed as void*, NULL = legacy default stream) the
+ * stream all later work of this context is queued on.  Pending work is synchronised first. */
+MR_API int mr_set_stream(mr_ctx *ctx, void *cuda_stream);
+
+/* Message of the last error of this context ("" if none).  Valid until the next call on ctx.
+ * mr_last_error(NULL) describes the last failed mr_create. */
+MR_API const char *mr_last_error(mr_ctx *ctx);
+
+/* ---- problem set-up ("continuous energy total cross section data ... 3-D
+ *      Cartesian mesh geometry"; geometry and tally share the mesh) ------------ */
+
+/* Rectilinear mesh given by its plane positions: xe[nx+1], ye[ny+1], ze[nz+1], host, strictly
+ * increasing, finite.  nx*ny*nz must be < 2^31.  Allocates and zeroes the fp64 tally; drops
+ * any material map loaded before.  Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA. */
+MR_API int mr_load_mesh(mr_ctx *ctx, int nx, int ny, int nz, const double *xe, const double *ye, const double *ze);
+
+/* Materials and per-cell composition.  density[M] g/cc (finite, >= 0); K slots per cell;
+ * cell_mat[ncell*K] material index per slot, -1 = empty slot; cell_frac[ncell*K] volume
+ * fractions (finite, >= 0; ignored for empty slots).  Slot k of cell c is element c*K+k.
+ * The library stores r = frac*density (rounded once to fp32 in MIXED mode) and the total
+ * cross section of cell c at energy E is Sigma_t = sum_k r[c,k] * sigma_{mat[c,k]}(E), summed
+ * in slot order (reading Q3).  Requires mr_load_mesh.  Drops loaded tables when M
+ * changes.  All host arrays.  Errors: INVALID_ARG, STATE, UNSUPPORTED (M > MR_MAX_MATERIALS,
+ * K > MR_MAX_SLOTS), OOM, CUDA. */
+MR_API int mr_load_materials(mr_ctx *ctx, int M, const double *density, int K, const int32_t *cell_mat,
+                      const double *cell_frac);
+
+/* Tabulated total cross section of material `material`: energy[n] MeV strictly increasing and
+ * > 0, sigma_t[n] cm^2/g finite and >= 0, host arrays, n >= 1.  sigma(E) is the lin-lin
+ * interpolant, clamped to the end values outside the grid (reading Q5).
+ * In MIXED mode the values are stored as fp32 (pass fp32-representable values to keep the
+ * bracket identical to a double evaluation).  Requires mr_load_materials.
+ * Errors: INVALID_ARG, STATE, OOM, CUDA. */
+MR_API int mr_load_xs(mr_ctx *ctx, int material, int64_t n, const double *energy, const double *sigma_t);
+
+/* ---- the hot path ------------------------------------------------------------------------ */
+
+/* Casts a batch of n rays and ADDS their scores to the resident tally (PAPER.md:77-85,
+ * Eq. (4)).  `rays` is an array of n records {x,y,z,u,v,w,E,W}: 8 floats in
+ * MIXED mode, 8 doubles in DOUBLE mode; where = MR_WHERE_HOST or MR_WHERE_DEVICE (device
+ * buffers must be 16-byte aligned).  W is the already divided weight W/N of Eq. (4).
+ * For every accepted ray, with tau = 0 at the origin, for each crossed cell i in order:
+ *     x = Sigma_i * l_i;   score = W * exp(-tau) * (x > 0 ? (1 - exp(-x)) / Sigma_i : l_i);
+ *     tally[i] += score;   tau += x
+ * until the ray leaves the mesh (no cut-off, no reflection: readings Q7, F5).  A ray is
+ * REJECTED (counted, no contribution) if any field is not finite, E <= 0, the direction is
+ * the zero vector, or the origin is outside the half-open box [lo, hi) on any axis.
+ * Asynchronous: returns once the batch is staged and the work is queued.  n = 0 is a no-op.
+ * Requires mesh, materials and all M tables.  Errors: INVALID_ARG, STATE, OOM, CUDA. */
+MR_API int mr_cast_rays(mr_ctx *ctx, int64_t n, const void *rays, int where);
+
+/* Synchronises and copies the ncell raw fp64 sums to the host array `out` ("the
+ * tally remained on the GPU until the termination of the simulation").  A consistent
+ * snapshot: all work queued before the call is included.  Errors: INVALID_ARG, STATE, CUDA. */
+MR_API int mr_read_tally(mr_ctx *ctx, double *out);
+
+/* Zeroes the tally and the ray/segment counters (queued on the stream). */
+MR_API int mr_clear_tally(mr_ctx *ctx);
+
+/* Blocks until all queued work of the context has finished. */
+MR_API int mr_sync(mr_ctx *ctx);
+
+/* Synchronises and fills *out. */
+MR_API int mr_get_stats(mr_ctx *ctx, mr_stats *out);
+
+/* Borrowed device pointer to the ncell fp64 tally (e.g. for a caller-side NCCL all-reduce
+ * across replicas).  Valid until the next mr_load_mesh / mr_destroy. */
+MR_API int mr_tally_device_ptr(mr_ctx *ctx, double **out);
+
+/* ---- test / diagnostic entry point ------------------------------------------------------- */
+
+/* The same walk as mr_cast_rays with no tally update.  Per ray r (host outputs, any may be
+ * NULL): nseg[r] = number of segments (0 if rejected); hash[r] = FNV-1a 64 over the
+ * little-endian bytes of the 32-bit cell indices in crossing order (0 if rejected);
+ * if cap > 0: cells[r*cap + j], lens[r*cap + j] for the first min(nseg, cap) segments
+ * (untouched beyond).  Needs only the mesh.  Synchronous.  Errors as mr_cast_rays. */
+MR_API int mr_trace_rays(mr_ctx *ctx, int64_t n, const void *rays, int where, uint32_t *nseg, uint64_t *hash,
+                  int32_t *cells, double *lens, int64_t cap);
+
+/* ---- tuning knobs (never change results beyond fp64 summation order) ---------------------- */
+enum {
+    MR_OPT_BLOCK_THREADS = 1, /* threads per CTA of the cast kernel (multiple of 32, <= 1024) */
+    MR_OPT_SORT_RAYS = 2,     /* 0: cast in buffer order; 1: bin rays by start slab and length first */
+    MR_OPT_STAGE_RAYS = 3     /* rays per pinned staging chunk for host batches */
+};
+MR_API int mr_set_option(mr_ctx *ctx, int option, int64_t value);
+MR_API int mr_get_option(mr_ctx *ctx, int option, int64_t *value);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MONTERAY_H */

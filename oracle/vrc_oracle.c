@@ -124,7 +124,11 @@ static int cast_one(const vrc_problem *p, const double *ray, double *tally, int 
     /* O1 validate */
     for (int f = 0; f < 8; ++f) if (!isfinite(ray[f])) accepted = 0;
     if (!(E > 0.0)) accepted = 0;
-    if (d[0] == 0.0 && d[1] == 0.0 && d[2] == 0.0) accepted = 0;
+    {   /* the ray must be able to move: an axis steps only if d_a != 0 and 1/d_a is finite (Q10) */
+        int movable = 0;
+        for (int a = 0; a < 3; ++a) if (d[a] != 0.0 && isfinite(1.0 / d[a])) movable = 1;
+        if (!movable) accepted = 0;
+    }
     for (int a = 0; a < 3 && accepted; ++a)
         if (!(o[a] >= edges[a][0] && o[a] < edges[a][n[a]])) accepted = 0;
 

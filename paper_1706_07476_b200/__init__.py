@@ -1,0 +1,21 @@
+"""B200-native VRC (volumetric-ray-casting) fluence-tally hot path of arXiv:1706.07476.
+
+The product is the C-ABI CUDA library libmonteray.so (include/monteray.h, csrc/); this package
+is its thin Python binding.  Importing the package does not load the library; the first use
+does, and fails loudly if it has not been built.  There is no CPU fallback.
+"""
+from .binding import (  # noqa: F401
+    EXPORTS,
+    LIB_PATH,
+    MR_OPT_BLOCK_THREADS,
+    MR_OPT_SORT_RAYS,
+    MR_OPT_STAGE_RAYS,
+    MR_PRECISION_DOUBLE,
+    MR_PRECISION_MIXED,
+    MR_WHERE_DEVICE,
+    MR_WHERE_HOST,
+    MonteRay,
+    MonteRayError,
+    Stats,
+    load_library,
+)

@@ -1,0 +1,300 @@
+"""Thin ctypes binding of libmonteray.so (include/monteray.h): argument marshalling only.
+
+Every step of the hot path runs inside the CUDA library; this module converts numpy / torch
+arguments to pointers and sizes and turns status codes into exceptions.  PyTorch supplies
+device memory (through the allocator callbacks) and the CUDA stream.  There is no CPU
+fallback: if the shared library is missing or no CUDA device is usable, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmonteray.so")
+
+MR_OK, MR_ERR_INVALID_ARG, MR_ERR_STATE, MR_ERR_CUDA, MR_ERR_OOM, MR_ERR_UNSUPPORTED = range(6)
+MR_PRECISION_MIXED, MR_PRECISION_DOUBLE = 0, 1
+MR_WHERE_HOST, MR_WHERE_DEVICE = 0, 1
+MR_OPT_BLOCK_THREADS, MR_OPT_SORT_RAYS, MR_OPT_STAGE_RAYS = 1, 2, 3
+_STATUS = {1: "MR_ERR_INVALID_ARG", 2: "MR_ERR_STATE", 3: "MR_ERR_CUDA", 4: "MR_ERR_OOM", 5: "MR_ERR_UNSUPPORTED"}
+
+EXPORTS = [
+    "mr_create", "mr_create_ex", "mr_destroy", "mr_set_stream", "mr_last_error", "mr_load_mesh",
+    "mr_load_materials", "mr_load_xs", "mr_cast_rays", "mr_read_tally", "mr_clear_tally", "mr_sync",
+    "mr_get_stats", "mr_tally_device_ptr", "mr_trace_rays", "mr_set_option", "mr_get_option",
+]
+
+
+class MonteRayError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{_STATUS.get(status, status)}: {message}")
+        self.status = status
+
+
+class mr_stats(C.Structure):
+    _fields_ = [("rays_accepted", C.c_int64), ("rays_rejected", C.c_int64), ("segments", C.c_int64),
+                ("kernel_launches", C.c_int64), ("last_cast_ms", C.c_double), ("reserved", C.c_int64 * 4)]
+
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_void_p, C.c_size_t, C.c_int)
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_int)
+
+
+class mr_allocator(C.Structure):
+    _fields_ = [("alloc", _ALLOC_FN), ("free", _FREE_FN), ("user", C.c_void_p)]
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """Loads libmonteray.so; raises if it has not been built (python -m paper_1706_07476_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_1706_07476_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64 = C.c_void_p, C.c_int, C.c_int64
+    sigs = {
+        "mr_create": [C.POINTER(vp), i32, i32],
+        "mr_create_ex": [C.POINTER(vp), i32, i32, C.POINTER(mr_allocator)],
+        "mr_destroy": [vp],
+        "mr_set_stream": [vp, vp],
+        "mr_load_mesh": [vp, i32, i32, i32, vp, vp, vp],
+        "mr_load_materials": [vp, i32, vp, i32, vp, vp],
+        "mr_load_xs": [vp, i32, i64, vp, vp],
+        "mr_cast_rays": [vp, i64, vp, i32],
+        "mr_read_tally": [vp, vp],
+        "mr_clear_tally": [vp],
+        "mr_sync": [vp],
+        "mr_get_stats": [vp, C.POINTER(mr_stats)],
+        "mr_tally_device_ptr": [vp, C.POINTER(vp)],
+        "mr_trace_rays": [vp, i64, vp, i32, vp, vp, vp, vp, i64],
+        "mr_set_option": [vp, i32, i64],
+        "mr_get_option": [vp, i32, C.POINTER(i64)],
+    }
+    for name, argtypes in sigs.items():
+        fn = getattr(lib, name)
+        fn.argtypes = argtypes
+        fn.restype = C.c_int
+    lib.mr_last_error.argtypes = [vp]
+    lib.mr_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+class _TorchAllocator:
+    """mr_allocator backed by torch's CUDA caching allocator (uint8 tensors kept alive by pointer)."""
+
+    def __init__(self):
+        import torch
+
+        self._torch = torch
+        self._live = {}
+        self._alloc_cb = _ALLOC_FN(self._alloc)
+        self._free_cb = _FREE_FN(self._free)
+        self.struct = mr_allocator(self._alloc_cb, self._free_cb, None)
+
+    def _alloc(self, user, nbytes, device):
+        try:
+            t = self._torch.empty(max(int(nbytes), 16), dtype=self._torch.uint8, device=f"cuda:{device}")
+        except Exception:  # out of memory -> NULL -> MR_ERR_OOM
+            return None
+        self._live[t.data_ptr()] = t
+        return t.data_ptr()
+
+    def _free(self, user, ptr, device):
+        self._live.pop(ptr, None)
+
+
+@dataclass
+class Stats:
+    rays_accepted: int
+    rays_rejected: int
+    segments: int
+    kernel_launches: int
+    last_cast_ms: float
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+class MonteRay:
+    """One library context.  Method names mirror the C entry points (mr_<name>)."""
+
+    def __init__(self, device: int = 0, precision: int = MR_PRECISION_MIXED, use_torch_allocator: bool = True,
+                 use_torch_stream: bool = True):
+        self.lib = load_library()
+        self.precision = precision
+        self.device = device
+        self._h = C.c_void_p()
+        self._allocator = None
+        if use_torch_allocator:
+            import torch
+
+            if not torch.cuda.is_available():
+                raise MonteRayError(MR_ERR_CUDA, "no CUDA device visible to torch (there is no CPU fallback)")
+            torch.cuda.init()
+            self._allocator = _TorchAllocator()
+            rc = self.lib.mr_create_ex(C.byref(self._h), device, precision, C.byref(self._allocator.struct))
+        else:
+            rc = self.lib.mr_create(C.byref(self._h), device, precision)
+        if rc != MR_OK:
+            raise MonteRayError(rc, (self.lib.mr_last_error(None) or b"").decode())
+        self.ncell = 0
+        if use_torch_stream:
+            self.use_current_torch_stream()
+
+    # ---- plumbing
+    def _check(self, rc: int):
+        if rc != MR_OK:
+            raise MonteRayError(rc, (self.lib.mr_last_error(self._h) or b"").decode())
+
+    def close(self):
+        if self._h:
+            self.lib.mr_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def use_current_torch_stream(self):
+        import torch
+
+        self.set_stream(torch.cuda.current_stream(self.device).cuda_stream)
+
+    def set_stream(self, cuda_stream: int):
+        self._check(self.lib.mr_set_stream(self._h, C.c_void_p(cuda_stream)))
+
+    @property
+    def ray_dtype(self):
+        return np.float64 if self.precision == MR_PRECISION_DOUBLE else np.float32
+
+    # ---- set-up
+    def load_mesh(self, xe, ye, ze):
+        xe, ye, ze = _f64(xe), _f64(ye), _f64(ze)
+        self._check(self.lib.mr_load_mesh(self._h, len(xe) - 1, len(ye) - 1, len(ze) - 1,
+                                          xe.ctypes.data, ye.ctypes.data, ze.ctypes.data))
+        self.ncell = (len(xe) - 1) * (len(ye) - 1) * (len(ze) - 1)
+
+    def load_materials(self, density, cell_mat, cell_frac):
+        density = _f64(density)
+        cell_mat = np.ascontiguousarray(cell_mat, dtype=np.int32)
+        cell_frac = _f64(cell_frac)
+        if cell_mat.size != cell_frac.size or self.ncell == 0 or cell_mat.size % self.ncell:
+            raise MonteRayError(MR_ERR_INVALID_ARG, "cell_mat / cell_frac must both hold ncell*K entries")
+        K = cell_mat.size // self.ncell
+        self._check(self.lib.mr_load_materials(self._h, len(density), density.ctypes.data, K,
+                                               cell_mat.ctypes.data, cell_frac.ctypes.data))
+
+    def load_xs(self, material: int, energy, sigma_t):
+        energy, sigma_t = _f64(energy), _f64(sigma_t)
+        if len(energy) != len(sigma_t):
+            raise MonteRayError(MR_ERR_INVALID_ARG, "energy and sigma_t differ in length")
+        self._check(self.lib.mr_load_xs(self._h, material, len(energy), energy.ctypes.data, sigma_t.ctypes.data))
+
+    def load_problem(self, prob):
+        """Convenience: mesh + materials + all tables of a workloads.Problem-like object."""
+        self.load_mesh(prob.xe, prob.ye, prob.ze)
+        self.load_materials(prob.density, prob.cell_mat, prob.cell_frac)
+        for m, (e, s) in enumerate(prob.xs):
+            self.load_xs(m, e, s)
+
+    # ---- hot path
+    def _ray_arg(self, rays):
+        """(pointer, n, where, keepalive) for a numpy array (host) or a torch CUDA tensor (device)."""
+        if isinstance(rays, np.ndarray):
+            a = np.ascontiguousarray(rays, dtype=self.ray_dtype).reshape(-1, 8)
+            return a.ctypes.data, a.shape[0], MR_WHERE_HOST, a
+        import torch
+
+        if isinstance(rays, torch.Tensor):
+            want = torch.float64 if self.precision == MR_PRECISION_DOUBLE else torch.float32
+            if rays.dtype != want or not rays.is_contiguous() or rays.numel() % 8:
+                raise MonteRayError(MR_ERR_INVALID_ARG, f"ray tensor must be contiguous {want} with 8 fields per ray")
+            n = rays.numel() // 8
+            if rays.is_cuda:
+                return rays.data_ptr(), n, MR_WHERE_DEVICE, rays
+            return rays.data_ptr(), n, MR_WHERE_HOST, rays  # CPU tensor (pinned or pageable)
+        raise MonteRayError(MR_ERR_INVALID_ARG, "rays must be a numpy array or a torch tensor")
+
+    def cast_rays(self, rays):
+        ptr, n, where, keep = self._ray_arg(rays)
+        self._check(self.lib.mr_cast_rays(self._h, n, C.c_void_p(ptr), where))
+        return n
+
+    def read_tally(self, out: Optional[np.ndarray] = None) -> np.ndarray:
+        if out is None:
+            out = np.empty(self.ncell, dtype=np.float64)
+        assert out.dtype == np.float64 and out.size == self.ncell and out.flags.c_contiguous
+        self._check(self.lib.mr_read_tally(self._h, out.ctypes.data))
+        return out
+
+    def read_tally_into(self, host_ptr: int):
+        """mr_read_tally into caller-owned host memory (e.g. a pinned torch tensor's data_ptr())."""
+        self._check(self.lib.mr_read_tally(self._h, C.c_void_p(host_ptr)))
+
+    def clear_tally(self):
+        self._check(self.lib.mr_clear_tally(self._h))
+
+    def sync(self):
+        self._check(self.lib.mr_sync(self._h))
+
+    def get_stats(self) -> Stats:
+        s = mr_stats()
+        self._check(self.lib.mr_get_stats(self._h, C.byref(s)))
+        return Stats(s.rays_accepted, s.rays_rejected, s.segments, s.kernel_launches, s.last_cast_ms)
+
+    def tally_device_ptr(self) -> int:
+        p = C.c_void_p()
+        self._check(self.lib.mr_tally_device_ptr(self._h, C.byref(p)))
+        return int(p.value)
+
+    def tally_tensor(self):
+        """The resident tally as a torch tensor view (no copy), e.g. for torch.distributed.all_reduce."""
+        import torch
+
+        class _Wrap:
+            pass
+
+        w = _Wrap()
+        w.__cuda_array_interface__ = {"shape": (self.ncell,), "typestr": "<f8", "data": (self.tally_device_ptr(), False),
+                                      "version": 3, "strides": None}
+        return torch.as_tensor(w, device=f"cuda:{self.device}")
+
+    def trace_rays(self, rays, cap: int = 0):
+        """mr_trace_rays -> (nseg uint32[n], hash uint64[n], cells int32[n,cap] | None, lens float64[n,cap] | None)."""
+        ptr, n, where, keep = self._ray_arg(rays)
+        nseg = np.zeros(n, dtype=np.uint32)
+        hsh = np.zeros(n, dtype=np.uint64)
+        cells = np.full((n, cap), -1, dtype=np.int32) if cap > 0 else None
+        lens = np.zeros((n, cap), dtype=np.float64) if cap > 0 else None
+        self._check(self.lib.mr_trace_rays(self._h, n, C.c_void_p(ptr), where, nseg.ctypes.data, hsh.ctypes.data,
+                                           cells.ctypes.data if cap > 0 else None,
+                                           lens.ctypes.data if cap > 0 else None, cap))
+        return nseg, hsh, cells, lens
+
+    def set_option(self, option: int, value: int):
+        self._check(self.lib.mr_set_option(self._h, option, value))
+
+    def get_option(self, option: int) -> int:
+        v = C.c_int64()
+        self._check(self.lib.mr_get_option(self._h, option, C.byref(v)))
+        return int(v.value)

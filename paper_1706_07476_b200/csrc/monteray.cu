@@ -1,0 +1,733 @@
+// monteray.cu -- host side of the C ABI declared in include/monteray.h.
+//
+// One translation unit: the context (device buffers, staging ring, options), argument
+// checking, and the kernel launches.  Device code lives in mr_device.cuh.  Nothing here
+// falls back to the CPU: without a CUDA device every entry point fails with MR_ERR_CUDA.
+#include "../../include/monteray.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#define MR_PACK_MAX_SLOTS MR_MAX_SLOTS
+#include "mr_device.cuh"
+
+using namespace mr;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+constexpr int kStageSlots = 2;
+constexpr size_t kEdgesSmemMax = 96 * 1024;  // larger meshes read their planes from global memory
+
+struct DeviceGuard {
+    int prev = -1;
+    bool changed = false;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) changed = (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~DeviceGuard()
+    {
+        if (changed) cudaSetDevice(prev);
+    }
+};
+
+}  // namespace
+
+struct mr_ctx {
+    int device = 0;
+    int precision = MR_PRECISION_MIXED;
+    cudaStream_t stream = nullptr;
+    cudaStream_t copy_stream = nullptr;
+    mr_allocator alloc{nullptr, nullptr, nullptr};
+    std::string err;
+    bool sticky_cuda = false;
+
+    // mesh + tally
+    int nx = 0, ny = 0, nz = 0, nedges = 0;
+    long long ncell = 0;
+    double *d_edges = nullptr;
+    double *d_tally = nullptr;
+
+    // materials
+    int M = 0, K = 0, layout = 0;
+    void *d_recs = nullptr;
+    uint8_t *d_ids = nullptr;
+
+    // tables
+    std::vector<void *> d_E, d_S;
+    std::vector<int> xs_n;
+    XsDesc *d_xs = nullptr;
+    bool xs_dirty = true;
+
+    unsigned long long *d_counters = nullptr;  // accepted, rejected, segments, spare
+
+    // host-batch staging ring
+    void *pinned[kStageSlots] = {nullptr, nullptr};
+    void *d_stage[kStageSlots] = {nullptr, nullptr};
+    cudaEvent_t ev_copied[kStageSlots] = {nullptr, nullptr};
+    cudaEvent_t ev_done[kStageSlots] = {nullptr, nullptr};
+    size_t stage_cap_rays = 0;       // rays each slot can hold now
+    long long stage_rays = 1 << 21;  // option MR_OPT_STAGE_RAYS
+    int next_slot = 0;
+
+    cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;
+    bool have_timing = false;
+    long long launches = 0;
+    int block_threads = 256;
+    int sort_rays = 0;
+
+    size_t ray_bytes() const { return precision == MR_PRECISION_DOUBLE ? 64 : 32; }
+    size_t real_bytes() const { return precision == MR_PRECISION_DOUBLE ? 8 : 4; }
+
+    int fail(int code, const std::string &msg)
+    {
+        err = msg;
+        return code;
+    }
+    int fail_cuda(cudaError_t e, const char *what)
+    {
+        sticky_cuda = true;
+        err = std::string("CUDA error in ") + what + ": " + cudaGetErrorString(e);
+        return e == cudaErrorMemoryAllocation ? MR_ERR_OOM : MR_ERR_CUDA;
+    }
+    void *dev_alloc(size_t bytes)
+    {
+        if (bytes == 0) bytes = 16;
+        if (alloc.alloc) return alloc.alloc(alloc.user, bytes, device);
+        void *p = nullptr;
+        if (cudaMalloc(&p, bytes) != cudaSuccess) {
+            cudaGetLastError();
+            return nullptr;
+        }
+        return p;
+    }
+    void dev_free(void *p)
+    {
+        if (!p) return;
+        if (alloc.free) alloc.free(alloc.user, p, device);
+        else cudaFree(p);
+    }
+};
+
+#define MR_CUDA(ctx, call)                                              \
+    do {                                                                \
+        cudaError_t e_ = (call);                                        \
+        if (e_ != cudaSuccess) return (ctx)->fail_cuda(e_, #call);      \
+    } while (0)
+
+#define MR_ENTER(ctx)                                                                      \
+    if (!(ctx)) return MR_ERR_INVALID_ARG;                                                 \
+    if ((ctx)->sticky_cuda) return MR_ERR_CUDA;                                            \
+    DeviceGuard guard_((ctx)->device);                                                     \
+    (ctx)->err.clear()
+
+namespace {
+
+void free_materials(mr_ctx *c)
+{
+    c->dev_free(c->d_recs);
+    c->dev_free(c->d_ids);
+    c->d_recs = nullptr;
+    c->d_ids = nullptr;
+    c->layout = 0;
+    c->K = 0;
+}
+
+void free_tables(mr_ctx *c)
+{
+    for (void *p : c->d_E) c->dev_free(p);
+    for (void *p : c->d_S) c->dev_free(p);
+    c->d_E.clear();
+    c->d_S.clear();
+    c->xs_n.clear();
+    c->dev_free(c->d_xs);
+    c->d_xs = nullptr;
+    c->xs_dirty = true;
+}
+
+void free_stage(mr_ctx *c)
+{
+    for (int s = 0; s < kStageSlots; ++s) {
+        if (c->pinned[s]) cudaFreeHost(c->pinned[s]);
+        c->dev_free(c->d_stage[s]);
+        c->pinned[s] = nullptr;
+        c->d_stage[s] = nullptr;
+    }
+    c->stage_cap_rays = 0;
+}
+
+bool finite_increasing(const double *a, int n)
+{
+    for (int i = 0; i < n; ++i) {
+        if (!std::isfinite(a[i])) return false;
+        if (i && !(a[i] > a[i - 1])) return false;
+    }
+    return true;
+}
+
+template <typename K>
+int set_smem(mr_ctx *c, K kernel, size_t bytes)
+{
+    if (bytes > 48 * 1024) MR_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return MR_OK;
+}
+
+size_t edges_smem_bytes(const mr_ctx *c) { return sizeof(double) * (size_t)((c->nedges + 1) & ~1); }
+
+template <typename Real, typename Rec>
+int launch_cast_t(mr_ctx *c, const CastParams &P)
+{
+    const int block = c->block_threads;
+    const size_t sig_bytes = (size_t)c->M * block * sizeof(Real);
+    const bool smem_edges = edges_smem_bytes(c) <= kEdgesSmemMax && edges_smem_bytes(c) + sig_bytes <= 200 * 1024;
+    const size_t smem = (smem_edges ? edges_smem_bytes(c) : 0) + sig_bytes;
+    if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "materials x block threads exceed shared memory; lower MR_OPT_BLOCK_THREADS");
+    const long long grid = (P.n + block - 1) / block;
+    if (grid > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
+    if (smem_edges) {
+        if (int rc = set_smem(c, cast_kernel<Real, Rec, true>, smem)) return rc;
+        cast_kernel<Real, Rec, true><<<(unsigned)grid, block, smem, c->stream>>>(P);
+    } else {
+        if (int rc = set_smem(c, cast_kernel<Real, Rec, false>, smem)) return rc;
+        cast_kernel<Real, Rec, false><<<(unsigned)grid, block, smem, c->stream>>>(P);
+    }
+    c->launches += 1;
+    MR_CUDA(c, cudaGetLastError());
+    return MR_OK;
+}
+
+int upload_xs_desc(mr_ctx *c)
+{
+    if (!c->xs_dirty) return MR_OK;
+    std::vector<XsDesc> h(c->M);
+    for (int m = 0; m < c->M; ++m) h[m] = XsDesc{c->d_E[m], c->d_S[m], c->xs_n[m], 0};
+    if (!c->d_xs) {
+        c->d_xs = (XsDesc *)c->dev_alloc(sizeof(XsDesc) * MR_MAX_MATERIALS);
+        if (!c->d_xs) return c->fail(MR_ERR_OOM, "device allocation failed (table descriptors)");
+    }
+    MR_CUDA(c, cudaMemcpyAsync(c->d_xs, h.data(), sizeof(XsDesc) * c->M, cudaMemcpyHostToDevice, c->stream));
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));  // h goes out of scope
+    c->xs_dirty = false;
+    return MR_OK;
+}
+
+int ready_to_cast(mr_ctx *c)
+{
+    if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    if (!c->d_recs) return c->fail(MR_ERR_STATE, "no materials loaded");
+    for (int m = 0; m < c->M; ++m)
+        if (m >= (int)c->xs_n.size() || c->xs_n[m] == 0)
+            return c->fail(MR_ERR_STATE, "cross-section table of material " + std::to_string(m) + " not loaded");
+    return MR_OK;
+}
+
+// Queue the cast of n device-resident rays on the context's stream.
+int cast_device(mr_ctx *c, long long n, const void *d_rays)
+{
+    CastParams P{};
+    P.mesh = MeshDev{c->nx, c->ny, c->nz, c->nedges, c->d_edges};
+    P.recs = c->d_recs;
+    P.ids = c->d_ids;
+    P.K = c->K;
+    P.M = c->M;
+    P.xs = c->d_xs;
+    P.rays = d_rays;
+    P.perm = nullptr;
+    P.n = n;
+    P.tally = c->d_tally;
+    P.counters = c->d_counters;
+    if (c->precision == MR_PRECISION_DOUBLE) return launch_cast_t<double, CellRecGeneric<double>>(c, P);
+    switch (c->layout) {
+    case LAYOUT_K1: return launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P);
+    case LAYOUT_K2: return launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P);
+    case LAYOUT_K3: return launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P);
+    case LAYOUT_K4: return launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P);
+    case LAYOUT_D8: return launch_cast_t<float, CellRec<LAYOUT_D8>>(c, P);
+    default: return launch_cast_t<float, CellRecGeneric<float>>(c, P);
+    }
+}
+
+int ensure_stage(mr_ctx *c, size_t rays_per_slot)
+{
+    if (c->stage_cap_rays >= rays_per_slot) return MR_OK;
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    MR_CUDA(c, cudaStreamSynchronize(c->copy_stream));
+    free_stage(c);
+    const size_t bytes = rays_per_slot * c->ray_bytes();
+    for (int s = 0; s < kStageSlots; ++s) {
+        if (cudaMallocHost(&c->pinned[s], bytes) != cudaSuccess) {
+            cudaGetLastError();
+            free_stage(c);
+            return c->fail(MR_ERR_OOM, "pinned host allocation failed (staging ring)");
+        }
+        c->d_stage[s] = c->dev_alloc(bytes);
+        if (!c->d_stage[s]) {
+            free_stage(c);
+            return c->fail(MR_ERR_OOM, "device allocation failed (staging ring)");
+        }
+    }
+    c->stage_cap_rays = rays_per_slot;
+    return MR_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+extern "C" {
+
+int mr_create_ex(mr_ctx **out, int device, int precision, const mr_allocator *alloc)
+{
+    if (!out) {
+        g_create_error = "out is NULL";
+        return MR_ERR_INVALID_ARG;
+    }
+    *out = nullptr;
+    if (precision != MR_PRECISION_MIXED && precision != MR_PRECISION_DOUBLE) {
+        g_create_error = "unknown precision mode";
+        return MR_ERR_INVALID_ARG;
+    }
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        g_create_error = std::string("no usable CUDA device: ") + cudaGetErrorString(e);
+        return MR_ERR_CUDA;
+    }
+    if (device < 0 || device >= count) {
+        g_create_error = "device index out of range";
+        return MR_ERR_INVALID_ARG;
+    }
+    if (alloc && (!alloc->alloc || !alloc->free)) {
+        g_create_error = "allocator needs both alloc and free";
+        return MR_ERR_INVALID_ARG;
+    }
+    mr_ctx *c = new mr_ctx();
+    c->device = device;
+    c->precision = precision;
+    if (alloc) c->alloc = *alloc;
+    DeviceGuard guard(device);
+    bool ok = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
+    for (int s = 0; s < kStageSlots && ok; ++s) {
+        ok = ok && cudaEventCreateWithFlags(&c->ev_copied[s], cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&c->ev_done[s], cudaEventDisableTiming) == cudaSuccess;
+    }
+    ok = ok && cudaEventCreate(&c->ev_t0) == cudaSuccess && cudaEventCreate(&c->ev_t1) == cudaSuccess;
+    if (ok) {
+        c->d_counters = (unsigned long long *)c->dev_alloc(4 * sizeof(unsigned long long));
+        ok = c->d_counters && cudaMemset(c->d_counters, 0, 4 * sizeof(unsigned long long)) == cudaSuccess;
+    }
+    if (!ok) {
+        g_create_error = std::string("context set-up failed: ") + cudaGetErrorString(cudaGetLastError());
+        mr_destroy(c);
+        return MR_ERR_CUDA;
+    }
+    *out = c;
+    return MR_OK;
+}
+
+int mr_create(mr_ctx **out, int device, int precision) { return mr_create_ex(out, device, precision, nullptr); }
+
+int mr_destroy(mr_ctx *c)
+{
+    if (!c) return MR_OK;
+    DeviceGuard guard(c->device);
+    cudaStreamSynchronize(c->stream);
+    if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
+    free_stage(c);
+    free_tables(c);
+    free_materials(c);
+    c->dev_free(c->d_edges);
+    c->dev_free(c->d_tally);
+    c->dev_free(c->d_counters);
+    for (int s = 0; s < kStageSlots; ++s) {
+        if (c->ev_copied[s]) cudaEventDestroy(c->ev_copied[s]);
+        if (c->ev_done[s]) cudaEventDestroy(c->ev_done[s]);
+    }
+    if (c->ev_t0) cudaEventDestroy(c->ev_t0);
+    if (c->ev_t1) cudaEventDestroy(c->ev_t1);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    cudaGetLastError();
+    delete c;
+    return MR_OK;
+}
+
+int mr_set_stream(mr_ctx *c, void *cuda_stream)
+{
+    MR_ENTER(c);
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    MR_CUDA(c, cudaStreamSynchronize(c->copy_stream));
+    c->stream = (cudaStream_t)cuda_stream;
+    return MR_OK;
+}
+
+const char *mr_last_error(mr_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+int mr_load_mesh(mr_ctx *c, int nx, int ny, int nz, const double *xe, const double *ye, const double *ze)
+{
+    MR_ENTER(c);
+    if (nx < 1 || ny < 1 || nz < 1 || !xe || !ye || !ze) return c->fail(MR_ERR_INVALID_ARG, "mesh: bad size or NULL edge array");
+    const long long ncell = (long long)nx * ny * nz;
+    if ((long long)nx * ny > 0x7fffffffLL || ncell >= 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "mesh: nx*ny*nz must be < 2^31");
+    if (!finite_increasing(xe, nx + 1) || !finite_increasing(ye, ny + 1) || !finite_increasing(ze, nz + 1))
+        return c->fail(MR_ERR_INVALID_ARG, "mesh: plane positions must be finite and strictly increasing");
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    free_materials(c);
+    c->dev_free(c->d_edges);
+    c->dev_free(c->d_tally);
+    c->d_edges = nullptr;
+    c->d_tally = nullptr;
+    const int ne = nx + ny + nz + 3;
+    std::vector<double> h(ne);
+    std::memcpy(h.data(), xe, sizeof(double) * (nx + 1));
+    std::memcpy(h.data() + nx + 1, ye, sizeof(double) * (ny + 1));
+    std::memcpy(h.data() + nx + ny + 2, ze, sizeof(double) * (nz + 1));
+    c->d_edges = (double *)c->dev_alloc(sizeof(double) * ne);
+    c->d_tally = (double *)c->dev_alloc(sizeof(double) * ncell);
+    if (!c->d_edges || !c->d_tally) {
+        c->dev_free(c->d_edges);
+        c->dev_free(c->d_tally);
+        c->d_edges = nullptr;
+        c->d_tally = nullptr;
+        return c->fail(MR_ERR_OOM, "device allocation failed (mesh / tally)");
+    }
+    c->nx = nx; c->ny = ny; c->nz = nz; c->nedges = ne; c->ncell = ncell;
+    MR_CUDA(c, cudaMemcpyAsync(c->d_edges, h.data(), sizeof(double) * ne, cudaMemcpyHostToDevice, c->stream));
+    MR_CUDA(c, cudaMemsetAsync(c->d_tally, 0, sizeof(double) * ncell, c->stream));
+    MR_CUDA(c, cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    return MR_OK;
+}
+
+int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int32_t *cell_mat, const double *cell_frac)
+{
+    MR_ENTER(c);
+    if (!c->d_tally) return c->fail(MR_ERR_STATE, "load the mesh before the materials");
+    if (M < 1 || K < 1 || !density || !cell_mat || !cell_frac) return c->fail(MR_ERR_INVALID_ARG, "materials: bad size or NULL array");
+    if (M > MR_MAX_MATERIALS) return c->fail(MR_ERR_UNSUPPORTED, "materials: M > MR_MAX_MATERIALS");
+    if (K > MR_MAX_SLOTS) return c->fail(MR_ERR_UNSUPPORTED, "materials: K > MR_MAX_SLOTS");
+    for (int m = 0; m < M; ++m)
+        if (!std::isfinite(density[m]) || density[m] < 0.0) return c->fail(MR_ERR_INVALID_ARG, "materials: densities must be finite and >= 0");
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (M != c->M) free_tables(c);
+    free_materials(c);
+
+    const bool dbl = c->precision == MR_PRECISION_DOUBLE;
+    int layout = LAYOUT_GENERIC;
+    if (!dbl) {
+        if (K <= 4) layout = K;  // LAYOUT_K1..K4
+        if (K == 8 && M == 8) {  // dense: every cell lists materials 0..7 in order (ids implicit)
+            bool dense = true;
+            for (long long i = 0; i < c->ncell * 8 && dense; ++i) dense = cell_mat[i] == (int32_t)(i & 7);
+            if (dense) layout = LAYOUT_D8;
+        }
+    }
+    size_t rec_bytes = 0, id_bytes = 0;
+    switch (layout) {
+    case LAYOUT_K1: rec_bytes = 8; break;
+    case LAYOUT_K2: case LAYOUT_K3: rec_bytes = 16; break;
+    case LAYOUT_K4: case LAYOUT_D8: rec_bytes = 32; break;
+    default: rec_bytes = (size_t)K * (dbl ? 8 : 4); id_bytes = (size_t)K;
+    }
+    const long long chunk = std::min<long long>(c->ncell, 1LL << 22);
+    void *recs = c->dev_alloc(rec_bytes * c->ncell);
+    uint8_t *ids = id_bytes ? (uint8_t *)c->dev_alloc(id_bytes * c->ncell) : nullptr;
+    int32_t *s_mat = (int32_t *)c->dev_alloc(sizeof(int32_t) * chunk * K);
+    double *s_frac = (double *)c->dev_alloc(sizeof(double) * chunk * K);
+    double *s_den = (double *)c->dev_alloc(sizeof(double) * M);
+    int *s_flags = (int *)c->dev_alloc(sizeof(int));
+    auto cleanup = [&](bool all) {
+        c->dev_free(s_mat); c->dev_free(s_frac); c->dev_free(s_den); c->dev_free(s_flags);
+        if (all) { c->dev_free(recs); c->dev_free(ids); }
+    };
+    if (!recs || (id_bytes && !ids) || !s_mat || !s_frac || !s_den || !s_flags) {
+        cleanup(true);
+        return c->fail(MR_ERR_OOM, "device allocation failed (cell records)");
+    }
+    cudaError_t e = cudaMemcpyAsync(s_den, density, sizeof(double) * M, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s_flags, 0, sizeof(int), c->stream);
+    for (long long first = 0; first < c->ncell && e == cudaSuccess; first += chunk) {
+        const long long count = std::min(chunk, c->ncell - first);
+        e = cudaMemcpyAsync(s_mat, cell_mat + first * K, sizeof(int32_t) * count * K, cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(s_frac, cell_frac + first * K, sizeof(double) * count * K, cudaMemcpyHostToDevice, c->stream);
+        if (e != cudaSuccess) break;
+        PackParams P{s_mat, s_frac, s_den, first, count, K, M, layout, dbl ? 1 : 0, recs, ids, s_flags};
+        pack_cells_kernel<<<(unsigned)((count + 255) / 256), 256, 0, c->stream>>>(P);
+        c->launches += 1;
+        e = cudaGetLastError();
+        // the pageable source is consumed when the copy call returns; the scratch is reused in stream order
+    }
+    int flags = 0;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&flags, s_flags, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) {
+        cleanup(true);
+        return c->fail_cuda(e, "mr_load_materials");
+    }
+    if (flags) {
+        cleanup(true);
+        return c->fail(MR_ERR_INVALID_ARG, (flags & 1) ? "materials: cell_mat entry outside [-1, M)" : "materials: cell_frac must be finite and >= 0");
+    }
+    cleanup(false);
+    c->d_recs = recs;
+    c->d_ids = ids;
+    c->layout = layout;
+    c->K = K;
+    if (M != c->M || (int)c->xs_n.size() != M) {
+        c->M = M;
+        c->d_E.assign(M, nullptr);
+        c->d_S.assign(M, nullptr);
+        c->xs_n.assign(M, 0);
+        c->xs_dirty = true;
+    }
+    return MR_OK;
+}
+
+int mr_load_xs(mr_ctx *c, int material, int64_t n, const double *energy, const double *sigma_t)
+{
+    MR_ENTER(c);
+    if (!c->d_recs) return c->fail(MR_ERR_STATE, "load the materials before the tables");
+    if (material < 0 || material >= c->M || n < 1 || n > 0x7fffffff || !energy || !sigma_t)
+        return c->fail(MR_ERR_INVALID_ARG, "xs: bad material index, size or NULL array");
+    const bool dbl = c->precision == MR_PRECISION_DOUBLE;
+    std::vector<float> ef, sf;
+    if (!dbl) { ef.resize(n); sf.resize(n); }
+    for (int64_t i = 0; i < n; ++i) {
+        if (!std::isfinite(energy[i]) || !(energy[i] > 0.0) || !std::isfinite(sigma_t[i]) || sigma_t[i] < 0.0)
+            return c->fail(MR_ERR_INVALID_ARG, "xs: energies must be finite and > 0, cross sections finite and >= 0");
+        if (!dbl) {
+            ef[i] = (float)energy[i];
+            sf[i] = (float)sigma_t[i];
+            if (!std::isfinite(ef[i]) || !std::isfinite(sf[i]) || !(ef[i] > 0.f))
+                return c->fail(MR_ERR_INVALID_ARG, "xs: value not representable in fp32");
+            if (i && !(ef[i] > ef[i - 1])) return c->fail(MR_ERR_INVALID_ARG, "xs: energy grid not strictly increasing (after fp32 rounding)");
+        } else if (i && !(energy[i] > energy[i - 1]))
+            return c->fail(MR_ERR_INVALID_ARG, "xs: energy grid not strictly increasing");
+    }
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    const size_t bytes = (size_t)n * c->real_bytes();
+    void *dE = c->dev_alloc(bytes), *dS = c->dev_alloc(bytes);
+    if (!dE || !dS) {
+        c->dev_free(dE);
+        c->dev_free(dS);
+        return c->fail(MR_ERR_OOM, "device allocation failed (cross-section table)");
+    }
+    const void *hE = dbl ? (const void *)energy : (const void *)ef.data();
+    const void *hS = dbl ? (const void *)sigma_t : (const void *)sf.data();
+    cudaError_t e = cudaMemcpyAsync(dE, hE, bytes, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dS, hS, bytes, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) {
+        c->dev_free(dE);
+        c->dev_free(dS);
+        return c->fail_cuda(e, "mr_load_xs");
+    }
+    c->dev_free(c->d_E[material]);
+    c->dev_free(c->d_S[material]);
+    c->d_E[material] = dE;
+    c->d_S[material] = dS;
+    c->xs_n[material] = (int)n;
+    c->xs_dirty = true;
+    return MR_OK;
+}
+
+int mr_cast_rays(mr_ctx *c, int64_t n, const void *rays, int where)
+{
+    MR_ENTER(c);
+    if (n < 0 || (n > 0 && !rays) || (where != MR_WHERE_HOST && where != MR_WHERE_DEVICE))
+        return c->fail(MR_ERR_INVALID_ARG, "cast: bad count, NULL buffer or unknown location");
+    if (int rc = ready_to_cast(c)) return rc;
+    if (n == 0) return MR_OK;
+    if (int rc = upload_xs_desc(c)) return rc;
+    if (where == MR_WHERE_DEVICE) {
+        if ((uintptr_t)rays & 15) return c->fail(MR_ERR_INVALID_ARG, "cast: device ray buffer must be 16-byte aligned");
+        MR_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
+        if (int rc = cast_device(c, n, rays)) return rc;
+        MR_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
+        c->have_timing = true;
+        return MR_OK;
+    }
+    // Host batch: chunks go through a 2-slot pinned ring; the H2D copy of chunk i+1 (copy stream)
+    // overlaps the kernel of chunk i (context stream), and the host memcpy overlaps both.
+    const size_t per = (size_t)std::max<long long>(1024, std::min<long long>(c->stage_rays, n));
+    if (int rc = ensure_stage(c, per)) return rc;
+    const size_t rb = c->ray_bytes();
+    MR_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
+    const int64_t chunk = (int64_t)std::min<size_t>(c->stage_cap_rays, per);
+    for (int64_t first = 0; first < n; first += chunk) {
+        const int64_t count = std::min<int64_t>(chunk, n - first);
+        const int s = c->next_slot;
+        c->next_slot = (s + 1) % kStageSlots;
+        MR_CUDA(c, cudaEventSynchronize(c->ev_copied[s]));           // pinned slot free again
+        std::memcpy(c->pinned[s], (const char *)rays + (size_t)first * rb, (size_t)count * rb);
+        MR_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_done[s], 0));  // device slot free again
+        MR_CUDA(c, cudaMemcpyAsync(c->d_stage[s], c->pinned[s], (size_t)count * rb, cudaMemcpyHostToDevice, c->copy_stream));
+        MR_CUDA(c, cudaEventRecord(c->ev_copied[s], c->copy_stream));
+        MR_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied[s], 0));
+        if (int rc = cast_device(c, count, c->d_stage[s])) return rc;
+        MR_CUDA(c, cudaEventRecord(c->ev_done[s], c->stream));
+    }
+    MR_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
+    c->have_timing = true;
+    return MR_OK;
+}
+
+int mr_read_tally(mr_ctx *c, double *out)
+{
+    MR_ENTER(c);
+    if (!out) return c->fail(MR_ERR_INVALID_ARG, "read_tally: out is NULL");
+    if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    MR_CUDA(c, cudaMemcpyAsync(out, c->d_tally, sizeof(double) * c->ncell, cudaMemcpyDeviceToHost, c->stream));
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    return MR_OK;
+}
+
+int mr_clear_tally(mr_ctx *c)
+{
+    MR_ENTER(c);
+    if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    MR_CUDA(c, cudaMemsetAsync(c->d_tally, 0, sizeof(double) * c->ncell, c->stream));
+    MR_CUDA(c, cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+    return MR_OK;
+}
+
+int mr_sync(mr_ctx *c)
+{
+    MR_ENTER(c);
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    return MR_OK;
+}
+
+int mr_get_stats(mr_ctx *c, mr_stats *out)
+{
+    MR_ENTER(c);
+    if (!out) return c->fail(MR_ERR_INVALID_ARG, "get_stats: out is NULL");
+    unsigned long long h[4] = {0, 0, 0, 0};
+    MR_CUDA(c, cudaMemcpyAsync(h, c->d_counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    std::memset(out, 0, sizeof(*out));
+    out->rays_accepted = (int64_t)h[0];
+    out->rays_rejected = (int64_t)h[1];
+    out->segments = (int64_t)h[2];
+    out->kernel_launches = c->launches;
+    if (c->have_timing) {
+        float ms = 0.f;
+        MR_CUDA(c, cudaEventElapsedTime(&ms, c->ev_t0, c->ev_t1));
+        out->last_cast_ms = ms;
+    }
+    return MR_OK;
+}
+
+int mr_tally_device_ptr(mr_ctx *c, double **out)
+{
+    MR_ENTER(c);
+    if (!out) return c->fail(MR_ERR_INVALID_ARG, "tally_device_ptr: out is NULL");
+    if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    *out = c->d_tally;
+    return MR_OK;
+}
+
+int mr_trace_rays(mr_ctx *c, int64_t n, const void *rays, int where, uint32_t *nseg, uint64_t *hash, int32_t *cells,
+                  double *lens, int64_t cap)
+{
+    MR_ENTER(c);
+    if (n < 0 || (n > 0 && !rays) || cap < 0 || (where != MR_WHERE_HOST && where != MR_WHERE_DEVICE))
+        return c->fail(MR_ERR_INVALID_ARG, "trace: bad count, NULL buffer or unknown location");
+    if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    if (n == 0) return MR_OK;
+    if (!cells && !lens) cap = 0;
+    const size_t rb = c->ray_bytes();
+    void *d_rays = nullptr;
+    uint32_t *d_nseg = nullptr;
+    unsigned long long *d_hash = nullptr;
+    int32_t *d_cells = nullptr;
+    double *d_lens = nullptr;
+    auto cleanup = [&]() {
+        if (where == MR_WHERE_HOST) c->dev_free(d_rays);
+        c->dev_free(d_nseg); c->dev_free(d_hash); c->dev_free(d_cells); c->dev_free(d_lens);
+    };
+    bool ok = true;
+    if (where == MR_WHERE_HOST) ok = ok && (d_rays = c->dev_alloc((size_t)n * rb));
+    if (nseg) ok = ok && (d_nseg = (uint32_t *)c->dev_alloc((size_t)n * 4));
+    if (hash) ok = ok && (d_hash = (unsigned long long *)c->dev_alloc((size_t)n * 8));
+    if (cells && cap) ok = ok && (d_cells = (int32_t *)c->dev_alloc((size_t)n * cap * 4));
+    if (lens && cap) ok = ok && (d_lens = (double *)c->dev_alloc((size_t)n * cap * 8));
+    if (!ok) {
+        cleanup();
+        return c->fail(MR_ERR_OOM, "device allocation failed (trace buffers)");
+    }
+    cudaError_t e = cudaSuccess;
+    if (where == MR_WHERE_HOST) e = cudaMemcpyAsync(d_rays, rays, (size_t)n * rb, cudaMemcpyHostToDevice, c->stream);
+    else {
+        if ((uintptr_t)rays & 15) { cleanup(); return c->fail(MR_ERR_INVALID_ARG, "trace: device ray buffer must be 16-byte aligned"); }
+        d_rays = const_cast<void *>(rays);
+    }
+    // cells/lens beyond nseg stay as the caller left them: seed the device copies from the host arrays
+    if (e == cudaSuccess && d_cells) e = cudaMemcpyAsync(d_cells, cells, (size_t)n * cap * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess && d_lens) e = cudaMemcpyAsync(d_lens, lens, (size_t)n * cap * 8, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) {
+        TraceParams P{MeshDev{c->nx, c->ny, c->nz, c->nedges, c->d_edges}, d_rays, n, d_nseg, d_hash, d_cells, d_lens, cap,
+                      c->precision == MR_PRECISION_DOUBLE ? 1 : 0};
+        const int block = 256;
+        const unsigned grid = (unsigned)((n + block - 1) / block);
+        if (edges_smem_bytes(c) <= kEdgesSmemMax) {
+            const size_t smem = edges_smem_bytes(c);
+            if (smem > 48 * 1024) e = cudaFuncSetAttribute(trace_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e == cudaSuccess) trace_kernel<true><<<grid, block, smem, c->stream>>>(P);
+        } else
+            trace_kernel<false><<<grid, block, 0, c->stream>>>(P);
+        c->launches += 1;
+        if (e == cudaSuccess) e = cudaGetLastError();
+    }
+    if (e == cudaSuccess && d_nseg) e = cudaMemcpyAsync(nseg, d_nseg, (size_t)n * 4, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess && d_hash) e = cudaMemcpyAsync(hash, d_hash, (size_t)n * 8, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess && d_cells) e = cudaMemcpyAsync(cells, d_cells, (size_t)n * cap * 4, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess && d_lens) e = cudaMemcpyAsync(lens, d_lens, (size_t)n * cap * 8, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cleanup();
+    if (e != cudaSuccess) return c->fail_cuda(e, "mr_trace_rays");
+    return MR_OK;
+}
+
+int mr_set_option(mr_ctx *c, int option, int64_t value)
+{
+    MR_ENTER(c);
+    switch (option) {
+    case MR_OPT_BLOCK_THREADS:
+        if (value < 32 || value > 1024 || (value & 31)) return c->fail(MR_ERR_INVALID_ARG, "block threads must be a multiple of 32 in [32, 1024]");
+        c->block_threads = (int)value;
+        return MR_OK;
+    case MR_OPT_SORT_RAYS:
+        if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "sort option is 0 or 1");
+        c->sort_rays = (int)value;
+        return MR_OK;
+    case MR_OPT_STAGE_RAYS:
+        if (value < 1024 || value > (1LL << 26)) return c->fail(MR_ERR_INVALID_ARG, "staging chunk must be in [1024, 2^26] rays");
+        c->stage_rays = value;
+        return MR_OK;
+    }
+    return c->fail(MR_ERR_INVALID_ARG, "unknown option");
+}
+
+int mr_get_option(mr_ctx *c, int option, int64_t *value)
+{
+    MR_ENTER(c);
+    if (!value) return c->fail(MR_ERR_INVALID_ARG, "value is NULL");
+    switch (option) {
+    case MR_OPT_BLOCK_THREADS: *value = c->block_threads; return MR_OK;
+    case MR_OPT_SORT_RAYS: *value = c->sort_rays; return MR_OK;
+    case MR_OPT_STAGE_RAYS: *value = c->stage_rays; return MR_OK;
+    }
+    return c->fail(MR_ERR_INVALID_ARG, "unknown option");
+}
+
+}  // extern "C"

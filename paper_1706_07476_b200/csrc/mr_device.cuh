@@ -1,0 +1,521 @@
+// mr_device.cuh -- device code of the VRC ray-cast hot path (sm_100a).
+//
+// Steps S1..S6 of DESIGN.md §1 ("first calculating all cross-sections, then ray
+// casting the particle, and finally calculating the VRC estimator", Eq. (4)).
+// Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mr {
+
+// ------------------------------------------------------------------------------------------------
+// Kernel parameter blocks (plain data, passed by value)
+// ------------------------------------------------------------------------------------------------
+struct XsDesc {            // one material's table (device pointers)
+    const void *E;         // float[n] (mixed) or double[n]
+    const void *S;
+    int n;
+    int pad;
+};
+
+enum CellLayout : int {
+    LAYOUT_K1 = 1,         // 8 B  {float r; u32 id}
+    LAYOUT_K2 = 2,         // 16 B {float r0,r1; u32 ids; u32 pad}
+    LAYOUT_K3 = 3,         // 16 B {float r0,r1,r2; u32 ids}
+    LAYOUT_K4 = 4,         // 32 B {float r0..r3; u32 ids; u32 pad[3]}
+    LAYOUT_D8 = 8,         // 32 B {float r[8]}  dense: slot k holds material k
+    LAYOUT_GENERIC = 100   // coef[ncell*K] (float or double) + ids[ncell*K] (u8, 0xff = empty)
+};
+
+struct MeshDev {
+    int nx, ny, nz;
+    int nedges;            // nx+1 + ny+1 + nz+1
+    const double *edges;   // x planes | y planes | z planes, concatenated
+};
+
+struct CastParams {
+    MeshDev mesh;
+    const void *recs;      // packed records (LAYOUT_K*, LAYOUT_D8) or coefficient array (generic)
+    const uint8_t *ids;    // generic layout only
+    int K, M;
+    const XsDesc *xs;      // [M]
+    const void *rays;      // 8 floats (mixed) or 8 doubles per ray
+    const uint32_t *perm;  // optional processing order (ray index per work item), may be null
+    long long n;
+    double *tally;
+    unsigned long long *counters;  // [0] accepted [1] rejected [2] segments
+};
+
+struct TraceParams {
+    MeshDev mesh;
+    const void *rays;
+    long long n;
+    uint32_t *nseg;        // may be null
+    unsigned long long *hash;  // may be null
+    int32_t *cells;        // may be null, [n*cap]
+    double *lens;          // may be null, [n*cap]
+    long long cap;
+    int ray_is_double;
+};
+
+// ------------------------------------------------------------------------------------------------
+// Small helpers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float4 ldg_f4(const void *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
+__device__ __forceinline__ uint4 ldg_u4(const void *p) { return __ldg(reinterpret_cast<const uint4 *>(p)); }
+__device__ __forceinline__ uint2 ldg_u2(const void *p) { return __ldg(reinterpret_cast<const uint2 *>(p)); }
+__device__ __forceinline__ double2 ldg_d2(const void *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
+
+// fp64 reduction into global memory without a return value (RED.E.ADD.F64 in SASS)
+__device__ __forceinline__ void red_add_f64(double *addr, double v)
+{
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(addr), "d"(v) : "memory");
+}
+
+// Ray record {x,y,z,u,v,w,E,W} -> doubles (exact promotion in mixed mode).  Returns the O1
+// validation verdict except for the box test (done by the walker once the mesh is known).
+template <typename Real>
+struct Ray {
+    double o[3], d[3];
+    Real E;
+    double W;
+    bool finite;
+};
+
+__device__ __forceinline__ Ray<float> load_ray_f32(const void *rays, long long r)
+{
+    const float4 *p = reinterpret_cast<const float4 *>(rays) + 2 * r;
+    float4 a = __ldg(p), b = __ldg(p + 1);
+    Ray<float> R;
+    R.o[0] = a.x; R.o[1] = a.y; R.o[2] = a.z;
+    R.d[0] = a.w; R.d[1] = b.x; R.d[2] = b.y;
+    R.E = b.z; R.W = b.w;
+    R.finite = isfinite(a.x) && isfinite(a.y) && isfinite(a.z) && isfinite(a.w) && isfinite(b.x) &&
+               isfinite(b.y) && isfinite(b.z) && isfinite(b.w);
+    return R;
+}
+
+__device__ __forceinline__ Ray<double> load_ray_f64(const void *rays, long long r)
+{
+    const double2 *p = reinterpret_cast<const double2 *>(rays) + 4 * r;
+    double2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2), e = __ldg(p + 3);
+    Ray<double> R;
+    R.o[0] = a.x; R.o[1] = a.y; R.o[2] = b.x;
+    R.d[0] = b.y; R.d[1] = c.x; R.d[2] = c.y;
+    R.E = e.x; R.W = e.y;
+    R.finite = isfinite(a.x) && isfinite(a.y) && isfinite(b.x) && isfinite(b.y) && isfinite(c.x) &&
+               isfinite(c.y) && isfinite(e.x) && isfinite(e.y);
+    return R;
+}
+
+template <typename Real> __device__ __forceinline__ Ray<Real> load_ray(const void *rays, long long r);
+template <> __device__ __forceinline__ Ray<float> load_ray<float>(const void *rays, long long r) { return load_ray_f32(rays, r); }
+template <> __device__ __forceinline__ Ray<double> load_ray<double>(const void *rays, long long r) { return load_ray_f64(rays, r); }
+
+// ------------------------------------------------------------------------------------------------
+// S1: sigma_m(E), lin-lin interpolation in a table, end values outside (Q5)
+// ------------------------------------------------------------------------------------------------
+template <typename Real>
+__device__ __forceinline__ Real sigma_lookup(const XsDesc &t, Real E)
+{
+    const Real *__restrict__ Eg = reinterpret_cast<const Real *>(t.E);
+    const Real *__restrict__ Sg = reinterpret_cast<const Real *>(t.S);
+    const int n = t.n;
+    if (n == 1 || E < __ldg(Eg)) return __ldg(Sg);
+    if (E >= __ldg(Eg + n - 1)) return __ldg(Sg + n - 1);
+    int lo = 1, hi = n - 1;  // invariant: Eg[lo-1] <= E < Eg[hi]
+    while (lo < hi) {
+        int mid = (lo + hi) >> 1;
+        if (__ldg(Eg + mid) <= E) lo = mid + 1; else hi = mid;
+    }
+    const int k = lo - 1;    // Eg[k] <= E < Eg[k+1], 0 <= k <= n-2
+    const Real e0 = __ldg(Eg + k), e1 = __ldg(Eg + k + 1);
+    const Real s0 = __ldg(Sg + k), s1 = __ldg(Sg + k + 1);
+    const Real t01 = (E - e0) / (e1 - e0);
+    return s0 + t01 * (s1 - s0);
+}
+
+// ------------------------------------------------------------------------------------------------
+// S2 + S3: the walker.  Crossing parameter of plane p on axis a is the pure function
+//   t_a(p) = (edges_a[p] - o_a) * inv_a          (one subtract, then one multiply, both RN)
+// and the trace is the 3-way merge of the three non-decreasing sequences, ties x < y < z
+// (O3-O5).  __dsub_rn/__dmul_rn keep the compiler from contracting anything.
+// Plane indices are absolute positions in the concatenated edge array.
+// ------------------------------------------------------------------------------------------------
+struct Walker {
+    double t0, t1, t2;     // pending crossing parameter per axis (+inf: the axis never steps)
+    double o0, o1, o2;
+    double iv0, iv1, iv2;
+    int p0, p1, p2;        // next plane (absolute index)
+    int lim0, lim1, lim2;  // crossing this plane leaves the mesh
+    int s0, s1, s2;        // +1 / -1 / 0
+    int dc1, dc2;          // cell-index increment of a y / z step (x: s0)
+    int c;                 // current cell
+    double tcur;
+};
+
+// number of entries of e[0..n) that are <= v
+__device__ __forceinline__ int upper_bound_edges(const double *e, int n, double v)
+{
+    int lo = 0, hi = n;
+    while (lo < hi) {
+        int mid = (lo + hi) >> 1;
+        if (e[mid] <= v) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+// Returns false if the ray is rejected by the box / direction rules of O1.
+__device__ __forceinline__ bool walker_init(Walker &w, const MeshDev &m, const double *e, const double o[3], const double d[3])
+{
+    const int bx = 0, by = m.nx + 1, bz = m.nx + m.ny + 2;
+    if (!(o[0] >= e[bx] && o[0] < e[bx + m.nx])) return false;
+    if (!(o[1] >= e[by] && o[1] < e[by + m.ny])) return false;
+    if (!(o[2] >= e[bz] && o[2] < e[bz + m.nz])) return false;
+    const int ix = upper_bound_edges(e + bx, m.nx + 1, o[0]) - 1;
+    const int iy = upper_bound_edges(e + by, m.ny + 1, o[1]) - 1;
+    const int iz = upper_bound_edges(e + bz, m.nz + 1, o[2]) - 1;
+    w.c = ix + m.nx * (iy + m.ny * iz);
+    w.o0 = o[0]; w.o1 = o[1]; w.o2 = o[2];
+    w.tcur = 0.0;
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    bool movable = false;
+#define MR_AXIS(A, IDX, BASE, N, DC)                                                            \
+    {                                                                                           \
+        const double dd = d[A];                                                                 \
+        const double inv = (dd != 0.0) ? __drcp_rn(dd) : 0.0;                                   \
+        if (dd == 0.0 || !isfinite(inv)) {                                                      \
+            w.s##A = 0; w.p##A = BASE; w.lim##A = -1; w.iv##A = 0.0; w.t##A = inf;              \
+        } else {                                                                                \
+            movable = true;                                                                     \
+            w.iv##A = inv;                                                                      \
+            w.s##A = dd > 0.0 ? 1 : -1;                                                         \
+            w.p##A = BASE + (dd > 0.0 ? IDX + 1 : IDX);                                         \
+            w.lim##A = BASE + (dd > 0.0 ? N : 0);                                               \
+            w.t##A = __dmul_rn(__dsub_rn(e[w.p##A], o[A]), inv);                                \
+        }                                                                                       \
+    }
+    MR_AXIS(0, ix, bx, m.nx, 1)
+    MR_AXIS(1, iy, by, m.ny, m.nx)
+    MR_AXIS(2, iz, bz, m.nz, m.nx * m.ny)
+#undef MR_AXIS
+    w.dc1 = w.s1 * m.nx;
+    w.dc2 = w.s2 * m.nx * m.ny;
+    return movable;
+}
+
+// One step of the merge.  On return: `cell` = the cell just traversed, `len` its segment length;
+// the return value is true when the ray has left the mesh.
+__device__ __forceinline__ bool walker_step(Walker &w, const double *e, int &cell, double &len)
+{
+    const bool ysel = w.t1 < w.t0;                 // ties keep x
+    const double tm = ysel ? w.t1 : w.t0;
+    const bool zsel = w.t2 < tm;                   // ties keep x / y
+    const double tn = zsel ? w.t2 : tm;
+    len = __dsub_rn(tn, w.tcur);
+    w.tcur = tn;
+    cell = w.c;
+    bool leave;
+    if (zsel) {
+        leave = (w.p2 == w.lim2);
+        w.c += w.dc2;
+        w.p2 += w.s2;
+        if (!leave) w.t2 = __dmul_rn(__dsub_rn(e[w.p2], w.o2), w.iv2);
+    } else if (ysel) {
+        leave = (w.p1 == w.lim1);
+        w.c += w.dc1;
+        w.p1 += w.s1;
+        if (!leave) w.t1 = __dmul_rn(__dsub_rn(e[w.p1], w.o1), w.iv1);
+    } else {
+        leave = (w.p0 == w.lim0);
+        w.c += w.s0;
+        w.p0 += w.s0;
+        if (!leave) w.t0 = __dmul_rn(__dsub_rn(e[w.p0], w.o0), w.iv0);
+    }
+    return leave;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S4: total cross section of a cell from its record and the ray's per-material sigma values.
+// sig[m * stride] is sigma of material m for this thread (shared memory, conflict-free).
+// ------------------------------------------------------------------------------------------------
+template <int LAYOUT> struct CellRec;
+
+template <> struct CellRec<LAYOUT_K1> {
+    uint2 v;
+    __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c) { v = ldg_u2(reinterpret_cast<const uint2 *>(recs) + c); }
+    __device__ __forceinline__ float sigma(const float *sig, int stride, int) const { return __uint_as_float(v.x) * sig[v.y * stride]; }
+};
+template <> struct CellRec<LAYOUT_K2> {
+    uint4 v;
+    __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c) { v = ldg_u4(reinterpret_cast<const uint4 *>(recs) + c); }
+    __device__ __forceinline__ float sigma(const float *sig, int stride, int) const
+    {
+        float s = __uint_as_float(v.x) * sig[(v.z & 0xffu) * stride];
+        return fmaf(__uint_as_float(v.y), sig[((v.z >> 8) & 0xffu) * stride], s);
+    }
+};
+template <> struct CellRec<LAYOUT_K3> {
+    uint4 v;
+    __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c) { v = ldg_u4(reinterpret_cast<const uint4 *>(recs) + c); }
+    __device__ __forceinline__ float sigma(const float *sig, int stride, int) const
+    {
+        float s = __uint_as_float(v.x) * sig[(v.w & 0xffu) * stride];
+        s = fmaf(__uint_as_float(v.y), sig[((v.w >> 8) & 0xffu) * stride], s);
+        return fmaf(__uint_as_float(v.z), sig[((v.w >> 16) & 0xffu) * stride], s);
+    }
+};
+template <> struct CellRec<LAYOUT_K4> {
+    uint4 v;
+    uint32_t ids;
+    __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c)
+    {
+        const uint4 *p = reinterpret_cast<const uint4 *>(recs) + 2 * (size_t)c;
+        v = ldg_u4(p);
+        ids = __ldg(reinterpret_cast<const uint32_t *>(p + 1));
+    }
+    __device__ __forceinline__ float sigma(const float *sig, int stride, int) const
+    {
+        float s = __uint_as_float(v.x) * sig[(ids & 0xffu) * stride];
+        s = fmaf(__uint_as_float(v.y), sig[((ids >> 8) & 0xffu) * stride], s);
+        s = fmaf(__uint_as_float(v.z), sig[((ids >> 16) & 0xffu) * stride], s);
+        return fmaf(__uint_as_float(v.w), sig[(ids >> 24) * stride], s);
+    }
+};
+template <> struct CellRec<LAYOUT_D8> {
+    float4 a, b;
+    __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c)
+    {
+        const float4 *p = reinterpret_cast<const float4 *>(recs) + 2 * (size_t)c;
+        a = __ldg(p); b = __ldg(p + 1);
+    }
+    __device__ __forceinline__ float sigma(const float *sig, int stride, int) const
+    {
+        float s = a.x * sig[0];
+        s = fmaf(a.y, sig[stride], s);
+        s = fmaf(a.z, sig[2 * stride], s);
+        s = fmaf(a.w, sig[3 * stride], s);
+        s = fmaf(b.x, sig[4 * stride], s);
+        s = fmaf(b.y, sig[5 * stride], s);
+        s = fmaf(b.z, sig[6 * stride], s);
+        return fmaf(b.w, sig[7 * stride], s);
+    }
+};
+
+// Generic layout, either precision: nothing is prefetched, the slots are read in sigma().
+template <typename Real> struct CellRecGeneric {
+    const Real *coef;
+    const uint8_t *ids;
+    __device__ __forceinline__ void load(const void *recs, const uint8_t *idp, int K, int c)
+    {
+        coef = reinterpret_cast<const Real *>(recs) + (size_t)c * K;
+        ids = idp + (size_t)c * K;
+    }
+    __device__ __forceinline__ Real sigma(const Real *sig, int stride, int K) const
+    {
+        Real s = 0;
+        for (int k = 0; k < K; ++k) {
+            const unsigned id = __ldg(ids + k);
+            if (id != 0xffu) s += __ldg(coef + k) * sig[id * stride];
+        }
+        return s;
+    }
+};
+
+// ------------------------------------------------------------------------------------------------
+// The cast kernel: one thread per ray (S1 -> S6).
+//   dynamic shared memory: [edges: nedges doubles (if EDGES_SMEM)] [sigma: M x blockDim Real]
+// ------------------------------------------------------------------------------------------------
+template <typename Real, typename Rec, bool EDGES_SMEM>
+__global__ void cast_kernel(const __grid_constant__ CastParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *s_edges = reinterpret_cast<double *>(smem_raw);
+    Real *s_sig = reinterpret_cast<Real *>(smem_raw + (EDGES_SMEM ? sizeof(double) * ((P.mesh.nedges + 1) & ~1) : 0));
+    const double *e = EDGES_SMEM ? s_edges : P.mesh.edges;
+    if (EDGES_SMEM) {
+        for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
+        __syncthreads();
+    }
+    const int stride = blockDim.x;
+    Real *sig = s_sig + threadIdx.x;
+
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned nseg = 0;
+    bool accepted = false, live = i < P.n;
+    if (live) {
+        const long long r = P.perm ? (long long)__ldg(P.perm + i) : i;
+        const Ray<Real> R = load_ray<Real>(P.rays, r);
+        Walker w;
+        accepted = R.finite && (R.E > (Real)0) && walker_init(w, P.mesh, e, R.o, R.d);
+        if (accepted) {
+            // S1: every material's sigma at the ray's energy, kept in this thread's shared column
+            for (int m = 0; m < P.M; ++m) sig[m * stride] = sigma_lookup<Real>(P.xs[m], R.E);
+
+            double wa = R.W;   // W * exp(-tau) as a running product
+            Rec rec;
+            rec.load(P.recs, P.ids, P.K, w.c);
+            for (;;) {
+                int cell;
+                double len;
+                const bool leave = walker_step(w, e, cell, len);
+                const Rec cur = rec;
+                if (!leave) rec.load(P.recs, P.ids, P.K, w.c);   // next cell's record: in flight during the score
+                // S4 + S5 (Eq. (4)): x = Sigma*l; score = W e^{-tau} (x > 0 ? (1-e^{-x})/Sigma : l)
+                const double S = (double)cur.sigma(sig, stride, P.K);
+                const double x = S * len;
+                const double em1 = expm1(-x);
+                const double g = (x > 0.0) ? (-em1 / S) : len;
+                const double score = wa * g;
+                wa = fma(wa, em1, wa);
+                // S6
+                if (len > 0.0) red_add_f64(P.tally + cell, score);
+                ++nseg;
+                if (leave) break;
+            }
+        }
+    }
+    // per-warp totals -> three global counters
+    const unsigned full = 0xffffffffu;
+    const unsigned acc = __popc(__ballot_sync(full, accepted));
+    const unsigned rej = __popc(__ballot_sync(full, live && !accepted));
+    unsigned long long segs = nseg;
+    for (int o = 16; o > 0; o >>= 1) segs += __shfl_xor_sync(full, segs, o);
+    if ((threadIdx.x & 31) == 0) {
+        if (acc) atomicAdd(P.counters + 0, (unsigned long long)acc);
+        if (rej) atomicAdd(P.counters + 1, (unsigned long long)rej);
+        if (segs) atomicAdd(P.counters + 2, segs);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// The trace kernel (test entry point mr_trace_rays): same walker, no cross sections, no tally.
+// ------------------------------------------------------------------------------------------------
+template <bool EDGES_SMEM>
+__global__ void trace_kernel(const __grid_constant__ TraceParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *s_edges = reinterpret_cast<double *>(smem_raw);
+    const double *e = EDGES_SMEM ? s_edges : P.mesh.edges;
+    if (EDGES_SMEM) {
+        for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
+        __syncthreads();
+    }
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= P.n) return;
+    double o[3], d[3];
+    bool ok;
+    if (P.ray_is_double) {
+        const Ray<double> R = load_ray_f64(P.rays, r);
+        for (int a = 0; a < 3; ++a) { o[a] = R.o[a]; d[a] = R.d[a]; }
+        ok = R.finite && R.E > 0.0;
+    } else {
+        const Ray<float> R = load_ray_f32(P.rays, r);
+        for (int a = 0; a < 3; ++a) { o[a] = R.o[a]; d[a] = R.d[a]; }
+        ok = R.finite && R.E > 0.0f;
+    }
+    Walker w;
+    ok = ok && walker_init(w, P.mesh, e, o, d);
+    unsigned nseg = 0;
+    unsigned long long h = 0;
+    if (ok) {
+        h = 0xcbf29ce484222325ULL;
+        for (;;) {
+            int cell;
+            double len;
+            const bool leave = walker_step(w, e, cell, len);
+            if ((long long)nseg < P.cap) {
+                if (P.cells) P.cells[r * P.cap + nseg] = cell;
+                if (P.lens) P.lens[r * P.cap + nseg] = len;
+            }
+            const unsigned cu = (unsigned)cell;
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                h ^= (unsigned long long)((cu >> (8 * b)) & 0xffu);
+                h *= 0x100000001b3ULL;
+            }
+            ++nseg;
+            if (leave) break;
+        }
+    }
+    if (P.nseg) P.nseg[r] = nseg;
+    if (P.hash) P.hash[r] = h;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Set-up kernels (mr_load_materials): validate and pack a chunk of the per-cell composition.
+//   flags[0] |= 1 on an invalid material id, |= 2 on a non-finite or negative fraction.
+// ------------------------------------------------------------------------------------------------
+struct PackParams {
+    const int32_t *cell_mat;   // chunk, [count*K]
+    const double *cell_frac;   // chunk, [count*K]
+    const double *density;     // [M]
+    long long first, count;    // cells [first, first+count)
+    int K, M, layout, is_double;
+    void *recs;
+    uint8_t *ids;
+    int *flags;
+};
+
+__global__ void pack_cells_kernel(const PackParams P)
+{
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= P.count) return;
+    const long long c = P.first + j;
+    float rf[MR_PACK_MAX_SLOTS];
+    double rd[MR_PACK_MAX_SLOTS];
+    unsigned id[MR_PACK_MAX_SLOTS];
+    int bad = 0;
+    for (int k = 0; k < P.K; ++k) {
+        const int m = P.cell_mat[j * P.K + k];
+        const double f = P.cell_frac[j * P.K + k];
+        if (m < -1 || m >= P.M) { bad |= 1; rd[k] = 0.0; rf[k] = 0.f; id[k] = 0xffu; continue; }
+        if (m == -1) { rd[k] = 0.0; rf[k] = 0.f; id[k] = 0xffu; continue; }
+        if (!(f >= 0.0) || !isfinite(f)) bad |= 2;
+        rd[k] = f * P.density[m];        // r = frac * density, rounded once to fp32 in mixed mode
+        rf[k] = (float)rd[k];
+        id[k] = (unsigned)m;
+    }
+    if (bad) atomicOr(P.flags, bad);
+    // packed layouts encode an empty slot as r = 0, id = 0 (adds +0 in the same slot order)
+    auto pid = [&](int k) { return id[k] == 0xffu ? 0u : id[k]; };
+    switch (P.layout) {
+    case LAYOUT_K1:
+        reinterpret_cast<uint2 *>(P.recs)[c] = make_uint2(__float_as_uint(rf[0]), pid(0));
+        break;
+    case LAYOUT_K2:
+        reinterpret_cast<uint4 *>(P.recs)[c] = make_uint4(__float_as_uint(rf[0]), __float_as_uint(rf[1]), pid(0) | (pid(1) << 8), 0u);
+        break;
+    case LAYOUT_K3:
+        reinterpret_cast<uint4 *>(P.recs)[c] = make_uint4(__float_as_uint(rf[0]), __float_as_uint(rf[1]), __float_as_uint(rf[2]),
+                                                         pid(0) | (pid(1) << 8) | (pid(2) << 16));
+        break;
+    case LAYOUT_K4: {
+        uint4 *p = reinterpret_cast<uint4 *>(P.recs) + 2 * c;
+        p[0] = make_uint4(__float_as_uint(rf[0]), __float_as_uint(rf[1]), __float_as_uint(rf[2]), __float_as_uint(rf[3]));
+        p[1] = make_uint4(pid(0) | (pid(1) << 8) | (pid(2) << 16) | (pid(3) << 24), 0u, 0u, 0u);
+        break;
+    }
+    case LAYOUT_D8: {
+        float4 *p = reinterpret_cast<float4 *>(P.recs) + 2 * c;
+        p[0] = make_float4(rf[0], rf[1], rf[2], rf[3]);
+        p[1] = make_float4(rf[4], rf[5], rf[6], rf[7]);
+        break;
+    }
+    default:
+        for (int k = 0; k < P.K; ++k) {
+            if (P.is_double) reinterpret_cast<double *>(P.recs)[c * P.K + k] = rd[k];
+            else reinterpret_cast<float *>(P.recs)[c * P.K + k] = rf[k];
+            P.ids[c * P.K + k] = (uint8_t)id[k];
+        }
+    }
+}
+
+__global__ void convert_f64_to_f32_kernel(const double *in, float *out, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = (float)in[i];
+}
+
+}  // namespace mr

@@ -1,0 +1,251 @@
+"""GPU parity: the CUDA library (through its C ABI / thin binding) against the CPU oracle, element by
+element, on the same seeded inputs.
+
+Bars (BASELINE.json north_star):
+  * traces (segment count, FNV-1a hash of the cell sequence, and for small cases the full cell and
+    length lists) bit-exact;
+  * per-cell tallies |d| <= 1e-4*|oracle| + 1e-7*max(tally) in MIXED mode,
+    |d| <= 1e-10*|oracle| (+1e-290 against denormals) in DOUBLE mode;
+  * the kernel's segment / accepted / rejected counters equal the oracle's exactly.
+"""
+import numpy as np
+import pytest
+
+from tests.tiny import tiny_problem, tiny_rays
+from workloads import make_problem, make_rays
+
+pytestmark = pytest.mark.gpu
+
+
+def _mr(prob, precision, **kw):
+    from paper_1706_07476_b200 import MonteRay
+
+    m = MonteRay(0, precision, **kw)
+    m.load_problem(prob)
+    return m
+
+
+def _oracle(prob):
+    from oracle.vrc_oracle import Oracle
+
+    return Oracle(prob)
+
+
+def _threads():
+    import os
+
+    return max(1, min(32, len(os.sched_getaffinity(0))))
+
+
+def assert_tally(got, want, precision):
+    d = np.abs(got - want)
+    if precision == 0:
+        bound = 1e-4 * np.abs(want) + 1e-7 * np.abs(want).max()
+    else:
+        bound = 1e-10 * np.abs(want) + 1e-290
+    bad = np.flatnonzero(d > bound)
+    assert bad.size == 0, (f"{bad.size} cells out of tolerance; worst cell {bad[np.argmax((d - bound)[bad])]}: "
+                           f"got {got[bad[0]]!r} want {want[bad[0]]!r}")
+
+
+def check_case(prob, rays32, precision, cap=0, threads=None, full_trace=False):
+    """Casts + traces `rays32` on the GPU and on the oracle and compares everything."""
+    orc = _oracle(prob)
+    ref = orc.cast(rays32, per_ray=True, cap=cap, threads=threads or _threads())
+    with _mr(prob, precision) as m:
+        rays = rays32.astype(m.ray_dtype)
+        n = m.cast_rays(rays)
+        assert n == len(rays32)
+        got = m.read_tally()
+        st = m.get_stats()
+        nseg, hsh, cells, lens = m.trace_rays(rays, cap=cap)
+    assert np.array_equal(nseg, ref.nseg), "segment counts differ"
+    assert np.array_equal(hsh, ref.hash), "cell-sequence hashes differ"
+    if cap:
+        assert np.array_equal(cells, ref.cells), "cell traces differ"
+        assert np.array_equal(lens, ref.lens), "segment lengths differ (must be bitwise equal)"
+    assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+    assert_tally(got, ref.tally, precision)
+    return got, ref
+
+
+# ------------------------------------------------------------------------------------- config 1 (full)
+@pytest.mark.parametrize("precision", [0, 1])
+def test_config1_full_traces_and_tally(precision):
+    prob = make_problem(1)
+    rays = make_rays(prob, 10_000)
+    got, ref = check_case(prob, rays, precision, cap=32)
+    assert ref.nseg.max() <= 32
+    assert ref.segments == 71239  # tests/golden/config1_oracle.txt
+
+
+# ------------------------------------------------------------------------------------- tiny random problems
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("seed,K,M,uniform", [(101, 1, 2, False), (102, 2, 3, False), (103, 3, 4, True),
+                                              (104, 4, 5, False), (105, 5, 6, False), (106, 8, 8, False),
+                                              (107, 16, 9, True)])
+def test_tiny_random_problems(seed, K, M, uniform, precision):
+    """Every cell layout (K1..K4 packed, generic K=5/8/16), non-uniform planes, empty slots, void cells,
+    axis-aligned and -0.0 directions; 3000 rays = several CTAs and a ragged last warp."""
+    prob = tiny_problem(seed, nx=7, ny=5, nz=6, M=M, K=K, n_e=33, uniform=uniform)
+    rays = tiny_rays(prob, seed, 3001, axis_aligned_share=0.1)
+    check_case(prob, rays, precision, cap=24, threads=1)
+
+
+def test_dense8_layout():
+    """K = M = 8 with ids 0..7 in every cell selects the dense 32-byte record (config 5's layout)."""
+    prob = tiny_problem(110, nx=6, ny=6, nz=6, M=8, K=8, n_e=65)
+    prob.cell_mat[:] = np.arange(8, dtype=np.int32)[None, :]
+    prob.cell_frac[:] = np.random.default_rng(110).random(prob.cell_frac.shape).astype(np.float32)
+    rays = tiny_rays(prob, 110, 5000)
+    check_case(prob, rays, 0, cap=24, threads=1)
+    check_case(prob, rays, 1, threads=1)
+
+
+def test_lattice_points_corners_and_faces():
+    prob = tiny_problem(21, nx=4, ny=4, nz=4, uniform=True)
+    rays = []
+    for o in ([-1.0, -1.0, -1.0], [-0.25, -0.25, 0.5], [0.5, -0.25, -0.25], [-1.0, 0.5, 1.25]):
+        for d in ([1, 1, 1], [1, 1, 0], [-1, 1, 1], [1, -1, -1], [0, 0, 1], [-1, -1, -1], [2, 1, 1], [0.0, -0.0, -1]):
+            rays.append(o + d + [1.0, 1.0])
+    rays = np.array(rays, dtype=np.float32)
+    for precision in (0, 1):
+        check_case(prob, rays, precision, cap=16, threads=1)
+
+
+def test_rejection_rules_and_counters():
+    prob = tiny_problem(81, uniform=True)  # box [-1,2] x [-1,1.25] x [-1,2.75]
+    ok = [0.0, 0.0, 0.0, 0.6, 0.0, 0.8, 1.0, 1.0]
+    rows = [ok]
+    for f, v in ((0, np.nan), (4, np.inf), (6, 0.0), (6, -1.0), (7, np.nan), (0, 2.0), (1, -1.0000001), (2, 2.75), (7, -np.inf)):
+        b = list(ok)
+        b[f] = v
+        rows.append(b)
+    rows.append([0.0, 0.0, 0.0, 0.0, -0.0, 0.0, 1.0, 1.0])
+    rows.append([-1.0, -1.0, -1.0, 0.6, 0.0, 0.8, 1.0, -2.5])  # on the lower faces, negative weight: accepted
+    rays = np.array(rows * 40, dtype=np.float32)  # 480 rays: rejected lanes interleaved with live ones
+    for precision in (0, 1):
+        got, ref = check_case(prob, rays, precision, cap=12, threads=1)
+        assert ref.rays_rejected == 40 * 10 and ref.rays_accepted == 40 * 2
+
+
+# ------------------------------------------------------------------------------------- shaped workloads
+@pytest.mark.parametrize("cfg,n_rays,kw", [
+    (2, 200_000, {}),
+    (3, 200_000, {}),
+    (4, 100_000, {"n": 128, "n_e": 20_000}),
+    (5, 200_000, {}),
+])
+def test_shaped_workloads_mixed(cfg, n_rays, kw):
+    prob = make_problem(cfg, **kw)
+    rays = make_rays(prob, n_rays)
+    check_case(prob, rays, 0)
+
+
+@pytest.mark.parametrize("cfg,n_rays,kw", [
+    (2, 50_000, {"nx": 100, "ny": 100, "nz": 50}),
+    (3, 50_000, {"nx": 85, "ny": 85, "nz": 60}),
+    (4, 30_000, {"n": 64, "n_e": 5_000}),
+    (5, 50_000, {"n_e": 50_000, "n_res": 500}),
+])
+def test_shaped_workloads_double(cfg, n_rays, kw):
+    prob = make_problem(cfg, **kw)
+    rays = make_rays(prob, n_rays)
+    check_case(prob, rays, 1)
+
+
+# ------------------------------------------------------------------------------------- API behaviour
+def test_host_device_and_chunked_staging_agree():
+    import torch
+
+    from paper_1706_07476_b200 import MR_OPT_STAGE_RAYS
+
+    prob = make_problem(1)
+    rays = make_rays(prob, 10_000)
+    ref = _oracle(prob).cast(rays)
+    with _mr(prob, 0) as m:
+        m.cast_rays(torch.from_numpy(rays).cuda())          # device buffer
+        t_dev = m.read_tally()
+        m.clear_tally()
+        m.set_option(MR_OPT_STAGE_RAYS, 1024)                # 10 chunks, ragged last one
+        m.cast_rays(rays)                                     # pageable host buffer
+        t_host = m.read_tally()
+        st = m.get_stats()
+        m.clear_tally()
+        m.cast_rays(torch.from_numpy(rays).pin_memory())     # pinned host buffer
+        t_pin = m.read_tally()
+        m.clear_tally()
+        assert m.cast_rays(rays[:0]) == 0                    # empty batch: no-op
+        assert not m.read_tally().any()
+        # additivity across calls: A then B == A u B
+        m.cast_rays(rays[:3333])
+        m.cast_rays(rays[3333:])
+        t_ab = m.read_tally()
+    assert st.segments == ref.segments and st.rays_accepted == 10_000
+    for t in (t_dev, t_host, t_pin, t_ab):
+        assert_tally(t, ref.tally, 0)
+    np.testing.assert_allclose(t_host, t_dev, rtol=1e-12, atol=1e-14)
+
+
+def test_block_size_option_and_torch_stream():
+    import torch
+
+    from paper_1706_07476_b200 import MR_OPT_BLOCK_THREADS
+
+    prob = make_problem(1)
+    rays = make_rays(prob, 10_000)
+    ref = _oracle(prob).cast(rays)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        with _mr(prob, 0) as m:
+            for bt in (64, 128, 512):
+                m.set_option(MR_OPT_BLOCK_THREADS, bt)
+                m.clear_tally()
+                m.cast_rays(rays)
+                assert_tally(m.read_tally(), ref.tally, 0)
+
+
+def test_call_order_and_argument_errors():
+    from paper_1706_07476_b200 import MonteRay, MonteRayError
+
+    prob = make_problem(1)
+    rays = make_rays(prob, 100)
+    with MonteRay(0, 0) as m:
+        with pytest.raises(MonteRayError) as e:
+            m.cast_rays(rays)
+        assert e.value.status == 2  # MR_ERR_STATE: no mesh
+        with pytest.raises(MonteRayError):
+            m.load_mesh([0.0, 1.0, 1.0], [0.0, 1.0], [0.0, 1.0])  # not strictly increasing
+        m.load_mesh(prob.xe, prob.ye, prob.ze)
+        with pytest.raises(MonteRayError) as e:
+            m.load_xs(0, prob.xs[0][0], prob.xs[0][1])
+        assert e.value.status == 2  # materials first
+        bad = prob.cell_mat.copy()
+        bad[17, 0] = 5
+        with pytest.raises(MonteRayError) as e:
+            m.load_materials(prob.density, bad, prob.cell_frac)
+        assert e.value.status == 1
+        m.load_materials(prob.density, prob.cell_mat, prob.cell_frac)
+        m.load_xs(0, *prob.xs[0])
+        with pytest.raises(MonteRayError) as e:
+            m.cast_rays(rays)
+        assert e.value.status == 2 and "material 1" in str(e.value)
+        with pytest.raises(MonteRayError):
+            m.load_xs(1, prob.xs[1][0][::-1], prob.xs[1][1])  # decreasing grid
+        m.load_xs(1, *prob.xs[1])
+        m.cast_rays(rays)
+        assert m.get_stats().rays_accepted == 100
+        # the trace needs only the mesh; the context stays usable after argument errors
+        nseg, _, _, _ = m.trace_rays(rays)
+        assert nseg.sum() == m.get_stats().segments
+
+
+def test_tally_tensor_view_is_the_resident_tally():
+    prob = make_problem(1)
+    rays = make_rays(prob, 2000)
+    with _mr(prob, 0) as m:
+        m.cast_rays(rays)
+        m.sync()
+        t = m.tally_tensor()
+        assert t.is_cuda and t.numel() == prob.ncell
+        assert np.array_equal(t.cpu().numpy(), m.read_tally())
