@@ -324,6 +324,40 @@ template <typename Real> struct CellRecGeneric {
 };
 
 // ------------------------------------------------------------------------------------------------
+// S5 helper: for x >= 0 returns ex = exp(-x) and omex = 1 - exp(-x), both to ~1 ulp, from ONE
+// polynomial.  y = -x = k ln2 + r, |r| <= ln2/2;  p = expm1(r) = r + r^2 q(r) (Taylor, 1/2! .. 1/13!);
+// exp(-x) = 2^k (1 + p);  1 - exp(-x) = (1 - 2^k) - 2^k p  (no cancellation: 2^k(1+p) <= 0.71 for k < 0,
+// and for k = 0 it is exactly -p).  A running product A *= exp(-x) built from 1 + expm1(-x) would lose
+// all precision once x > ~37; carrying ex itself does not ("attenuation").
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void exp_pair(double x, double &ex, double &omex)
+{
+    const double y = -x;
+    const double kf = rint(y * 1.4426950408889634074);           // k = round(y / ln2) <= 0
+    double r = fma(kf, -6.93147180369123816490e-01, y);           // Cody-Waite: ln2 = hi + lo
+    r = fma(kf, -1.90821492927058770002e-10, r);
+    double q = 1.0 / 6227020800.0;                                 // 1/13!
+    q = fma(q, r, 1.0 / 479001600.0);                              // 1/12!
+    q = fma(q, r, 1.0 / 39916800.0);                               // 1/11!
+    q = fma(q, r, 1.0 / 3628800.0);                                // 1/10!
+    q = fma(q, r, 1.0 / 362880.0);                                 // 1/9!
+    q = fma(q, r, 1.0 / 40320.0);                                  // 1/8!
+    q = fma(q, r, 1.0 / 5040.0);                                   // 1/7!
+    q = fma(q, r, 1.0 / 720.0);                                    // 1/6!
+    q = fma(q, r, 1.0 / 120.0);                                    // 1/5!
+    q = fma(q, r, 1.0 / 24.0);                                     // 1/4!
+    q = fma(q, r, 1.0 / 6.0);                                      // 1/3!
+    q = fma(q, r, 0.5);                                            // 1/2!
+    const double p = fma(r * r, q, r);
+    const int k = (int)kf;
+    // 2^k for k in [-1022, 0]; beyond that exp(-x) < 2.3e-308 and is flushed to 0 (x > 708)
+    const double scale = __longlong_as_double((long long)(k + 1023) << 52);
+    const bool tiny = k < -1022;
+    ex = tiny ? 0.0 : fma(scale, p, scale);
+    omex = tiny ? 1.0 : fma(-scale, p, 1.0 - scale);
+}
+
+// ------------------------------------------------------------------------------------------------
 // The cast kernel: one thread per ray (S1 -> S6).
 //   dynamic shared memory: [edges: nedges doubles (if EDGES_SMEM)] [sigma: M x blockDim Real]
 // ------------------------------------------------------------------------------------------------
@@ -365,10 +399,11 @@ __global__ void cast_kernel(const __grid_constant__ CastParams P)
                 // S4 + S5 (Eq. (4)): x = Sigma*l; score = W e^{-tau} (x > 0 ? (1-e^{-x})/Sigma : l)
                 const double S = (double)cur.sigma(sig, stride, P.K);
                 const double x = S * len;
-                const double em1 = expm1(-x);
-                const double g = (x > 0.0) ? (-em1 / S) : len;
+                double ex, omex;
+                exp_pair(x, ex, omex);
+                const double g = (x > 0.0) ? (omex / S) : len;
                 const double score = wa * g;
-                wa = fma(wa, em1, wa);
+                wa *= ex;
                 // S6
                 if (len > 0.0) red_add_f64(P.tally + cell, score);
                 ++nseg;
