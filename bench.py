@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the VRC ray-cast hot path on B200 (driver contract).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C]
+
+A "step" is one pass of the whole hot path over one batch of synthetic rays: S1 cross sections ->
+S2/S3 mesh walk -> S4/S5 Eq. (4) score -> S6 fp64 tally accumulation (mr_cast_rays).  The default
+workload is BASELINE.json configs[2], the PWR 17x17-like lattice (170x170x300 cells, K = 3,
+10^7 rays per batch): the configuration north_star's roofline target is quoted on.
+
+  value   : whole-job ray-cell segments/s with the ray batch already resident in HBM
+  e2e     : the same metric through the C ABI with HOST buffers: each step copies the batch from
+            pinned host memory (mr_cast_rays, where = host) and reads the tally back (mr_read_tally)
+  roofline: algorithmic bytes (31 B/segment + 96 B/ray on this config) / cast-kernel time, against
+            the measured copy bandwidth in MEASURED_PEAKS.json
+  cpu_baseline: the CPU oracle, as it stands, on the box's host cores over a bounded sample
+
+N > 1 (torchrun, one rank per GPU): every rank holds the whole problem and casts its own batches
+(weak scaling, no data-path collective); time = max over ranks.  --impl reference times the
+oracle on the host cores (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ray_cell_segments_per_sec"
+UNIT = "segments/s"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def algorithmic_bytes(prob, segments: int, rays: int, dense: bool = False) -> int:
+    """B_seg = 16 + 5K (dense: 16 + 4K), B_ray = 32 + 16 M (mixed mode)."""
+    b_seg = 16 + (4 if dense else 5) * prob.K
+    b_ray = 32 + 16 * prob.M
+    return segments * b_seg + rays * b_ray
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def committed_traffic(workload: str):
+    """dram bytes per cast-kernel launch from the committed ncu capture (profiles/traffic.txt), or None."""
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "traffic.txt")):
+            w = line.split()
+            if len(w) >= 2 and w[0] == workload:
+                return float(w[1])
+    except OSError:
+        pass
+    return None
+
+
+class ClockSampler:
+    """Polls SM clock and throttle reasons through NVML while `active` (the timed regions)."""
+
+    def __init__(self, cuda_index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.active = False
+        self._stop = False
+        self._thread = None
+        try:
+            import pynvml
+            import torch
+
+            pynvml.nvmlInit()
+            try:
+                uuid = str(torch.cuda.get_device_properties(cuda_index).uuid)
+                uuid = uuid if uuid.startswith("GPU-") else "GPU-" + uuid
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode())
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(cuda_index)
+            self.nv = pynvml
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        except Exception as e:  # no NVML: report that instead of numbers
+            self.error = repr(e)
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        while not self._stop:
+            if self.active:
+                try:
+                    self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                    try:
+                        mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                    except Exception:
+                        mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                    for bit, nm in names.items():
+                        if mask & bit:
+                            self.reasons.add(nm)
+                except Exception:
+                    pass
+            time.sleep(0.01)
+
+    def report(self):
+        self._stop = True
+        if self._thread is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "error": getattr(self, "error", "nvml unavailable")}
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def cpu_oracle_rate(prob, rays, threads: int):
+    """segments/s of the oracle as it stands on `threads` host threads over `rays`."""
+    from oracle.vrc_oracle import Oracle
+
+    orc = Oracle(prob)
+    t0 = time.perf_counter()
+    res = orc.cast(rays, threads=threads)
+    dt = time.perf_counter() - t0
+    return res.segments / dt, res.segments, dt, res.threads
+
+
+def run_reference(args, prob_kw):
+    """--impl reference: the CPU oracle on a bounded sample of the same workload, rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle.vrc_oracle import Oracle, max_threads
+    from workloads import CONFIG_NAMES, make_problem, make_rays
+
+    prob = make_problem(args.config, **prob_kw)
+    threads = max(1, min(max_threads(), len(os.sched_getaffinity(0))))
+    n_sample = args.ref_rays
+    rays = make_rays(prob, n_sample)
+    orc = Oracle(prob)
+    for _ in range(args.warmup):
+        orc.cast(rays[: max(1000, n_sample // 10)], threads=threads)
+    t0 = time.perf_counter()
+    segs = 0
+    for _ in range(args.steps):
+        segs += orc.cast(rays, threads=threads).segments
+    dt = time.perf_counter() - t0
+    value = segs / dt
+    sample = f"{n_sample} rays ({segs // args.steps} segments) of the workload per step, all host threads"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": CONFIG_NAMES[args.config], "reference": "CPU oracle (oracle/vrc_oracle.c), host cores",
+                   "rays_per_step": n_sample},
+        "rays_per_sec": n_sample * args.steps / dt,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="1-based index into BASELINE.json configs (default 3 = PWR)")
+    ap.add_argument("--rays", type=int, default=0, help="rays per batch (default: the config's full batch)")
+    ap.add_argument("--ref-rays", type=int, default=200_000, help="rays per step of the CPU reference arm")
+    ap.add_argument("--cpu-sample-rays", type=int, default=1_000_000, help="rays of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--block-threads", type=int, default=0)
+    ap.add_argument("--sort", type=int, default=-1, help="override MR_OPT_SORT_RAYS (default: library default)")
+    args = ap.parse_args()
+    prob_kw = {}
+
+    if args.impl == "reference":
+        return run_reference(args, prob_kw)
+
+    import numpy as np
+    import torch
+
+    from paper_1706_07476_b200 import MR_OPT_BLOCK_THREADS, MR_OPT_SORT_RAYS, MonteRay, multi
+    from workloads import CONFIG_NAMES, FULL_RAYS, make_problem, make_rays
+
+    rank, local_rank, world = multi.env_rank_world()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        multi.init_process_group("nccl")
+    n_rays = args.rays or FULL_RAYS[args.config]
+
+    prob = make_problem(args.config, **prob_kw)
+    rays = make_rays(prob, n_rays, batch=rank)  # every rank its own batch: weak scaling
+    m = MonteRay(local_rank, 0)
+    m.load_problem(prob)
+    if args.block_threads:
+        m.set_option(MR_OPT_BLOCK_THREADS, args.block_threads)
+    if args.sort >= 0:
+        m.set_option(MR_OPT_SORT_RAYS, args.sort)
+    d_rays = torch.from_numpy(rays).to(dev)
+    h_rays = torch.from_numpy(rays).pin_memory()
+    h_tally = torch.empty(prob.ncell, dtype=torch.float64).pin_memory()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------------------------------------------------------- device-resident steps (value)
+    for _ in range(max(args.warmup, 3)):
+        m.cast_rays(d_rays)
+    barrier()
+    st0 = m.get_stats()
+    if sampler:
+        sampler.active = True
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        m.cast_rays(d_rays)
+    e1.record()
+    barrier()
+    if sampler:
+        sampler.active = False
+    ms_total = multi.max_over_ranks(e0.elapsed_time(e1), dev)
+    st1 = m.get_stats()
+    seg_step = (st1.segments - st0.segments) // args.steps
+    launches = st1.kernel_launches - st0.kernel_launches
+    seg_all = multi.sum_over_ranks(seg_step, dev)
+    value = seg_all * args.steps / (ms_total * 1e-3)
+    rays_all = n_rays * world
+
+    # ---------------------------------------------------------------- dominant-kernel time (roofline)
+    kms = []
+    for _ in range(min(args.steps, 10)):
+        m.cast_rays(d_rays)
+        kms.append(m.get_stats().last_kernel_ms)
+    kernel_ms = statistics.mean(kms)
+    peak, peak_src = measured_peak()
+    dense = prob.config == 5
+    alg_bytes = algorithmic_bytes(prob, seg_step, n_rays, dense)
+    achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
+    traffic = committed_traffic(CONFIG_NAMES[args.config])
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": traffic, "peak_source": peak_src, "kernel": "mr::cast_kernel", "kernel_ms": kernel_ms,
+                "algorithmic_bytes_per_launch": alg_bytes,
+                "segments_per_sec_at_roofline": peak * 1e9 / (alg_bytes / seg_step)}
+
+    # ---------------------------------------------------------------- end to end through the C ABI, host buffers
+    e2e = None
+    if not args.no_e2e:
+        for _ in range(2):
+            m.cast_rays(h_rays)
+            m.read_tally_into(h_tally.data_ptr())
+        barrier()
+        if sampler:
+            sampler.active = True
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            m.cast_rays(h_rays)                    # H2D of the batch from pinned memory, inside the call
+            m.read_tally_into(h_tally.data_ptr())  # D2H of the ncell doubles (synchronises)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if sampler:
+            sampler.active = False
+        dt = multi.max_over_ranks(dt, dev)
+        e2e = {"value": seg_all * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(rays.nbytes),
+               "d2h_bytes_per_step": int(prob.ncell * 8), "ms_per_step": 1e3 * dt / args.steps}
+    total_launches = m.get_stats().kernel_launches
+
+    # ---------------------------------------------------------------- CPU oracle beside it (rank 0, N = 1)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle.vrc_oracle import max_threads
+
+        threads = max(1, min(max_threads(), len(os.sched_getaffinity(0))))
+        n_s = min(args.cpu_sample_rays, n_rays)
+        rate, segs, dt, used = cpu_oracle_rate(prob, rays[:n_s], threads)
+        cpu = {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle",
+               "sample": f"first {n_s} rays of the batch ({segs} segments), {dt:.1f} s wall on {used} threads"}
+
+    if rank == 0:
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": CONFIG_NAMES[args.config], "mesh": [prob.nx, prob.ny, prob.nz], "K": prob.K, "M": prob.M,
+                       "rays_per_step_per_gpu": n_rays, "segments_per_step_per_gpu": int(seg_step),
+                       "precision": "mixed (fp32 tables/rays/coefficients, fp64 walk/score/tally)",
+                       "parallelism": f"replicas x{world}" if world > 1 else "1 GPU",
+                       "l2": "inputs larger than L2 (rays 320 MB + cell records 139 MB + tally 69 MB), no flush"
+                       if args.config == 3 else "no flush"},
+            "rays_per_sec": rays_all * args.steps / (ms_total * 1e-3),
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": int(launches), "gpu_launches_total": int(total_launches),
+            "clocks": sampler.report() if sampler else None,
+        }
+        print(json.dumps(out))
+    m.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -83,8 +83,9 @@ typedef struct {
     int64_t rays_rejected;  /* rays refused by the validation rule below */
     int64_t segments;       /* ray-cell segments scored (zero-length ones included) */
     int64_t kernel_launches;/* kernels this context has launched since creation */
-    double last_cast_ms;    /* device time of the most recent mr_cast_rays work (all its kernels) */
-    int64_t reserved[4];
+    double last_cast_ms;    /* device time of the most recent mr_cast_rays work (copies and all kernels) */
+    double last_kernel_ms;  /* device time of the cast kernel alone in that call (summed over its chunks) */
+    int64_t reserved[3];
 } mr_stats;
 
 /* ---- life cycle -------------------------------------------------------------------------- */

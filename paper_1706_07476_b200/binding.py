@@ -38,7 +38,8 @@ class MonteRayError(RuntimeError):
 
 class mr_stats(C.Structure):
     _fields_ = [("rays_accepted", C.c_int64), ("rays_rejected", C.c_int64), ("segments", C.c_int64),
-                ("kernel_launches", C.c_int64), ("last_cast_ms", C.c_double), ("reserved", C.c_int64 * 4)]
+                ("kernel_launches", C.c_int64), ("last_cast_ms", C.c_double), ("last_kernel_ms", C.c_double),
+                ("reserved", C.c_int64 * 3)]
 
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_void_p, C.c_size_t, C.c_int)
@@ -121,6 +122,7 @@ class Stats:
     segments: int
     kernel_launches: int
     last_cast_ms: float
+    last_kernel_ms: float
 
 
 def _f64(a) -> np.ndarray:
@@ -260,7 +262,7 @@ class MonteRay:
     def get_stats(self) -> Stats:
         s = mr_stats()
         self._check(self.lib.mr_get_stats(self._h, C.byref(s)))
-        return Stats(s.rays_accepted, s.rays_rejected, s.segments, s.kernel_launches, s.last_cast_ms)
+        return Stats(s.rays_accepted, s.rays_rejected, s.segments, s.kernel_launches, s.last_cast_ms, s.last_kernel_ms)
 
     def tally_device_ptr(self) -> int:
         p = C.c_void_p()

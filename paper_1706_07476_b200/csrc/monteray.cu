@@ -80,6 +80,8 @@ struct mr_ctx {
 
     cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;
     bool have_timing = false;
+    std::vector<cudaEvent_t> kev;  // (start, stop) pairs around each cast-kernel launch of the last call
+    size_t kev_used = 0;
     long long launches = 0;
     int block_threads = 256;
     int sort_rays = 0;
@@ -244,15 +246,28 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     P.n = n;
     P.tally = c->d_tally;
     P.counters = c->d_counters;
-    if (c->precision == MR_PRECISION_DOUBLE) return launch_cast_t<double, CellRecGeneric<double>>(c, P);
-    switch (c->layout) {
-    case LAYOUT_K1: return launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P);
-    case LAYOUT_K2: return launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P);
-    case LAYOUT_K3: return launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P);
-    case LAYOUT_K4: return launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P);
-    case LAYOUT_D8: return launch_cast_t<float, CellRec<LAYOUT_D8>>(c, P);
-    default: return launch_cast_t<float, CellRecGeneric<float>>(c, P);
+    if (c->kev_used + 2 > c->kev.size()) {
+        cudaEvent_t a = nullptr, b = nullptr;
+        MR_CUDA(c, cudaEventCreate(&a));
+        MR_CUDA(c, cudaEventCreate(&b));
+        c->kev.push_back(a);
+        c->kev.push_back(b);
     }
+    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->stream));
+    int rc;
+    if (c->precision == MR_PRECISION_DOUBLE) rc = launch_cast_t<double, CellRecGeneric<double>>(c, P);
+    else switch (c->layout) {
+    case LAYOUT_K1: rc = launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P); break;
+    case LAYOUT_K2: rc = launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
+    case LAYOUT_K3: rc = launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P); break;
+    case LAYOUT_K4: rc = launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P); break;
+    case LAYOUT_D8: rc = launch_cast_t<float, CellRec<LAYOUT_D8>>(c, P); break;
+    default: rc = launch_cast_t<float, CellRecGeneric<float>>(c, P);
+    }
+    if (rc) return rc;
+    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used + 1], c->stream));
+    c->kev_used += 2;
+    return MR_OK;
 }
 
 int ensure_stage(mr_ctx *c, size_t rays_per_slot)
@@ -353,6 +368,7 @@ int mr_destroy(mr_ctx *c)
         if (c->ev_copied[s]) cudaEventDestroy(c->ev_copied[s]);
         if (c->ev_done[s]) cudaEventDestroy(c->ev_done[s]);
     }
+    for (cudaEvent_t e : c->kev) cudaEventDestroy(e);
     if (c->ev_t0) cudaEventDestroy(c->ev_t0);
     if (c->ev_t1) cudaEventDestroy(c->ev_t1);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
@@ -548,6 +564,7 @@ int mr_cast_rays(mr_ctx *c, int64_t n, const void *rays, int where)
     if (int rc = ready_to_cast(c)) return rc;
     if (n == 0) return MR_OK;
     if (int rc = upload_xs_desc(c)) return rc;
+    c->kev_used = 0;
     if (where == MR_WHERE_DEVICE) {
         if ((uintptr_t)rays & 15) return c->fail(MR_ERR_INVALID_ARG, "cast: device ray buffer must be 16-byte aligned");
         MR_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
@@ -623,6 +640,10 @@ int mr_get_stats(mr_ctx *c, mr_stats *out)
         float ms = 0.f;
         MR_CUDA(c, cudaEventElapsedTime(&ms, c->ev_t0, c->ev_t1));
         out->last_cast_ms = ms;
+        for (size_t i = 0; i + 1 < c->kev_used; i += 2) {
+            MR_CUDA(c, cudaEventElapsedTime(&ms, c->kev[i], c->kev[i + 1]));
+            out->last_kernel_ms += ms;
+        }
     }
     return MR_OK;
 }
