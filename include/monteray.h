@@ -179,7 +179,7 @@ MR_API int mr_trace_rays(mr_ctx *ctx, int64_t n, const void *rays, int where, ui
 
 /* ---- tuning knobs (never change results beyond fp64 summation order) ---------------------- */
 enum {
-    MR_OPT_BLOCK_THREADS = 1, /* threads per CTA of the cast kernel (multiple of 32, <= 1024) */
+    MR_OPT_BLOCK_THREADS = 1, /* threads per CTA of the cast kernel (multiple of 32, <= 256) */
     MR_OPT_SORT_RAYS = 2,     /* 0: cast in buffer order; 1: bin rays by start slab and length first */
     MR_OPT_STAGE_RAYS = 3     /* rays per pinned staging chunk for host batches */
 };

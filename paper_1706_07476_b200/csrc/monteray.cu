@@ -16,6 +16,7 @@
 
 #define MR_PACK_MAX_SLOTS MR_MAX_SLOTS
 #include "mr_device.cuh"
+#include "mr_sort.cuh"
 
 using namespace mr;
 
@@ -83,8 +84,13 @@ struct mr_ctx {
     std::vector<cudaEvent_t> kev;  // (start, stop) pairs around each cast-kernel launch of the last call
     size_t kev_used = 0;
     long long launches = 0;
-    int block_threads = 256;
-    int sort_rays = 0;
+    int block_threads = 128;
+    int sort_rays = 1;
+
+    // ray-ordering pre-pass scratch (grown on demand)
+    uint32_t *d_keys = nullptr, *d_perm = nullptr, *d_hist = nullptr;
+    long long sort_cap = 0;
+    int hist_cap = 0;
 
     size_t ray_bytes() const { return precision == MR_PRECISION_DOUBLE ? 64 : 32; }
     size_t real_bytes() const { return precision == MR_PRECISION_DOUBLE ? 8 : 4; }
@@ -188,9 +194,9 @@ template <typename Real, typename Rec>
 int launch_cast_t(mr_ctx *c, const CastParams &P)
 {
     const int block = c->block_threads;
-    const size_t sig_bytes = (size_t)c->M * block * sizeof(Real);
-    const bool smem_edges = edges_smem_bytes(c) <= kEdgesSmemMax && edges_smem_bytes(c) + sig_bytes <= 200 * 1024;
-    const size_t smem = (smem_edges ? edges_smem_bytes(c) : 0) + sig_bytes;
+    const size_t per_block = walker_smem_bytes(block) + (size_t)c->M * block * sizeof(Real);
+    const bool smem_edges = edges_smem_bytes(c) <= kEdgesSmemMax && edges_smem_bytes(c) + per_block <= 200 * 1024;
+    const size_t smem = (smem_edges ? edges_smem_bytes(c) : 0) + per_block;
     if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "materials x block threads exceed shared memory; lower MR_OPT_BLOCK_THREADS");
     const long long grid = (P.n + block - 1) / block;
     if (grid > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
@@ -231,6 +237,56 @@ int ready_to_cast(mr_ctx *c)
     return MR_OK;
 }
 
+constexpr long long kSortMinRays = 1 << 14;   // below this a batch is a handful of CTAs: ordering buys nothing
+
+// Queue the ordering pre-pass for n device-resident rays; *perm_out = null if the batch is cast in buffer order.
+int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm_out)
+{
+    *perm_out = nullptr;
+    if (!c->sort_rays || n < kSortMinRays || n > 0xffffffffLL || edges_smem_bytes(c) > kEdgesSmemMax) return MR_OK;
+    const int nlen = 128;
+    const int zdiv = (c->nz + 255) / 256;
+    const int nslab = (c->nz + zdiv - 1) / zdiv;
+    const int maxlen = c->nx + c->ny + c->nz;
+    int lshift = 0;
+    while ((maxlen >> lshift) >= nlen) ++lshift;
+    const int nkeys = nslab * nlen + 1;
+    if (n > c->sort_cap) {
+        MR_CUDA(c, cudaStreamSynchronize(c->stream));
+        c->dev_free(c->d_keys);
+        c->dev_free(c->d_perm);
+        c->d_keys = (uint32_t *)c->dev_alloc((size_t)n * 4);
+        c->d_perm = (uint32_t *)c->dev_alloc((size_t)n * 4);
+        c->sort_cap = (c->d_keys && c->d_perm) ? n : 0;
+        if (!c->sort_cap) {
+            c->dev_free(c->d_keys);
+            c->dev_free(c->d_perm);
+            c->d_keys = c->d_perm = nullptr;
+            return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering scratch)");
+        }
+    }
+    if (nkeys + 1 > c->hist_cap) {
+        MR_CUDA(c, cudaStreamSynchronize(c->stream));
+        c->dev_free(c->d_hist);
+        c->d_hist = (uint32_t *)c->dev_alloc((size_t)(nkeys + 1) * 4);
+        c->hist_cap = c->d_hist ? nkeys + 1 : 0;
+        if (!c->d_hist) return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering histogram)");
+    }
+    SortParams S{MeshDev{c->nx, c->ny, c->nz, c->nedges, c->d_edges}, d_rays, n, c->precision == MR_PRECISION_DOUBLE ? 1 : 0,
+                 zdiv, lshift, nlen, nkeys, c->d_keys, c->d_hist, c->d_perm};
+    MR_CUDA(c, cudaMemsetAsync(c->d_hist, 0, (size_t)(nkeys + 1) * 4, c->stream));
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    const size_t smem = edges_smem_bytes(c);
+    if (int rc = set_smem(c, classify_kernel, smem)) return rc;
+    classify_kernel<<<grid, 256, smem, c->stream>>>(S);
+    scan_kernel<<<1, 1024, 0, c->stream>>>(c->d_hist, nkeys);
+    scatter_kernel<<<grid, 256, 0, c->stream>>>(S);
+    c->launches += 3;
+    MR_CUDA(c, cudaGetLastError());
+    *perm_out = c->d_perm;
+    return MR_OK;
+}
+
 // Queue the cast of n device-resident rays on the context's stream.
 int cast_device(mr_ctx *c, long long n, const void *d_rays)
 {
@@ -242,7 +298,7 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     P.M = c->M;
     P.xs = c->d_xs;
     P.rays = d_rays;
-    P.perm = nullptr;
+    if (int rc = order_rays(c, n, d_rays, &P.perm)) return rc;
     P.n = n;
     P.tally = c->d_tally;
     P.counters = c->d_counters;
@@ -364,6 +420,9 @@ int mr_destroy(mr_ctx *c)
     c->dev_free(c->d_edges);
     c->dev_free(c->d_tally);
     c->dev_free(c->d_counters);
+    c->dev_free(c->d_keys);
+    c->dev_free(c->d_perm);
+    c->dev_free(c->d_hist);
     for (int s = 0; s < kStageSlots; ++s) {
         if (c->ev_copied[s]) cudaEventDestroy(c->ev_copied[s]);
         if (c->ev_done[s]) cudaEventDestroy(c->ev_done[s]);
@@ -701,11 +760,11 @@ int mr_trace_rays(mr_ctx *c, int64_t n, const void *rays, int where, uint32_t *n
         const int block = 256;
         const unsigned grid = (unsigned)((n + block - 1) / block);
         if (edges_smem_bytes(c) <= kEdgesSmemMax) {
-            const size_t smem = edges_smem_bytes(c);
+            const size_t smem = edges_smem_bytes(c) + walker_smem_bytes(block);
             if (smem > 48 * 1024) e = cudaFuncSetAttribute(trace_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e == cudaSuccess) trace_kernel<true><<<grid, block, smem, c->stream>>>(P);
         } else
-            trace_kernel<false><<<grid, block, 0, c->stream>>>(P);
+            trace_kernel<false><<<grid, block, walker_smem_bytes(block), c->stream>>>(P);
         c->launches += 1;
         if (e == cudaSuccess) e = cudaGetLastError();
     }
@@ -724,7 +783,7 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
     MR_ENTER(c);
     switch (option) {
     case MR_OPT_BLOCK_THREADS:
-        if (value < 32 || value > 1024 || (value & 31)) return c->fail(MR_ERR_INVALID_ARG, "block threads must be a multiple of 32 in [32, 1024]");
+        if (value < 32 || value > 256 || (value & 31)) return c->fail(MR_ERR_INVALID_ARG, "block threads must be a multiple of 32 in [32, 256]");
         c->block_threads = (int)value;
         return MR_OK;
     case MR_OPT_SORT_RAYS:

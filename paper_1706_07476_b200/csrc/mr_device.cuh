@@ -141,18 +141,22 @@ __device__ __forceinline__ Real sigma_lookup(const XsDesc &t, Real E)
 //   t_a(p) = (edges_a[p] - o_a) * inv_a          (one subtract, then one multiply, both RN)
 // and the trace is the 3-way merge of the three non-decreasing sequences, ties x < y < z
 // (O3-O5).  __dsub_rn/__dmul_rn keep the compiler from contracting anything.
-// Plane indices are absolute positions in the concatenated edge array.
+//
+// Register budget: only the three pending crossing parameters, the current parameter and the cell
+// index live in registers.  The per-axis constants (o_a, inv_a) and counters (next plane, step,
+// exit plane, cell-index increment) sit in shared memory as two 16-byte records per axis per
+// thread, laid out [axis][thread] so that a warp's accesses are bank-conflict free whatever axis
+// each lane picks (the axis offset is a multiple of 512 B).  One step = pick the axis (2 DSETP +
+// selects), 2 LDS.128, 1 LDS.64 (plane position), 1 STS (next plane), DADD, DMUL: no divergent
+// branches.  Plane indices are absolute positions in the concatenated edge array.
 // ------------------------------------------------------------------------------------------------
+struct __align__(16) AxisF { double o, iv; };
+struct __align__(16) AxisI { int p, s, lim, dc; };   // next plane, step, exit plane, cell increment
+
 struct Walker {
     double t0, t1, t2;     // pending crossing parameter per axis (+inf: the axis never steps)
-    double o0, o1, o2;
-    double iv0, iv1, iv2;
-    int p0, p1, p2;        // next plane (absolute index)
-    int lim0, lim1, lim2;  // crossing this plane leaves the mesh
-    int s0, s1, s2;        // +1 / -1 / 0
-    int dc1, dc2;          // cell-index increment of a y / z step (x: s0)
-    int c;                 // current cell
     double tcur;
+    int c;                 // current cell
 };
 
 // number of entries of e[0..n) that are <= v
@@ -166,73 +170,76 @@ __device__ __forceinline__ int upper_bound_edges(const double *e, int n, double 
     return lo;
 }
 
-// Returns false if the ray is rejected by the box / direction rules of O1.
-__device__ __forceinline__ bool walker_init(Walker &w, const MeshDev &m, const double *e, const double o[3], const double d[3])
+// bytes of walker state in shared memory for a CTA of `block` threads
+__host__ __device__ constexpr size_t walker_smem_bytes(int block) { return (size_t)block * 3 * (sizeof(AxisF) + sizeof(AxisI)); }
+
+// Returns false if the ray is rejected by the box / direction rules of O1.  axf/axi point at this
+// thread's axis-0 records; axis a is at [a * stride].
+__device__ __forceinline__ bool walker_init(Walker &w, AxisF *axf, AxisI *axi, int stride, const MeshDev &m,
+                                            const double *e, const double o[3], const double d[3])
 {
-    const int bx = 0, by = m.nx + 1, bz = m.nx + m.ny + 2;
-    if (!(o[0] >= e[bx] && o[0] < e[bx + m.nx])) return false;
-    if (!(o[1] >= e[by] && o[1] < e[by + m.ny])) return false;
-    if (!(o[2] >= e[bz] && o[2] < e[bz + m.nz])) return false;
-    const int ix = upper_bound_edges(e + bx, m.nx + 1, o[0]) - 1;
-    const int iy = upper_bound_edges(e + by, m.ny + 1, o[1]) - 1;
-    const int iz = upper_bound_edges(e + bz, m.nz + 1, o[2]) - 1;
-    w.c = ix + m.nx * (iy + m.ny * iz);
-    w.o0 = o[0]; w.o1 = o[1]; w.o2 = o[2];
-    w.tcur = 0.0;
+    const int base[3] = {0, m.nx + 1, m.nx + m.ny + 2};
+    const int n[3] = {m.nx, m.ny, m.nz};
+    const int dcell[3] = {1, m.nx, m.nx * m.ny};
     const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    int idx[3];
+    double t[3];
     bool movable = false;
-#define MR_AXIS(A, IDX, BASE, N, DC)                                                            \
-    {                                                                                           \
-        const double dd = d[A];                                                                 \
-        const double inv = (dd != 0.0) ? __drcp_rn(dd) : 0.0;                                   \
-        if (dd == 0.0 || !isfinite(inv)) {                                                      \
-            w.s##A = 0; w.p##A = BASE; w.lim##A = -1; w.iv##A = 0.0; w.t##A = inf;              \
-        } else {                                                                                \
-            movable = true;                                                                     \
-            w.iv##A = inv;                                                                      \
-            w.s##A = dd > 0.0 ? 1 : -1;                                                         \
-            w.p##A = BASE + (dd > 0.0 ? IDX + 1 : IDX);                                         \
-            w.lim##A = BASE + (dd > 0.0 ? N : 0);                                               \
-            w.t##A = __dmul_rn(__dsub_rn(e[w.p##A], o[A]), inv);                                \
-        }                                                                                       \
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (!(o[a] >= e[base[a]] && o[a] < e[base[a] + n[a]])) return false;   // half-open box (Q8)
+        idx[a] = upper_bound_edges(e + base[a], n[a] + 1, o[a]) - 1;          // O3: pure comparisons
     }
-    MR_AXIS(0, ix, bx, m.nx, 1)
-    MR_AXIS(1, iy, by, m.ny, m.nx)
-    MR_AXIS(2, iz, bz, m.nz, m.nx * m.ny)
-#undef MR_AXIS
-    w.dc1 = w.s1 * m.nx;
-    w.dc2 = w.s2 * m.nx * m.ny;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double dd = d[a];
+        const double inv = (dd != 0.0) ? __drcp_rn(dd) : 0.0;
+        AxisI ai;
+        if (dd == 0.0 || !isfinite(inv)) {                                     // Q10: the axis never steps
+            ai = AxisI{base[a], 0, -1, 0};
+            axf[a * stride] = AxisF{o[a], 0.0};
+            t[a] = inf;
+        } else {
+            movable = true;
+            const bool up = dd > 0.0;
+            ai.p = base[a] + (up ? idx[a] + 1 : idx[a]);
+            ai.s = up ? 1 : -1;
+            ai.lim = base[a] + (up ? n[a] : 0);
+            ai.dc = up ? dcell[a] : -dcell[a];
+            axf[a * stride] = AxisF{o[a], inv};
+            t[a] = __dmul_rn(__dsub_rn(e[ai.p], o[a]), inv);                   // O4
+        }
+        axi[a * stride] = ai;
+    }
+    w.t0 = t[0]; w.t1 = t[1]; w.t2 = t[2];
+    w.tcur = 0.0;
+    w.c = idx[0] + m.nx * (idx[1] + m.ny * idx[2]);
     return movable;
 }
 
-// One step of the merge.  On return: `cell` = the cell just traversed, `len` its segment length;
+// One step of the merge (O5).  On return `cell` = the cell just traversed, `len` its segment length;
 // the return value is true when the ray has left the mesh.
-__device__ __forceinline__ bool walker_step(Walker &w, const double *e, int &cell, double &len)
+__device__ __forceinline__ bool walker_step(Walker &w, AxisF *axf, AxisI *axi, int stride, const double *e,
+                                            int &cell, double &len)
 {
     const bool ysel = w.t1 < w.t0;                 // ties keep x
     const double tm = ysel ? w.t1 : w.t0;
     const bool zsel = w.t2 < tm;                   // ties keep x / y
     const double tn = zsel ? w.t2 : tm;
+    const int off = zsel ? 2 * stride : (ysel ? stride : 0);
+    const AxisI ai = axi[off];
+    const AxisF af = axf[off];
     len = __dsub_rn(tn, w.tcur);
     w.tcur = tn;
     cell = w.c;
-    bool leave;
-    if (zsel) {
-        leave = (w.p2 == w.lim2);
-        w.c += w.dc2;
-        w.p2 += w.s2;
-        if (!leave) w.t2 = __dmul_rn(__dsub_rn(e[w.p2], w.o2), w.iv2);
-    } else if (ysel) {
-        leave = (w.p1 == w.lim1);
-        w.c += w.dc1;
-        w.p1 += w.s1;
-        if (!leave) w.t1 = __dmul_rn(__dsub_rn(e[w.p1], w.o1), w.iv1);
-    } else {
-        leave = (w.p0 == w.lim0);
-        w.c += w.s0;
-        w.p0 += w.s0;
-        if (!leave) w.t0 = __dmul_rn(__dsub_rn(e[w.p0], w.o0), w.iv0);
-    }
+    const bool leave = (ai.p == ai.lim);
+    const int pn = ai.p + ai.s;
+    w.c += ai.dc;
+    axi[off].p = pn;
+    const double tnew = __dmul_rn(__dsub_rn(e[leave ? ai.p : pn], af.o), af.iv);
+    w.t0 = (zsel || ysel) ? w.t0 : tnew;
+    w.t1 = (!zsel && ysel) ? tnew : w.t1;
+    w.t2 = zsel ? tnew : w.t2;
     return leave;
 }
 
@@ -324,56 +331,88 @@ template <typename Real> struct CellRecGeneric {
 };
 
 // ------------------------------------------------------------------------------------------------
-// S5 helper: for x >= 0 returns ex = exp(-x) and omex = 1 - exp(-x), both to ~1 ulp, from ONE
-// polynomial.  y = -x = k ln2 + r, |r| <= ln2/2;  p = expm1(r) = r + r^2 q(r) (Taylor, 1/2! .. 1/13!);
-// exp(-x) = 2^k (1 + p);  1 - exp(-x) = (1 - 2^k) - 2^k p  (no cancellation: 2^k(1+p) <= 0.71 for k < 0,
-// and for k = 0 it is exactly -p).  A running product A *= exp(-x) built from 1 + expm1(-x) would lose
-// all precision once x > ~37; carrying ex itself does not ("attenuation").
+// S5: the two factors of Eq. (4) for one segment, x = Sigma * len >= 0:
+//     g  = (1 - exp(-x)) / Sigma   (-> len as x -> 0, reading Q12),     ex = exp(-x)
+// from ONE polynomial.  -x = k ln2 + r, |r| <= ln2/2; p = expm1(r) = r + r^2 q(r), q = Taylor
+// 1/2! + r/3! + ...; exp(-x) = 2^k (1 + p); 1 - exp(-x) = (1 - 2^k) - 2^k p (no cancellation:
+// 2^k (1+p) <= 0.71 for k < 0).  For k = 0 (x <= ln2/2, the common case in thin cells) g needs no
+// division at all: (1 - e^{-x})/Sigma = len * (p/r) = len * (1 + r q(r)), which is also exact at x = 0.
+// The attenuation is carried as a running product of ex itself: 1 + expm1(-x) would lose all
+// precision once x > ~37.
+//   FULL  (double mode): q to 1/13!, error ~1e-16; the k < 0 branch divides.
+//   !FULL (mixed mode) : q to 1/8!, error < 6e-10 (the fp32 cross sections carry ~1e-7); the
+//                        k < 0 branch uses rcp.approx + 2 Newton steps (error ~1e-16).
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void exp_pair(double x, double &ex, double &omex)
+__constant__ double c_expq[12] = {
+    1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 39916800.0, 1.0 / 3628800.0, 1.0 / 362880.0, 1.0 / 40320.0,
+    1.0 / 5040.0, 1.0 / 720.0, 1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0, 0.5};
+
+template <bool FULL>
+__device__ __forceinline__ void score_terms(double S, double len, double &g, double &ex)
 {
-    const double y = -x;
-    const double kf = rint(y * 1.4426950408889634074);           // k = round(y / ln2) <= 0
-    double r = fma(kf, -6.93147180369123816490e-01, y);           // Cody-Waite: ln2 = hi + lo
-    r = fma(kf, -1.90821492927058770002e-10, r);
-    double q = 1.0 / 6227020800.0;                                 // 1/13!
-    q = fma(q, r, 1.0 / 479001600.0);                              // 1/12!
-    q = fma(q, r, 1.0 / 39916800.0);                               // 1/11!
-    q = fma(q, r, 1.0 / 3628800.0);                                // 1/10!
-    q = fma(q, r, 1.0 / 362880.0);                                 // 1/9!
-    q = fma(q, r, 1.0 / 40320.0);                                  // 1/8!
-    q = fma(q, r, 1.0 / 5040.0);                                   // 1/7!
-    q = fma(q, r, 1.0 / 720.0);                                    // 1/6!
-    q = fma(q, r, 1.0 / 120.0);                                    // 1/5!
-    q = fma(q, r, 1.0 / 24.0);                                     // 1/4!
-    q = fma(q, r, 1.0 / 6.0);                                      // 1/3!
-    q = fma(q, r, 0.5);                                            // 1/2!
-    const double p = fma(r * r, q, r);
-    const int k = (int)kf;
-    // 2^k for k in [-1022, 0]; beyond that exp(-x) < 2.3e-308 and is flushed to 0 (x > 708)
-    const double scale = __longlong_as_double((long long)(k + 1023) << 52);
-    const bool tiny = k < -1022;
-    ex = tiny ? 0.0 : fma(scale, p, scale);
-    omex = tiny ? 1.0 : fma(-scale, p, 1.0 - scale);
+    const double x = S * len;
+    double r = -x;
+    int k = 0;
+    if (x > 0.34657359027997264) {                                   // ln2 / 2
+        const double kf = rint(x * -1.4426950408889634074);          // k = round(-x / ln2) < 0
+        r = fma(kf, -6.93147180369123816490e-01, -x);                // Cody-Waite: ln2 = hi + lo
+        r = fma(kf, -1.90821492927058770002e-10, r);
+        k = (int)kf;                                                 // saturates for huge x
+    }
+    constexpr int first = FULL ? 0 : 5;
+    double q = c_expq[first];
+#pragma unroll
+    for (int i = first + 1; i < 12; ++i) q = fma(q, r, c_expq[i]);
+    const double p = fma(r * r, q, r);                               // expm1(r)
+    if (k == 0) {
+        ex = 1.0 + p;
+        g = fma(len * r, q, len);                                    // len * (1 + r q)
+    } else if (k >= -1022) {
+        const double scale = __longlong_as_double((long long)(k + 1023) << 52);   // 2^k
+        ex = fma(scale, p, scale);
+        const double omex = fma(-scale, p, 1.0 - scale);
+        if (FULL) {
+            g = omex / S;
+        } else {
+            double y;
+            asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(S));
+            double err = fma(-S, y, 1.0);
+            y = fma(y, err, y);
+            err = fma(-S, y, 1.0);
+            y = fma(y, err, y);
+            g = omex * y;
+        }
+    } else {                                                         // x > 708: exp(-x) < 2.3e-308, flushed
+        ex = 0.0;
+        g = 1.0 / S;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
 // The cast kernel: one thread per ray (S1 -> S6).
-//   dynamic shared memory: [edges: nedges doubles (if EDGES_SMEM)] [sigma: M x blockDim Real]
+//   dynamic shared memory: [edges: nedges doubles (if EDGES_SMEM)] [walker: 3 x blockDim x 32 B]
+//                          [sigma: M x blockDim Real]
 // ------------------------------------------------------------------------------------------------
+__host__ __device__ constexpr size_t edges_smem_bytes_for(int nedges) { return sizeof(double) * (size_t)((nedges + 1) & ~1); }
+
 template <typename Real, typename Rec, bool EDGES_SMEM>
-__global__ void cast_kernel(const __grid_constant__ CastParams P)
+__global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double *s_edges = reinterpret_cast<double *>(smem_raw);
-    Real *s_sig = reinterpret_cast<Real *>(smem_raw + (EDGES_SMEM ? sizeof(double) * ((P.mesh.nedges + 1) & ~1) : 0));
+    const int stride = blockDim.x;
+    unsigned char *sp = smem_raw;
+    double *s_edges = reinterpret_cast<double *>(sp);
+    if (EDGES_SMEM) sp += edges_smem_bytes_for(P.mesh.nedges);
+    AxisF *axf = reinterpret_cast<AxisF *>(sp) + threadIdx.x;
+    sp += sizeof(AxisF) * 3 * stride;
+    AxisI *axi = reinterpret_cast<AxisI *>(sp) + threadIdx.x;
+    sp += sizeof(AxisI) * 3 * stride;
+    Real *sig = reinterpret_cast<Real *>(sp) + threadIdx.x;
     const double *e = EDGES_SMEM ? s_edges : P.mesh.edges;
     if (EDGES_SMEM) {
         for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
         __syncthreads();
     }
-    const int stride = blockDim.x;
-    Real *sig = s_sig + threadIdx.x;
 
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     unsigned nseg = 0;
@@ -382,30 +421,28 @@ __global__ void cast_kernel(const __grid_constant__ CastParams P)
         const long long r = P.perm ? (long long)__ldg(P.perm + i) : i;
         const Ray<Real> R = load_ray<Real>(P.rays, r);
         Walker w;
-        accepted = R.finite && (R.E > (Real)0) && walker_init(w, P.mesh, e, R.o, R.d);
+        accepted = R.finite && (R.E > (Real)0) && walker_init(w, axf, axi, stride, P.mesh, e, R.o, R.d);
         if (accepted) {
             // S1: every material's sigma at the ray's energy, kept in this thread's shared column
             for (int m = 0; m < P.M; ++m) sig[m * stride] = sigma_lookup<Real>(P.xs[m], R.E);
 
-            double wa = R.W;   // W * exp(-tau) as a running product
+            double wa = R.W;   // W * exp(-tau), a running product of exp(-x)
+            double *const tally = P.tally;
             Rec rec;
             rec.load(P.recs, P.ids, P.K, w.c);
             for (;;) {
                 int cell;
                 double len;
-                const bool leave = walker_step(w, e, cell, len);
+                const bool leave = walker_step(w, axf, axi, stride, e, cell, len);
                 const Rec cur = rec;
                 if (!leave) rec.load(P.recs, P.ids, P.K, w.c);   // next cell's record: in flight during the score
-                // S4 + S5 (Eq. (4)): x = Sigma*l; score = W e^{-tau} (x > 0 ? (1-e^{-x})/Sigma : l)
+                // S4 + S5 (Eq. (4)): score = W e^{-tau} (1 - e^{-x}) / Sigma,  x = Sigma * len
                 const double S = (double)cur.sigma(sig, stride, P.K);
-                const double x = S * len;
-                double ex, omex;
-                exp_pair(x, ex, omex);
-                const double g = (x > 0.0) ? (omex / S) : len;
-                const double score = wa * g;
+                double g, ex;
+                score_terms<sizeof(Real) == 8>(S, len, g, ex);
+                // S6 (a zero-length segment scores exactly 0: nothing to add)
+                if (len > 0.0) red_add_f64(tally + cell, wa * g);
                 wa *= ex;
-                // S6
-                if (len > 0.0) red_add_f64(P.tally + cell, score);
                 ++nseg;
                 if (leave) break;
             }
@@ -425,13 +462,20 @@ __global__ void cast_kernel(const __grid_constant__ CastParams P)
 }
 
 // ------------------------------------------------------------------------------------------------
-// The trace kernel (test entry point mr_trace_rays): same walker, no cross sections, no tally.
+// The trace kernel (test entry point mr_trace_rays): the same walker, no cross sections, no tally.
+//   dynamic shared memory: [edges (if EDGES_SMEM)] [walker: 3 x blockDim x 32 B]
 // ------------------------------------------------------------------------------------------------
 template <bool EDGES_SMEM>
-__global__ void trace_kernel(const __grid_constant__ TraceParams P)
+__global__ void __launch_bounds__(256) trace_kernel(const __grid_constant__ TraceParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double *s_edges = reinterpret_cast<double *>(smem_raw);
+    const int stride = blockDim.x;
+    unsigned char *sp = smem_raw;
+    double *s_edges = reinterpret_cast<double *>(sp);
+    if (EDGES_SMEM) sp += edges_smem_bytes_for(P.mesh.nedges);
+    AxisF *axf = reinterpret_cast<AxisF *>(sp) + threadIdx.x;
+    sp += sizeof(AxisF) * 3 * stride;
+    AxisI *axi = reinterpret_cast<AxisI *>(sp) + threadIdx.x;
     const double *e = EDGES_SMEM ? s_edges : P.mesh.edges;
     if (EDGES_SMEM) {
         for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
@@ -451,7 +495,7 @@ __global__ void trace_kernel(const __grid_constant__ TraceParams P)
         ok = R.finite && R.E > 0.0f;
     }
     Walker w;
-    ok = ok && walker_init(w, P.mesh, e, o, d);
+    ok = ok && walker_init(w, axf, axi, stride, P.mesh, e, o, d);
     unsigned nseg = 0;
     unsigned long long h = 0;
     if (ok) {
@@ -459,7 +503,7 @@ __global__ void trace_kernel(const __grid_constant__ TraceParams P)
         for (;;) {
             int cell;
             double len;
-            const bool leave = walker_step(w, e, cell, len);
+            const bool leave = walker_step(w, axf, axi, stride, e, cell, len);
             if ((long long)nseg < P.cap) {
                 if (P.cells) P.cells[r * P.cap + nseg] = cell;
                 if (P.lens) P.lens[r * P.cap + nseg] = len;

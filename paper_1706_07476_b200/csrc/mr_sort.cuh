@@ -1,0 +1,125 @@
+// mr_sort.cuh -- batch pre-pass: order the rays of a batch by (start z-slab, estimated segment count).
+//
+// Why (DESIGN.md §4 "ray ordering"): one thread walks one ray, so a warp runs as long as its longest
+// ray and touches cell records / tally lines wherever its 32 rays happen to be.  Ordering a batch so
+// that (a) rays of one warp need about the same number of steps and (b) CTAs resident at the same
+// time work in the same few z-slabs raises lane utilisation and keeps the working set (a z-slab of
+// records + tally is contiguous in memory, x fastest) inside the 126 MB L2.  The order only changes
+// which thread walks which ray: every ray's trace and score are unchanged, and the tally differs by
+// fp64 summation order only (reading Q18).
+//
+// Three kernels: classify (key per ray + histogram), scan (exclusive prefix over the keys), scatter
+// (ray index -> sorted position).  A counting sort: O(n), no library call.
+#pragma once
+#include "mr_device.cuh"
+
+namespace mr {
+
+struct SortParams {
+    MeshDev mesh;
+    const void *rays;
+    long long n;
+    int ray_is_double;
+    int zdiv;        // z-slab thickness in cells
+    int lshift;      // estimated segments >> lshift = length bucket
+    int nlen;        // length buckets per slab
+    int nkeys;       // slabs * nlen + 1 (last key: rejected rays)
+    uint32_t *keys;  // [n]
+    uint32_t *hist;  // [nkeys + 1], zeroed before classify; becomes the exclusive prefix after scan
+    uint32_t *perm;  // [n]
+};
+
+// dynamic shared memory: [edges] (always staged: the search would otherwise hammer global memory)
+__global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *e = reinterpret_cast<double *>(smem_raw);
+    for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) e[i] = __ldg(P.mesh.edges + i);
+    __syncthreads();
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= P.n) return;
+    double o[3], d[3];
+    bool ok;
+    if (P.ray_is_double) {
+        const Ray<double> R = load_ray_f64(P.rays, r);
+        for (int a = 0; a < 3; ++a) { o[a] = R.o[a]; d[a] = R.d[a]; }
+        ok = R.finite && R.E > 0.0;
+    } else {
+        const Ray<float> R = load_ray_f32(P.rays, r);
+        for (int a = 0; a < 3; ++a) { o[a] = R.o[a]; d[a] = R.d[a]; }
+        ok = R.finite && R.E > 0.0f;
+    }
+    const int base[3] = {0, P.mesh.nx + 1, P.mesh.nx + P.mesh.ny + 2};
+    const int n[3] = {P.mesh.nx, P.mesh.ny, P.mesh.nz};
+    int idx[3] = {0, 0, 0};
+    double t_exit = __longlong_as_double(0x7ff0000000000000LL);
+    for (int a = 0; a < 3 && ok; ++a) {
+        ok = (o[a] >= e[base[a]] && o[a] < e[base[a] + n[a]]);
+        if (!ok) break;
+        idx[a] = upper_bound_edges(e + base[a], n[a] + 1, o[a]) - 1;
+        if (d[a] != 0.0) {
+            const double t = (e[base[a] + (d[a] > 0.0 ? n[a] : 0)] - o[a]) / d[a];
+            t_exit = fmin(t_exit, t);
+        }
+    }
+    ok = ok && isfinite(t_exit);
+    uint32_t key = (uint32_t)(P.nkeys - 1);
+    if (ok) {
+        int est = 1;   // cells crossed ~ 1 + sum of index distances between the origin and the exit point
+        for (int a = 0; a < 3; ++a) {
+            double x = fma(t_exit, d[a], o[a]);
+            x = fmin(fmax(x, e[base[a]]), e[base[a] + n[a]]);
+            int j = upper_bound_edges(e + base[a], n[a] + 1, x) - 1;
+            j = min(max(j, 0), n[a] - 1);
+            est += abs(j - idx[a]);
+        }
+        key = (uint32_t)((idx[2] / P.zdiv) * P.nlen + min(est >> P.lshift, P.nlen - 1));
+    }
+    P.keys[r] = key;
+    atomicAdd(P.hist + key, 1u);
+}
+
+// one CTA: exclusive prefix sum of hist[0..nkeys) in place
+__global__ void __launch_bounds__(1024) scan_kernel(uint32_t *hist, int nkeys)
+{
+    __shared__ uint32_t warp_tot[32];
+    __shared__ uint32_t carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int first = 0; first < nkeys; first += 1024) {
+        const int i = first + threadIdx.x;
+        const uint32_t v = i < nkeys ? hist[i] : 0u;
+        uint32_t s = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= o) s += u;
+        }
+        if (lane == 31) warp_tot[wid] = s;
+        __syncthreads();
+        if (wid == 0) {
+            uint32_t w = warp_tot[lane];
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, w, o);
+                if (lane >= o) w += u;
+            }
+            warp_tot[lane] = w;
+        }
+        __syncthreads();
+        const uint32_t before = carry + (wid ? warp_tot[wid - 1] : 0u) + (s - v);
+        if (i < nkeys) hist[i] = before;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry = before + v;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(256) scatter_kernel(const SortParams P)
+{
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= P.n) return;
+    const uint32_t pos = atomicAdd(P.hist + P.keys[r], 1u);
+    P.perm[pos] = (uint32_t)r;
+}
+
+}  // namespace mr

@@ -198,7 +198,7 @@ def test_block_size_option_and_torch_stream():
     s = torch.cuda.Stream()
     with torch.cuda.stream(s):
         with _mr(prob, 0) as m:
-            for bt in (64, 128, 512):
+            for bt in (64, 128, 256):
                 m.set_option(MR_OPT_BLOCK_THREADS, bt)
                 m.clear_tally()
                 m.cast_rays(rays)
@@ -249,3 +249,28 @@ def test_tally_tensor_view_is_the_resident_tally():
         t = m.tally_tensor()
         assert t.is_cuda and t.numel() == prob.ncell
         assert np.array_equal(t.cpu().numpy(), m.read_tally())
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_ray_ordering_prepass_on_and_off(precision):
+    """MR_OPT_SORT_RAYS only changes which thread walks which ray: same counters, tally within tolerance
+    either way; includes rejected rays (they get the last key) and a batch that is not a multiple of 256."""
+    from paper_1706_07476_b200 import MR_OPT_SORT_RAYS
+
+    prob = make_problem(3, nx=68, ny=68, nz=40, n_e=2000)
+    rays = make_rays(prob, 70_001)
+    rays[::1000, 6] = -1.0        # E <= 0: rejected
+    rays[5::1000, 0] = 1.0e6      # origin outside the box: rejected
+    ref = _oracle(prob).cast(rays, threads=_threads())
+    assert ref.rays_rejected == 141
+    with _mr(prob, precision) as m:
+        r = rays.astype(m.ray_dtype)
+        for sort in (0, 1):
+            m.set_option(MR_OPT_SORT_RAYS, sort)
+            m.clear_tally()
+            before = m.get_stats().kernel_launches
+            m.cast_rays(r)
+            st = m.get_stats()
+            assert st.kernel_launches - before == (4 if sort else 1)
+            assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+            assert_tally(m.read_tally(), ref.tally, precision)
