@@ -110,7 +110,7 @@ MR_API const char *mr_last_error(mr_ctx *ctx);
  *      Cartesian mesh geometry"; geometry and tally share the mesh) ------------ */
 
 /* Rectilinear mesh given by its plane positions: xe[nx+1], ye[ny+1], ze[nz+1], host, strictly
- * increasing, finite.  nx*ny*nz must be < 2^31.  Allocates and zeroes the fp64 tally; drops
+ * increasing, finite.  nx*ny*nz must be < 2^31 and each of nx, ny, nz <= 32767.  Allocates and zeroes the fp64 tally; drops
  * any material map loaded before.  Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA. */
 MR_API int mr_load_mesh(mr_ctx *ctx, int nx, int ny, int nz, const double *xe, const double *ye, const double *ze);
 

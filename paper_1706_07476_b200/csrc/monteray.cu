@@ -54,6 +54,8 @@ struct mr_ctx {
     // mesh + tally
     int nx = 0, ny = 0, nz = 0, nedges = 0;
     long long ncell = 0;
+    bool mesh_arith = false;           // every plane position equals fma(p, h, e0) bit for bit
+    double mesh_e0[3] = {0, 0, 0}, mesh_h[3] = {0, 0, 0};
     double *d_edges = nullptr;
     double *d_tally = nullptr;
 
@@ -190,26 +192,45 @@ int set_smem(mr_ctx *c, K kernel, size_t bytes)
 
 size_t edges_smem_bytes(const mr_ctx *c) { return sizeof(double) * (size_t)((c->nedges + 1) & ~1); }
 
+MeshDev mesh_dev(const mr_ctx *c)
+{
+    MeshDev m{c->nx, c->ny, c->nz, c->nedges, c->d_edges, {c->mesh_e0[0], c->mesh_e0[1], c->mesh_e0[2]},
+              {c->mesh_h[0], c->mesh_h[1], c->mesh_h[2]}};
+    return m;
+}
+
+int edge_mode(const mr_ctx *c, size_t other_smem)
+{
+    if (c->mesh_arith) return EDGES_ARITH;
+    if (edges_smem_bytes(c) <= kEdgesSmemMax && edges_smem_bytes(c) + other_smem <= 200 * 1024) return EDGES_SHARED;
+    return EDGES_GLOBAL;
+}
+
+template <typename Real, typename Rec, int MODE>
+int launch_cast_m(mr_ctx *c, const CastParams &P, int block, size_t smem)
+{
+    const long long grid = (P.n + block - 1) / block;
+    if (grid > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
+    if (int rc = set_smem(c, cast_kernel<Real, Rec, MODE>, smem)) return rc;
+    cast_kernel<Real, Rec, MODE><<<(unsigned)grid, block, smem, c->stream>>>(P);
+    c->launches += 1;
+    MR_CUDA(c, cudaGetLastError());
+    return MR_OK;
+}
+
 template <typename Real, typename Rec>
 int launch_cast_t(mr_ctx *c, const CastParams &P)
 {
     const int block = c->block_threads;
     const size_t per_block = walker_smem_bytes(block) + (size_t)c->M * block * sizeof(Real);
-    const bool smem_edges = edges_smem_bytes(c) <= kEdgesSmemMax && edges_smem_bytes(c) + per_block <= 200 * 1024;
-    const size_t smem = (smem_edges ? edges_smem_bytes(c) : 0) + per_block;
+    const int mode = edge_mode(c, per_block);
+    const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
     if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "materials x block threads exceed shared memory; lower MR_OPT_BLOCK_THREADS");
-    const long long grid = (P.n + block - 1) / block;
-    if (grid > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
-    if (smem_edges) {
-        if (int rc = set_smem(c, cast_kernel<Real, Rec, true>, smem)) return rc;
-        cast_kernel<Real, Rec, true><<<(unsigned)grid, block, smem, c->stream>>>(P);
-    } else {
-        if (int rc = set_smem(c, cast_kernel<Real, Rec, false>, smem)) return rc;
-        cast_kernel<Real, Rec, false><<<(unsigned)grid, block, smem, c->stream>>>(P);
+    switch (mode) {
+    case EDGES_ARITH: return launch_cast_m<Real, Rec, EDGES_ARITH>(c, P, block, smem);
+    case EDGES_SHARED: return launch_cast_m<Real, Rec, EDGES_SHARED>(c, P, block, smem);
+    default: return launch_cast_m<Real, Rec, EDGES_GLOBAL>(c, P, block, smem);
     }
-    c->launches += 1;
-    MR_CUDA(c, cudaGetLastError());
-    return MR_OK;
 }
 
 int upload_xs_desc(mr_ctx *c)
@@ -272,7 +293,7 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
         c->hist_cap = c->d_hist ? nkeys + 1 : 0;
         if (!c->d_hist) return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering histogram)");
     }
-    SortParams S{MeshDev{c->nx, c->ny, c->nz, c->nedges, c->d_edges}, d_rays, n, c->precision == MR_PRECISION_DOUBLE ? 1 : 0,
+    SortParams S{mesh_dev(c), d_rays, n, c->precision == MR_PRECISION_DOUBLE ? 1 : 0,
                  zdiv, lshift, nlen, nkeys, c->d_keys, c->d_hist, c->d_perm};
     MR_CUDA(c, cudaMemsetAsync(c->d_hist, 0, (size_t)(nkeys + 1) * 4, c->stream));
     const unsigned grid = (unsigned)((n + 255) / 256);
@@ -291,7 +312,7 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
 int cast_device(mr_ctx *c, long long n, const void *d_rays)
 {
     CastParams P{};
-    P.mesh = MeshDev{c->nx, c->ny, c->nz, c->nedges, c->d_edges};
+    P.mesh = mesh_dev(c);
     P.recs = c->d_recs;
     P.ids = c->d_ids;
     P.K = c->K;
@@ -453,6 +474,7 @@ int mr_load_mesh(mr_ctx *c, int nx, int ny, int nz, const double *xe, const doub
     if (nx < 1 || ny < 1 || nz < 1 || !xe || !ye || !ze) return c->fail(MR_ERR_INVALID_ARG, "mesh: bad size or NULL edge array");
     const long long ncell = (long long)nx * ny * nz;
     if ((long long)nx * ny > 0x7fffffffLL || ncell >= 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "mesh: nx*ny*nz must be < 2^31");
+    if (nx > 32767 || ny > 32767 || nz > 32767) return c->fail(MR_ERR_UNSUPPORTED, "mesh: at most 32767 cells per axis");
     if (!finite_increasing(xe, nx + 1) || !finite_increasing(ye, ny + 1) || !finite_increasing(ze, nz + 1))
         return c->fail(MR_ERR_INVALID_ARG, "mesh: plane positions must be finite and strictly increasing");
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -476,6 +498,17 @@ int mr_load_mesh(mr_ctx *c, int nx, int ny, int nz, const double *xe, const doub
         return c->fail(MR_ERR_OOM, "device allocation failed (mesh / tally)");
     }
     c->nx = nx; c->ny = ny; c->nz = nz; c->nedges = ne; c->ncell = ncell;
+    {   // arithmetic mesh?  (uniform spacing reproduced exactly by one fma per plane, checked plane by plane)
+        const double *ax[3] = {xe, ye, ze};
+        const int na[3] = {nx, ny, nz};
+        c->mesh_arith = true;
+        for (int a = 0; a < 3; ++a) {
+            c->mesh_e0[a] = ax[a][0];
+            c->mesh_h[a] = ax[a][1] - ax[a][0];
+            for (int p = 0; p <= na[a] && c->mesh_arith; ++p)
+                c->mesh_arith = (std::fma((double)p, c->mesh_h[a], c->mesh_e0[a]) == ax[a][p]);
+        }
+    }
     MR_CUDA(c, cudaMemcpyAsync(c->d_edges, h.data(), sizeof(double) * ne, cudaMemcpyHostToDevice, c->stream));
     MR_CUDA(c, cudaMemsetAsync(c->d_tally, 0, sizeof(double) * ncell, c->stream));
     MR_CUDA(c, cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
@@ -755,16 +788,17 @@ int mr_trace_rays(mr_ctx *c, int64_t n, const void *rays, int where, uint32_t *n
     if (e == cudaSuccess && d_cells) e = cudaMemcpyAsync(d_cells, cells, (size_t)n * cap * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess && d_lens) e = cudaMemcpyAsync(d_lens, lens, (size_t)n * cap * 8, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) {
-        TraceParams P{MeshDev{c->nx, c->ny, c->nz, c->nedges, c->d_edges}, d_rays, n, d_nseg, d_hash, d_cells, d_lens, cap,
-                      c->precision == MR_PRECISION_DOUBLE ? 1 : 0};
+        TraceParams P{mesh_dev(c), d_rays, n, d_nseg, d_hash, d_cells, d_lens, cap, c->precision == MR_PRECISION_DOUBLE ? 1 : 0};
         const int block = 256;
         const unsigned grid = (unsigned)((n + block - 1) / block);
-        if (edges_smem_bytes(c) <= kEdgesSmemMax) {
-            const size_t smem = edges_smem_bytes(c) + walker_smem_bytes(block);
-            if (smem > 48 * 1024) e = cudaFuncSetAttribute(trace_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e == cudaSuccess) trace_kernel<true><<<grid, block, smem, c->stream>>>(P);
+        const int mode = edge_mode(c, walker_smem_bytes(block));
+        const size_t smem = walker_smem_bytes(block) + (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0);
+        if (mode == EDGES_ARITH) trace_kernel<EDGES_ARITH><<<grid, block, smem, c->stream>>>(P);
+        else if (mode == EDGES_SHARED) {
+            if (smem > 48 * 1024) e = cudaFuncSetAttribute(trace_kernel<EDGES_SHARED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e == cudaSuccess) trace_kernel<EDGES_SHARED><<<grid, block, smem, c->stream>>>(P);
         } else
-            trace_kernel<false><<<grid, block, walker_smem_bytes(block), c->stream>>>(P);
+            trace_kernel<EDGES_GLOBAL><<<grid, block, smem, c->stream>>>(P);
         c->launches += 1;
         if (e == cudaSuccess) e = cudaGetLastError();
     }

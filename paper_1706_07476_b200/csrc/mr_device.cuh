@@ -32,7 +32,13 @@ struct MeshDev {
     int nx, ny, nz;
     int nedges;            // nx+1 + ny+1 + nz+1
     const double *edges;   // x planes | y planes | z planes, concatenated
+    // "arithmetic" axes: mr_load_mesh verified edges_a[p] == fma((double)p, h[a], e0[a]) bit for bit for
+    // every plane, so the walker may recompute a plane position instead of looking it up
+    double e0[3], h[3];
 };
+
+// where the walker finds plane positions
+enum EdgeMode : int { EDGES_GLOBAL = 0, EDGES_SHARED = 1, EDGES_ARITH = 2 };
 
 struct CastParams {
     MeshDev mesh;
@@ -142,21 +148,22 @@ __device__ __forceinline__ Real sigma_lookup(const XsDesc &t, Real E)
 // and the trace is the 3-way merge of the three non-decreasing sequences, ties x < y < z
 // (O3-O5).  __dsub_rn/__dmul_rn keep the compiler from contracting anything.
 //
-// Register budget: only the three pending crossing parameters, the current parameter and the cell
-// index live in registers.  The per-axis constants (o_a, inv_a) and counters (next plane, step,
-// exit plane, cell-index increment) sit in shared memory as two 16-byte records per axis per
-// thread, laid out [axis][thread] so that a warp's accesses are bank-conflict free whatever axis
-// each lane picks (the axis offset is a multiple of 512 B).  One step = pick the axis (2 DSETP +
-// selects), 2 LDS.128, 1 LDS.64 (plane position), 1 STS (next plane), DADD, DMUL: no divergent
-// branches.  Plane indices are absolute positions in the concatenated edge array.
+// State: the three pending crossing parameters, the current parameter, the cell index, and per
+// axis one packed word (next plane | exit plane << 16) and the signed cell-index increment live in
+// registers; the per-axis doubles (o_a, inv_a) sit in shared memory, [axis][thread], 16 B each, so a
+// warp's LDS.128 is bank-conflict free whatever axis each lane picks.  The kernel is bound by
+// L1TEX data-pipe wavefronts (two uncoalesced global accesses per segment), so shared-memory
+// traffic per step is kept to that one LDS.128 (+ the sigma reads); when the mesh is arithmetic
+// (EDGES_ARITH) the plane position is recomputed with one I2F + DFMA instead of a table read.
 // ------------------------------------------------------------------------------------------------
 struct __align__(16) AxisF { double o, iv; };
-struct __align__(16) AxisI { int p, s, lim, dc; };   // next plane, step, exit plane, cell increment
 
 struct Walker {
     double t0, t1, t2;     // pending crossing parameter per axis (+inf: the axis never steps)
     double tcur;
     int c;                 // current cell
+    int pl0, pl1, pl2;     // next plane (low 16 bits) | plane whose crossing leaves the mesh (high 16 bits)
+    int dc0, dc1, dc2;     // signed cell-index increment of a step (sign = step direction; 0: never steps)
 };
 
 // number of entries of e[0..n) that are <= v
@@ -171,47 +178,63 @@ __device__ __forceinline__ int upper_bound_edges(const double *e, int n, double 
 }
 
 // bytes of walker state in shared memory for a CTA of `block` threads
-__host__ __device__ constexpr size_t walker_smem_bytes(int block) { return (size_t)block * 3 * (sizeof(AxisF) + sizeof(AxisI)); }
+__host__ __device__ constexpr size_t walker_smem_bytes(int block) { return (size_t)block * 3 * sizeof(AxisF); }
 
-// Returns false if the ray is rejected by the box / direction rules of O1.  axf/axi point at this
-// thread's axis-0 records; axis a is at [a * stride].
-__device__ __forceinline__ bool walker_init(Walker &w, AxisF *axf, AxisI *axi, int stride, const MeshDev &m,
-                                            const double *e, const double o[3], const double d[3])
+// position of plane p (relative index) of axis a
+template <int EDGE_MODE>
+__device__ __forceinline__ double plane_pos(const MeshDev &m, const double *e, int a, int base, int p)
+{
+    if (EDGE_MODE == EDGES_ARITH) return fma((double)p, m.h[a], m.e0[a]);
+    return e[base + p];
+}
+
+// Returns false if the ray is rejected by the box / direction rules of O1.  axf points at this thread's
+// axis-0 record; axis a is at [a * stride].  `e` = the concatenated plane table (global or shared).
+template <int EDGE_MODE>
+__device__ __forceinline__ bool walker_init(Walker &w, AxisF *axf, int stride, const MeshDev &m, const double *e,
+                                            const double o[3], const double d[3])
 {
     const int base[3] = {0, m.nx + 1, m.nx + m.ny + 2};
     const int n[3] = {m.nx, m.ny, m.nz};
     const int dcell[3] = {1, m.nx, m.nx * m.ny};
     const double inf = __longlong_as_double(0x7ff0000000000000LL);
-    int idx[3];
+    int idx[3], pl[3], dc[3];
     double t[3];
     bool movable = false;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        if (!(o[a] >= e[base[a]] && o[a] < e[base[a] + n[a]])) return false;   // half-open box (Q8)
-        idx[a] = upper_bound_edges(e + base[a], n[a] + 1, o[a]) - 1;          // O3: pure comparisons
+        const double lo = plane_pos<EDGE_MODE>(m, e, a, base[a], 0), hi = plane_pos<EDGE_MODE>(m, e, a, base[a], n[a]);
+        if (!(o[a] >= lo && o[a] < hi)) return false;                          // half-open box (Q8)
+        // O3: i = upper_bound(edges, o) - 1, by pure comparisons against the plane positions
+        int l = 0, r = n[a] + 1;
+        while (l < r) {
+            const int mid = (l + r) >> 1;
+            if (plane_pos<EDGE_MODE>(m, e, a, base[a], mid) <= o[a]) l = mid + 1; else r = mid;
+        }
+        idx[a] = l - 1;
     }
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const double dd = d[a];
         const double inv = (dd != 0.0) ? __drcp_rn(dd) : 0.0;
-        AxisI ai;
         if (dd == 0.0 || !isfinite(inv)) {                                     // Q10: the axis never steps
-            ai = AxisI{base[a], 0, -1, 0};
+            pl[a] = 0xffff << 16;
+            dc[a] = 0;
             axf[a * stride] = AxisF{o[a], 0.0};
             t[a] = inf;
         } else {
             movable = true;
             const bool up = dd > 0.0;
-            ai.p = base[a] + (up ? idx[a] + 1 : idx[a]);
-            ai.s = up ? 1 : -1;
-            ai.lim = base[a] + (up ? n[a] : 0);
-            ai.dc = up ? dcell[a] : -dcell[a];
+            const int p = up ? idx[a] + 1 : idx[a];
+            pl[a] = p | ((up ? n[a] : 0) << 16);
+            dc[a] = up ? dcell[a] : -dcell[a];
             axf[a * stride] = AxisF{o[a], inv};
-            t[a] = __dmul_rn(__dsub_rn(e[ai.p], o[a]), inv);                   // O4
+            t[a] = __dmul_rn(__dsub_rn(plane_pos<EDGE_MODE>(m, e, a, base[a], p), o[a]), inv);   // O4
         }
-        axi[a * stride] = ai;
     }
     w.t0 = t[0]; w.t1 = t[1]; w.t2 = t[2];
+    w.pl0 = pl[0]; w.pl1 = pl[1]; w.pl2 = pl[2];
+    w.dc0 = dc[0]; w.dc1 = dc[1]; w.dc2 = dc[2];
     w.tcur = 0.0;
     w.c = idx[0] + m.nx * (idx[1] + m.ny * idx[2]);
     return movable;
@@ -219,27 +242,35 @@ __device__ __forceinline__ bool walker_init(Walker &w, AxisF *axf, AxisI *axi, i
 
 // One step of the merge (O5).  On return `cell` = the cell just traversed, `len` its segment length;
 // the return value is true when the ray has left the mesh.
-__device__ __forceinline__ bool walker_step(Walker &w, AxisF *axf, AxisI *axi, int stride, const double *e,
+template <int EDGE_MODE>
+__device__ __forceinline__ bool walker_step(Walker &w, const AxisF *axf, int stride, const MeshDev &m, const double *e,
                                             int &cell, double &len)
 {
     const bool ysel = w.t1 < w.t0;                 // ties keep x
     const double tm = ysel ? w.t1 : w.t0;
     const bool zsel = w.t2 < tm;                   // ties keep x / y
     const double tn = zsel ? w.t2 : tm;
-    const int off = zsel ? 2 * stride : (ysel ? stride : 0);
-    const AxisI ai = axi[off];
-    const AxisF af = axf[off];
+    const int a = zsel ? 2 : (ysel ? 1 : 0);
+    const AxisF af = axf[a * stride];
+    const int pl = zsel ? w.pl2 : (ysel ? w.pl1 : w.pl0);
+    const int dc = zsel ? w.dc2 : (ysel ? w.dc1 : w.dc0);
     len = __dsub_rn(tn, w.tcur);
     w.tcur = tn;
     cell = w.c;
-    const bool leave = (ai.p == ai.lim);
-    const int pn = ai.p + ai.s;
-    w.c += ai.dc;
-    axi[off].p = pn;
-    const double tnew = __dmul_rn(__dsub_rn(e[leave ? ai.p : pn], af.o), af.iv);
+    const int p = pl & 0xffff;
+    const bool leave = (p == (int)((unsigned)pl >> 16));
+    const int s = dc > 0 ? 1 : -1;
+    w.c += dc;
+    const int pq = leave ? p : p + s;              // never read outside the table
+    const int base = (EDGE_MODE == EDGES_ARITH) ? 0 : (zsel ? m.nx + m.ny + 2 : (ysel ? m.nx + 1 : 0));
+    const double tnew = __dmul_rn(__dsub_rn(plane_pos<EDGE_MODE>(m, e, a, base, pq), af.o), af.iv);
+    const int pln = pl + s;
     w.t0 = (zsel || ysel) ? w.t0 : tnew;
     w.t1 = (!zsel && ysel) ? tnew : w.t1;
     w.t2 = zsel ? tnew : w.t2;
+    w.pl0 = (zsel || ysel) ? w.pl0 : pln;
+    w.pl1 = (!zsel && ysel) ? pln : w.pl1;
+    w.pl2 = zsel ? pln : w.pl2;
     return leave;
 }
 
@@ -390,26 +421,24 @@ __device__ __forceinline__ void score_terms(double S, double len, double &g, dou
 
 // ------------------------------------------------------------------------------------------------
 // The cast kernel: one thread per ray (S1 -> S6).
-//   dynamic shared memory: [edges: nedges doubles (if EDGES_SMEM)] [walker: 3 x blockDim x 32 B]
+//   dynamic shared memory: [edges: nedges doubles (EDGES_SHARED only)] [walker: 3 x blockDim x 16 B]
 //                          [sigma: M x blockDim Real]
 // ------------------------------------------------------------------------------------------------
 __host__ __device__ constexpr size_t edges_smem_bytes_for(int nedges) { return sizeof(double) * (size_t)((nedges + 1) & ~1); }
 
-template <typename Real, typename Rec, bool EDGES_SMEM>
+template <typename Real, typename Rec, int EDGE_MODE>
 __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int stride = blockDim.x;
     unsigned char *sp = smem_raw;
     double *s_edges = reinterpret_cast<double *>(sp);
-    if (EDGES_SMEM) sp += edges_smem_bytes_for(P.mesh.nedges);
+    if (EDGE_MODE == EDGES_SHARED) sp += edges_smem_bytes_for(P.mesh.nedges);
     AxisF *axf = reinterpret_cast<AxisF *>(sp) + threadIdx.x;
     sp += sizeof(AxisF) * 3 * stride;
-    AxisI *axi = reinterpret_cast<AxisI *>(sp) + threadIdx.x;
-    sp += sizeof(AxisI) * 3 * stride;
     Real *sig = reinterpret_cast<Real *>(sp) + threadIdx.x;
-    const double *e = EDGES_SMEM ? s_edges : P.mesh.edges;
-    if (EDGES_SMEM) {
+    const double *e = (EDGE_MODE == EDGES_SHARED) ? s_edges : P.mesh.edges;
+    if (EDGE_MODE == EDGES_SHARED) {
         for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
         __syncthreads();
     }
@@ -421,7 +450,7 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
         const long long r = P.perm ? (long long)__ldg(P.perm + i) : i;
         const Ray<Real> R = load_ray<Real>(P.rays, r);
         Walker w;
-        accepted = R.finite && (R.E > (Real)0) && walker_init(w, axf, axi, stride, P.mesh, e, R.o, R.d);
+        accepted = R.finite && (R.E > (Real)0) && walker_init<EDGE_MODE>(w, axf, stride, P.mesh, e, R.o, R.d);
         if (accepted) {
             // S1: every material's sigma at the ray's energy, kept in this thread's shared column
             for (int m = 0; m < P.M; ++m) sig[m * stride] = sigma_lookup<Real>(P.xs[m], R.E);
@@ -433,7 +462,7 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
             for (;;) {
                 int cell;
                 double len;
-                const bool leave = walker_step(w, axf, axi, stride, e, cell, len);
+                const bool leave = walker_step<EDGE_MODE>(w, axf, stride, P.mesh, e, cell, len);
                 const Rec cur = rec;
                 if (!leave) rec.load(P.recs, P.ids, P.K, w.c);   // next cell's record: in flight during the score
                 // S4 + S5 (Eq. (4)): score = W e^{-tau} (1 - e^{-x}) / Sigma,  x = Sigma * len
@@ -463,21 +492,19 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
 
 // ------------------------------------------------------------------------------------------------
 // The trace kernel (test entry point mr_trace_rays): the same walker, no cross sections, no tally.
-//   dynamic shared memory: [edges (if EDGES_SMEM)] [walker: 3 x blockDim x 32 B]
+//   dynamic shared memory: [edges (EDGES_SHARED only)] [walker: 3 x blockDim x 16 B]
 // ------------------------------------------------------------------------------------------------
-template <bool EDGES_SMEM>
+template <int EDGE_MODE>
 __global__ void __launch_bounds__(256) trace_kernel(const __grid_constant__ TraceParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int stride = blockDim.x;
     unsigned char *sp = smem_raw;
     double *s_edges = reinterpret_cast<double *>(sp);
-    if (EDGES_SMEM) sp += edges_smem_bytes_for(P.mesh.nedges);
+    if (EDGE_MODE == EDGES_SHARED) sp += edges_smem_bytes_for(P.mesh.nedges);
     AxisF *axf = reinterpret_cast<AxisF *>(sp) + threadIdx.x;
-    sp += sizeof(AxisF) * 3 * stride;
-    AxisI *axi = reinterpret_cast<AxisI *>(sp) + threadIdx.x;
-    const double *e = EDGES_SMEM ? s_edges : P.mesh.edges;
-    if (EDGES_SMEM) {
+    const double *e = (EDGE_MODE == EDGES_SHARED) ? s_edges : P.mesh.edges;
+    if (EDGE_MODE == EDGES_SHARED) {
         for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
         __syncthreads();
     }
@@ -495,7 +522,7 @@ __global__ void __launch_bounds__(256) trace_kernel(const __grid_constant__ Trac
         ok = R.finite && R.E > 0.0f;
     }
     Walker w;
-    ok = ok && walker_init(w, axf, axi, stride, P.mesh, e, o, d);
+    ok = ok && walker_init<EDGE_MODE>(w, axf, stride, P.mesh, e, o, d);
     unsigned nseg = 0;
     unsigned long long h = 0;
     if (ok) {
@@ -503,7 +530,7 @@ __global__ void __launch_bounds__(256) trace_kernel(const __grid_constant__ Trac
         for (;;) {
             int cell;
             double len;
-            const bool leave = walker_step(w, axf, axi, stride, e, cell, len);
+            const bool leave = walker_step<EDGE_MODE>(w, axf, stride, P.mesh, e, cell, len);
             if ((long long)nseg < P.cap) {
                 if (P.cells) P.cells[r * P.cap + nseg] = cell;
                 if (P.lens) P.lens[r * P.cap + nseg] = len;
