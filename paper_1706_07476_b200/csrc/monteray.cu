@@ -64,8 +64,18 @@ struct mr_ctx {
     void *d_recs = nullptr;
     uint8_t *d_ids = nullptr;
 
-    // tables
-    std::vector<void *> d_E, d_S;
+    // tables: sigma per material; energy grids are shared between materials whose grids are bitwise identical
+    struct Grid {
+        std::vector<unsigned char> host;  // the grid as stored on the device (fp32 or fp64 bytes)
+        void *d_E = nullptr;
+        uint32_t *d_first = nullptr;      // bucket index, nb + 1 entries (XsDesc::first)
+        uint32_t b0 = 0;
+        int sh = 0, n = 0, refs = 0, id = 0;
+    };
+    std::vector<Grid *> grids;
+    std::vector<Grid *> grid_of;          // [M]
+    int next_grid_id = 0;
+    std::vector<void *> d_S;
     std::vector<int> xs_n;
     XsDesc *d_xs = nullptr;
     bool xs_dirty = true;
@@ -151,11 +161,20 @@ void free_materials(mr_ctx *c)
     c->K = 0;
 }
 
+void unref_grid(mr_ctx *c, mr_ctx::Grid *g)
+{
+    if (!g || --g->refs > 0) return;
+    c->dev_free(g->d_E);
+    c->dev_free(g->d_first);
+    c->grids.erase(std::remove(c->grids.begin(), c->grids.end(), g), c->grids.end());
+    delete g;
+}
+
 void free_tables(mr_ctx *c)
 {
-    for (void *p : c->d_E) c->dev_free(p);
+    for (mr_ctx::Grid *g : c->grid_of) unref_grid(c, g);
     for (void *p : c->d_S) c->dev_free(p);
-    c->d_E.clear();
+    c->grid_of.clear();
     c->d_S.clear();
     c->xs_n.clear();
     c->dev_free(c->d_xs);
@@ -237,7 +256,10 @@ int upload_xs_desc(mr_ctx *c)
 {
     if (!c->xs_dirty) return MR_OK;
     std::vector<XsDesc> h(c->M);
-    for (int m = 0; m < c->M; ++m) h[m] = XsDesc{c->d_E[m], c->d_S[m], c->xs_n[m], 0};
+    for (int m = 0; m < c->M; ++m) {
+        const mr_ctx::Grid *g = c->grid_of[m];
+        h[m] = XsDesc{g->d_E, c->d_S[m], c->xs_n[m], g->id, g->d_first, g->b0, g->sh};
+    }
     if (!c->d_xs) {
         c->d_xs = (XsDesc *)c->dev_alloc(sizeof(XsDesc) * MR_MAX_MATERIALS);
         if (!c->d_xs) return c->fail(MR_ERR_OOM, "device allocation failed (table descriptors)");
@@ -592,7 +614,7 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
     c->K = K;
     if (M != c->M || (int)c->xs_n.size() != M) {
         c->M = M;
-        c->d_E.assign(M, nullptr);
+        c->grid_of.assign(M, nullptr);
         c->d_S.assign(M, nullptr);
         c->xs_n.assign(M, 0);
         c->xs_dirty = true;
@@ -623,25 +645,71 @@ int mr_load_xs(mr_ctx *c, int material, int64_t n, const double *energy, const d
     }
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
     const size_t bytes = (size_t)n * c->real_bytes();
-    void *dE = c->dev_alloc(bytes), *dS = c->dev_alloc(bytes);
-    if (!dE || !dS) {
-        c->dev_free(dE);
-        c->dev_free(dS);
-        return c->fail(MR_ERR_OOM, "device allocation failed (cross-section table)");
-    }
     const void *hE = dbl ? (const void *)energy : (const void *)ef.data();
     const void *hS = dbl ? (const void *)sigma_t : (const void *)sf.data();
-    cudaError_t e = cudaMemcpyAsync(dE, hE, bytes, cudaMemcpyHostToDevice, c->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dS, hS, bytes, cudaMemcpyHostToDevice, c->stream);
+
+    // the energy grid: reuse a resident one if it is bitwise identical, else upload it with its bucket index
+    mr_ctx::Grid *g = nullptr;
+    for (mr_ctx::Grid *q : c->grids)
+        if (q->n == (int)n && q->host.size() == bytes && std::memcmp(q->host.data(), hE, bytes) == 0) { g = q; break; }
+    bool new_grid = false;
+    std::vector<uint32_t> first;
+    if (!g) {
+        new_grid = true;
+        g = new mr_ctx::Grid();
+        g->n = (int)n;
+        g->host.assign((const unsigned char *)hE, (const unsigned char *)hE + bytes);
+        // bucket(E) = (bits((float)E) >> sh) - b0: positive floats order like their bit patterns and double -> float
+        // rounding is monotone, so bucket() is non-decreasing in E in both precision modes
+        auto fbits = [&](int64_t i) {
+            const float f = dbl ? (float)energy[i] : ef[i];
+            uint32_t u;
+            std::memcpy(&u, &f, 4);
+            return u;
+        };
+        const uint32_t lo_bits = fbits(0), hi_bits = fbits(n - 1);
+        const uint64_t want = std::min<uint64_t>(std::max<uint64_t>(2 * (uint64_t)n, 1024), 1u << 20);
+        int sh = 0;
+        while ((uint64_t)(hi_bits >> sh) - (lo_bits >> sh) + 1 > want) ++sh;
+        g->sh = sh;
+        g->b0 = lo_bits >> sh;
+        const uint32_t nb = (hi_bits >> sh) - g->b0 + 1;
+        first.assign((size_t)nb + 1, 0);
+        for (int64_t i = 0; i < n; ++i) first[(fbits(i) >> sh) - g->b0 + 1] += 1;   // counts, shifted by one
+        for (uint32_t b2 = 0; b2 < nb; ++b2) first[b2 + 1] += first[b2];            // first[b] = #points with bucket < b
+        g->d_E = c->dev_alloc(bytes);
+        g->d_first = (uint32_t *)c->dev_alloc(first.size() * sizeof(uint32_t));
+    }
+    void *dS = c->dev_alloc(bytes);
+    auto drop_new = [&]() {
+        if (new_grid) {
+            c->dev_free(g->d_E);
+            c->dev_free(g->d_first);
+            delete g;
+        }
+        c->dev_free(dS);
+    };
+    if (!dS || !g->d_E || !g->d_first) {
+        drop_new();
+        return c->fail(MR_ERR_OOM, "device allocation failed (cross-section table)");
+    }
+    cudaError_t e = cudaMemcpyAsync(dS, hS, bytes, cudaMemcpyHostToDevice, c->stream);
+    if (new_grid && e == cudaSuccess) e = cudaMemcpyAsync(g->d_E, hE, bytes, cudaMemcpyHostToDevice, c->stream);
+    if (new_grid && e == cudaSuccess)
+        e = cudaMemcpyAsync(g->d_first, first.data(), first.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) {
-        c->dev_free(dE);
-        c->dev_free(dS);
+        drop_new();
         return c->fail_cuda(e, "mr_load_xs");
     }
-    c->dev_free(c->d_E[material]);
+    if (new_grid) {
+        g->id = c->next_grid_id++;
+        c->grids.push_back(g);
+    }
+    g->refs += 1;
+    unref_grid(c, c->grid_of[material]);   // the table this call replaces, if any
     c->dev_free(c->d_S[material]);
-    c->d_E[material] = dE;
+    c->grid_of[material] = g;
     c->d_S[material] = dS;
     c->xs_n[material] = (int)n;
     c->xs_dirty = true;

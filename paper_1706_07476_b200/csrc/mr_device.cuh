@@ -16,7 +16,12 @@ struct XsDesc {            // one material's table (device pointers)
     const void *E;         // float[n] (mixed) or double[n]
     const void *S;
     int n;
-    int pad;
+    int grid;              // materials whose energy grids are bitwise identical share a grid id (and E, first)
+    // bucket index of the grid (the paper's hash-based lookup): bucket(E) = (bits((float)E) >> sh) - b0
+    // is non-decreasing in E; first[b] = number of grid points whose bucket is < b, for b = 0..nb
+    const uint32_t *first;
+    uint32_t b0;
+    int sh;
 };
 
 enum CellLayout : int {
@@ -120,26 +125,47 @@ template <> __device__ __forceinline__ Ray<float> load_ray<float>(const void *ra
 template <> __device__ __forceinline__ Ray<double> load_ray<double>(const void *rays, long long r) { return load_ray_f64(rays, r); }
 
 // ------------------------------------------------------------------------------------------------
-// S1: sigma_m(E), lin-lin interpolation in a table, end values outside (Q5)
+// S1: sigma_m(E), lin-lin interpolation in a table, end values outside (Q5).
+// The bracket k (E_k <= E < E_{k+1}) is the one a plain upper_bound gives (reading Q4); the bucket index
+// only narrows the range the binary search starts from: every grid point in a lower bucket is < E and
+// every point in a higher bucket is > E because bucket() is monotone.  Materials that share a grid share
+// the bracket and the interpolation weight, so the search runs once per distinct grid.
 // ------------------------------------------------------------------------------------------------
 template <typename Real>
-__device__ __forceinline__ Real sigma_lookup(const XsDesc &t, Real E)
+struct Bracket {
+    int k;       // -1: E below the grid (or n == 1), -2: E at or above the last point, else the bracket
+    Real t01;    // (E - E_k) / (E_{k+1} - E_k)
+};
+
+template <typename Real>
+__device__ __forceinline__ Bracket<Real> find_bracket(const XsDesc &t, Real E)
 {
     const Real *__restrict__ Eg = reinterpret_cast<const Real *>(t.E);
-    const Real *__restrict__ Sg = reinterpret_cast<const Real *>(t.S);
     const int n = t.n;
-    if (n == 1 || E < __ldg(Eg)) return __ldg(Sg);
-    if (E >= __ldg(Eg + n - 1)) return __ldg(Sg + n - 1);
-    int lo = 1, hi = n - 1;  // invariant: Eg[lo-1] <= E < Eg[hi]
-    while (lo < hi) {
-        int mid = (lo + hi) >> 1;
+    Bracket<Real> b;
+    b.t01 = (Real)0;
+    if (n == 1 || E < __ldg(Eg)) { b.k = -1; return b; }
+    if (E >= __ldg(Eg + n - 1)) { b.k = -2; return b; }
+    const uint32_t bk = (__float_as_uint((float)E) >> t.sh) - t.b0;
+    int lo = max((int)__ldg(t.first + bk), 1), hi = min((int)__ldg(t.first + bk + 1), n - 1);
+    while (lo < hi) {        // invariant: Eg[lo-1] <= E < Eg[hi]
+        const int mid = (lo + hi) >> 1;
         if (__ldg(Eg + mid) <= E) lo = mid + 1; else hi = mid;
     }
-    const int k = lo - 1;    // Eg[k] <= E < Eg[k+1], 0 <= k <= n-2
-    const Real e0 = __ldg(Eg + k), e1 = __ldg(Eg + k + 1);
-    const Real s0 = __ldg(Sg + k), s1 = __ldg(Sg + k + 1);
-    const Real t01 = (E - e0) / (e1 - e0);
-    return s0 + t01 * (s1 - s0);
+    b.k = lo - 1;            // Eg[k] <= E < Eg[k+1], 0 <= k <= n-2
+    const Real e0 = __ldg(Eg + b.k), e1 = __ldg(Eg + b.k + 1);
+    b.t01 = (E - e0) / (e1 - e0);
+    return b;
+}
+
+template <typename Real>
+__device__ __forceinline__ Real sigma_at(const XsDesc &t, const Bracket<Real> &b)
+{
+    const Real *__restrict__ Sg = reinterpret_cast<const Real *>(t.S);
+    if (b.k == -1) return __ldg(Sg);
+    if (b.k == -2) return __ldg(Sg + t.n - 1);
+    const Real s0 = __ldg(Sg + b.k), s1 = __ldg(Sg + b.k + 1);
+    return s0 + b.t01 * (s1 - s0);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -453,7 +479,13 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
         accepted = R.finite && (R.E > (Real)0) && walker_init<EDGE_MODE>(w, axf, stride, P.mesh, e, R.o, R.d);
         if (accepted) {
             // S1: every material's sigma at the ray's energy, kept in this thread's shared column
-            for (int m = 0; m < P.M; ++m) sig[m * stride] = sigma_lookup<Real>(P.xs[m], R.E);
+            Bracket<Real> br;
+            int grid = -1;
+            for (int m = 0; m < P.M; ++m) {
+                const XsDesc t = P.xs[m];
+                if (t.grid != grid) { br = find_bracket<Real>(t, R.E); grid = t.grid; }
+                sig[m * stride] = sigma_at<Real>(t, br);
+            }
 
             double wa = R.W;   // W * exp(-tau), a running product of exp(-x)
             double *const tally = P.tally;
