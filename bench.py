@@ -184,6 +184,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--sort", type=int, default=-1, help="override MR_OPT_SORT_RAYS (default: library default)")
+    ap.add_argument("--opt", action="append", default=[], help="library option as ID=VALUE (MR_OPT_* of include/monteray.h), repeatable")
+    ap.add_argument("--stage-rays", type=int, default=0, help="override MR_OPT_STAGE_RAYS (rays per H2D chunk of a host batch)")
     args = ap.parse_args()
     prob_kw = {}
 
@@ -193,7 +195,7 @@ def main():
     import numpy as np
     import torch
 
-    from paper_1706_07476_b200 import MR_OPT_BLOCK_THREADS, MR_OPT_SORT_RAYS, MonteRay, multi
+    from paper_1706_07476_b200 import MR_OPT_BLOCK_THREADS, MR_OPT_SORT_RAYS, MR_OPT_STAGE_RAYS, MonteRay, multi
     from workloads import CONFIG_NAMES, FULL_RAYS, make_problem, make_rays
 
     rank, local_rank, world = multi.env_rank_world()
@@ -213,6 +215,11 @@ def main():
         m.set_option(MR_OPT_BLOCK_THREADS, args.block_threads)
     if args.sort >= 0:
         m.set_option(MR_OPT_SORT_RAYS, args.sort)
+    if args.stage_rays:
+        m.set_option(MR_OPT_STAGE_RAYS, args.stage_rays)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        m.set_option(int(k), int(v))
     d_rays = torch.from_numpy(rays).to(dev)
     h_rays = torch.from_numpy(rays).pin_memory()
     h_tally = torch.empty(prob.ncell, dtype=torch.float64).pin_memory()

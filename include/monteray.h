@@ -145,7 +145,8 @@ MR_API int mr_load_xs(mr_ctx *ctx, int material, int64_t n, const double *energy
  * until the ray leaves the mesh (no cut-off, no reflection: readings Q7, F5).  A ray is
  * REJECTED (counted, no contribution) if any field is not finite, E <= 0, the direction is
  * the zero vector, or the origin is outside the half-open box [lo, hi) on any axis.
- * Asynchronous: returns once the batch is staged and the work is queued.  n = 0 is a no-op.
+ * Asynchronous: returns once the batch is staged (a host buffer has been copied out of, or,
+ * if it is page-locked, DMA'd out of) and the work is queued.  n = 0 is a no-op.
  * Requires mesh, materials and all M tables.  Errors: INVALID_ARG, STATE, OOM, CUDA. */
 MR_API int mr_cast_rays(mr_ctx *ctx, int64_t n, const void *rays, int where);
 
@@ -181,7 +182,9 @@ MR_API int mr_trace_rays(mr_ctx *ctx, int64_t n, const void *rays, int where, ui
 enum {
     MR_OPT_BLOCK_THREADS = 1, /* threads per CTA of the cast kernel (multiple of 32, <= 256) */
     MR_OPT_SORT_RAYS = 2,     /* 0: cast in buffer order; 1: bin rays by start slab and length first */
-    MR_OPT_STAGE_RAYS = 3     /* rays per pinned staging chunk for host batches */
+    MR_OPT_STAGE_RAYS = 3,    /* rays per staging chunk for host batches (H2D of chunk i+1 overlaps the cast of chunk i) */
+    MR_OPT_COPY_THREADS = 4,  /* host threads that copy a PAGEABLE batch into the pinned ring (a pinned batch is DMA'd directly) */
+    MR_OPT_PAIR_RECORDS = 5   /* 1: 16-byte cell records (K = 2, 3, MIXED) are fetched as 32-byte pairs kept in registers; 0: one by one */
 };
 MR_API int mr_set_option(mr_ctx *ctx, int option, int64_t value);
 MR_API int mr_get_option(mr_ctx *ctx, int option, int64_t *value);

@@ -8,6 +8,8 @@ from .binding import (  # noqa: F401
     EXPORTS,
     LIB_PATH,
     MR_OPT_BLOCK_THREADS,
+    MR_OPT_COPY_THREADS,
+    MR_OPT_PAIR_RECORDS,
     MR_OPT_SORT_RAYS,
     MR_OPT_STAGE_RAYS,
     MR_PRECISION_DOUBLE,

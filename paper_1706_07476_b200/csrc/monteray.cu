@@ -12,6 +12,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <thread>
 #include <vector>
 
 #define MR_PACK_MAX_SLOTS MR_MAX_SLOTS
@@ -90,6 +91,7 @@ struct mr_ctx {
     size_t stage_cap_rays = 0;       // rays each slot can hold now
     long long stage_rays = 1 << 21;  // option MR_OPT_STAGE_RAYS
     int next_slot = 0;
+    int copy_threads = 4;            // option MR_OPT_COPY_THREADS
 
     cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;
     bool have_timing = false;
@@ -98,6 +100,7 @@ struct mr_ctx {
     long long launches = 0;
     int block_threads = 128;
     int sort_rays = 1;
+    int pair_records = 1;            // option MR_OPT_PAIR_RECORDS
 
     // ray-ordering pre-pass scratch (grown on demand)
     uint32_t *d_keys = nullptr, *d_perm = nullptr, *d_hist = nullptr;
@@ -357,8 +360,8 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     if (c->precision == MR_PRECISION_DOUBLE) rc = launch_cast_t<double, CellRecGeneric<double>>(c, P);
     else switch (c->layout) {
     case LAYOUT_K1: rc = launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P); break;
-    case LAYOUT_K2: rc = launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
-    case LAYOUT_K3: rc = launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P); break;
+    case LAYOUT_K2: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
+    case LAYOUT_K3: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K3P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P); break;
     case LAYOUT_K4: rc = launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P); break;
     case LAYOUT_D8: rc = launch_cast_t<float, CellRec<LAYOUT_D8>>(c, P); break;
     default: rc = launch_cast_t<float, CellRecGeneric<float>>(c, P);
@@ -369,15 +372,41 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     return MR_OK;
 }
 
-int ensure_stage(mr_ctx *c, size_t rays_per_slot)
+// parallel host copy into a pinned staging slot (a single memcpy thread moves ~10 GB/s, less than the PCIe link)
+void host_copy(void *dst, const void *src, size_t bytes, int threads)
 {
-    if (c->stage_cap_rays >= rays_per_slot) return MR_OK;
+    const size_t kMinPerThread = 4u << 20;
+    int t = (int)std::min<size_t>((size_t)std::max(1, threads), bytes / kMinPerThread);
+    if (t <= 1) {
+        std::memcpy(dst, src, bytes);
+        return;
+    }
+    std::vector<std::thread> pool;
+    const size_t piece = ((bytes / t) + 4095) & ~(size_t)4095;
+    for (int i = 1; i < t; ++i) {
+        const size_t off = (size_t)i * piece;
+        if (off >= bytes) break;
+        const size_t len = std::min(piece, bytes - off);
+        pool.emplace_back([=]() { std::memcpy((char *)dst + off, (const char *)src + off, len); });
+    }
+    std::memcpy(dst, src, std::min(piece, bytes));
+    for (std::thread &th : pool) th.join();
+}
+
+// Grows the staging ring to `rays_per_slot` rays per slot; the pinned host halves are only allocated when a
+// pageable batch needs them.
+int ensure_stage(mr_ctx *c, size_t rays_per_slot, bool need_pinned)
+{
+    const bool have_pinned = c->pinned[0] != nullptr;
+    if (c->stage_cap_rays >= rays_per_slot && (have_pinned || !need_pinned)) return MR_OK;
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
     MR_CUDA(c, cudaStreamSynchronize(c->copy_stream));
+    const size_t cap = std::max(c->stage_cap_rays, rays_per_slot);
+    const bool want_pinned = need_pinned || have_pinned;
     free_stage(c);
-    const size_t bytes = rays_per_slot * c->ray_bytes();
+    const size_t bytes = cap * c->ray_bytes();
     for (int s = 0; s < kStageSlots; ++s) {
-        if (cudaMallocHost(&c->pinned[s], bytes) != cudaSuccess) {
+        if (want_pinned && cudaMallocHost(&c->pinned[s], bytes) != cudaSuccess) {
             cudaGetLastError();
             free_stage(c);
             return c->fail(MR_ERR_OOM, "pinned host allocation failed (staging ring)");
@@ -388,7 +417,7 @@ int ensure_stage(mr_ctx *c, size_t rays_per_slot)
             return c->fail(MR_ERR_OOM, "device allocation failed (staging ring)");
         }
     }
-    c->stage_cap_rays = rays_per_slot;
+    c->stage_cap_rays = cap;
     return MR_OK;
 }
 
@@ -569,7 +598,7 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
     default: rec_bytes = (size_t)K * (dbl ? 8 : 4); id_bytes = (size_t)K;
     }
     const long long chunk = std::min<long long>(c->ncell, 1LL << 22);
-    void *recs = c->dev_alloc(rec_bytes * c->ncell);
+    void *recs = c->dev_alloc(rec_bytes * (c->ncell + 1));   // + 1: 16-byte records are read as aligned pairs
     uint8_t *ids = id_bytes ? (uint8_t *)c->dev_alloc(id_bytes * c->ncell) : nullptr;
     int32_t *s_mat = (int32_t *)c->dev_alloc(sizeof(int32_t) * chunk * K);
     double *s_frac = (double *)c->dev_alloc(sizeof(double) * chunk * K);
@@ -733,28 +762,52 @@ int mr_cast_rays(mr_ctx *c, int64_t n, const void *rays, int where)
         c->have_timing = true;
         return MR_OK;
     }
-    // Host batch: chunks go through a 2-slot pinned ring; the H2D copy of chunk i+1 (copy stream)
-    // overlaps the kernel of chunk i (context stream), and the host memcpy overlaps both.
-    const size_t per = (size_t)std::max<long long>(1024, std::min<long long>(c->stage_rays, n));
-    if (int rc = ensure_stage(c, per)) return rc;
+    // Host batch, in chunks of MR_OPT_STAGE_RAYS rays through a 2-slot device ring: the H2D copy of chunk i+1
+    // (copy stream) overlaps the kernels of chunk i (context stream) -- the CPU/GPU overlap of Fig. 4
+    // inside one call.  A pinned (page-locked) caller buffer is the DMA source itself; a
+    // pageable one is first copied, by a few host threads, into a pinned ring slot.
     const size_t rb = c->ray_bytes();
+    const size_t per = (size_t)std::max<long long>(1024, std::min<long long>(c->stage_rays, n));
+    bool pinned_src = false;
+    {
+        cudaPointerAttributes at{};
+        if (cudaPointerGetAttributes(&at, rays) == cudaSuccess) pinned_src = (at.type == cudaMemoryTypeHost);
+        else cudaGetLastError();
+        if (pinned_src) {   // the whole batch must lie inside the registered range
+            cudaPointerAttributes at2{};
+            const char *last = (const char *)rays + (size_t)n * rb - 1;
+            if (cudaPointerGetAttributes(&at2, last) != cudaSuccess || at2.type != cudaMemoryTypeHost) {
+                cudaGetLastError();
+                pinned_src = false;
+            }
+        }
+    }
+    if (int rc = ensure_stage(c, per, !pinned_src)) return rc;
     MR_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
     const int64_t chunk = (int64_t)std::min<size_t>(c->stage_cap_rays, per);
+    int last_slot = -1;
     for (int64_t first = 0; first < n; first += chunk) {
         const int64_t count = std::min<int64_t>(chunk, n - first);
         const int s = c->next_slot;
         c->next_slot = (s + 1) % kStageSlots;
-        MR_CUDA(c, cudaEventSynchronize(c->ev_copied[s]));           // pinned slot free again
-        std::memcpy(c->pinned[s], (const char *)rays + (size_t)first * rb, (size_t)count * rb);
+        const char *src = (const char *)rays + (size_t)first * rb;
+        if (!pinned_src) {
+            MR_CUDA(c, cudaEventSynchronize(c->ev_copied[s]));       // pinned slot free again
+            host_copy(c->pinned[s], src, (size_t)count * rb, c->copy_threads);
+            src = (const char *)c->pinned[s];
+        }
         MR_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_done[s], 0));  // device slot free again
-        MR_CUDA(c, cudaMemcpyAsync(c->d_stage[s], c->pinned[s], (size_t)count * rb, cudaMemcpyHostToDevice, c->copy_stream));
+        MR_CUDA(c, cudaMemcpyAsync(c->d_stage[s], src, (size_t)count * rb, cudaMemcpyHostToDevice, c->copy_stream));
         MR_CUDA(c, cudaEventRecord(c->ev_copied[s], c->copy_stream));
         MR_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied[s], 0));
         if (int rc = cast_device(c, count, c->d_stage[s])) return rc;
         MR_CUDA(c, cudaEventRecord(c->ev_done[s], c->stream));
+        last_slot = s;
     }
     MR_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
     c->have_timing = true;
+    // the caller's buffer is consumed when the call returns: wait for the last DMA out of it
+    if (pinned_src && last_slot >= 0) MR_CUDA(c, cudaEventSynchronize(c->ev_copied[last_slot]));
     return MR_OK;
 }
 
@@ -896,6 +949,14 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         if (value < 1024 || value > (1LL << 26)) return c->fail(MR_ERR_INVALID_ARG, "staging chunk must be in [1024, 2^26] rays");
         c->stage_rays = value;
         return MR_OK;
+    case MR_OPT_PAIR_RECORDS:
+        if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "pair-records option is 0 or 1");
+        c->pair_records = (int)value;
+        return MR_OK;
+    case MR_OPT_COPY_THREADS:
+        if (value < 1 || value > 64) return c->fail(MR_ERR_INVALID_ARG, "copy threads must be in [1, 64]");
+        c->copy_threads = (int)value;
+        return MR_OK;
     }
     return c->fail(MR_ERR_INVALID_ARG, "unknown option");
 }
@@ -908,6 +969,8 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     case MR_OPT_BLOCK_THREADS: *value = c->block_threads; return MR_OK;
     case MR_OPT_SORT_RAYS: *value = c->sort_rays; return MR_OK;
     case MR_OPT_STAGE_RAYS: *value = c->stage_rays; return MR_OK;
+    case MR_OPT_COPY_THREADS: *value = c->copy_threads; return MR_OK;
+    case MR_OPT_PAIR_RECORDS: *value = c->pair_records; return MR_OK;
     }
     return c->fail(MR_ERR_INVALID_ARG, "unknown option");
 }

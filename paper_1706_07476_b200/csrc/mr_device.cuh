@@ -30,6 +30,8 @@ enum CellLayout : int {
     LAYOUT_K3 = 3,         // 16 B {float r0,r1,r2; u32 ids}
     LAYOUT_K4 = 4,         // 32 B {float r0..r3; u32 ids; u32 pad[3]}
     LAYOUT_D8 = 8,         // 32 B {float r[8]}  dense: slot k holds material k
+    LAYOUT_K2P = 12,       // kernel-side only: LAYOUT_K2 / LAYOUT_K3 records fetched as 32-byte pairs
+    LAYOUT_K3P = 13,
     LAYOUT_GENERIC = 100   // coef[ncell*K] (float or double) + ids[ncell*K] (u8, 0xff = empty)
 };
 
@@ -77,6 +79,14 @@ __device__ __forceinline__ float4 ldg_f4(const void *p) { return __ldg(reinterpr
 __device__ __forceinline__ uint4 ldg_u4(const void *p) { return __ldg(reinterpret_cast<const uint4 *>(p)); }
 __device__ __forceinline__ uint2 ldg_u2(const void *p) { return __ldg(reinterpret_cast<const uint2 *>(p)); }
 __device__ __forceinline__ double2 ldg_d2(const void *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
+
+// 32-byte read-only load (LDG.E.256 on sm_100a); p must be 32-byte aligned
+__device__ __forceinline__ void ldg_256(const void *p, uint4 &lo, uint4 &hi)
+{
+    asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(lo.x), "=r"(lo.y), "=r"(lo.z), "=r"(lo.w), "=r"(hi.x), "=r"(hi.y), "=r"(hi.z), "=r"(hi.w)
+                 : "l"(p));
+}
 
 // fp64 reduction into global memory without a return value (RED.E.ADD.F64 in SASS)
 __device__ __forceinline__ void red_add_f64(double *addr, double v)
@@ -304,84 +314,129 @@ __device__ __forceinline__ bool walker_step(Walker &w, const AxisF *axf, int str
 // S4: total cross section of a cell from its record and the ray's per-material sigma values.
 // sig[m * stride] is sigma of material m for this thread (shared memory, conflict-free).
 // ------------------------------------------------------------------------------------------------
+// Interface of a record type (the kernel is a template over it):
+//   reset()                      once per ray
+//   load(recs, ids, K, c)        start fetching cell c's record (issued one step ahead of its use)
+//   value()                      the fetched record of the cell last passed to load(), as a small value
+//   sigma(value, sig, stride, K) Sigma_t of that cell
 template <int LAYOUT> struct CellRec;
 
 template <> struct CellRec<LAYOUT_K1> {
+    typedef uint2 Value;
     uint2 v;
+    __device__ __forceinline__ void reset() {}
     __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c) { v = ldg_u2(reinterpret_cast<const uint2 *>(recs) + c); }
-    __device__ __forceinline__ float sigma(const float *sig, int stride, int) const { return __uint_as_float(v.x) * sig[v.y * stride]; }
+    __device__ __forceinline__ Value value() const { return v; }
+    static __device__ __forceinline__ float sigma(const Value &v, const float *sig, int stride, int) { return __uint_as_float(v.x) * sig[v.y * stride]; }
 };
-template <> struct CellRec<LAYOUT_K2> {
+
+// 16-byte records (K = 2, 3) are fetched as 32-byte aligned PAIRS (cells 2j, 2j+1: x neighbours) with one
+// LDG.E.256 and the pair is kept in registers: a step in x that stays inside the pair (about a quarter of
+// all steps on a mesh with square xy cells) needs no load at all.  The kernel is bound by L1TEX wavefronts
+// (one per lane for an uncoalesced access), so every load not issued is time saved.
+struct PairRec {
+    uint4 a, b;
+    int tag;       // index of the resident pair, -1: none
+    bool odd;      // which half the current cell is
+    __device__ __forceinline__ void reset() { tag = -1; }
+    __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c)
+    {
+        odd = c & 1;
+        if ((c >> 1) != tag) {
+            tag = c >> 1;
+            ldg_256(reinterpret_cast<const uint4 *>(recs) + 2 * (size_t)tag, a, b);
+        }
+    }
+    __device__ __forceinline__ uint4 value() const { return odd ? b : a; }
+};
+struct SingleRec {
     uint4 v;
+    __device__ __forceinline__ void reset() {}
     __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c) { v = ldg_u4(reinterpret_cast<const uint4 *>(recs) + c); }
-    __device__ __forceinline__ float sigma(const float *sig, int stride, int) const
+    __device__ __forceinline__ uint4 value() const { return v; }
+};
+template <typename Fetch> struct RecK2 : Fetch {
+    typedef uint4 Value;
+    static __device__ __forceinline__ float sigma(const Value &v, const float *sig, int stride, int)
     {
         float s = __uint_as_float(v.x) * sig[(v.z & 0xffu) * stride];
         return fmaf(__uint_as_float(v.y), sig[((v.z >> 8) & 0xffu) * stride], s);
     }
 };
-template <> struct CellRec<LAYOUT_K3> {
-    uint4 v;
-    __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c) { v = ldg_u4(reinterpret_cast<const uint4 *>(recs) + c); }
-    __device__ __forceinline__ float sigma(const float *sig, int stride, int) const
+template <typename Fetch> struct RecK3 : Fetch {
+    typedef uint4 Value;
+    static __device__ __forceinline__ float sigma(const Value &v, const float *sig, int stride, int)
     {
         float s = __uint_as_float(v.x) * sig[(v.w & 0xffu) * stride];
         s = fmaf(__uint_as_float(v.y), sig[((v.w >> 8) & 0xffu) * stride], s);
         return fmaf(__uint_as_float(v.z), sig[((v.w >> 16) & 0xffu) * stride], s);
     }
 };
+template <> struct CellRec<LAYOUT_K2> : RecK2<SingleRec> {};
+template <> struct CellRec<LAYOUT_K3> : RecK3<SingleRec> {};
+template <> struct CellRec<LAYOUT_K2P> : RecK2<PairRec> {};
+template <> struct CellRec<LAYOUT_K3P> : RecK3<PairRec> {};
 template <> struct CellRec<LAYOUT_K4> {
-    uint4 v;
-    uint32_t ids;
+    struct Value { uint4 v; uint32_t ids; };
+    Value q;
+    __device__ __forceinline__ void reset() {}
     __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c)
     {
         const uint4 *p = reinterpret_cast<const uint4 *>(recs) + 2 * (size_t)c;
-        v = ldg_u4(p);
-        ids = __ldg(reinterpret_cast<const uint32_t *>(p + 1));
+        q.v = ldg_u4(p);
+        q.ids = __ldg(reinterpret_cast<const uint32_t *>(p + 1));
     }
-    __device__ __forceinline__ float sigma(const float *sig, int stride, int) const
+    __device__ __forceinline__ Value value() const { return q; }
+    static __device__ __forceinline__ float sigma(const Value &q, const float *sig, int stride, int)
     {
-        float s = __uint_as_float(v.x) * sig[(ids & 0xffu) * stride];
-        s = fmaf(__uint_as_float(v.y), sig[((ids >> 8) & 0xffu) * stride], s);
-        s = fmaf(__uint_as_float(v.z), sig[((ids >> 16) & 0xffu) * stride], s);
-        return fmaf(__uint_as_float(v.w), sig[(ids >> 24) * stride], s);
+        float s = __uint_as_float(q.v.x) * sig[(q.ids & 0xffu) * stride];
+        s = fmaf(__uint_as_float(q.v.y), sig[((q.ids >> 8) & 0xffu) * stride], s);
+        s = fmaf(__uint_as_float(q.v.z), sig[((q.ids >> 16) & 0xffu) * stride], s);
+        return fmaf(__uint_as_float(q.v.w), sig[(q.ids >> 24) * stride], s);
     }
 };
 template <> struct CellRec<LAYOUT_D8> {
-    float4 a, b;
+    struct Value { float4 a, b; };
+    Value q;
+    __device__ __forceinline__ void reset() {}
     __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c)
     {
-        const float4 *p = reinterpret_cast<const float4 *>(recs) + 2 * (size_t)c;
-        a = __ldg(p); b = __ldg(p + 1);
+        uint4 lo, hi;
+        ldg_256(reinterpret_cast<const uint4 *>(recs) + 2 * (size_t)c, lo, hi);
+        q.a = make_float4(__uint_as_float(lo.x), __uint_as_float(lo.y), __uint_as_float(lo.z), __uint_as_float(lo.w));
+        q.b = make_float4(__uint_as_float(hi.x), __uint_as_float(hi.y), __uint_as_float(hi.z), __uint_as_float(hi.w));
     }
-    __device__ __forceinline__ float sigma(const float *sig, int stride, int) const
+    __device__ __forceinline__ Value value() const { return q; }
+    static __device__ __forceinline__ float sigma(const Value &q, const float *sig, int stride, int)
     {
-        float s = a.x * sig[0];
-        s = fmaf(a.y, sig[stride], s);
-        s = fmaf(a.z, sig[2 * stride], s);
-        s = fmaf(a.w, sig[3 * stride], s);
-        s = fmaf(b.x, sig[4 * stride], s);
-        s = fmaf(b.y, sig[5 * stride], s);
-        s = fmaf(b.z, sig[6 * stride], s);
-        return fmaf(b.w, sig[7 * stride], s);
+        float s = q.a.x * sig[0];
+        s = fmaf(q.a.y, sig[stride], s);
+        s = fmaf(q.a.z, sig[2 * stride], s);
+        s = fmaf(q.a.w, sig[3 * stride], s);
+        s = fmaf(q.b.x, sig[4 * stride], s);
+        s = fmaf(q.b.y, sig[5 * stride], s);
+        s = fmaf(q.b.z, sig[6 * stride], s);
+        return fmaf(q.b.w, sig[7 * stride], s);
     }
 };
 
 // Generic layout, either precision: nothing is prefetched, the slots are read in sigma().
 template <typename Real> struct CellRecGeneric {
-    const Real *coef;
-    const uint8_t *ids;
+    struct Value { const Real *coef; const uint8_t *ids; };
+    Value q;
+    __device__ __forceinline__ void reset() {}
     __device__ __forceinline__ void load(const void *recs, const uint8_t *idp, int K, int c)
     {
-        coef = reinterpret_cast<const Real *>(recs) + (size_t)c * K;
-        ids = idp + (size_t)c * K;
+        q.coef = reinterpret_cast<const Real *>(recs) + (size_t)c * K;
+        q.ids = idp + (size_t)c * K;
     }
-    __device__ __forceinline__ Real sigma(const Real *sig, int stride, int K) const
+    __device__ __forceinline__ Value value() const { return q; }
+    static __device__ __forceinline__ Real sigma(const Value &q, const Real *sig, int stride, int K)
     {
         Real s = 0;
         for (int k = 0; k < K; ++k) {
-            const unsigned id = __ldg(ids + k);
-            if (id != 0xffu) s += __ldg(coef + k) * sig[id * stride];
+            const unsigned id = __ldg(q.ids + k);
+            if (id != 0xffu) s += __ldg(q.coef + k) * sig[id * stride];
         }
         return s;
     }
@@ -490,15 +545,16 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
             double wa = R.W;   // W * exp(-tau), a running product of exp(-x)
             double *const tally = P.tally;
             Rec rec;
+            rec.reset();
             rec.load(P.recs, P.ids, P.K, w.c);
             for (;;) {
                 int cell;
                 double len;
                 const bool leave = walker_step<EDGE_MODE>(w, axf, stride, P.mesh, e, cell, len);
-                const Rec cur = rec;
+                const typename Rec::Value cur = rec.value();
                 if (!leave) rec.load(P.recs, P.ids, P.K, w.c);   // next cell's record: in flight during the score
                 // S4 + S5 (Eq. (4)): score = W e^{-tau} (1 - e^{-x}) / Sigma,  x = Sigma * len
-                const double S = (double)cur.sigma(sig, stride, P.K);
+                const double S = (double)Rec::sigma(cur, sig, stride, P.K);
                 double g, ex;
                 score_terms<sizeof(Real) == 8>(S, len, g, ex);
                 // S6 (a zero-length segment scores exactly 0: nothing to add)
