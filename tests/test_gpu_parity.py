@@ -154,6 +154,31 @@ def test_shaped_workloads_double(cfg, n_rays, kw):
     check_case(prob, rays, 1)
 
 
+# ------------------------------------------------------------------------------------- full sizes, bench launch configuration
+@pytest.mark.parametrize("cfg", [2, 3, 5, 4])
+def test_full_size_configs_in_bench_configuration(cfg):
+    """BASELINE.json's full sizes (config 4: one of its 10^6-ray batches on the full 512^3 mesh), library
+    defaults = the launch configuration bench.py times (ray-ordering pre-pass on, device-resident batch):
+    every ray's segment count and cell-sequence hash, the counters and the WHOLE tally against the oracle."""
+    import torch
+
+    from workloads import FULL_RAYS
+
+    prob = make_problem(cfg)
+    rays = make_rays(prob, FULL_RAYS[cfg])
+    ref = _oracle(prob).cast(rays, per_ray=True, threads=_threads())
+    with _mr(prob, 0) as m:
+        d_rays = torch.from_numpy(rays).cuda()
+        m.cast_rays(d_rays)
+        got = m.read_tally()
+        st = m.get_stats()
+        nseg, hsh, _, _ = m.trace_rays(d_rays)
+    assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+    assert np.array_equal(nseg, ref.nseg), "segment counts differ"
+    assert np.array_equal(hsh, ref.hash), "cell-sequence hashes differ"
+    assert_tally(got, ref.tally, 0)
+
+
 # ------------------------------------------------------------------------------------- API behaviour
 def test_host_device_and_chunked_staging_agree():
     import torch
