@@ -24,6 +24,11 @@
  * homogeneous closed form W/S(1-exp(-S L)); the collision-probability invariant; the S->0
  * track-length limit; the two-slab closed form; fine-step quadrature of the plain
  * definition; linearity, additivity and mirror symmetry; published FNV-1a test vectors.
+ * The next-event function further down (vrc_next_event, steps N1..N6) is pinned in
+ * tests/test_oracle_next_event_pins.py: homogeneous closed form W exp(-S R)/R^2, the void
+ * inverse-square law, fine-step quadrature of Sigma_t along the line (detectors inside and outside
+ * the mesh), brute-force crossing lists for the cell sequence, detectors on planes / lattice
+ * points, reciprocity tau(a->b) = tau(b->a), linearity in W, every rejection rule.
  * Nothing in this file is "parity unpinned".
  */
 #include <math.h>
@@ -267,6 +272,133 @@ int vrc_cast_mt(const vrc_problem *p, int64_t n, const double *rays, double *tal
     }
     if (counts) { counts->rays_accepted = acc; counts->rays_rejected = rej; counts->segments = seg; }
     return threads;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * Next-event (point-detector) estimator -- SURVEY.md §8(f) NEXT-3.
+ *
+ * "The next-event estimator (Kalos, 1963) requires a ray-cast from each source and
+ * collision event to the estimator location."  The paper gives no formula; the estimator's plain
+ * definition (Kalos 1963) for an event at r with weight W and a detector point r_d is
+ *     score = W p(Omega_d) exp(-tau(r, r_d)) / |r_d - r|^2,   tau = int_0^R Sigma_t(r + s Omega_d, E) ds
+ * with Omega_d the unit vector towards the detector and R the distance.  The caller passes the
+ * weight already multiplied by the angular density p(Omega_d) (reading N-Q1, like W/N of Eq. (4)),
+ * so the ray cast owes  W exp(-tau) / R^2.  Outside the mesh is void (reading N-Q2).
+ *
+ * Steps (all IEEE double):
+ *   N1 reject (count, no contribution) an event with non-finite x,y,z,E,W, E <= 0, origin outside the
+ *      half-open box, or R2 = dx*dx + dy*dy + dz*dz not finite or == 0 (d = r_d - r, one subtract per axis);
+ *      the direction fields of the record are ignored
+ *   N2 sigma_m(E) as O2;  N3 start cell as O3
+ *   N4 crossing parameters as O4 with the UNNORMALISED direction d: t_a(p) = (edges_a[p] - o_a) * (1/d_a),
+ *      so that t = 1 is the detector, exactly
+ *   N5 walk as O5 (ties x<y<z); a segment whose pending crossing has t >= 1 ends AT the detector
+ *      (l = 1 - t_cur) and is the last; a step that leaves the mesh is the last too.
+ *      tau += Sigma_i * (l_i * R),  R = sqrt(R2)
+ *   N6 score = W * exp(-tau) / R2
+ * Per-event outputs: nseg, FNV-1a hash of the cell sequence, tau, score; *det_sum += score.
+ * ------------------------------------------------------------------------------------------------ */
+typedef struct {
+    uint32_t *nseg;   /* [n] */
+    uint64_t *hash;   /* [n] */
+    double *tau;      /* [n] */
+    double *score;    /* [n] */
+} vrc_ne_diag;
+
+static int next_event_one(const vrc_problem *p, const double *ray, const double *det, const vrc_ne_diag *dg,
+                          int64_t r, double *score_out, int64_t *segments_out)
+{
+    const double o[3] = {ray[0], ray[1], ray[2]};
+    const double E = ray[6], W = ray[7];
+    const int32_t n[3] = {p->nx, p->ny, p->nz};
+    const double *edges[3] = {p->xe, p->ye, p->ze};
+    double d[3];
+    uint32_t nseg = 0;
+    uint64_t hash = FNV_BASIS;
+    double tau = 0.0, score = 0.0;
+    int accepted = 1;
+
+    /* N1 */
+    for (int a = 0; a < 3; ++a) if (!isfinite(o[a])) accepted = 0;
+    if (!isfinite(E) || !isfinite(W) || !(E > 0.0)) accepted = 0;
+    for (int a = 0; a < 3; ++a) d[a] = det[a] - o[a];
+    const double R2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    if (!isfinite(R2) || !(R2 > 0.0)) accepted = 0;
+    for (int a = 0; a < 3 && accepted; ++a)
+        if (!(o[a] >= edges[a][0] && o[a] < edges[a][n[a]])) accepted = 0;
+
+    if (accepted) {
+        const double R = sqrt(R2);
+        double sig[64];
+        for (int32_t m = 0; m < p->M; ++m) sig[m] = vrc_sigma(p, m, E);        /* N2 */
+        int32_t i[3], step[3], plane[3];
+        double inv[3], t[3], t_cur = 0.0;
+        for (int a = 0; a < 3; ++a)                                              /* N3 */
+            i[a] = (int32_t)(upper_bound(edges[a], n[a] + 1, o[a]) - 1);
+        for (int a = 0; a < 3; ++a) {                                            /* N4 */
+            inv[a] = (d[a] != 0.0) ? 1.0 / d[a] : 0.0;
+            if (d[a] == 0.0 || !isfinite(inv[a])) {
+                step[a] = 0; plane[a] = 0; t[a] = INFINITY;
+            } else {
+                step[a] = d[a] > 0.0 ? 1 : -1;
+                plane[a] = d[a] > 0.0 ? i[a] + 1 : i[a];
+                t[a] = (edges[a][plane[a]] - o[a]) * inv[a];
+            }
+        }
+        for (;;) {                                                               /* N5 */
+            int a = 0;
+            if (t[1] < t[a]) a = 1;
+            if (t[2] < t[a]) a = 2;
+            const int last = t[a] >= 1.0;
+            const double l = (last ? 1.0 : t[a]) - t_cur;
+            int64_t c = (int64_t)i[0] + (int64_t)n[0] * ((int64_t)i[1] + (int64_t)n[1] * (int64_t)i[2]);
+            double S = 0.0;
+            for (int32_t k = 0; k < p->K; ++k) {
+                int32_t m = p->cell_mat[c * p->K + k];
+                if (m >= 0) S += (p->cell_frac[c * p->K + k] * p->density[m]) * sig[m];
+            }
+            tau += S * (l * R);
+            for (int b = 0; b < 4; ++b) {
+                hash ^= (uint64_t)(((uint32_t)c >> (8 * b)) & 0xffu);
+                hash *= FNV_PRIME;
+            }
+            nseg += 1;
+            if (last) break;
+            t_cur = t[a];
+            i[a] += step[a];
+            if (i[a] < 0 || i[a] >= n[a]) break;     /* the rest of the way is void (N-Q2) */
+            plane[a] += step[a];
+            t[a] = (edges[a][plane[a]] - o[a]) * inv[a];
+        }
+        score = W * exp(-tau) / R2;                                              /* N6 */
+    }
+    if (dg) {
+        if (dg->nseg) dg->nseg[r] = nseg;
+        if (dg->hash) dg->hash[r] = accepted ? hash : 0;
+        if (dg->tau) dg->tau[r] = tau;
+        if (dg->score) dg->score[r] = score;
+    }
+    *score_out = score;
+    *segments_out += nseg;
+    return accepted;
+}
+
+/* n events against ONE detector point det[3]; *det_sum += sum of scores (event order). */
+int vrc_next_event(const vrc_problem *p, int64_t n, const double *rays, const double *det, double *det_sum,
+                   const vrc_ne_diag *dg, vrc_counts *counts)
+{
+    if (p->M > 64) return -1;
+    vrc_counts cnt = {0, 0, 0};
+    double total = 0.0;
+    for (int64_t r = 0; r < n; ++r) {
+        double s;
+        if (next_event_one(p, rays + 8 * r, det, dg, r, &s, &cnt.segments)) cnt.rays_accepted++;
+        else cnt.rays_rejected++;
+        total += s;
+    }
+    if (det_sum) *det_sum += total;
+    if (counts) *counts = cnt;
+    return 0;
 }
 
 int vrc_max_threads(void)

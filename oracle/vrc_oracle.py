@@ -45,6 +45,10 @@ class _Counts(C.Structure):
     _fields_ = [("rays_accepted", C.c_int64), ("rays_rejected", C.c_int64), ("segments", C.c_int64)]
 
 
+class _NeDiag(C.Structure):
+    _fields_ = [("nseg", C.c_void_p), ("hash", C.c_void_p), ("tau", C.c_void_p), ("score", C.c_void_p)]
+
+
 class _Diag(C.Structure):
     _fields_ = [("nseg", C.c_void_p), ("hash", C.c_void_p), ("sum_l", C.c_void_p), ("t_exit", C.c_void_p),
                 ("tau_exit", C.c_void_p), ("sum_score", C.c_void_p), ("sum_sig_score", C.c_void_p),
@@ -62,6 +66,9 @@ def _load():
         _lib.vrc_cast_mt.restype = C.c_int
         _lib.vrc_cast_mt.argtypes = [C.POINTER(_Problem), C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_int, C.c_int64]
+        _lib.vrc_next_event.restype = C.c_int
+        _lib.vrc_next_event.argtypes = [C.POINTER(_Problem), C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
+                                        C.c_void_p, C.c_void_p]
         _lib.vrc_fnv1a_cells.restype = C.c_uint64
         _lib.vrc_fnv1a_cells.argtypes = [C.c_void_p, C.c_int64]
         _lib.vrc_max_threads.restype = C.c_int
@@ -94,6 +101,18 @@ class CastResult:
     cells: Optional[np.ndarray] = None
     lens: Optional[np.ndarray] = None
     scores: Optional[np.ndarray] = None
+
+
+@dataclass
+class NextEventResult:
+    det_sum: float
+    rays_accepted: int
+    rays_rejected: int
+    segments: int
+    nseg: np.ndarray
+    hash: np.ndarray
+    tau: np.ndarray
+    score: np.ndarray
 
 
 class Oracle:
@@ -174,3 +193,52 @@ class Oracle:
         res.rays_accepted, res.rays_rejected, res.segments, res.threads = (
             int(cnt.rays_accepted), int(cnt.rays_rejected), int(cnt.segments), int(used))
         return res
+
+    def next_event(self, rays, det) -> NextEventResult:
+        """Next-event (point-detector) estimator of `rays` ([n,8]; direction fields ignored) for ONE detector
+        point `det` (x, y, z): steps N1..N6 of vrc_oracle.c.  Returns the detector sum and per-event outputs."""
+        r = np.ascontiguousarray(np.asarray(rays, dtype=np.float64).reshape(-1, 8))
+        n = r.shape[0]
+        d = np.ascontiguousarray(np.asarray(det, dtype=np.float64).reshape(3))
+        nseg = np.zeros(n, dtype=np.uint32)
+        hsh = np.zeros(n, dtype=np.uint64)
+        tau = np.zeros(n, dtype=np.float64)
+        score = np.zeros(n, dtype=np.float64)
+        dg = _NeDiag(nseg.ctypes.data, hsh.ctypes.data, tau.ctypes.data, score.ctypes.data)
+        total = C.c_double(0.0)
+        cnt = _Counts()
+        rc = self.lib.vrc_next_event(C.byref(self._p), n, r.ctypes.data, d.ctypes.data,
+                                     C.cast(C.byref(total), C.c_void_p), C.cast(C.byref(dg), C.c_void_p),
+                                     C.cast(C.byref(cnt), C.c_void_p))
+        if rc < 0:
+            raise RuntimeError(f"oracle error {rc}")
+        return NextEventResult(float(total.value), int(cnt.rays_accepted), int(cnt.rays_rejected), int(cnt.segments),
+                               nseg, hsh, tau, score)
+
+
+# ---------------------------------------------------------------------------------------------------
+# Per-batch moments (SURVEY.md §8(f) NEXT-2): PAPER.md:93 Eq. (5) FOM = 1/(sigma^2 T) with "sigma the
+# standard deviation of the tally mean".  Plain numpy, fp64, one statement per definition.
+# ---------------------------------------------------------------------------------------------------
+def batch_moments(batch_tallies):
+    """batch_tallies [B, ncell] (the tally of each batch on its own) -> (sum_b x_b, sum_b x_b^2) per cell."""
+    x = np.asarray(batch_tallies, dtype=np.float64)
+    s1 = np.zeros(x.shape[1])
+    s2 = np.zeros(x.shape[1])
+    for b in range(x.shape[0]):           # batch order, one add per batch (the order the device folds in)
+        s1 = s1 + x[b]
+        s2 = s2 + x[b] * x[b]
+    return s1, s2
+
+
+def mean_and_sigma(s1, s2, B: int):
+    """Batch mean and the standard deviation OF THE MEAN per cell:
+    mean = s1/B;  sigma^2 = (s2/B - mean^2) / (B - 1)  (unbiased sample variance / B), clamped at 0."""
+    mean = s1 / B
+    var = (s2 / B - mean * mean) / (B - 1) if B > 1 else np.full_like(mean, np.inf)
+    return mean, np.sqrt(np.maximum(var, 0.0))
+
+
+def figure_of_merit(sigma, T: float):
+    """PAPER.md:93 Eq. (5): FOM = 1 / (sigma^2 T)."""
+    return 1.0 / (sigma * sigma * T)
