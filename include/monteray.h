@@ -85,7 +85,9 @@ typedef struct {
     int64_t kernel_launches;/* kernels this context has launched since creation */
     double last_cast_ms;    /* device time of the most recent mr_cast_rays work (copies and all kernels) */
     double last_kernel_ms;  /* device time of the cast kernel alone in that call (summed over its chunks) */
-    int64_t reserved[3];
+    int64_t ne_pairs_accepted; /* next-event: (event, detector) pairs scored since mr_load_detectors / mr_clear_detectors */
+    int64_t ne_pairs_rejected; /* next-event: pairs refused by the rule of mr_cast_next_event */
+    int64_t ne_segments;       /* next-event: cells crossed between events and detectors */
 } mr_stats;
 
 /* ---- life cycle -------------------------------------------------------------------------- */
@@ -167,6 +169,57 @@ MR_API int mr_get_stats(mr_ctx *ctx, mr_stats *out);
 /* Borrowed device pointer to the ncell fp64 tally (e.g. for a caller-side NCCL all-reduce
  * across replicas).  Valid until the next mr_load_mesh / mr_destroy. */
 MR_API int mr_tally_device_ptr(mr_ctx *ctx, double **out);
+
+/* ---- per-batch moments (Eq. (5) FOM = 1/(sigma^2 T), "sigma the
+ *      standard deviation of the tally mean") -------------------------------------------------- */
+
+/* Closes a batch: with x_b[c] = what was added to tally[c] since the previous mr_end_batch (or since
+ * creation / mr_clear_tally), accumulates sumsq[c] += x_b[c]^2 on the device and counts the batch.  The
+ * tally itself stays the running total (sum_b x_b), so mr_read_tally is unchanged.  Queued on the stream.
+ * The first call allocates two more ncell-double arrays.  Errors: STATE (no mesh), OOM, CUDA. */
+MR_API int mr_end_batch(mr_ctx *ctx);
+
+/* Synchronises and returns the moments over the CLOSED batches: sum[c] = sum_b x_b[c] (the tally as of the
+ * last mr_end_batch), sumsq[c] = sum_b x_b[c]^2, *nbatch = B.  Host arrays of ncell doubles; any of the
+ * three may be NULL.  Before the first mr_end_batch: zeros and B = 0.  Errors: STATE, CUDA. */
+MR_API int mr_read_moments(mr_ctx *ctx, double *sum, double *sumsq, int64_t *nbatch);
+
+/* Synchronises, evaluates on the device and returns per cell the batch mean  mean = sum/B  and the standard
+ * deviation OF THE MEAN  sigma = sqrt(max((sumsq/B - mean^2)/(B-1), 0))  (+inf when B = 1), the sigma of
+ * Eq. (5).  Host arrays of ncell doubles, either may be NULL.  Errors: STATE (no closed batch), OOM, CUDA. */
+MR_API int mr_read_mean_sigma(mr_ctx *ctx, double *mean, double *sigma, int64_t *nbatch);
+
+/* ---- next-event (point-detector) estimator ("requires a ray-cast
+ *      from each source and collision event to the estimator location") ------------------------ */
+
+/* Detector points xyz[ndet*3] (host, finite; inside or outside the mesh).  Allocates and zeroes the ndet
+ * resident fp64 detector sums and the next-event counters; replaces any earlier set.  1 <= ndet <= 65535.
+ * Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA. */
+MR_API int mr_load_detectors(mr_ctx *ctx, int ndet, const double *xyz);
+
+/* For every event (the same records as mr_cast_rays; only x,y,z,E,W are used, the direction fields are
+ * ignored) and every detector d: with dvec = det_d - origin (fp64), R^2 = |dvec|^2, the cells between the
+ * origin and the detector are walked exactly as in mr_cast_rays but with the unnormalised direction dvec,
+ * so the crossing parameter t = 1 IS the detector; the segment whose pending crossing has t >= 1 ends at
+ * the detector and is the last; leaving the mesh ends the walk too (outside the mesh is void);
+ *     tau = sum_i Sigma_i * (l_i * R);     det_sum[d] += W * exp(-tau) / R^2
+ * W must already carry the angular density p(Omega -> detector) of the event (reading N-Q1).
+ * A pair is REJECTED (counted, no contribution) if x,y,z,E or W is not finite, E <= 0, the origin is outside
+ * the half-open box, or R^2 is 0 or not finite.  Asynchronous like mr_cast_rays.  n = 0 is a no-op.
+ * Requires mesh, materials, all tables and detectors.  Errors: INVALID_ARG, STATE, OOM, CUDA. */
+MR_API int mr_cast_next_event(mr_ctx *ctx, int64_t n, const void *rays, int where);
+
+/* Synchronises and copies the ndet detector sums to the host array `out`. */
+MR_API int mr_read_detectors(mr_ctx *ctx, double *out);
+
+/* Zeroes the detector sums and the next-event counters (queued on the stream). */
+MR_API int mr_clear_detectors(mr_ctx *ctx);
+
+/* Test entry: the same walk for ONE detector `det`, nothing is added to the detector sums or counters.  Per event r (host
+ * outputs, any may be NULL): nseg[r] cells crossed (0 if rejected), hash[r] FNV-1a 64 of the cell sequence
+ * (0 if rejected), tau[r], score[r].  Synchronous. */
+MR_API int mr_trace_next_event(mr_ctx *ctx, int64_t n, const void *rays, int where, int det, uint32_t *nseg,
+                               uint64_t *hash, double *tau, double *score);
 
 /* ---- test / diagnostic entry point ------------------------------------------------------- */
 

@@ -27,6 +27,8 @@ EXPORTS = [
     "mr_create", "mr_create_ex", "mr_destroy", "mr_set_stream", "mr_last_error", "mr_load_mesh",
     "mr_load_materials", "mr_load_xs", "mr_cast_rays", "mr_read_tally", "mr_clear_tally", "mr_sync",
     "mr_get_stats", "mr_tally_device_ptr", "mr_trace_rays", "mr_set_option", "mr_get_option",
+    "mr_end_batch", "mr_read_moments", "mr_read_mean_sigma",
+    "mr_load_detectors", "mr_cast_next_event", "mr_read_detectors", "mr_clear_detectors", "mr_trace_next_event",
 ]
 
 
@@ -39,7 +41,7 @@ class MonteRayError(RuntimeError):
 class mr_stats(C.Structure):
     _fields_ = [("rays_accepted", C.c_int64), ("rays_rejected", C.c_int64), ("segments", C.c_int64),
                 ("kernel_launches", C.c_int64), ("last_cast_ms", C.c_double), ("last_kernel_ms", C.c_double),
-                ("reserved", C.c_int64 * 3)]
+                ("ne_pairs_accepted", C.c_int64), ("ne_pairs_rejected", C.c_int64), ("ne_segments", C.c_int64)]
 
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_void_p, C.c_size_t, C.c_int)
@@ -80,6 +82,14 @@ def load_library() -> C.CDLL:
         "mr_trace_rays": [vp, i64, vp, i32, vp, vp, vp, vp, i64],
         "mr_set_option": [vp, i32, i64],
         "mr_get_option": [vp, i32, C.POINTER(i64)],
+        "mr_end_batch": [vp],
+        "mr_read_moments": [vp, vp, vp, C.POINTER(i64)],
+        "mr_read_mean_sigma": [vp, vp, vp, C.POINTER(i64)],
+        "mr_load_detectors": [vp, i32, vp],
+        "mr_cast_next_event": [vp, i64, vp, i32],
+        "mr_read_detectors": [vp, vp],
+        "mr_clear_detectors": [vp],
+        "mr_trace_next_event": [vp, i64, vp, i32, i32, vp, vp, vp, vp],
     }
     for name, argtypes in sigs.items():
         fn = getattr(lib, name)
@@ -123,6 +133,9 @@ class Stats:
     kernel_launches: int
     last_cast_ms: float
     last_kernel_ms: float
+    ne_pairs_accepted: int = 0
+    ne_pairs_rejected: int = 0
+    ne_segments: int = 0
 
 
 def _f64(a) -> np.ndarray:
@@ -262,7 +275,8 @@ class MonteRay:
     def get_stats(self) -> Stats:
         s = mr_stats()
         self._check(self.lib.mr_get_stats(self._h, C.byref(s)))
-        return Stats(s.rays_accepted, s.rays_rejected, s.segments, s.kernel_launches, s.last_cast_ms, s.last_kernel_ms)
+        return Stats(s.rays_accepted, s.rays_rejected, s.segments, s.kernel_launches, s.last_cast_ms, s.last_kernel_ms,
+                     s.ne_pairs_accepted, s.ne_pairs_rejected, s.ne_segments)
 
     def tally_device_ptr(self) -> int:
         p = C.c_void_p()
@@ -292,6 +306,56 @@ class MonteRay:
                                            cells.ctypes.data if cap > 0 else None,
                                            lens.ctypes.data if cap > 0 else None, cap))
         return nseg, hsh, cells, lens
+
+    # ---- per-batch moments (NEXT-2)
+    def end_batch(self):
+        self._check(self.lib.mr_end_batch(self._h))
+
+    def read_moments(self):
+        """mr_read_moments -> (sum float64[ncell], sumsq float64[ncell], nbatch)."""
+        s1 = np.empty(self.ncell, dtype=np.float64)
+        s2 = np.empty(self.ncell, dtype=np.float64)
+        nb = C.c_int64()
+        self._check(self.lib.mr_read_moments(self._h, s1.ctypes.data, s2.ctypes.data, C.byref(nb)))
+        return s1, s2, int(nb.value)
+
+    def read_mean_sigma(self):
+        """mr_read_mean_sigma -> (mean float64[ncell], sigma float64[ncell], nbatch)."""
+        mean = np.empty(self.ncell, dtype=np.float64)
+        sigma = np.empty(self.ncell, dtype=np.float64)
+        nb = C.c_int64()
+        self._check(self.lib.mr_read_mean_sigma(self._h, mean.ctypes.data, sigma.ctypes.data, C.byref(nb)))
+        return mean, sigma, int(nb.value)
+
+    # ---- next-event estimator (NEXT-3)
+    def load_detectors(self, xyz):
+        xyz = _f64(xyz).reshape(-1, 3)
+        self._check(self.lib.mr_load_detectors(self._h, xyz.shape[0], xyz.ctypes.data))
+        self.ndet = xyz.shape[0]
+
+    def cast_next_event(self, rays):
+        ptr, n, where, keep = self._ray_arg(rays)
+        self._check(self.lib.mr_cast_next_event(self._h, n, C.c_void_p(ptr), where))
+        return n
+
+    def read_detectors(self) -> np.ndarray:
+        out = np.empty(self.ndet, dtype=np.float64)
+        self._check(self.lib.mr_read_detectors(self._h, out.ctypes.data))
+        return out
+
+    def clear_detectors(self):
+        self._check(self.lib.mr_clear_detectors(self._h))
+
+    def trace_next_event(self, rays, det: int):
+        """mr_trace_next_event -> (nseg uint32[n], hash uint64[n], tau float64[n], score float64[n])."""
+        ptr, n, where, keep = self._ray_arg(rays)
+        nseg = np.zeros(n, dtype=np.uint32)
+        hsh = np.zeros(n, dtype=np.uint64)
+        tau = np.zeros(n, dtype=np.float64)
+        score = np.zeros(n, dtype=np.float64)
+        self._check(self.lib.mr_trace_next_event(self._h, n, C.c_void_p(ptr), where, det, nseg.ctypes.data,
+                                                 hsh.ctypes.data, tau.ctypes.data, score.ctypes.data))
+        return nseg, hsh, tau, score
 
     def set_option(self, option: int, value: int):
         self._check(self.lib.mr_set_option(self._h, option, value))

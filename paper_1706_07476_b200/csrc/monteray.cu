@@ -81,7 +81,15 @@ struct mr_ctx {
     XsDesc *d_xs = nullptr;
     bool xs_dirty = true;
 
-    unsigned long long *d_counters = nullptr;  // accepted, rejected, segments, spare
+    unsigned long long *d_counters = nullptr;  // accepted, rejected, segments, spare | next-event: accepted, rejected, segments, spare
+
+    // per-batch moments (allocated by the first mr_end_batch)
+    double *d_prev = nullptr, *d_s2 = nullptr;
+    long long nbatch = 0;
+
+    // next-event detectors
+    int ndet = 0;
+    double *d_det = nullptr, *d_det_sum = nullptr;
 
     // host-batch staging ring
     void *pinned[kStageSlots] = {nullptr, nullptr};
@@ -466,8 +474,8 @@ int mr_create_ex(mr_ctx **out, int device, int precision, const mr_allocator *al
     }
     ok = ok && cudaEventCreate(&c->ev_t0) == cudaSuccess && cudaEventCreate(&c->ev_t1) == cudaSuccess;
     if (ok) {
-        c->d_counters = (unsigned long long *)c->dev_alloc(4 * sizeof(unsigned long long));
-        ok = c->d_counters && cudaMemset(c->d_counters, 0, 4 * sizeof(unsigned long long)) == cudaSuccess;
+        c->d_counters = (unsigned long long *)c->dev_alloc(8 * sizeof(unsigned long long));
+        ok = c->d_counters && cudaMemset(c->d_counters, 0, 8 * sizeof(unsigned long long)) == cudaSuccess;
     }
     if (!ok) {
         g_create_error = std::string("context set-up failed: ") + cudaGetErrorString(cudaGetLastError());
@@ -492,6 +500,10 @@ int mr_destroy(mr_ctx *c)
     c->dev_free(c->d_edges);
     c->dev_free(c->d_tally);
     c->dev_free(c->d_counters);
+    c->dev_free(c->d_prev);
+    c->dev_free(c->d_s2);
+    c->dev_free(c->d_det);
+    c->dev_free(c->d_det_sum);
     c->dev_free(c->d_keys);
     c->dev_free(c->d_perm);
     c->dev_free(c->d_hist);
@@ -532,8 +544,12 @@ int mr_load_mesh(mr_ctx *c, int nx, int ny, int nz, const double *xe, const doub
     free_materials(c);
     c->dev_free(c->d_edges);
     c->dev_free(c->d_tally);
+    c->dev_free(c->d_prev);
+    c->dev_free(c->d_s2);
     c->d_edges = nullptr;
     c->d_tally = nullptr;
+    c->d_prev = c->d_s2 = nullptr;
+    c->nbatch = 0;
     const int ne = nx + ny + nz + 3;
     std::vector<double> h(ne);
     std::memcpy(h.data(), xe, sizeof(double) * (nx + 1));
@@ -745,19 +761,19 @@ int mr_load_xs(mr_ctx *c, int material, int64_t n, const double *energy, const d
     return MR_OK;
 }
 
-int mr_cast_rays(mr_ctx *c, int64_t n, const void *rays, int where)
+}  // extern "C"
+
+namespace {
+
+// Runs `work(count, device rays)` over a batch: a device batch in one piece, a host batch in staged chunks.
+template <typename Work>
+int run_batch(mr_ctx *c, int64_t n, const void *rays, int where, Work work)
 {
-    MR_ENTER(c);
-    if (n < 0 || (n > 0 && !rays) || (where != MR_WHERE_HOST && where != MR_WHERE_DEVICE))
-        return c->fail(MR_ERR_INVALID_ARG, "cast: bad count, NULL buffer or unknown location");
-    if (int rc = ready_to_cast(c)) return rc;
-    if (n == 0) return MR_OK;
-    if (int rc = upload_xs_desc(c)) return rc;
     c->kev_used = 0;
     if (where == MR_WHERE_DEVICE) {
         if ((uintptr_t)rays & 15) return c->fail(MR_ERR_INVALID_ARG, "cast: device ray buffer must be 16-byte aligned");
         MR_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
-        if (int rc = cast_device(c, n, rays)) return rc;
+        if (int rc = work((long long)n, rays)) return rc;
         MR_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
         c->have_timing = true;
         return MR_OK;
@@ -800,7 +816,7 @@ int mr_cast_rays(mr_ctx *c, int64_t n, const void *rays, int where)
         MR_CUDA(c, cudaMemcpyAsync(c->d_stage[s], src, (size_t)count * rb, cudaMemcpyHostToDevice, c->copy_stream));
         MR_CUDA(c, cudaEventRecord(c->ev_copied[s], c->copy_stream));
         MR_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied[s], 0));
-        if (int rc = cast_device(c, count, c->d_stage[s])) return rc;
+        if (int rc = work((long long)count, (const void *)c->d_stage[s])) return rc;
         MR_CUDA(c, cudaEventRecord(c->ev_done[s], c->stream));
         last_slot = s;
     }
@@ -809,6 +825,21 @@ int mr_cast_rays(mr_ctx *c, int64_t n, const void *rays, int where)
     // the caller's buffer is consumed when the call returns: wait for the last DMA out of it
     if (pinned_src && last_slot >= 0) MR_CUDA(c, cudaEventSynchronize(c->ev_copied[last_slot]));
     return MR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mr_cast_rays(mr_ctx *c, int64_t n, const void *rays, int where)
+{
+    MR_ENTER(c);
+    if (n < 0 || (n > 0 && !rays) || (where != MR_WHERE_HOST && where != MR_WHERE_DEVICE))
+        return c->fail(MR_ERR_INVALID_ARG, "cast: bad count, NULL buffer or unknown location");
+    if (int rc = ready_to_cast(c)) return rc;
+    if (n == 0) return MR_OK;
+    if (int rc = upload_xs_desc(c)) return rc;
+    return run_batch(c, n, rays, where, [c](long long count, const void *d_rays) { return cast_device(c, count, d_rays); });
 }
 
 int mr_read_tally(mr_ctx *c, double *out)
@@ -827,6 +858,11 @@ int mr_clear_tally(mr_ctx *c)
     if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
     MR_CUDA(c, cudaMemsetAsync(c->d_tally, 0, sizeof(double) * c->ncell, c->stream));
     MR_CUDA(c, cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
+    if (c->d_prev) {   // the batch moments restart with the tally
+        MR_CUDA(c, cudaMemsetAsync(c->d_prev, 0, sizeof(double) * c->ncell, c->stream));
+        MR_CUDA(c, cudaMemsetAsync(c->d_s2, 0, sizeof(double) * c->ncell, c->stream));
+    }
+    c->nbatch = 0;
     return MR_OK;
 }
 
@@ -841,13 +877,16 @@ int mr_get_stats(mr_ctx *c, mr_stats *out)
 {
     MR_ENTER(c);
     if (!out) return c->fail(MR_ERR_INVALID_ARG, "get_stats: out is NULL");
-    unsigned long long h[4] = {0, 0, 0, 0};
+    unsigned long long h[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     MR_CUDA(c, cudaMemcpyAsync(h, c->d_counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
     std::memset(out, 0, sizeof(*out));
     out->rays_accepted = (int64_t)h[0];
     out->rays_rejected = (int64_t)h[1];
     out->segments = (int64_t)h[2];
+    out->ne_pairs_accepted = (int64_t)h[4];
+    out->ne_pairs_rejected = (int64_t)h[5];
+    out->ne_segments = (int64_t)h[6];
     out->kernel_launches = c->launches;
     if (c->have_timing) {
         float ms = 0.f;
@@ -930,6 +969,278 @@ int mr_trace_rays(mr_ctx *c, int64_t n, const void *rays, int where, uint32_t *n
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     cleanup();
     if (e != cudaSuccess) return c->fail_cuda(e, "mr_trace_rays");
+    return MR_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+template <typename Real, typename Rec, int MODE, bool TRACE>
+int launch_ne_m(mr_ctx *c, const NextEventParams &P, int ndet_launch, int block, size_t smem)
+{
+    const long long gx = (P.n + block - 1) / block;
+    if (gx > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
+    if (int rc = set_smem(c, next_event_kernel<Real, Rec, MODE, TRACE>, smem)) return rc;
+    next_event_kernel<Real, Rec, MODE, TRACE><<<dim3((unsigned)gx, (unsigned)ndet_launch), block, smem, c->stream>>>(P);
+    c->launches += 1;
+    MR_CUDA(c, cudaGetLastError());
+    return MR_OK;
+}
+
+template <typename Real, typename Rec, bool TRACE>
+int launch_ne_t(mr_ctx *c, const NextEventParams &P, int ndet_launch)
+{
+    const int block = c->block_threads;
+    const size_t per_block = walker_smem_bytes(block) + (size_t)c->M * block * sizeof(Real);
+    const int mode = edge_mode(c, per_block);
+    const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
+    if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "materials x block threads exceed shared memory; lower MR_OPT_BLOCK_THREADS");
+    switch (mode) {
+    case EDGES_ARITH: return launch_ne_m<Real, Rec, EDGES_ARITH, TRACE>(c, P, ndet_launch, block, smem);
+    case EDGES_SHARED: return launch_ne_m<Real, Rec, EDGES_SHARED, TRACE>(c, P, ndet_launch, block, smem);
+    default: return launch_ne_m<Real, Rec, EDGES_GLOBAL, TRACE>(c, P, ndet_launch, block, smem);
+    }
+}
+
+template <bool TRACE>
+int launch_next_event(mr_ctx *c, const NextEventParams &P, int ndet_launch)
+{
+    if (c->precision == MR_PRECISION_DOUBLE) return launch_ne_t<double, CellRecGeneric<double>, TRACE>(c, P, ndet_launch);
+    switch (c->layout) {
+    case LAYOUT_K1: return launch_ne_t<float, CellRec<LAYOUT_K1>, TRACE>(c, P, ndet_launch);
+    case LAYOUT_K2: return c->pair_records ? launch_ne_t<float, CellRec<LAYOUT_K2P>, TRACE>(c, P, ndet_launch) : launch_ne_t<float, CellRec<LAYOUT_K2>, TRACE>(c, P, ndet_launch);
+    case LAYOUT_K3: return c->pair_records ? launch_ne_t<float, CellRec<LAYOUT_K3P>, TRACE>(c, P, ndet_launch) : launch_ne_t<float, CellRec<LAYOUT_K3>, TRACE>(c, P, ndet_launch);
+    case LAYOUT_K4: return launch_ne_t<float, CellRec<LAYOUT_K4>, TRACE>(c, P, ndet_launch);
+    case LAYOUT_D8: return launch_ne_t<float, CellRec<LAYOUT_D8>, TRACE>(c, P, ndet_launch);
+    default: return launch_ne_t<float, CellRecGeneric<float>, TRACE>(c, P, ndet_launch);
+    }
+}
+
+NextEventParams ne_params(mr_ctx *c, long long n, const void *d_rays)
+{
+    NextEventParams P{};
+    P.mesh = mesh_dev(c);
+    P.recs = c->d_recs;
+    P.ids = c->d_ids;
+    P.K = c->K;
+    P.M = c->M;
+    P.xs = c->d_xs;
+    P.rays = d_rays;
+    P.n = n;
+    P.det = c->d_det;
+    return P;
+}
+
+// all detectors against n device-resident events (grid.y = detectors, at most 65535 per launch)
+int next_event_device(mr_ctx *c, long long n, const void *d_rays)
+{
+    NextEventParams P = ne_params(c, n, d_rays);
+    P.det_sum = c->d_det_sum;
+    P.counters = c->d_counters + 4;
+    if (c->kev_used + 2 > c->kev.size()) {
+        cudaEvent_t a = nullptr, b = nullptr;
+        MR_CUDA(c, cudaEventCreate(&a));
+        MR_CUDA(c, cudaEventCreate(&b));
+        c->kev.push_back(a);
+        c->kev.push_back(b);
+    }
+    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->stream));
+    P.det_first = 0;
+    if (int rc = launch_next_event<false>(c, P, c->ndet)) return rc;
+    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used + 1], c->stream));
+    c->kev_used += 2;
+    return MR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mr_end_batch(mr_ctx *c)
+{
+    MR_ENTER(c);
+    if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    if (!c->d_prev) {
+        c->d_prev = (double *)c->dev_alloc(sizeof(double) * c->ncell);
+        c->d_s2 = (double *)c->dev_alloc(sizeof(double) * c->ncell);
+        if (!c->d_prev || !c->d_s2) {
+            c->dev_free(c->d_prev);
+            c->dev_free(c->d_s2);
+            c->d_prev = c->d_s2 = nullptr;
+            return c->fail(MR_ERR_OOM, "device allocation failed (batch moments)");
+        }
+        MR_CUDA(c, cudaMemsetAsync(c->d_prev, 0, sizeof(double) * c->ncell, c->stream));
+        MR_CUDA(c, cudaMemsetAsync(c->d_s2, 0, sizeof(double) * c->ncell, c->stream));
+    }
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    const long long want = (c->ncell / 2 + 255) / 256 + 1;
+    const unsigned grid = (unsigned)std::min<long long>(want, (long long)sms * 8);
+    fold_batch_kernel<<<grid, 256, 0, c->stream>>>(c->d_tally, c->d_prev, c->d_s2, c->ncell);
+    c->launches += 1;
+    MR_CUDA(c, cudaGetLastError());
+    c->nbatch += 1;
+    return MR_OK;
+}
+
+int mr_read_moments(mr_ctx *c, double *sum, double *sumsq, int64_t *nbatch)
+{
+    MR_ENTER(c);
+    if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    if (nbatch) *nbatch = c->nbatch;
+    if (!c->d_prev) {
+        MR_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (sum) std::memset(sum, 0, sizeof(double) * c->ncell);
+        if (sumsq) std::memset(sumsq, 0, sizeof(double) * c->ncell);
+        return MR_OK;
+    }
+    if (sum) MR_CUDA(c, cudaMemcpyAsync(sum, c->d_prev, sizeof(double) * c->ncell, cudaMemcpyDeviceToHost, c->stream));
+    if (sumsq) MR_CUDA(c, cudaMemcpyAsync(sumsq, c->d_s2, sizeof(double) * c->ncell, cudaMemcpyDeviceToHost, c->stream));
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    return MR_OK;
+}
+
+int mr_read_mean_sigma(mr_ctx *c, double *mean, double *sigma, int64_t *nbatch)
+{
+    MR_ENTER(c);
+    if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    if (!c->d_prev || c->nbatch < 1) return c->fail(MR_ERR_STATE, "no closed batch (call mr_end_batch first)");
+    if (nbatch) *nbatch = c->nbatch;
+    double *d_mean = (double *)c->dev_alloc(sizeof(double) * c->ncell);
+    double *d_sigma = (double *)c->dev_alloc(sizeof(double) * c->ncell);
+    if (!d_mean || !d_sigma) {
+        c->dev_free(d_mean);
+        c->dev_free(d_sigma);
+        return c->fail(MR_ERR_OOM, "device allocation failed (mean / sigma)");
+    }
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    const unsigned grid = (unsigned)std::min<long long>((c->ncell + 255) / 256, (long long)sms * 8);
+    mean_sigma_kernel<<<grid, 256, 0, c->stream>>>(c->d_prev, c->d_s2, d_mean, d_sigma, c->ncell, c->nbatch);
+    c->launches += 1;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && mean) e = cudaMemcpyAsync(mean, d_mean, sizeof(double) * c->ncell, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess && sigma) e = cudaMemcpyAsync(sigma, d_sigma, sizeof(double) * c->ncell, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    c->dev_free(d_mean);
+    c->dev_free(d_sigma);
+    if (e != cudaSuccess) return c->fail_cuda(e, "mr_read_mean_sigma");
+    return MR_OK;
+}
+
+int mr_load_detectors(mr_ctx *c, int ndet, const double *xyz)
+{
+    MR_ENTER(c);
+    if (ndet < 1 || !xyz) return c->fail(MR_ERR_INVALID_ARG, "detectors: bad count or NULL array");
+    if (ndet > 65535) return c->fail(MR_ERR_UNSUPPORTED, "detectors: at most 65535 points");
+    for (int i = 0; i < 3 * ndet; ++i)
+        if (!std::isfinite(xyz[i])) return c->fail(MR_ERR_INVALID_ARG, "detectors: coordinates must be finite");
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->dev_free(c->d_det);
+    c->dev_free(c->d_det_sum);
+    c->ndet = 0;
+    c->d_det = (double *)c->dev_alloc(sizeof(double) * 3 * ndet);
+    c->d_det_sum = (double *)c->dev_alloc(sizeof(double) * ndet);
+    if (!c->d_det || !c->d_det_sum) {
+        c->dev_free(c->d_det);
+        c->dev_free(c->d_det_sum);
+        c->d_det = c->d_det_sum = nullptr;
+        return c->fail(MR_ERR_OOM, "device allocation failed (detectors)");
+    }
+    MR_CUDA(c, cudaMemcpyAsync(c->d_det, xyz, sizeof(double) * 3 * ndet, cudaMemcpyHostToDevice, c->stream));
+    MR_CUDA(c, cudaMemsetAsync(c->d_det_sum, 0, sizeof(double) * ndet, c->stream));
+    MR_CUDA(c, cudaMemsetAsync(c->d_counters + 4, 0, 4 * sizeof(unsigned long long), c->stream));
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->ndet = ndet;
+    return MR_OK;
+}
+
+int mr_cast_next_event(mr_ctx *c, int64_t n, const void *rays, int where)
+{
+    MR_ENTER(c);
+    if (n < 0 || (n > 0 && !rays) || (where != MR_WHERE_HOST && where != MR_WHERE_DEVICE))
+        return c->fail(MR_ERR_INVALID_ARG, "next_event: bad count, NULL buffer or unknown location");
+    if (int rc = ready_to_cast(c)) return rc;
+    if (!c->ndet) return c->fail(MR_ERR_STATE, "no detectors loaded");
+    if (n == 0) return MR_OK;
+    if (int rc = upload_xs_desc(c)) return rc;
+    return run_batch(c, n, rays, where, [c](long long count, const void *d_rays) { return next_event_device(c, count, d_rays); });
+}
+
+int mr_read_detectors(mr_ctx *c, double *out)
+{
+    MR_ENTER(c);
+    if (!out) return c->fail(MR_ERR_INVALID_ARG, "read_detectors: out is NULL");
+    if (!c->ndet) return c->fail(MR_ERR_STATE, "no detectors loaded");
+    MR_CUDA(c, cudaMemcpyAsync(out, c->d_det_sum, sizeof(double) * c->ndet, cudaMemcpyDeviceToHost, c->stream));
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    return MR_OK;
+}
+
+int mr_clear_detectors(mr_ctx *c)
+{
+    MR_ENTER(c);
+    if (!c->ndet) return c->fail(MR_ERR_STATE, "no detectors loaded");
+    MR_CUDA(c, cudaMemsetAsync(c->d_det_sum, 0, sizeof(double) * c->ndet, c->stream));
+    MR_CUDA(c, cudaMemsetAsync(c->d_counters + 4, 0, 4 * sizeof(unsigned long long), c->stream));
+    return MR_OK;
+}
+
+int mr_trace_next_event(mr_ctx *c, int64_t n, const void *rays, int where, int det, uint32_t *nseg, uint64_t *hash,
+                        double *tau, double *score)
+{
+    MR_ENTER(c);
+    if (n < 0 || (n > 0 && !rays) || (where != MR_WHERE_HOST && where != MR_WHERE_DEVICE))
+        return c->fail(MR_ERR_INVALID_ARG, "trace_next_event: bad count, NULL buffer or unknown location");
+    if (int rc = ready_to_cast(c)) return rc;
+    if (!c->ndet) return c->fail(MR_ERR_STATE, "no detectors loaded");
+    if (det < 0 || det >= c->ndet) return c->fail(MR_ERR_INVALID_ARG, "trace_next_event: detector index out of range");
+    if (n == 0) return MR_OK;
+    if (int rc = upload_xs_desc(c)) return rc;
+    const size_t rb = c->ray_bytes();
+    void *d_rays = nullptr;
+    uint32_t *d_nseg = nullptr;
+    unsigned long long *d_hash = nullptr;
+    double *d_tau = nullptr, *d_score = nullptr;
+    auto cleanup = [&]() {
+        if (where == MR_WHERE_HOST) c->dev_free(d_rays);
+        c->dev_free(d_nseg); c->dev_free(d_hash); c->dev_free(d_tau); c->dev_free(d_score);
+    };
+    bool ok = true;
+    if (where == MR_WHERE_HOST) ok = ok && (d_rays = c->dev_alloc((size_t)n * rb));
+    if (nseg) ok = ok && (d_nseg = (uint32_t *)c->dev_alloc((size_t)n * 4));
+    if (hash) ok = ok && (d_hash = (unsigned long long *)c->dev_alloc((size_t)n * 8));
+    if (tau) ok = ok && (d_tau = (double *)c->dev_alloc((size_t)n * 8));
+    if (score) ok = ok && (d_score = (double *)c->dev_alloc((size_t)n * 8));
+    if (!ok) {
+        cleanup();
+        return c->fail(MR_ERR_OOM, "device allocation failed (next-event trace buffers)");
+    }
+    cudaError_t e = cudaSuccess;
+    if (where == MR_WHERE_HOST) e = cudaMemcpyAsync(d_rays, rays, (size_t)n * rb, cudaMemcpyHostToDevice, c->stream);
+    else {
+        if ((uintptr_t)rays & 15) { cleanup(); return c->fail(MR_ERR_INVALID_ARG, "trace_next_event: device ray buffer must be 16-byte aligned"); }
+        d_rays = const_cast<void *>(rays);
+    }
+    int rc = MR_OK;
+    if (e == cudaSuccess) {
+        NextEventParams P = ne_params(c, n, d_rays);
+        P.det_first = det;
+        P.nseg = d_nseg; P.hash = d_hash; P.tau = d_tau; P.score = d_score;
+        rc = launch_next_event<true>(c, P, 1);
+    }
+    if (rc == MR_OK) {
+        if (e == cudaSuccess && d_nseg) e = cudaMemcpyAsync(nseg, d_nseg, (size_t)n * 4, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess && d_hash) e = cudaMemcpyAsync(hash, d_hash, (size_t)n * 8, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess && d_tau) e = cudaMemcpyAsync(tau, d_tau, (size_t)n * 8, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess && d_score) e = cudaMemcpyAsync(score, d_score, (size_t)n * 8, cudaMemcpyDeviceToHost, c->stream);
+    }
+    cudaError_t e2 = cudaStreamSynchronize(c->stream);
+    if (e == cudaSuccess) e = e2;
+    cleanup();
+    if (rc != MR_OK) return rc;
+    if (e != cudaSuccess) return c->fail_cuda(e, "mr_trace_next_event");
     return MR_OK;
 }
 

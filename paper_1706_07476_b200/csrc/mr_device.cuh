@@ -638,6 +638,201 @@ __global__ void __launch_bounds__(256) trace_kernel(const __grid_constant__ Trac
 }
 
 // ------------------------------------------------------------------------------------------------
+// Next-event (point-detector) estimator, SURVEY.md §8(f) NEXT-3 ("requires a ray-cast from
+// each source and collision event to the estimator location").  One thread per (event, detector): the same
+// S1 look-up and S2/S3 walker, with the UNNORMALISED direction d = det - o so that the crossing parameter
+// t = 1 is the detector exactly (steps N1-N6); no tally atomics -- only the optical
+// thickness tau = sum_i Sigma_i (l_i R) is carried, and score = W exp(-tau) / R^2 is reduced per CTA into
+// the detector's fp64 sum.  blockIdx.y = detector (or P.det_first + blockIdx.y).
+//   dynamic shared memory: as cast_kernel.
+// ------------------------------------------------------------------------------------------------
+struct NextEventParams {
+    MeshDev mesh;
+    const void *recs;
+    const uint8_t *ids;
+    int K, M;
+    const XsDesc *xs;
+    const void *rays;
+    long long n;
+    const double *det;             // [ndet*3] detector points
+    int det_first;                 // first detector of this launch
+    double *det_sum;               // [ndet] resident sums (may be null in a trace launch)
+    unsigned long long *counters;  // [0] accepted pairs [1] rejected pairs [2] segments (may be null)
+    // per-event outputs of the test entry point (one detector per launch), any may be null
+    uint32_t *nseg;
+    unsigned long long *hash;
+    double *tau;
+    double *score;
+};
+
+// accurate exp(-x), x >= 0, from the same reduction as score_terms (full series)
+__device__ __forceinline__ double exp_neg(double x)
+{
+    const double kf = rint(x * -1.4426950408889634074);
+    double r = fma(kf, -6.93147180369123816490e-01, -x);
+    r = fma(kf, -1.90821492927058770002e-10, r);
+    double q = c_expq[0];
+#pragma unroll
+    for (int i = 1; i < 12; ++i) q = fma(q, r, c_expq[i]);
+    const double p = fma(r * r, q, r);
+    const int k = (int)kf;
+    if (k < -1022) return 0.0;
+    const double scale = __longlong_as_double((long long)(k + 1023) << 52);
+    return fma(scale, p, scale);
+}
+
+template <typename Real, typename Rec, int EDGE_MODE, bool TRACE>
+__global__ void __launch_bounds__(256) next_event_kernel(const __grid_constant__ NextEventParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double s_part[8];
+    const int stride = blockDim.x;
+    unsigned char *sp = smem_raw;
+    double *s_edges = reinterpret_cast<double *>(sp);
+    if (EDGE_MODE == EDGES_SHARED) sp += edges_smem_bytes_for(P.mesh.nedges);
+    AxisF *axf = reinterpret_cast<AxisF *>(sp) + threadIdx.x;
+    sp += sizeof(AxisF) * 3 * stride;
+    Real *sig = reinterpret_cast<Real *>(sp) + threadIdx.x;
+    const double *e = (EDGE_MODE == EDGES_SHARED) ? s_edges : P.mesh.edges;
+    if (EDGE_MODE == EDGES_SHARED) {
+        for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
+        __syncthreads();
+    }
+    const int det = P.det_first + blockIdx.y;
+    const double D[3] = {__ldg(P.det + 3 * det), __ldg(P.det + 3 * det + 1), __ldg(P.det + 3 * det + 2)};
+
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = r < P.n;
+    bool accepted = false;
+    unsigned nseg = 0;
+    unsigned long long h = 0;
+    double tau = 0.0, score = 0.0;
+    if (live) {
+        const Ray<Real> R = load_ray<Real>(P.rays, r);
+        // N1: only x, y, z, E, W are looked at (the direction fields of the record are ignored)
+        const bool fin = isfinite(R.o[0]) && isfinite(R.o[1]) && isfinite(R.o[2]) && isfinite((double)R.E) && isfinite(R.W);
+        const double d[3] = {__dsub_rn(D[0], R.o[0]), __dsub_rn(D[1], R.o[1]), __dsub_rn(D[2], R.o[2])};
+        const double R2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+        Walker w;
+        accepted = fin && (R.E > (Real)0) && isfinite(R2) && (R2 > 0.0) &&
+                   walker_init<EDGE_MODE>(w, axf, stride, P.mesh, e, R.o, d);
+        if (accepted) {
+            const double Rd = sqrt(R2);
+            Bracket<Real> br;
+            int grid = -1;
+            for (int m = 0; m < P.M; ++m) {                          // N2
+                const XsDesc t = P.xs[m];
+                if (t.grid != grid) { br = find_bracket<Real>(t, R.E); grid = t.grid; }
+                sig[m * stride] = sigma_at<Real>(t, br);
+            }
+            if (TRACE) h = 0xcbf29ce484222325ULL;
+            Rec rec;
+            rec.reset();
+            rec.load(P.recs, P.ids, P.K, w.c);
+            for (;;) {                                               // N5
+                const double tm = fmin(fmin(w.t0, w.t1), w.t2);      // value of the pending crossing (ties: same value)
+                const bool last = tm >= 1.0;
+                int cell = w.c;
+                double len;
+                bool leave = true;
+                const typename Rec::Value cur = rec.value();
+                if (last) len = __dsub_rn(1.0, w.tcur);
+                else {
+                    leave = walker_step<EDGE_MODE>(w, axf, stride, P.mesh, e, cell, len);
+                    if (!leave) rec.load(P.recs, P.ids, P.K, w.c);
+                }
+                const double S = (double)Rec::sigma(cur, sig, stride, P.K);
+                tau = fma(S, len * Rd, tau);
+                if (TRACE) {
+                    const unsigned cu = (unsigned)cell;
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        h ^= (unsigned long long)((cu >> (8 * b)) & 0xffu);
+                        h *= 0x100000001b3ULL;
+                    }
+                }
+                ++nseg;
+                if (leave) break;
+            }
+            score = R.W * exp_neg(tau) / R2;                         // N6
+        }
+        if (TRACE) {
+            if (P.nseg) P.nseg[r] = nseg;
+            if (P.hash) P.hash[r] = h;
+            if (P.tau) P.tau[r] = tau;
+            if (P.score) P.score[r] = score;
+        }
+    }
+    // CTA totals: one fp64 atomic per CTA into the detector's sum, three counter atomics per warp
+    const unsigned full = 0xffffffffu;
+    double v = score;
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(full, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) s_part[warp] = v;
+    const unsigned acc = __popc(__ballot_sync(full, accepted));
+    const unsigned rej = __popc(__ballot_sync(full, live && !accepted));
+    unsigned long long segs = nseg;
+    for (int o = 16; o > 0; o >>= 1) segs += __shfl_xor_sync(full, segs, o);
+    if (lane == 0 && P.counters) {
+        if (acc) atomicAdd(P.counters + 0, (unsigned long long)acc);
+        if (rej) atomicAdd(P.counters + 1, (unsigned long long)rej);
+        if (segs) atomicAdd(P.counters + 2, segs);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && P.det_sum) {
+        double t = 0.0;
+        for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += s_part[i];
+        if (t != 0.0) red_add_f64(P.det_sum + det, t);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Per-batch moments, SURVEY.md §8(f) NEXT-2 (Eq. (5): FOM = 1/(sigma^2 T), sigma the standard
+// deviation of the tally mean).  mr_end_batch folds the batch that just ended:
+//     x = tally[c] - prev[c];   s2[c] += x*x;   prev[c] = tally[c]
+// (the tally itself stays the running total, so sum_b x_b is the tally).  A pure stream: 40 B per cell.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) fold_batch_kernel(const double *__restrict__ tally, double *__restrict__ prev,
+                                                         double *__restrict__ s2, long long ncell)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x * 2;
+    for (long long c = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 2; c < ncell; c += stride) {
+        if (c + 1 < ncell) {
+            const double2 t = *reinterpret_cast<const double2 *>(tally + c);
+            double2 p = *reinterpret_cast<double2 *>(prev + c);
+            double2 q = *reinterpret_cast<double2 *>(s2 + c);
+            const double x0 = t.x - p.x, x1 = t.y - p.y;
+            q.x = fma(x0, x0, q.x);
+            q.y = fma(x1, x1, q.y);
+            *reinterpret_cast<double2 *>(s2 + c) = q;
+            *reinterpret_cast<double2 *>(prev + c) = t;
+        } else {
+            const double t = tally[c], x = t - prev[c];
+            s2[c] = fma(x, x, s2[c]);
+            prev[c] = t;
+        }
+    }
+}
+
+// mean = prev/B;  sigma = sqrt(max((s2/B - mean^2)/(B-1), 0))   (standard deviation OF THE MEAN; B = 1: +inf)
+__global__ void __launch_bounds__(256) mean_sigma_kernel(const double *__restrict__ prev, const double *__restrict__ s2,
+                                                         double *__restrict__ mean, double *__restrict__ sigma,
+                                                         long long ncell, long long B)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const double Bd = (double)B;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += stride) {
+        const double m = prev[c] / Bd;
+        mean[c] = m;
+        if (B > 1) {
+            const double var = (s2[c] / Bd - m * m) / (double)(B - 1);
+            sigma[c] = sqrt(fmax(var, 0.0));
+        } else
+            sigma[c] = __longlong_as_double(0x7ff0000000000000LL);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Set-up kernels (mr_load_materials): validate and pack a chunk of the per-cell composition.
 //   flags[0] |= 1 on an invalid material id, |= 2 on a non-finite or negative fraction.
 // ------------------------------------------------------------------------------------------------
