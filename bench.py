@@ -182,6 +182,9 @@ def main():
     ap.add_argument("--cpu-sample-rays", type=int, default=1_000_000, help="rays of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-next", action="store_true", help="skip the SURVEY 8(f) rows (next-event cast, batch-moment fold)")
+    ap.add_argument("--ne-rays", type=int, default=2_000_000, help="events per next-event step")
+    ap.add_argument("--ne-detectors", type=int, default=4)
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--sort", type=int, default=-1, help="override MR_OPT_SORT_RAYS (default: library default)")
     ap.add_argument("--opt", action="append", default=[], help="library option as ID=VALUE (MR_OPT_* of include/monteray.h), repeatable")
@@ -290,6 +293,53 @@ def main():
         dt = multi.max_over_ranks(dt, dev)
         e2e = {"value": seg_all * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(rays.nbytes),
                "d2h_bytes_per_step": int(prob.ncell * 8), "ms_per_step": 1e3 * dt / args.steps}
+    # ---------------------------------------------------------------- next-event cast, batch-moment fold
+    next_rows = None
+    if not args.no_next:
+        next_rows = {}
+        lo = np.array([prob.xe[0], prob.ye[0], prob.ze[0]])
+        hi = np.array([prob.xe[-1], prob.ye[-1], prob.ze[-1]])
+        g = np.random.default_rng(7)
+        dets = lo + (0.05 + 0.9 * g.random((args.ne_detectors, 3))) * (hi - lo)   # detector points inside the mesh
+        n_ne = min(args.ne_rays, n_rays)
+        m.load_detectors(dets)
+        d_ev = d_rays[:n_ne]
+        for _ in range(3):
+            m.cast_next_event(d_ev)
+        barrier()
+        s0 = m.get_stats()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = max(3, min(args.steps, 10))
+        a0.record()
+        for _ in range(reps):
+            m.cast_next_event(d_ev)
+        a1.record()
+        barrier()
+        ms = a0.elapsed_time(a1) / reps
+        s1 = m.get_stats()
+        ne_seg = (s1.ne_segments - s0.ne_segments) // reps
+        ne_bytes = ne_seg * (4 if dense else 5) * prob.K + n_ne * args.ne_detectors * (32 + 16 * prob.M)
+        next_rows["next_event"] = {
+            "value": ne_seg / (ms * 1e-3), "unit": "segments/s", "pairs_per_sec": n_ne * args.ne_detectors / (ms * 1e-3),
+            "ms_per_step": ms, "events": n_ne, "detectors": args.ne_detectors, "segments_per_step": int(ne_seg),
+            "roofline": {"bound": "hbm", "achieved": ne_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": ne_bytes / (ms * 1e-3) / 1e9 / peak,
+                         "algorithmic_bytes": "5K (4K dense) per segment + (32 + 16 M) per (event, detector) pair"}}
+        for _ in range(3):
+            m.end_batch()
+        barrier()
+        a0.record()
+        for _ in range(reps):
+            m.end_batch()
+        a1.record()
+        barrier()
+        ms = a0.elapsed_time(a1) / reps
+        fold_bytes = prob.ncell * 40
+        next_rows["end_batch"] = {
+            "value": prob.ncell / (ms * 1e-3), "unit": "cells/s", "ms_per_step": ms,
+            "roofline": {"bound": "hbm", "achieved": fold_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": fold_bytes / (ms * 1e-3) / 1e9 / peak,
+                         "algorithmic_bytes": "40 per cell (read tally, read+write previous total and sum of squares)"}}
     total_launches = m.get_stats().kernel_launches
 
     # ---------------------------------------------------------------- CPU oracle beside it (rank 0, N = 1)
@@ -315,7 +365,7 @@ def main():
                        "l2": "inputs larger than L2 (rays 320 MB + cell records 139 MB + tally 69 MB), no flush"
                        if args.config == 3 else "no flush"},
             "rays_per_sec": rays_all * args.steps / (ms_total * 1e-3),
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "next_rows": next_rows,
             "gpu_launches": int(launches), "gpu_launches_total": int(total_launches),
             "clocks": sampler.report() if sampler else None,
         }

@@ -221,6 +221,41 @@ MR_API int mr_clear_detectors(mr_ctx *ctx);
 MR_API int mr_trace_next_event(mr_ctx *ctx, int64_t n, const void *rays, int where, int det, uint32_t *nseg,
                                uint64_t *hash, double *tau, double *score);
 
+/* ---- producer ring (Fig. 4: "rays were stored in a buffer and
+ *      transferred to the GPU when the buffer became full ... the CPU cleared the buffer and resumed";
+ *      one buffer per node shared by the ranks that feed one GPU) ------------------- */
+
+typedef struct {
+    int64_t rays_pushed;      /* rays accepted by mr_ring_push since mr_ring_open */
+    int64_t slots_shipped;    /* buffers handed to the GPU (full ones and flushed partial ones) */
+    double producer_wait_ms;  /* total time producers spent blocked because every slot was in flight */
+    double reserved[3];
+} mr_ring_stats;
+
+/* Opens a ring of `slots` (2..16) page-locked host buffers of `rays_per_slot` rays each (>= 1024), with as many
+ * device buffers behind them.  Producers append rays with mr_ring_push; a buffer that becomes full is shipped:
+ * H2D copy on the copy stream, then the ordering pre-pass and the cast kernel on the context's stream, without
+ * blocking the producer -- which goes on filling the next buffer while the GPU works (Fig. 4).  A producer
+ * blocks only when every buffer is still being copied out.  Requires mesh, materials and all tables.
+ * Errors: INVALID_ARG, STATE (ring already open, set-up incomplete), OOM, CUDA. */
+MR_API int mr_ring_open(mr_ctx *ctx, int slots, int64_t rays_per_slot);
+
+/* Appends n rays (HOST array of the context's record type) to the ring.  THREAD-SAFE: any number of host
+ * threads may push concurrently (space is reserved under a lock, the copy into the page-locked buffer runs
+ * outside it); this is the only entry point, with mr_ring_flush, that may be called while other threads are
+ * inside the same context, and no other mr_* call may run at the same time.  The rays are consumed when the
+ * call returns.  n may exceed a buffer.  Errors: INVALID_ARG, STATE (ring not open), CUDA. */
+MR_API int mr_ring_push(mr_ctx *ctx, int64_t n, const void *rays);
+
+/* Ships the partly filled buffer, if any.  After mr_ring_flush (and once every producer has returned from its
+ * last push) all pushed rays are queued on the context's stream: mr_read_tally then includes them. */
+MR_API int mr_ring_flush(mr_ctx *ctx);
+
+/* Flushes, waits for the copies and frees the ring. */
+MR_API int mr_ring_close(mr_ctx *ctx);
+
+MR_API int mr_ring_get_stats(mr_ctx *ctx, mr_ring_stats *out);
+
 /* ---- test / diagnostic entry point ------------------------------------------------------- */
 
 /* The same walk as mr_cast_rays with no tally update.  Per ray r (host outputs, any may be

@@ -28,6 +28,7 @@ EXPORTS = [
     "mr_load_materials", "mr_load_xs", "mr_cast_rays", "mr_read_tally", "mr_clear_tally", "mr_sync",
     "mr_get_stats", "mr_tally_device_ptr", "mr_trace_rays", "mr_set_option", "mr_get_option",
     "mr_end_batch", "mr_read_moments", "mr_read_mean_sigma",
+    "mr_ring_open", "mr_ring_push", "mr_ring_flush", "mr_ring_close", "mr_ring_get_stats",
     "mr_load_detectors", "mr_cast_next_event", "mr_read_detectors", "mr_clear_detectors", "mr_trace_next_event",
 ]
 
@@ -42,6 +43,11 @@ class mr_stats(C.Structure):
     _fields_ = [("rays_accepted", C.c_int64), ("rays_rejected", C.c_int64), ("segments", C.c_int64),
                 ("kernel_launches", C.c_int64), ("last_cast_ms", C.c_double), ("last_kernel_ms", C.c_double),
                 ("ne_pairs_accepted", C.c_int64), ("ne_pairs_rejected", C.c_int64), ("ne_segments", C.c_int64)]
+
+
+class mr_ring_stats(C.Structure):
+    _fields_ = [("rays_pushed", C.c_int64), ("slots_shipped", C.c_int64), ("producer_wait_ms", C.c_double),
+                ("reserved", C.c_double * 3)]
 
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_void_p, C.c_size_t, C.c_int)
@@ -82,6 +88,11 @@ def load_library() -> C.CDLL:
         "mr_trace_rays": [vp, i64, vp, i32, vp, vp, vp, vp, i64],
         "mr_set_option": [vp, i32, i64],
         "mr_get_option": [vp, i32, C.POINTER(i64)],
+        "mr_ring_open": [vp, i32, i64],
+        "mr_ring_push": [vp, i64, vp],
+        "mr_ring_flush": [vp],
+        "mr_ring_close": [vp],
+        "mr_ring_get_stats": [vp, C.POINTER(mr_ring_stats)],
         "mr_end_batch": [vp],
         "mr_read_moments": [vp, vp, vp, C.POINTER(i64)],
         "mr_read_mean_sigma": [vp, vp, vp, C.POINTER(i64)],
@@ -306,6 +317,30 @@ class MonteRay:
                                            cells.ctypes.data if cap > 0 else None,
                                            lens.ctypes.data if cap > 0 else None, cap))
         return nseg, hsh, cells, lens
+
+    # ---- producer ring (NEXT-1)
+    def ring_open(self, slots: int, rays_per_slot: int):
+        self._check(self.lib.mr_ring_open(self._h, slots, rays_per_slot))
+
+    def ring_push(self, rays: np.ndarray):
+        """mr_ring_push of a host array; thread-safe (ctypes releases the GIL for the duration of the call)."""
+        a = rays if (isinstance(rays, np.ndarray) and rays.dtype == self.ray_dtype and rays.flags.c_contiguous) \
+            else np.ascontiguousarray(rays, dtype=self.ray_dtype)
+        rc = self.lib.mr_ring_push(self._h, a.size // 8, C.c_void_p(a.ctypes.data))
+        if rc != MR_OK:
+            raise MonteRayError(rc, "mr_ring_push failed")
+
+    def ring_flush(self):
+        self._check(self.lib.mr_ring_flush(self._h))
+
+    def ring_close(self):
+        self._check(self.lib.mr_ring_close(self._h))
+
+    def ring_stats(self):
+        s = mr_ring_stats()
+        self._check(self.lib.mr_ring_get_stats(self._h, C.byref(s)))
+        return {"rays_pushed": int(s.rays_pushed), "slots_shipped": int(s.slots_shipped),
+                "producer_wait_ms": float(s.producer_wait_ms)}
 
     # ---- per-batch moments (NEXT-2)
     def end_batch(self):

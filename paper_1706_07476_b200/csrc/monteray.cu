@@ -8,7 +8,11 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
+#include <chrono>
 #include <cmath>
+#include <condition_variable>
+#include <mutex>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -43,7 +47,33 @@ struct DeviceGuard {
 
 }  // namespace
 
+// Producer ring (mr_ring_*): `slots` page-locked buffers, each with a device buffer behind it.
+struct RingSlot {
+    enum State { FREE = 0, FILLING = 1, SHIPPING = 2, IN_FLIGHT = 3 };
+    void *pinned = nullptr;
+    void *d_buf = nullptr;
+    cudaEvent_t ev_copied = nullptr;   // H2D out of `pinned` finished: the host buffer may be refilled
+    cudaEvent_t ev_done = nullptr;     // kernels reading `d_buf` finished: the device buffer may be overwritten
+    int state = FREE;                  // guarded by Ring::m
+    long long cursor = 0;              // rays reserved (guarded by Ring::m)
+    std::atomic<long long> committed{0};   // rays whose copy into `pinned` has finished
+};
+
+struct Ring {
+    std::mutex m;                      // slot states, cursors, `open`
+    std::condition_variable cv;
+    std::mutex ship_m;                 // serialises the CUDA calls that ship a slot
+    std::vector<RingSlot *> slots;
+    long long cap = 0;                 // rays per slot
+    int open = 0;                      // slot being filled
+    long long rays_pushed = 0, slots_shipped = 0;
+    double wait_ms = 0.0;
+    int error = MR_OK;                 // first error of a ship
+    std::string error_msg;
+};
+
 struct mr_ctx {
+    Ring *ring = nullptr;
     int device = 0;
     int precision = MR_PRECISION_MIXED;
     cudaStream_t stream = nullptr;
@@ -494,6 +524,17 @@ int mr_destroy(mr_ctx *c)
     DeviceGuard guard(c->device);
     cudaStreamSynchronize(c->stream);
     if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
+    if (c->ring) {
+        for (RingSlot *s : c->ring->slots) {
+            if (s->ev_copied) { cudaEventSynchronize(s->ev_copied); cudaEventDestroy(s->ev_copied); }
+            if (s->ev_done) { cudaEventSynchronize(s->ev_done); cudaEventDestroy(s->ev_done); }
+            if (s->pinned) cudaFreeHost(s->pinned);
+            c->dev_free(s->d_buf);
+            delete s;
+        }
+        delete c->ring;
+        c->ring = nullptr;
+    }
     free_stage(c);
     free_tables(c);
     free_materials(c);
@@ -1241,6 +1282,215 @@ int mr_trace_next_event(mr_ctx *c, int64_t n, const void *rays, int where, int d
     cleanup();
     if (rc != MR_OK) return rc;
     if (e != cudaSuccess) return c->fail_cuda(e, "mr_trace_next_event");
+    return MR_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+void ring_free(mr_ctx *c)
+{
+    Ring *r = c->ring;
+    if (!r) return;
+    for (RingSlot *s : r->slots) {
+        if (s->ev_copied) { cudaEventSynchronize(s->ev_copied); cudaEventDestroy(s->ev_copied); }
+        if (s->ev_done) { cudaEventSynchronize(s->ev_done); cudaEventDestroy(s->ev_done); }
+        if (s->pinned) cudaFreeHost(s->pinned);
+        c->dev_free(s->d_buf);
+        delete s;
+    }
+    delete r;
+    c->ring = nullptr;
+}
+
+// Hands slot s (count rays, all reserved) to the GPU.  Called by the thread that filled it, no ring lock held.
+void ring_ship(mr_ctx *c, RingSlot *s, long long count)
+{
+    Ring *r = c->ring;
+    while (s->committed.load(std::memory_order_acquire) < count) std::this_thread::yield();   // other producers still copying in
+    int rc = MR_OK;
+    std::string msg;
+    {
+        std::lock_guard<std::mutex> g(r->ship_m);
+        DeviceGuard guard(c->device);
+        const size_t bytes = (size_t)count * c->ray_bytes();
+        cudaError_t e = cudaStreamWaitEvent(c->copy_stream, s->ev_done, 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(s->d_buf, s->pinned, bytes, cudaMemcpyHostToDevice, c->copy_stream);
+        if (e == cudaSuccess) e = cudaEventRecord(s->ev_copied, c->copy_stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(c->stream, s->ev_copied, 0);
+        if (e != cudaSuccess) {
+            rc = MR_ERR_CUDA;
+            msg = std::string("CUDA error while shipping a ring buffer: ") + cudaGetErrorString(e);
+        } else {
+            c->kev_used = 0;
+            rc = cast_device(c, count, s->d_buf);
+            if (rc != MR_OK) msg = c->err;
+            else if ((e = cudaEventRecord(s->ev_done, c->stream)) != cudaSuccess) {
+                rc = MR_ERR_CUDA;
+                msg = std::string("CUDA error while shipping a ring buffer: ") + cudaGetErrorString(e);
+            }
+        }
+    }
+    std::lock_guard<std::mutex> g(r->m);
+    if (rc != MR_OK && r->error == MR_OK) { r->error = rc; r->error_msg = msg; }
+    r->slots_shipped += 1;
+    s->state = RingSlot::IN_FLIGHT;
+    r->cv.notify_all();
+}
+
+// With r->m held: make r->open a slot that can take rays (waits for its last H2D copy if it is still in flight).
+void ring_acquire_open(mr_ctx *c, std::unique_lock<std::mutex> &lk)
+{
+    Ring *r = c->ring;
+    RingSlot *s = r->slots[r->open];
+    if (s->state == RingSlot::FILLING) return;
+    const auto t0 = std::chrono::steady_clock::now();
+    bool waited = false;
+    while (s->state == RingSlot::SHIPPING) { waited = true; r->cv.wait(lk); }    // its filler has not queued it yet
+    if (s->state == RingSlot::IN_FLIGHT) {
+        if (cudaEventQuery(s->ev_copied) != cudaSuccess) {
+            waited = true;
+            cudaGetLastError();
+            DeviceGuard guard(c->device);
+            cudaEventSynchronize(s->ev_copied);     // every slot is in flight: the producers have to wait (lock held on purpose)
+        }
+    }
+    if (waited) r->wait_ms += std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    s->state = RingSlot::FILLING;
+    s->cursor = 0;
+    s->committed.store(0, std::memory_order_release);
+}
+
+}  // namespace
+
+extern "C" {
+
+int mr_ring_open(mr_ctx *c, int slots, int64_t rays_per_slot)
+{
+    MR_ENTER(c);
+    if (c->ring) return c->fail(MR_ERR_STATE, "ring already open");
+    if (slots < 2 || slots > 16 || rays_per_slot < 1024 || rays_per_slot > (1LL << 28))
+        return c->fail(MR_ERR_INVALID_ARG, "ring: 2..16 slots of 1024..2^28 rays");
+    if (int rc = ready_to_cast(c)) return rc;
+    if (int rc = upload_xs_desc(c)) return rc;
+    Ring *r = new Ring();
+    c->ring = r;
+    r->cap = rays_per_slot;
+    const size_t bytes = (size_t)rays_per_slot * c->ray_bytes();
+    for (int i = 0; i < slots; ++i) {
+        RingSlot *s = new RingSlot();
+        r->slots.push_back(s);
+        bool ok = cudaMallocHost(&s->pinned, bytes) == cudaSuccess;
+        ok = ok && (s->d_buf = c->dev_alloc(bytes)) != nullptr;
+        ok = ok && cudaEventCreateWithFlags(&s->ev_copied, cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&s->ev_done, cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) {
+            cudaGetLastError();
+            ring_free(c);
+            return c->fail(MR_ERR_OOM, "ring: page-locked or device allocation failed");
+        }
+    }
+    // grow the ordering scratch now: cast_device must not synchronise the stream while producers run
+    if (c->sort_rays && rays_per_slot >= kSortMinRays) {
+        const uint32_t *perm = nullptr;
+        MR_CUDA(c, cudaMemsetAsync(r->slots[0]->d_buf, 0, bytes, c->stream));
+        if (int rc = order_rays(c, rays_per_slot, r->slots[0]->d_buf, &perm)) { ring_free(c); return rc; }
+        MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    return MR_OK;
+}
+
+int mr_ring_push(mr_ctx *c, int64_t n, const void *rays)
+{
+    if (!c) return MR_ERR_INVALID_ARG;
+    Ring *r = c->ring;
+    if (!r) return MR_ERR_STATE;
+    if (n < 0 || (n > 0 && !rays)) return MR_ERR_INVALID_ARG;
+    const size_t rb = c->ray_bytes();
+    const char *src = (const char *)rays;
+    while (n > 0) {
+        RingSlot *s;
+        long long off, take;
+        bool full;
+        {
+            std::unique_lock<std::mutex> lk(r->m);
+            if (r->error != MR_OK) return r->error;
+            ring_acquire_open(c, lk);
+            s = r->slots[r->open];
+            off = s->cursor;
+            take = std::min<long long>(n, r->cap - off);
+            s->cursor += take;
+            full = s->cursor == r->cap;
+            if (full) {
+                s->state = RingSlot::SHIPPING;
+                r->open = (r->open + 1) % (int)r->slots.size();
+            }
+            r->rays_pushed += take;
+        }
+        std::memcpy((char *)s->pinned + (size_t)off * rb, src, (size_t)take * rb);
+        s->committed.fetch_add(take, std::memory_order_acq_rel);
+        if (full) ring_ship(c, s, r->cap);
+        src += (size_t)take * rb;
+        n -= take;
+    }
+    return MR_OK;
+}
+
+int mr_ring_flush(mr_ctx *c)
+{
+    if (!c) return MR_ERR_INVALID_ARG;
+    Ring *r = c->ring;
+    if (!r) return MR_ERR_STATE;
+    RingSlot *s = nullptr;
+    long long count = 0;
+    {
+        std::unique_lock<std::mutex> lk(r->m);
+        RingSlot *o = r->slots[r->open];
+        if (o->state == RingSlot::FILLING && o->cursor > 0) {
+            s = o;
+            count = o->cursor;
+            o->state = RingSlot::SHIPPING;
+            r->open = (r->open + 1) % (int)r->slots.size();
+        }
+    }
+    if (s) ring_ship(c, s, count);
+    std::unique_lock<std::mutex> lk(r->m);
+    while (true) {   // every slot a producer marked SHIPPING has been queued
+        bool pending = false;
+        for (RingSlot *q : r->slots) pending = pending || q->state == RingSlot::SHIPPING;
+        if (!pending) break;
+        r->cv.wait(lk);
+    }
+    if (r->error != MR_OK) {
+        c->err = r->error_msg;
+        return r->error;
+    }
+    return MR_OK;
+}
+
+int mr_ring_close(mr_ctx *c)
+{
+    if (!c) return MR_ERR_INVALID_ARG;
+    if (!c->ring) return MR_OK;
+    const int rc = mr_ring_flush(c);
+    DeviceGuard guard(c->device);
+    cudaStreamSynchronize(c->copy_stream);
+    cudaStreamSynchronize(c->stream);
+    ring_free(c);
+    return rc;
+}
+
+int mr_ring_get_stats(mr_ctx *c, mr_ring_stats *out)
+{
+    if (!c || !out) return MR_ERR_INVALID_ARG;
+    std::memset(out, 0, sizeof(*out));
+    Ring *r = c->ring;
+    if (!r) return MR_ERR_STATE;
+    std::lock_guard<std::mutex> g(r->m);
+    out->rays_pushed = r->rays_pushed;
+    out->slots_shipped = r->slots_shipped;
+    out->producer_wait_ms = r->wait_ms;
     return MR_OK;
 }
 

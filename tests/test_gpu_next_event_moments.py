@@ -204,3 +204,65 @@ def test_mean_sigma_needs_a_closed_batch():
         m.end_batch()
         mean, sigma, nb = m.read_mean_sigma()
         assert nb == 1 and np.all(np.isinf(sigma)) and np.array_equal(mean, m.read_tally())
+
+
+# ------------------------------------------------------------------------------------- producer ring (NEXT-1)
+@pytest.mark.parametrize("precision,producers", [(0, 1), (0, 4), (1, 3)])
+def test_producer_ring_many_threads_equals_one_call(precision, producers):
+    """PAPER.md:77-83 (Fig. 4): producers fill a buffer, full buffers go to the GPU while the producers go on.
+    Several host threads push ragged pieces concurrently; after flush the tally and counters equal the oracle's
+    for the union of all pushed rays (buffers of 5000 rays: many ships, pieces that straddle buffers, a partial
+    last buffer)."""
+    import threading
+
+    prob = make_problem(3, nx=68, ny=68, nz=40, n_e=2000)
+    rays32 = make_rays(prob, 60_007)
+    ref = _oracle(prob).cast(rays32, threads=8)
+    with _mr(prob, precision) as m:
+        rays = np.ascontiguousarray(rays32.astype(m.ray_dtype))
+        m.ring_open(3, 5000)
+        bounds = np.linspace(0, len(rays), producers + 1).astype(int)
+
+        def produce(lo, hi, piece):
+            i = lo
+            while i < hi:
+                j = min(hi, i + piece)
+                m.ring_push(rays[i:j])
+                i = j
+
+        ts = [threading.Thread(target=produce, args=(bounds[k], bounds[k + 1], 777 + 1300 * k)) for k in range(producers)]
+        for t in ts:
+            t.start()
+        for t in ts:
+            t.join()
+        m.ring_flush()
+        got = m.read_tally()
+        st = m.get_stats()
+        rs = m.ring_stats()
+        m.ring_push(rays[:100])          # the ring stays usable after a flush
+        m.ring_close()
+        assert m.get_stats().rays_accepted == ref.rays_accepted + 100
+    assert rs["rays_pushed"] == len(rays) and rs["slots_shipped"] == -(-len(rays) // 5000)
+    assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+    d = np.abs(got - ref.tally)
+    bound = (1e-4 * np.abs(ref.tally) + 1e-7 * ref.tally.max()) if precision == 0 else (1e-10 * np.abs(ref.tally) + 1e-290)
+    assert np.all(d <= bound)
+
+
+def test_ring_call_order_errors():
+    from paper_1706_07476_b200 import MonteRay, MonteRayError
+
+    prob = make_problem(1)
+    with MonteRay(0, 0) as m:
+        with pytest.raises(MonteRayError):
+            m.ring_open(2, 4096)                 # nothing loaded
+        m.load_problem(prob)
+        with pytest.raises(MonteRayError):
+            m.ring_push(make_rays(prob, 10))     # ring not open
+        with pytest.raises(MonteRayError):
+            m.ring_open(1, 4096)
+        m.ring_open(2, 4096)
+        with pytest.raises(MonteRayError):
+            m.ring_open(2, 4096)                 # already open
+        m.ring_close()
+        m.ring_close()                           # idempotent
