@@ -185,6 +185,9 @@ def main():
     ap.add_argument("--no-next", action="store_true", help="skip the SURVEY 8(f) rows (next-event cast, batch-moment fold)")
     ap.add_argument("--ne-rays", type=int, default=2_000_000, help="events per next-event step")
     ap.add_argument("--ne-detectors", type=int, default=4)
+    ap.add_argument("--producers", type=int, default=4, help="host threads feeding the producer ring")
+    ap.add_argument("--ring-slots", type=int, default=4)
+    ap.add_argument("--ring-slot-rays", type=int, default=1 << 20)
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--sort", type=int, default=-1, help="override MR_OPT_SORT_RAYS (default: library default)")
     ap.add_argument("--opt", action="append", default=[], help="library option as ID=VALUE (MR_OPT_* of include/monteray.h), repeatable")
@@ -340,6 +343,45 @@ def main():
             "roofline": {"bound": "hbm", "achieved": fold_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                          "frac": fold_bytes / (ms * 1e-3) / 1e9 / peak,
                          "algorithmic_bytes": "40 per cell (read tally, read+write previous total and sum of squares)"}}
+        # NEXT-1 (Fig. 4): P host threads push the batch piecewise into the producer ring; buffers ship as they fill
+        P = max(1, args.producers)
+        bounds = np.linspace(0, n_rays, P + 1).astype(np.int64)
+        piece = 8192                      # rays per push: a burst of collision events
+
+        def produce(lo, hi):
+            i = lo
+            while i < hi:
+                j = min(hi, i + piece)
+                m.ring_push(rays[i:j])
+                i = j
+
+        def ring_step():
+            ts = [threading.Thread(target=produce, args=(int(bounds[k]), int(bounds[k + 1]))) for k in range(P)]
+            for t in ts:
+                t.start()
+            for t in ts:
+                t.join()
+            m.ring_flush()
+            m.read_tally_into(h_tally.data_ptr())
+
+        m.ring_open(args.ring_slots, min(args.ring_slot_rays, max(1024, n_rays)))
+        ring_step()
+        w0 = m.ring_stats()["producer_wait_ms"]
+        barrier()
+        reps = max(2, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            ring_step()
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / reps
+        rs = m.ring_stats()
+        m.ring_close()
+        next_rows["producer_ring"] = {
+            "value": seg_step / dt, "unit": UNIT, "ms_per_step": 1e3 * dt, "producers": P, "rays_per_push": piece,
+            "slots": args.ring_slots, "rays_per_slot": min(args.ring_slot_rays, max(1024, n_rays)),
+            "producer_wait_ms_per_step": (rs["producer_wait_ms"] - w0) / reps,
+            "device_only_ms_per_step": ms_total / args.steps,
+            "h2d_bytes_per_step": int(rays.nbytes), "d2h_bytes_per_step": int(prob.ncell * 8)}
     total_launches = m.get_stats().kernel_launches
 
     # ---------------------------------------------------------------- CPU oracle beside it (rank 0, N = 1)
