@@ -143,7 +143,7 @@ struct mr_ctx {
     // ray-ordering pre-pass scratch (grown on demand)
     uint32_t *d_keys = nullptr, *d_perm = nullptr, *d_hist = nullptr;
     long long sort_cap = 0;
-    int hist_cap = 0;
+    long long hist_cap = 0;
 
     size_t ray_bytes() const { return precision == MR_PRECISION_DOUBLE ? 64 : 32; }
     size_t real_bytes() const { return precision == MR_PRECISION_DOUBLE ? 8 : 4; }
@@ -324,10 +324,13 @@ int ready_to_cast(mr_ctx *c)
 constexpr long long kSortMinRays = 1 << 14;   // below this a batch is a handful of CTAs: ordering buys nothing
 
 // Queue the ordering pre-pass for n device-resident rays; *perm_out = null if the batch is cast in buffer order.
-int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm_out)
+// nsec > 0: next-event mode, one section per detector det_first .. det_first + nsec - 1 (keys, perm: n entries per
+// section; histogram: nkeys + 1 entries per section).
+int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm_out, int nsec = 0, int det_first = 0)
 {
     *perm_out = nullptr;
     if (!c->sort_rays || n < kSortMinRays || n > 0xffffffffLL || edges_smem_bytes(c) > kEdgesSmemMax) return MR_OK;
+    const int sections = std::max(nsec, 1);
     const int nlen = 128;
     const int zdiv = (c->nz + 255) / 256;
     const int nslab = (c->nz + zdiv - 1) / zdiv;
@@ -335,13 +338,14 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
     int lshift = 0;
     while ((maxlen >> lshift) >= nlen) ++lshift;
     const int nkeys = nslab * nlen + 1;
-    if (n > c->sort_cap) {
+    const long long entries = n * sections;
+    if (entries > c->sort_cap) {
         MR_CUDA(c, cudaStreamSynchronize(c->stream));
         c->dev_free(c->d_keys);
         c->dev_free(c->d_perm);
-        c->d_keys = (uint32_t *)c->dev_alloc((size_t)n * 4);
-        c->d_perm = (uint32_t *)c->dev_alloc((size_t)n * 4);
-        c->sort_cap = (c->d_keys && c->d_perm) ? n : 0;
+        c->d_keys = (uint32_t *)c->dev_alloc((size_t)entries * 4);
+        c->d_perm = (uint32_t *)c->dev_alloc((size_t)entries * 4);
+        c->sort_cap = (c->d_keys && c->d_perm) ? entries : 0;
         if (!c->sort_cap) {
             c->dev_free(c->d_keys);
             c->dev_free(c->d_perm);
@@ -349,21 +353,22 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
             return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering scratch)");
         }
     }
-    if (nkeys + 1 > c->hist_cap) {
+    const long long hist_entries = (long long)(nkeys + 1) * sections;
+    if (hist_entries > c->hist_cap) {
         MR_CUDA(c, cudaStreamSynchronize(c->stream));
         c->dev_free(c->d_hist);
-        c->d_hist = (uint32_t *)c->dev_alloc((size_t)(nkeys + 1) * 4);
-        c->hist_cap = c->d_hist ? nkeys + 1 : 0;
+        c->d_hist = (uint32_t *)c->dev_alloc((size_t)hist_entries * 4);
+        c->hist_cap = c->d_hist ? hist_entries : 0;
         if (!c->d_hist) return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering histogram)");
     }
     SortParams S{mesh_dev(c), d_rays, n, c->precision == MR_PRECISION_DOUBLE ? 1 : 0,
-                 zdiv, lshift, nlen, nkeys, c->d_keys, c->d_hist, c->d_perm};
-    MR_CUDA(c, cudaMemsetAsync(c->d_hist, 0, (size_t)(nkeys + 1) * 4, c->stream));
-    const unsigned grid = (unsigned)((n + 255) / 256);
+                 zdiv, lshift, nlen, nkeys, c->d_keys, c->d_hist, c->d_perm, nsec > 0 ? c->d_det : nullptr, det_first};
+    MR_CUDA(c, cudaMemsetAsync(c->d_hist, 0, (size_t)hist_entries * 4, c->stream));
+    const dim3 grid((unsigned)((n + 255) / 256), (unsigned)sections);
     const size_t smem = edges_smem_bytes(c);
     if (int rc = set_smem(c, classify_kernel, smem)) return rc;
     classify_kernel<<<grid, 256, smem, c->stream>>>(S);
-    scan_kernel<<<1, 1024, 0, c->stream>>>(c->d_hist, nkeys);
+    scan_kernel<<<sections, 1024, 0, c->stream>>>(c->d_hist, nkeys);
     scatter_kernel<<<grid, 256, 0, c->stream>>>(S);
     c->launches += 3;
     MR_CUDA(c, cudaGetLastError());
@@ -1087,8 +1092,14 @@ int next_event_device(mr_ctx *c, long long n, const void *d_rays)
         c->kev.push_back(b);
     }
     MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->stream));
-    P.det_first = 0;
-    if (int rc = launch_next_event<false>(c, P, c->ndet)) return rc;
+    // detectors in groups whose ordering scratch stays below 2^25 (event, detector) pairs
+    const int group = (int)std::max<long long>(1, std::min<long long>(c->ndet, (1LL << 25) / std::max<long long>(n, 1)));
+    for (int first = 0; first < c->ndet; first += group) {
+        const int count = std::min(group, c->ndet - first);
+        P.det_first = first;
+        if (int rc = order_rays(c, n, d_rays, &P.perm, count, first)) return rc;
+        if (int rc = launch_next_event<false>(c, P, count)) return rc;
+    }
     MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used + 1], c->stream));
     c->kev_used += 2;
     return MR_OK;
@@ -1340,26 +1351,33 @@ void ring_ship(mr_ctx *c, RingSlot *s, long long count)
 }
 
 // With r->m held: make r->open a slot that can take rays (waits for its last H2D copy if it is still in flight).
+// r->open may move while this thread sleeps on the condition variable, so it is re-read after every wait.
 void ring_acquire_open(mr_ctx *c, std::unique_lock<std::mutex> &lk)
 {
     Ring *r = c->ring;
-    RingSlot *s = r->slots[r->open];
-    if (s->state == RingSlot::FILLING) return;
+    if (r->slots[r->open]->state == RingSlot::FILLING) return;
     const auto t0 = std::chrono::steady_clock::now();
     bool waited = false;
-    while (s->state == RingSlot::SHIPPING) { waited = true; r->cv.wait(lk); }    // its filler has not queued it yet
-    if (s->state == RingSlot::IN_FLIGHT) {
-        if (cudaEventQuery(s->ev_copied) != cudaSuccess) {
+    for (;;) {
+        RingSlot *s = r->slots[r->open];
+        if (s->state == RingSlot::FILLING) break;                 // another producer re-opened it meanwhile
+        if (s->state == RingSlot::SHIPPING) {                     // its filler has not queued it yet
+            waited = true;
+            r->cv.wait(lk);
+            continue;
+        }
+        if (s->state == RingSlot::IN_FLIGHT && cudaEventQuery(s->ev_copied) != cudaSuccess) {
             waited = true;
             cudaGetLastError();
             DeviceGuard guard(c->device);
             cudaEventSynchronize(s->ev_copied);     // every slot is in flight: the producers have to wait (lock held on purpose)
         }
+        s->state = RingSlot::FILLING;
+        s->cursor = 0;
+        s->committed.store(0, std::memory_order_release);
+        break;
     }
     if (waited) r->wait_ms += std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
-    s->state = RingSlot::FILLING;
-    s->cursor = 0;
-    s->committed.store(0, std::memory_order_release);
 }
 
 }  // namespace

@@ -278,7 +278,8 @@ __device__ __forceinline__ bool walker_init(Walker &w, AxisF *axf, int stride, c
 
 // One step of the merge (O5).  On return `cell` = the cell just traversed, `len` its segment length;
 // the return value is true when the ray has left the mesh.
-template <int EDGE_MODE>
+// LIMIT (next-event walk): a pending crossing with parameter >= 1 ends the walk AT the detector (t = 1).
+template <int EDGE_MODE, bool LIMIT = false>
 __device__ __forceinline__ bool walker_step(Walker &w, const AxisF *axf, int stride, const MeshDev &m, const double *e,
                                             int &cell, double &len)
 {
@@ -286,6 +287,11 @@ __device__ __forceinline__ bool walker_step(Walker &w, const AxisF *axf, int str
     const double tm = ysel ? w.t1 : w.t0;
     const bool zsel = w.t2 < tm;                   // ties keep x / y
     const double tn = zsel ? w.t2 : tm;
+    if (LIMIT && tn >= 1.0) {
+        len = __dsub_rn(1.0, w.tcur);
+        cell = w.c;
+        return true;
+    }
     const int a = zsel ? 2 : (ysel ? 1 : 0);
     const AxisF af = axf[a * stride];
     const int pl = zsel ? w.pl2 : (ysel ? w.pl1 : w.pl0);
@@ -653,6 +659,7 @@ struct NextEventParams {
     int K, M;
     const XsDesc *xs;
     const void *rays;
+    const uint32_t *perm;          // optional processing order, one section of n entries per detector of the launch
     long long n;
     const double *det;             // [ndet*3] detector points
     int det_first;                 // first detector of this launch
@@ -701,13 +708,14 @@ __global__ void __launch_bounds__(256) next_event_kernel(const __grid_constant__
     const int det = P.det_first + blockIdx.y;
     const double D[3] = {__ldg(P.det + 3 * det), __ldg(P.det + 3 * det + 1), __ldg(P.det + 3 * det + 2)};
 
-    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = r < P.n;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = i < P.n;
     bool accepted = false;
     unsigned nseg = 0;
     unsigned long long h = 0;
     double tau = 0.0, score = 0.0;
     if (live) {
+        const long long r = P.perm ? (long long)__ldg(P.perm + (size_t)blockIdx.y * P.n + i) : i;
         const Ray<Real> R = load_ray<Real>(P.rays, r);
         // N1: only x, y, z, E, W are looked at (the direction fields of the record are ignored)
         const bool fin = isfinite(R.o[0]) && isfinite(R.o[1]) && isfinite(R.o[2]) && isfinite((double)R.E) && isfinite(R.W);
@@ -730,17 +738,11 @@ __global__ void __launch_bounds__(256) next_event_kernel(const __grid_constant__
             rec.reset();
             rec.load(P.recs, P.ids, P.K, w.c);
             for (;;) {                                               // N5
-                const double tm = fmin(fmin(w.t0, w.t1), w.t2);      // value of the pending crossing (ties: same value)
-                const bool last = tm >= 1.0;
-                int cell = w.c;
+                int cell;
                 double len;
-                bool leave = true;
                 const typename Rec::Value cur = rec.value();
-                if (last) len = __dsub_rn(1.0, w.tcur);
-                else {
-                    leave = walker_step<EDGE_MODE>(w, axf, stride, P.mesh, e, cell, len);
-                    if (!leave) rec.load(P.recs, P.ids, P.K, w.c);
-                }
+                const bool leave = walker_step<EDGE_MODE, true>(w, axf, stride, P.mesh, e, cell, len);
+                if (!leave) rec.load(P.recs, P.ids, P.K, w.c);
                 const double S = (double)Rec::sigma(cur, sig, stride, P.K);
                 tau = fma(S, len * Rd, tau);
                 if (TRACE) {
@@ -757,6 +759,7 @@ __global__ void __launch_bounds__(256) next_event_kernel(const __grid_constant__
             score = R.W * exp_neg(tau) / R2;                         // N6
         }
         if (TRACE) {
+            const long long r = i;                                   // trace launches are never reordered
             if (P.nseg) P.nseg[r] = nseg;
             if (P.hash) P.hash[r] = h;
             if (P.tau) P.tau[r] = tau;

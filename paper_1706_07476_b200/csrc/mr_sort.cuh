@@ -27,6 +27,10 @@ struct SortParams {
     uint32_t *keys;  // [n]
     uint32_t *hist;  // [nkeys + 1], zeroed before classify; becomes the exclusive prefix after scan
     uint32_t *perm;  // [n]
+    // next-event mode (det != null): blockIdx.y = detector det_first + y; the "direction" of ray r is det - origin,
+    // the walk ends at the detector (t = 1); keys / hist / perm hold one section per detector of the launch
+    const double *det;
+    int det_first;
 };
 
 // dynamic shared memory: [edges] (always staged: the search would otherwise hammer global memory)
@@ -43,11 +47,19 @@ __global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
     if (P.ray_is_double) {
         const Ray<double> R = load_ray_f64(P.rays, r);
         for (int a = 0; a < 3; ++a) { o[a] = R.o[a]; d[a] = R.d[a]; }
-        ok = R.finite && R.E > 0.0;
+        ok = (P.det ? (isfinite(o[0]) && isfinite(o[1]) && isfinite(o[2]) && isfinite(R.E) && isfinite(R.W)) : R.finite) && R.E > 0.0;
     } else {
         const Ray<float> R = load_ray_f32(P.rays, r);
         for (int a = 0; a < 3; ++a) { o[a] = R.o[a]; d[a] = R.d[a]; }
-        ok = R.finite && R.E > 0.0f;
+        ok = (P.det ? (isfinite(o[0]) && isfinite(o[1]) && isfinite(o[2]) && isfinite(R.E) && isfinite(R.W)) : R.finite) && R.E > 0.0f;
+    }
+    uint32_t *keys = P.keys, *hist = P.hist;
+    if (P.det) {
+        const double *D = P.det + 3 * (size_t)(P.det_first + blockIdx.y);
+        for (int a = 0; a < 3; ++a) d[a] = __ldg(D + a) - o[a];
+        ok = ok && isfinite(d[0]) && isfinite(d[1]) && isfinite(d[2]);
+        keys += (size_t)blockIdx.y * P.n;
+        hist += (size_t)blockIdx.y * (P.nkeys + 1);
     }
     const int base[3] = {0, P.mesh.nx + 1, P.mesh.nx + P.mesh.ny + 2};
     const int n[3] = {P.mesh.nx, P.mesh.ny, P.mesh.nz};
@@ -62,6 +74,7 @@ __global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
             t_exit = fmin(t_exit, t);
         }
     }
+    if (P.det) t_exit = fmin(t_exit, 1.0);   // the walk ends at the detector
     ok = ok && isfinite(t_exit);
     uint32_t key = (uint32_t)(P.nkeys - 1);
     if (ok) {
@@ -75,13 +88,14 @@ __global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
         }
         key = (uint32_t)((idx[2] / P.zdiv) * P.nlen + min(est >> P.lshift, P.nlen - 1));
     }
-    P.keys[r] = key;
-    atomicAdd(P.hist + key, 1u);
+    keys[r] = key;
+    atomicAdd(hist + key, 1u);
 }
 
-// one CTA: exclusive prefix sum of hist[0..nkeys) in place
+// one CTA per histogram (blockIdx.x = section, nkeys + 1 entries apart): exclusive prefix sum of hist[0..nkeys) in place
 __global__ void __launch_bounds__(1024) scan_kernel(uint32_t *hist, int nkeys)
 {
+    hist += (size_t)blockIdx.x * (nkeys + 1);
     __shared__ uint32_t warp_tot[32];
     __shared__ uint32_t carry;
     if (threadIdx.x == 0) carry = 0;
@@ -118,8 +132,9 @@ __global__ void __launch_bounds__(256) scatter_kernel(const SortParams P)
 {
     const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= P.n) return;
-    const uint32_t pos = atomicAdd(P.hist + P.keys[r], 1u);
-    P.perm[pos] = (uint32_t)r;
+    const size_t sec = P.det ? blockIdx.y : 0;
+    const uint32_t pos = atomicAdd(P.hist + sec * (P.nkeys + 1) + P.keys[sec * P.n + r], 1u);
+    P.perm[sec * P.n + pos] = (uint32_t)r;
 }
 
 }  // namespace mr

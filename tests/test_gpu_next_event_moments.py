@@ -207,8 +207,8 @@ def test_mean_sigma_needs_a_closed_batch():
 
 
 # ------------------------------------------------------------------------------------- producer ring (NEXT-1)
-@pytest.mark.parametrize("precision,producers", [(0, 1), (0, 4), (1, 3)])
-def test_producer_ring_many_threads_equals_one_call(precision, producers):
+@pytest.mark.parametrize("precision,producers,slots,cap", [(0, 1, 3, 5000), (0, 4, 3, 5000), (1, 3, 3, 5000), (0, 8, 2, 1024)])
+def test_producer_ring_many_threads_equals_one_call(precision, producers, slots, cap):
     """PAPER.md:77-83 (Fig. 4): producers fill a buffer, full buffers go to the GPU while the producers go on.
     Several host threads push ragged pieces concurrently; after flush the tally and counters equal the oracle's
     for the union of all pushed rays (buffers of 5000 rays: many ships, pieces that straddle buffers, a partial
@@ -220,7 +220,7 @@ def test_producer_ring_many_threads_equals_one_call(precision, producers):
     ref = _oracle(prob).cast(rays32, threads=8)
     with _mr(prob, precision) as m:
         rays = np.ascontiguousarray(rays32.astype(m.ray_dtype))
-        m.ring_open(3, 5000)
+        m.ring_open(slots, cap)
         bounds = np.linspace(0, len(rays), producers + 1).astype(int)
 
         def produce(lo, hi, piece):
@@ -230,7 +230,7 @@ def test_producer_ring_many_threads_equals_one_call(precision, producers):
                 m.ring_push(rays[i:j])
                 i = j
 
-        ts = [threading.Thread(target=produce, args=(bounds[k], bounds[k + 1], 777 + 1300 * k)) for k in range(producers)]
+        ts = [threading.Thread(target=produce, args=(bounds[k], bounds[k + 1], 777 + 1300 * (k % 3))) for k in range(producers)]
         for t in ts:
             t.start()
         for t in ts:
@@ -242,7 +242,7 @@ def test_producer_ring_many_threads_equals_one_call(precision, producers):
         m.ring_push(rays[:100])          # the ring stays usable after a flush
         m.ring_close()
         assert m.get_stats().rays_accepted == ref.rays_accepted + 100
-    assert rs["rays_pushed"] == len(rays) and rs["slots_shipped"] == -(-len(rays) // 5000)
+    assert rs["rays_pushed"] == len(rays) and rs["slots_shipped"] == -(-len(rays) // cap)
     assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
     d = np.abs(got - ref.tally)
     bound = (1e-4 * np.abs(ref.tally) + 1e-7 * ref.tally.max()) if precision == 0 else (1e-10 * np.abs(ref.tally) + 1e-290)
