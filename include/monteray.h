@@ -272,7 +272,10 @@ enum {
     MR_OPT_SORT_RAYS = 2,     /* 0: cast in buffer order; 1: bin rays by start slab and length first */
     MR_OPT_STAGE_RAYS = 3,    /* rays per staging chunk for host batches (H2D of chunk i+1 overlaps the cast of chunk i) */
     MR_OPT_COPY_THREADS = 4,  /* host threads that copy a PAGEABLE batch into the pinned ring (a pinned batch is DMA'd directly) */
-    MR_OPT_PAIR_RECORDS = 5   /* 1: 16-byte cell records (K = 2, 3, MIXED) are fetched as 32-byte pairs kept in registers; 0: one by one */
+    MR_OPT_PAIR_RECORDS = 5,  /* 1: 16-byte cell records (K = 2, 3, MIXED) are fetched as 32-byte pairs kept in registers; 0: one by one */
+    MR_OPT_ORDER_MODE = 6     /* key of the MR_OPT_SORT_RAYS pre-pass: 1 = (start z-slab, length): CTAs resident together work in the
+                                 same slabs (L2 reuse); 2 = longest rays first: no tail; 0 = auto: 2 when tally + cell records fit
+                                 in half the L2, else 1 */
 };
 MR_API int mr_set_option(mr_ctx *ctx, int option, int64_t value);
 MR_API int mr_get_option(mr_ctx *ctx, int option, int64_t *value);

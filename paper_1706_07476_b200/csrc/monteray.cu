@@ -145,6 +145,11 @@ struct mr_ctx {
     long long sort_cap = 0;
     long long hist_cap = 0;
 
+    int order_mode = 0;              // option MR_OPT_ORDER_MODE: 0 auto, 1 slab-major, 2 longest first
+    size_t l2_bytes = 0;             // device L2 size
+    size_t rec_bytes_per_cell = 0;
+    size_t resident_bytes() const { return (size_t)ncell * (8 + rec_bytes_per_cell); }   // tally + cell records
+
     size_t ray_bytes() const { return precision == MR_PRECISION_DOUBLE ? 64 : 32; }
     size_t real_bytes() const { return precision == MR_PRECISION_DOUBLE ? 8 : 4; }
 
@@ -362,7 +367,9 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
         if (!c->d_hist) return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering histogram)");
     }
     SortParams S{mesh_dev(c), d_rays, n, c->precision == MR_PRECISION_DOUBLE ? 1 : 0,
-                 zdiv, lshift, nlen, nkeys, c->d_keys, c->d_hist, c->d_perm, nsec > 0 ? c->d_det : nullptr, det_first};
+                 zdiv, lshift, nlen, nkeys, c->d_keys, c->d_hist, c->d_perm, nsec > 0 ? c->d_det : nullptr, det_first,
+                 c->order_mode == 2 || (c->order_mode == 0 && c->resident_bytes() <= c->l2_bytes / 2) ? 1 : 0, nslab,
+                 c->mesh_arith ? 1 : 0};
     MR_CUDA(c, cudaMemsetAsync(c->d_hist, 0, (size_t)hist_entries * 4, c->stream));
     const dim3 grid((unsigned)((n + 255) / 256), (unsigned)sections);
     const size_t smem = edges_smem_bytes(c);
@@ -500,6 +507,11 @@ int mr_create_ex(mr_ctx **out, int device, int precision, const mr_allocator *al
     mr_ctx *c = new mr_ctx();
     c->device = device;
     c->precision = precision;
+    {
+        int l2 = 0;
+        if (cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, device) != cudaSuccess) cudaGetLastError();
+        c->l2_bytes = (size_t)std::max(l2, 0);
+    }
     if (alloc) c->alloc = *alloc;
     DeviceGuard guard(device);
     bool ok = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
@@ -702,6 +714,7 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
     c->d_recs = recs;
     c->d_ids = ids;
     c->layout = layout;
+    c->rec_bytes_per_cell = rec_bytes + id_bytes;
     c->K = K;
     if (M != c->M || (int)c->xs_n.size() != M) {
         c->M = M;
@@ -1532,6 +1545,10 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "pair-records option is 0 or 1");
         c->pair_records = (int)value;
         return MR_OK;
+    case MR_OPT_ORDER_MODE:
+        if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "order mode is 0 (auto), 1 (slab-major) or 2 (longest first)");
+        c->order_mode = (int)value;
+        return MR_OK;
     case MR_OPT_COPY_THREADS:
         if (value < 1 || value > 64) return c->fail(MR_ERR_INVALID_ARG, "copy threads must be in [1, 64]");
         c->copy_threads = (int)value;
@@ -1550,6 +1567,7 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     case MR_OPT_STAGE_RAYS: *value = c->stage_rays; return MR_OK;
     case MR_OPT_COPY_THREADS: *value = c->copy_threads; return MR_OK;
     case MR_OPT_PAIR_RECORDS: *value = c->pair_records; return MR_OK;
+    case MR_OPT_ORDER_MODE: *value = c->order_mode; return MR_OK;
     }
     return c->fail(MR_ERR_INVALID_ARG, "unknown option");
 }

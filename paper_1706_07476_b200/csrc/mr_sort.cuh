@@ -31,6 +31,11 @@ struct SortParams {
     // the walk ends at the detector (t = 1); keys / hist / perm hold one section per detector of the launch
     const double *det;
     int det_first;
+    // 1: length-major order, longest rays first (working set fits in L2, so slab locality buys nothing and the
+    // kernel's tail -- the last CTAs still walking long rays -- is what costs); 0: slab-major, length within a slab
+    int longest_first;
+    int nslab;
+    int arith;       // the mesh is arithmetic (MeshDev::e0, h valid): cell indices by one multiply instead of a search
 };
 
 // dynamic shared memory: [edges] (always staged: the search would otherwise hammer global memory)
@@ -42,6 +47,11 @@ __global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
     __syncthreads();
     const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= P.n) return;
+    // the key only orders the work: an index that is off by one near a plane is harmless here
+    auto cell_of = [&](int a, int base, int n, double x) {
+        if (P.arith) return min(max((int)floor((x - P.mesh.e0[a]) / P.mesh.h[a]), 0), n - 1);
+        return min(max(upper_bound_edges(e + base, n + 1, x) - 1, 0), n - 1);
+    };
     double o[3], d[3];
     bool ok;
     if (P.ray_is_double) {
@@ -68,7 +78,7 @@ __global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
     for (int a = 0; a < 3 && ok; ++a) {
         ok = (o[a] >= e[base[a]] && o[a] < e[base[a] + n[a]]);
         if (!ok) break;
-        idx[a] = upper_bound_edges(e + base[a], n[a] + 1, o[a]) - 1;
+        idx[a] = cell_of(a, base[a], n[a], o[a]);
         if (d[a] != 0.0) {
             const double t = (e[base[a] + (d[a] > 0.0 ? n[a] : 0)] - o[a]) / d[a];
             t_exit = fmin(t_exit, t);
@@ -82,14 +92,17 @@ __global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
         for (int a = 0; a < 3; ++a) {
             double x = fma(t_exit, d[a], o[a]);
             x = fmin(fmax(x, e[base[a]]), e[base[a] + n[a]]);
-            int j = upper_bound_edges(e + base[a], n[a] + 1, x) - 1;
-            j = min(max(j, 0), n[a] - 1);
-            est += abs(j - idx[a]);
+            est += abs(cell_of(a, base[a], n[a], x) - idx[a]);
         }
-        key = (uint32_t)((idx[2] / P.zdiv) * P.nlen + min(est >> P.lshift, P.nlen - 1));
+        const int lb = min(est >> P.lshift, P.nlen - 1);
+        key = P.longest_first ? (uint32_t)((P.nlen - 1 - lb) * P.nslab + idx[2] / P.zdiv)
+                              : (uint32_t)((idx[2] / P.zdiv) * P.nlen + lb);
     }
     keys[r] = key;
-    atomicAdd(hist + key, 1u);
+    // one atomic per distinct key of the warp (rays born in one small region share a handful of keys)
+    const unsigned act = __activemask();
+    const unsigned peers = __match_any_sync(act, key);
+    if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(hist + key, (unsigned)__popc(peers));
 }
 
 // one CTA per histogram (blockIdx.x = section, nkeys + 1 entries apart): exclusive prefix sum of hist[0..nkeys) in place
@@ -133,7 +146,14 @@ __global__ void __launch_bounds__(256) scatter_kernel(const SortParams P)
     const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= P.n) return;
     const size_t sec = P.det ? blockIdx.y : 0;
-    const uint32_t pos = atomicAdd(P.hist + sec * (P.nkeys + 1) + P.keys[sec * P.n + r], 1u);
+    const uint32_t key = P.keys[sec * P.n + r];
+    const unsigned act = __activemask();
+    const unsigned peers = __match_any_sync(act, key);
+    const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
+    uint32_t base = 0;
+    if (lane == leader) base = atomicAdd(P.hist + sec * (P.nkeys + 1) + key, (unsigned)__popc(peers));
+    base = __shfl_sync(peers, base, leader);
+    const uint32_t pos = base + __popc(peers & ((1u << lane) - 1u));
     P.perm[sec * P.n + pos] = (uint32_t)r;
 }
 

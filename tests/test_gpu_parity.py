@@ -299,3 +299,25 @@ def test_ray_ordering_prepass_on_and_off(precision):
             assert st.kernel_launches - before == (4 if sort else 1)
             assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
             assert_tally(m.read_tally(), ref.tally, precision)
+
+
+def test_order_modes_give_the_same_result():
+    """MR_OPT_ORDER_MODE (slab-major / longest first / auto) only permutes the work: counters identical,
+    tally within tolerance of the oracle in every mode."""
+    from paper_1706_07476_b200 import MR_OPT_ORDER_MODE
+
+    prob = make_problem(2, nx=60, ny=60, nz=30, n_e=2000)
+    rays = make_rays(prob, 50_003)
+    ref = _oracle(prob).cast(rays, threads=_threads())
+    with _mr(prob, 0) as m:
+        assert m.get_option(MR_OPT_ORDER_MODE) == 0
+        for mode in (1, 2, 0):
+            m.set_option(MR_OPT_ORDER_MODE, mode)
+            m.clear_tally()
+            m.cast_rays(rays)
+            st = m.get_stats()
+            assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+            assert_tally(m.read_tally(), ref.tally, 0)
+        from paper_1706_07476_b200 import MonteRayError
+        with pytest.raises(MonteRayError):
+            m.set_option(MR_OPT_ORDER_MODE, 3)
