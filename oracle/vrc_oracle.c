@@ -50,6 +50,18 @@ typedef struct {
     const int64_t *xs_off;     /* [M+1] offsets of each material's table in xs_E / xs_sig */
     const double *xs_E;        /* energies, MeV, strictly increasing per table */
     const double *xs_sig;      /* total cross sections, cm^2/g */
+    /* Multi-nuclide materials ("first calculating all cross-sections"): a
+     * material m with mix_off[m+1] > mix_off[m] has no table of its own; its cross section is the weighted sum
+     * of nuclide tables  sigma_m(E) = sum_j mix_w[j] * sigma_{mix_nuc[j]}(E),  j = mix_off[m] .. mix_off[m+1]-1,
+     * added in that order, each nuclide table lin-lin interpolated and end-clamped like a material table.
+     * N = 0 (and NULL pointers): no nuclides. */
+    int32_t N;
+    const int64_t *nxs_off;    /* [N+1] offsets of each nuclide's table in nxs_E / nxs_sig */
+    const double *nxs_E;
+    const double *nxs_sig;
+    const int64_t *mix_off;    /* [M+1] */
+    const int32_t *mix_nuc;    /* nuclide index per entry */
+    const double *mix_w;       /* weight per entry (e.g. mass fraction: sigma stays in cm^2/g) */
 } vrc_problem;
 
 typedef struct {
@@ -96,12 +108,26 @@ static int64_t upper_bound(const double *a, int64_t n, double v)
     return lo;
 }
 
-/* O2: lin-lin interpolated sigma_m(E), clamped to the end values (reading Q5). */
+/* lin-lin interpolation in one table, clamped to the end values (reading Q5) */
+static double table_sigma(const double *Eg, const double *Sg, int64_t n, double E);
+
+/* O2: sigma_m(E): the material's own table, or the weighted sum of its nuclides' tables. */
 double vrc_sigma(const vrc_problem *p, int32_t m, double E)
 {
-    const double *Eg = p->xs_E + p->xs_off[m];
-    const double *Sg = p->xs_sig + p->xs_off[m];
-    int64_t n = p->xs_off[m + 1] - p->xs_off[m];
+    if (p->N > 0 && p->mix_off && p->mix_off[m + 1] > p->mix_off[m]) {
+        double s = 0.0;
+        for (int64_t j = p->mix_off[m]; j < p->mix_off[m + 1]; ++j) {
+            int32_t q = p->mix_nuc[j];
+            s += p->mix_w[j] * table_sigma(p->nxs_E + p->nxs_off[q], p->nxs_sig + p->nxs_off[q],
+                                           p->nxs_off[q + 1] - p->nxs_off[q], E);
+        }
+        return s;
+    }
+    return table_sigma(p->xs_E + p->xs_off[m], p->xs_sig + p->xs_off[m], p->xs_off[m + 1] - p->xs_off[m], E);
+}
+
+static double table_sigma(const double *Eg, const double *Sg, int64_t n, double E)
+{
     if (n == 1 || E < Eg[0]) return Sg[0];
     if (E >= Eg[n - 1]) return Sg[n - 1];
     int64_t k = upper_bound(Eg, n, E) - 1;

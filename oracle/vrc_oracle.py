@@ -38,7 +38,9 @@ class _Problem(C.Structure):
                 ("xe", C.c_void_p), ("ye", C.c_void_p), ("ze", C.c_void_p),
                 ("M", C.c_int32), ("density", C.c_void_p), ("K", C.c_int32),
                 ("cell_mat", C.c_void_p), ("cell_frac", C.c_void_p),
-                ("xs_off", C.c_void_p), ("xs_E", C.c_void_p), ("xs_sig", C.c_void_p)]
+                ("xs_off", C.c_void_p), ("xs_E", C.c_void_p), ("xs_sig", C.c_void_p),
+                ("N", C.c_int32), ("nxs_off", C.c_void_p), ("nxs_E", C.c_void_p), ("nxs_sig", C.c_void_p),
+                ("mix_off", C.c_void_p), ("mix_nuc", C.c_void_p), ("mix_w", C.c_void_p)]
 
 
 class _Counts(C.Structure):
@@ -136,16 +138,49 @@ class Oracle:
         self._frac = np.ascontiguousarray(prob.cell_frac, dtype=np.float64).reshape(-1)
         assert self._mat.size == self.ncell * self.K and self._frac.size == self.ncell * self.K
         assert len(prob.xs) == self.M and self.M <= 64
+        # optional multi-nuclide materials: prob.nuclide_xs = [(E, sigma)], prob.mixtures[m] = (nuclide ids, weights) | None
+        mixtures = getattr(prob, "mixtures", None) or [None] * self.M
+        nuclide_xs = getattr(prob, "nuclide_xs", None) or []
         off = np.zeros(self.M + 1, dtype=np.int64)
-        for m, (e, s) in enumerate(prob.xs):
+        tabs = []
+        for m, t in enumerate(prob.xs):
+            if mixtures[m] is not None:
+                off[m + 1] = off[m]          # no table of its own
+                continue
+            e, s = t
             assert len(e) == len(s) and len(e) >= 1
             off[m + 1] = off[m] + len(e)
+            tabs.append((e, s))
         self._off = off
-        self._E = np.ascontiguousarray(np.concatenate([np.asarray(e, dtype=np.float64) for e, _ in prob.xs]))
-        self._S = np.ascontiguousarray(np.concatenate([np.asarray(s, dtype=np.float64) for _, s in prob.xs]))
+        self._E = np.ascontiguousarray(np.concatenate([np.asarray(e, dtype=np.float64) for e, _ in tabs] or [np.zeros(1)]))
+        self._S = np.ascontiguousarray(np.concatenate([np.asarray(s, dtype=np.float64) for _, s in tabs] or [np.zeros(1)]))
+        self.N = len(nuclide_xs)
+        noff = np.zeros(self.N + 1, dtype=np.int64)
+        for q, (e, s) in enumerate(nuclide_xs):
+            assert len(e) == len(s) and len(e) >= 1
+            noff[q + 1] = noff[q] + len(e)
+        self._noff = noff
+        self._nE = np.ascontiguousarray(np.concatenate([np.asarray(e, dtype=np.float64) for e, _ in nuclide_xs] or [np.zeros(1)]))
+        self._nS = np.ascontiguousarray(np.concatenate([np.asarray(s, dtype=np.float64) for _, s in nuclide_xs] or [np.zeros(1)]))
+        moff = np.zeros(self.M + 1, dtype=np.int64)
+        mn, mw = [], []
+        for m in range(self.M):
+            k = 0
+            if mixtures[m] is not None:
+                ids, w = mixtures[m]
+                assert len(ids) == len(w) and len(ids) >= 1 and all(0 <= int(q) < self.N for q in ids)
+                mn += [int(q) for q in ids]
+                mw += [float(x) for x in w]
+                k = len(ids)
+            moff[m + 1] = moff[m] + k
+        self._moff = moff
+        self._mn = np.ascontiguousarray(np.array(mn or [0], dtype=np.int32))
+        self._mw = np.ascontiguousarray(np.array(mw or [0.0], dtype=np.float64))
         self._p = _Problem(self.nx, self.ny, self.nz, self._xe.ctypes.data, self._ye.ctypes.data,
                            self._ze.ctypes.data, self.M, self._den.ctypes.data, self.K, self._mat.ctypes.data,
-                           self._frac.ctypes.data, self._off.ctypes.data, self._E.ctypes.data, self._S.ctypes.data)
+                           self._frac.ctypes.data, self._off.ctypes.data, self._E.ctypes.data, self._S.ctypes.data,
+                           self.N, self._noff.ctypes.data, self._nE.ctypes.data, self._nS.ctypes.data,
+                           self._moff.ctypes.data, self._mn.ctypes.data, self._mw.ctypes.data)
 
     def sigma(self, m: int, E: float) -> float:
         return float(self.lib.vrc_sigma(C.byref(self._p), int(m), float(E)))

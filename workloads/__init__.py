@@ -9,6 +9,7 @@ from .configs import (  # noqa: F401
     CONFIG_NAMES,
     FULL_RAYS,
     Problem,
+    add_nuclides,
     make_problem,
     make_rays,
     rng_for,

@@ -344,3 +344,32 @@ def make_rays(prob: Problem, n: int, batch: int = 0) -> np.ndarray:
     d = _isotropic(g, n)
     w = 0.5 + g.random(n)
     return _pack(pos, d, e, w, lo, hi)
+
+
+# --------------------------------------------------------------------------- multi-nuclide materials (NEXT-4)
+def add_nuclides(prob, n_nuclides: int = 6, max_per_material: int = 4, keep_direct: int = 1, seed_stream: int = 20):
+    """Returns a shallow copy of `prob` in which every material but the first `keep_direct` is a mixture of
+    nuclides: sigma_m(E) = sum_j w_j sigma_nuclide_j(E).  Nuclide tables are synthetic (same recipe as the
+    material tables) on grids of DIFFERENT sizes (no unionised grid), weights are fp32-representable mass
+    fractions that sum to about 1.  Input generation only: no method arithmetic."""
+    import copy
+
+    g = rng_for(prob.config, seed_stream)
+    q = copy.copy(prob)
+    n_e = max(len(e) for e, _ in prob.xs)
+    sizes = [max(9, int(n_e * f)) for f in (1.0, 0.5, 0.37, 0.81, 0.25, 0.66, 0.45, 0.9)]
+    q.nuclide_xs = [xs_table(prob.config, seed_stream + 1 + j, sizes[j % len(sizes)], 0.05 + 0.3 * g.random(),
+                             0.01 * 10.0 ** (2.0 * g.random()), max(3, min(200, sizes[j % len(sizes)] // 200)))
+                    for j in range(n_nuclides)]
+    q.mixtures = []
+    q.xs = list(prob.xs)
+    for m in range(prob.M):
+        if m < keep_direct:
+            q.mixtures.append(None)
+            continue
+        k = int(g.integers(1, max_per_material + 1))
+        ids = g.choice(n_nuclides, size=min(k, n_nuclides), replace=False).astype(np.int32)
+        w = g.random(len(ids)) + 0.05
+        q.mixtures.append((ids, f32r(w / w.sum())))
+        q.xs[m] = None
+    return q
