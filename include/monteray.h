@@ -66,6 +66,8 @@ enum { MR_WHERE_HOST = 0, MR_WHERE_DEVICE = 1 };
 
 #define MR_MAX_MATERIALS 64
 #define MR_MAX_SLOTS 16
+#define MR_MAX_NUCLIDES 64
+#define MR_MAX_MIX 16
 
 /* Optional device-memory allocator supplied by the caller (the Python binding passes one that
  * hands out torch caching-allocator blocks).  alloc returns a device pointer aligned to 256 B
@@ -134,6 +136,17 @@ MR_API int mr_load_materials(mr_ctx *ctx, int M, const double *density, int K, c
  * bracket identical to a double evaluation).  Requires mr_load_materials.
  * Errors: INVALID_ARG, STATE, OOM, CUDA. */
 MR_API int mr_load_xs(mr_ctx *ctx, int material, int64_t n, const double *energy, const double *sigma_t);
+
+/* Multi-nuclide materials ("first calculating all cross-sections"): instead of a
+ * table of its own a material may be a mixture of nuclides, each with its own energy grid:
+ *     sigma_m(E) = sum_j weights[j] * sigma_{nuclides[j]}(E)        (added in list order)
+ * mr_load_nuclide_xs loads nuclide `nuclide`'s table (0 <= nuclide < MR_MAX_NUCLIDES; same rules as mr_load_xs; may be
+ * called any time after mr_create); mr_define_material makes material `material` the mixture of nnuc (1..MR_MAX_MIX)
+ * nuclides with the given weights (finite, >= 0; e.g. mass fractions, so that sigma stays in cm^2/g; stored as fp32 in
+ * MIXED mode) and drops the material's own table, if any; a later mr_load_xs for that material drops the mixture.
+ * mr_cast_rays needs the table of every nuclide a mixture names.  Errors: INVALID_ARG, STATE, OOM, CUDA. */
+MR_API int mr_load_nuclide_xs(mr_ctx *ctx, int nuclide, int64_t n, const double *energy, const double *sigma);
+MR_API int mr_define_material(mr_ctx *ctx, int material, int nnuc, const int32_t *nuclides, const double *weights);
 
 /* ---- the hot path ------------------------------------------------------------------------ */
 

@@ -28,7 +28,7 @@ EXPORTS = [
     "mr_create", "mr_create_ex", "mr_destroy", "mr_set_stream", "mr_last_error", "mr_load_mesh",
     "mr_load_materials", "mr_load_xs", "mr_cast_rays", "mr_read_tally", "mr_clear_tally", "mr_sync",
     "mr_get_stats", "mr_tally_device_ptr", "mr_trace_rays", "mr_set_option", "mr_get_option",
-    "mr_end_batch", "mr_read_moments", "mr_read_mean_sigma",
+    "mr_end_batch", "mr_read_moments", "mr_read_mean_sigma", "mr_load_nuclide_xs", "mr_define_material",
     "mr_ring_open", "mr_ring_push", "mr_ring_flush", "mr_ring_close", "mr_ring_get_stats",
     "mr_load_detectors", "mr_cast_next_event", "mr_read_detectors", "mr_clear_detectors", "mr_trace_next_event",
 ]
@@ -94,6 +94,8 @@ def load_library() -> C.CDLL:
         "mr_ring_flush": [vp],
         "mr_ring_close": [vp],
         "mr_ring_get_stats": [vp, C.POINTER(mr_ring_stats)],
+        "mr_load_nuclide_xs": [vp, i32, i64, vp, vp],
+        "mr_define_material": [vp, i32, i32, vp, vp],
         "mr_end_batch": [vp],
         "mr_read_moments": [vp, vp, vp, C.POINTER(i64)],
         "mr_read_mean_sigma": [vp, vp, vp, C.POINTER(i64)],
@@ -237,12 +239,31 @@ class MonteRay:
             raise MonteRayError(MR_ERR_INVALID_ARG, "energy and sigma_t differ in length")
         self._check(self.lib.mr_load_xs(self._h, material, len(energy), energy.ctypes.data, sigma_t.ctypes.data))
 
+    def load_nuclide_xs(self, nuclide: int, energy, sigma):
+        energy, sigma = _f64(energy), _f64(sigma)
+        if len(energy) != len(sigma):
+            raise MonteRayError(MR_ERR_INVALID_ARG, "energy and sigma differ in length")
+        self._check(self.lib.mr_load_nuclide_xs(self._h, nuclide, len(energy), energy.ctypes.data, sigma.ctypes.data))
+
+    def define_material(self, material: int, nuclides, weights):
+        nuclides = np.ascontiguousarray(nuclides, dtype=np.int32)
+        weights = _f64(weights)
+        if len(nuclides) != len(weights):
+            raise MonteRayError(MR_ERR_INVALID_ARG, "nuclides and weights differ in length")
+        self._check(self.lib.mr_define_material(self._h, material, len(nuclides), nuclides.ctypes.data, weights.ctypes.data))
+
     def load_problem(self, prob):
-        """Convenience: mesh + materials + all tables of a workloads.Problem-like object."""
+        """Convenience: mesh + materials + all tables (and nuclide mixtures) of a workloads.Problem-like object."""
         self.load_mesh(prob.xe, prob.ye, prob.ze)
         self.load_materials(prob.density, prob.cell_mat, prob.cell_frac)
-        for m, (e, s) in enumerate(prob.xs):
-            self.load_xs(m, e, s)
+        mixtures = getattr(prob, "mixtures", None) or [None] * len(prob.xs)
+        for q, (e, s) in enumerate(getattr(prob, "nuclide_xs", None) or []):
+            self.load_nuclide_xs(q, e, s)
+        for m, t in enumerate(prob.xs):
+            if mixtures[m] is not None:
+                self.define_material(m, *mixtures[m])
+            else:
+                self.load_xs(m, *t)
 
     # ---- hot path
     def _ray_arg(self, rays):

@@ -110,6 +110,14 @@ struct mr_ctx {
     std::vector<int> xs_n;
     XsDesc *d_xs = nullptr;
     bool xs_dirty = true;
+    // nuclide tables and per-material mixtures (mr_load_nuclide_xs / mr_define_material)
+    Grid *nuc_grid_of[MR_MAX_NUCLIDES] = {};
+    void *nuc_S[MR_MAX_NUCLIDES] = {};
+    int nuc_n[MR_MAX_NUCLIDES] = {};
+    std::vector<std::vector<std::pair<int, double>>> mix;   // [M]: (nuclide, weight) list, empty = own table
+    int N = 0;                             // nuclide slots in use by the resident descriptors (highest loaded index + 1)
+    int *d_mix_off = nullptr, *d_mix_nuc = nullptr;
+    void *d_mix_w = nullptr;
 
     unsigned long long *d_counters = nullptr;  // accepted, rejected, segments, spare | next-event: accepted, rejected, segments, spare
 
@@ -223,6 +231,7 @@ void free_tables(mr_ctx *c)
     c->grid_of.clear();
     c->d_S.clear();
     c->xs_n.clear();
+    c->mix.clear();
     c->dev_free(c->d_xs);
     c->d_xs = nullptr;
     c->xs_dirty = true;
@@ -287,7 +296,7 @@ template <typename Real, typename Rec>
 int launch_cast_t(mr_ctx *c, const CastParams &P)
 {
     const int block = c->block_threads;
-    const size_t per_block = walker_smem_bytes(block) + (size_t)c->M * block * sizeof(Real);
+    const size_t per_block = walker_smem_bytes(block) + (size_t)(c->M + c->N) * block * sizeof(Real);
     const int mode = edge_mode(c, per_block);
     const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
     if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "materials x block threads exceed shared memory; lower MR_OPT_BLOCK_THREADS");
@@ -301,17 +310,54 @@ int launch_cast_t(mr_ctx *c, const CastParams &P)
 int upload_xs_desc(mr_ctx *c)
 {
     if (!c->xs_dirty) return MR_OK;
-    std::vector<XsDesc> h(c->M);
+    // descriptors: [0, M) materials (n = 0: a nuclide mixture), [M, M + N) nuclides (n = 0: not loaded)
+    int N = 0;
+    for (int q = 0; q < MR_MAX_NUCLIDES; ++q)
+        if (c->nuc_n[q] > 0) N = q + 1;
+    bool any_mix = false;
+    for (int m = 0; m < c->M; ++m) any_mix = any_mix || !c->mix[m].empty();
+    if (!any_mix) N = 0;
+    std::vector<XsDesc> h(c->M + N);
     for (int m = 0; m < c->M; ++m) {
         const mr_ctx::Grid *g = c->grid_of[m];
-        h[m] = XsDesc{g->d_E, c->d_S[m], c->xs_n[m], g->id, g->d_first, g->b0, g->sh};
+        h[m] = g ? XsDesc{g->d_E, c->d_S[m], c->xs_n[m], g->id, g->d_first, g->b0, g->sh} : XsDesc{nullptr, nullptr, 0, -1, nullptr, 0, 0};
+    }
+    for (int q = 0; q < N; ++q) {
+        const mr_ctx::Grid *g = c->nuc_grid_of[q];
+        h[c->M + q] = g ? XsDesc{g->d_E, c->nuc_S[q], c->nuc_n[q], g->id, g->d_first, g->b0, g->sh} : XsDesc{nullptr, nullptr, 0, -1, nullptr, 0, 0};
     }
     if (!c->d_xs) {
-        c->d_xs = (XsDesc *)c->dev_alloc(sizeof(XsDesc) * MR_MAX_MATERIALS);
+        c->d_xs = (XsDesc *)c->dev_alloc(sizeof(XsDesc) * (MR_MAX_MATERIALS + MR_MAX_NUCLIDES));
         if (!c->d_xs) return c->fail(MR_ERR_OOM, "device allocation failed (table descriptors)");
     }
-    MR_CUDA(c, cudaMemcpyAsync(c->d_xs, h.data(), sizeof(XsDesc) * c->M, cudaMemcpyHostToDevice, c->stream));
-    MR_CUDA(c, cudaStreamSynchronize(c->stream));  // h goes out of scope
+    MR_CUDA(c, cudaMemcpyAsync(c->d_xs, h.data(), sizeof(XsDesc) * h.size(), cudaMemcpyHostToDevice, c->stream));
+    // mixtures: offsets per material, then (nuclide, weight) entries; weights rounded once to fp32 in MIXED mode
+    std::vector<int> off(c->M + 1, 0), nuc;
+    std::vector<double> wd;
+    std::vector<float> wf;
+    for (int m = 0; m < c->M; ++m) {
+        for (const auto &e : c->mix[m]) {
+            nuc.push_back(e.first);
+            wd.push_back(e.second);
+            wf.push_back((float)e.second);
+        }
+        off[m + 1] = (int)nuc.size();
+    }
+    if (N > 0) {
+        if (!c->d_mix_off) {
+            c->d_mix_off = (int *)c->dev_alloc(sizeof(int) * (MR_MAX_MATERIALS + 1));
+            c->d_mix_nuc = (int *)c->dev_alloc(sizeof(int) * MR_MAX_MATERIALS * MR_MAX_MIX);
+            c->d_mix_w = c->dev_alloc(sizeof(double) * MR_MAX_MATERIALS * MR_MAX_MIX);
+            if (!c->d_mix_off || !c->d_mix_nuc || !c->d_mix_w) return c->fail(MR_ERR_OOM, "device allocation failed (mixtures)");
+        }
+        const bool dbl = c->precision == MR_PRECISION_DOUBLE;
+        MR_CUDA(c, cudaMemcpyAsync(c->d_mix_off, off.data(), sizeof(int) * off.size(), cudaMemcpyHostToDevice, c->stream));
+        MR_CUDA(c, cudaMemcpyAsync(c->d_mix_nuc, nuc.data(), sizeof(int) * nuc.size(), cudaMemcpyHostToDevice, c->stream));
+        MR_CUDA(c, cudaMemcpyAsync(c->d_mix_w, dbl ? (const void *)wd.data() : (const void *)wf.data(),
+                                   (dbl ? sizeof(double) : sizeof(float)) * nuc.size(), cudaMemcpyHostToDevice, c->stream));
+    }
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));  // the host vectors go out of scope
+    c->N = N;
     c->xs_dirty = false;
     return MR_OK;
 }
@@ -320,9 +366,14 @@ int ready_to_cast(mr_ctx *c)
 {
     if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
     if (!c->d_recs) return c->fail(MR_ERR_STATE, "no materials loaded");
-    for (int m = 0; m < c->M; ++m)
-        if (m >= (int)c->xs_n.size() || c->xs_n[m] == 0)
+    for (int m = 0; m < c->M; ++m) {
+        if (m < (int)c->xs_n.size() && c->xs_n[m] > 0) continue;
+        if (m >= (int)c->mix.size() || c->mix[m].empty())
             return c->fail(MR_ERR_STATE, "cross-section table of material " + std::to_string(m) + " not loaded");
+        for (const auto &e : c->mix[m])
+            if (c->nuc_n[e.first] == 0)
+                return c->fail(MR_ERR_STATE, "material " + std::to_string(m) + " needs nuclide " + std::to_string(e.first) + ", whose table is not loaded");
+    }
     return MR_OK;
 }
 
@@ -393,6 +444,10 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     P.K = c->K;
     P.M = c->M;
     P.xs = c->d_xs;
+    P.N = c->N;
+    P.mix_off = c->d_mix_off;
+    P.mix_nuc = c->d_mix_nuc;
+    P.mix_w = c->d_mix_w;
     P.rays = d_rays;
     if (int rc = order_rays(c, n, d_rays, &P.perm)) return rc;
     P.n = n;
@@ -554,6 +609,13 @@ int mr_destroy(mr_ctx *c)
     }
     free_stage(c);
     free_tables(c);
+    for (int q = 0; q < MR_MAX_NUCLIDES; ++q) {
+        unref_grid(c, c->nuc_grid_of[q]);
+        c->dev_free(c->nuc_S[q]);
+    }
+    c->dev_free(c->d_mix_off);
+    c->dev_free(c->d_mix_nuc);
+    c->dev_free(c->d_mix_w);
     free_materials(c);
     c->dev_free(c->d_edges);
     c->dev_free(c->d_tally);
@@ -718,6 +780,7 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
     c->K = K;
     if (M != c->M || (int)c->xs_n.size() != M) {
         c->M = M;
+        c->mix.assign(M, {});
         c->grid_of.assign(M, nullptr);
         c->d_S.assign(M, nullptr);
         c->xs_n.assign(M, 0);
@@ -726,12 +789,14 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
     return MR_OK;
 }
 
-int mr_load_xs(mr_ctx *c, int material, int64_t n, const double *energy, const double *sigma_t)
+}  // extern "C"
+
+namespace {
+
+// Validates and uploads one (energy, sigma) table into the given slot (a material's or a nuclide's).
+int load_table(mr_ctx *c, mr_ctx::Grid **grid_slot, void **S_slot, int *n_slot, int64_t n, const double *energy,
+               const double *sigma_t)
 {
-    MR_ENTER(c);
-    if (!c->d_recs) return c->fail(MR_ERR_STATE, "load the materials before the tables");
-    if (material < 0 || material >= c->M || n < 1 || n > 0x7fffffff || !energy || !sigma_t)
-        return c->fail(MR_ERR_INVALID_ARG, "xs: bad material index, size or NULL array");
     const bool dbl = c->precision == MR_PRECISION_DOUBLE;
     std::vector<float> ef, sf;
     if (!dbl) { ef.resize(n); sf.resize(n); }
@@ -811,11 +876,57 @@ int mr_load_xs(mr_ctx *c, int material, int64_t n, const double *energy, const d
         c->grids.push_back(g);
     }
     g->refs += 1;
-    unref_grid(c, c->grid_of[material]);   // the table this call replaces, if any
+    unref_grid(c, *grid_slot);   // the table this call replaces, if any
+    c->dev_free(*S_slot);
+    *grid_slot = g;
+    *S_slot = dS;
+    *n_slot = (int)n;
+    c->xs_dirty = true;
+    return MR_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int mr_load_xs(mr_ctx *c, int material, int64_t n, const double *energy, const double *sigma_t)
+{
+    MR_ENTER(c);
+    if (!c->d_recs) return c->fail(MR_ERR_STATE, "load the materials before the tables");
+    if (material < 0 || material >= c->M || n < 1 || n > 0x7fffffff || !energy || !sigma_t)
+        return c->fail(MR_ERR_INVALID_ARG, "xs: bad material index, size or NULL array");
+    if (int rc = load_table(c, &c->grid_of[material], &c->d_S[material], &c->xs_n[material], n, energy, sigma_t)) return rc;
+    c->mix[material].clear();       // a table of its own replaces a nuclide mixture
+    return MR_OK;
+}
+
+int mr_load_nuclide_xs(mr_ctx *c, int nuclide, int64_t n, const double *energy, const double *sigma)
+{
+    MR_ENTER(c);
+    if (nuclide < 0 || nuclide >= MR_MAX_NUCLIDES || n < 1 || n > 0x7fffffff || !energy || !sigma)
+        return c->fail(MR_ERR_INVALID_ARG, "nuclide xs: bad nuclide index, size or NULL array");
+    return load_table(c, &c->nuc_grid_of[nuclide], &c->nuc_S[nuclide], &c->nuc_n[nuclide], n, energy, sigma);
+}
+
+int mr_define_material(mr_ctx *c, int material, int nnuc, const int32_t *nuclides, const double *weights)
+{
+    MR_ENTER(c);
+    if (!c->d_recs) return c->fail(MR_ERR_STATE, "load the materials before defining their composition");
+    if (material < 0 || material >= c->M || nnuc < 1 || nnuc > MR_MAX_MIX || !nuclides || !weights)
+        return c->fail(MR_ERR_INVALID_ARG, "define_material: bad material index, nuclide count or NULL array");
+    std::vector<std::pair<int, double>> mix;
+    for (int j = 0; j < nnuc; ++j) {
+        if (nuclides[j] < 0 || nuclides[j] >= MR_MAX_NUCLIDES) return c->fail(MR_ERR_INVALID_ARG, "define_material: nuclide index out of range");
+        if (!std::isfinite(weights[j]) || weights[j] < 0.0 || (c->precision == MR_PRECISION_MIXED && !std::isfinite((float)weights[j])))
+            return c->fail(MR_ERR_INVALID_ARG, "define_material: weights must be finite and >= 0");
+        mix.emplace_back(nuclides[j], weights[j]);
+    }
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    unref_grid(c, c->grid_of[material]);    // the mixture replaces a table of its own
     c->dev_free(c->d_S[material]);
-    c->grid_of[material] = g;
-    c->d_S[material] = dS;
-    c->xs_n[material] = (int)n;
+    c->grid_of[material] = nullptr;
+    c->d_S[material] = nullptr;
+    c->xs_n[material] = 0;
+    c->mix[material] = mix;
     c->xs_dirty = true;
     return MR_OK;
 }
@@ -1051,7 +1162,7 @@ template <typename Real, typename Rec, bool TRACE>
 int launch_ne_t(mr_ctx *c, const NextEventParams &P, int ndet_launch)
 {
     const int block = c->block_threads;
-    const size_t per_block = walker_smem_bytes(block) + (size_t)c->M * block * sizeof(Real);
+    const size_t per_block = walker_smem_bytes(block) + (size_t)(c->M + c->N) * block * sizeof(Real);
     const int mode = edge_mode(c, per_block);
     const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
     if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "materials x block threads exceed shared memory; lower MR_OPT_BLOCK_THREADS");
@@ -1085,6 +1196,10 @@ NextEventParams ne_params(mr_ctx *c, long long n, const void *d_rays)
     P.K = c->K;
     P.M = c->M;
     P.xs = c->d_xs;
+    P.N = c->N;
+    P.mix_off = c->d_mix_off;
+    P.mix_nuc = c->d_mix_nuc;
+    P.mix_w = c->d_mix_w;
     P.rays = d_rays;
     P.n = n;
     P.det = c->d_det;

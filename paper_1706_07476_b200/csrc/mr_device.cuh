@@ -52,7 +52,11 @@ struct CastParams {
     const void *recs;      // packed records (LAYOUT_K*, LAYOUT_D8) or coefficient array (generic)
     const uint8_t *ids;    // generic layout only
     int K, M;
-    const XsDesc *xs;      // [M]
+    const XsDesc *xs;      // [M + N]: materials (n = 0: a nuclide mixture), then nuclides
+    int N;                 // nuclide descriptors (0: every material has a table of its own)
+    const int *mix_off;    // [M + 1] entries of material m: mix_off[m] .. mix_off[m+1]-1
+    const int *mix_nuc;    // nuclide per entry
+    const void *mix_w;     // weight per entry (Real)
     const void *rays;      // 8 floats (mixed) or 8 doubles per ray
     const uint32_t *perm;  // optional processing order (ray index per work item), may be null
     long long n;
@@ -176,6 +180,36 @@ __device__ __forceinline__ Real sigma_at(const XsDesc &t, const Bracket<Real> &b
     if (b.k == -2) return __ldg(Sg + t.n - 1);
     const Real s0 = __ldg(Sg + b.k), s1 = __ldg(Sg + b.k + 1);
     return s0 + b.t01 * (s1 - s0);
+}
+
+// S1 for a whole ray ("first calculating all cross-sections"): sigma of every material into the
+// thread's shared column sig[m * stride], m < M.  With nuclides (N > 0) the nuclide values go to columns
+// M .. M+N-1 first and a mixture material is the weighted sum of its nuclides, added in list order.
+template <typename Real>
+__device__ __forceinline__ void sigma_all(const XsDesc *xs, int M, int N, const int *mix_off, const int *mix_nuc,
+                                          const void *mix_w, Real E, Real *sig, int stride)
+{
+    Bracket<Real> br;
+    int grid = -1;
+    for (int q = M; q < M + N; ++q) {
+        const XsDesc t = xs[q];
+        if (t.n == 0) continue;                     // nuclide not loaded (and, checked on the host, not used)
+        if (t.grid != grid) { br = find_bracket<Real>(t, E); grid = t.grid; }
+        sig[q * stride] = sigma_at<Real>(t, br);
+    }
+    for (int m = 0; m < M; ++m) {
+        const XsDesc t = xs[m];
+        if (t.n > 0) {
+            if (t.grid != grid) { br = find_bracket<Real>(t, E); grid = t.grid; }
+            sig[m * stride] = sigma_at<Real>(t, br);
+        } else {
+            const Real *w = reinterpret_cast<const Real *>(mix_w);
+            Real s = 0;
+            for (int j = __ldg(mix_off + m); j < __ldg(mix_off + m + 1); ++j)
+                s += __ldg(w + j) * sig[(M + __ldg(mix_nuc + j)) * stride];
+            sig[m * stride] = s;
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -540,13 +574,7 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
         accepted = R.finite && (R.E > (Real)0) && walker_init<EDGE_MODE>(w, axf, stride, P.mesh, e, R.o, R.d);
         if (accepted) {
             // S1: every material's sigma at the ray's energy, kept in this thread's shared column
-            Bracket<Real> br;
-            int grid = -1;
-            for (int m = 0; m < P.M; ++m) {
-                const XsDesc t = P.xs[m];
-                if (t.grid != grid) { br = find_bracket<Real>(t, R.E); grid = t.grid; }
-                sig[m * stride] = sigma_at<Real>(t, br);
-            }
+            sigma_all<Real>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, R.E, sig, stride);
 
             double wa = R.W;   // W * exp(-tau), a running product of exp(-x)
             double *const tally = P.tally;
@@ -657,7 +685,11 @@ struct NextEventParams {
     const void *recs;
     const uint8_t *ids;
     int K, M;
-    const XsDesc *xs;
+    const XsDesc *xs;              // as CastParams
+    int N;
+    const int *mix_off;
+    const int *mix_nuc;
+    const void *mix_w;
     const void *rays;
     const uint32_t *perm;          // optional processing order, one section of n entries per detector of the launch
     long long n;
@@ -726,13 +758,7 @@ __global__ void __launch_bounds__(256) next_event_kernel(const __grid_constant__
                    walker_init<EDGE_MODE>(w, axf, stride, P.mesh, e, R.o, d);
         if (accepted) {
             const double Rd = sqrt(R2);
-            Bracket<Real> br;
-            int grid = -1;
-            for (int m = 0; m < P.M; ++m) {                          // N2
-                const XsDesc t = P.xs[m];
-                if (t.grid != grid) { br = find_bracket<Real>(t, R.E); grid = t.grid; }
-                sig[m * stride] = sigma_at<Real>(t, br);
-            }
+            sigma_all<Real>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, R.E, sig, stride);   // N2
             if (TRACE) h = 0xcbf29ce484222325ULL;
             Rec rec;
             rec.reset();

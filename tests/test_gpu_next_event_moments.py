@@ -266,3 +266,70 @@ def test_ring_call_order_errors():
             m.ring_open(2, 4096)                 # already open
         m.ring_close()
         m.ring_close()                           # idempotent
+
+
+# ------------------------------------------------------------------------------------- multi-nuclide materials (NEXT-4)
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("cfg,kw,n", [(1, {}, 10_000), (3, {"nx": 68, "ny": 68, "nz": 40, "n_e": 3000}, 60_000),
+                                      (5, {"n": 24, "n_e": 4000, "n_res": 50}, 30_000)])
+def test_nuclide_mixtures_against_oracle(cfg, kw, n, precision):
+    """Materials that are mixtures of nuclides on grids of different sizes, beside materials with their own table:
+    cast tally, counters, traces, and the next-event detector sum against the oracle."""
+    from workloads import add_nuclides
+
+    prob = add_nuclides(make_problem(cfg, **kw), n_nuclides=6)
+    assert any(mx is not None for mx in prob.mixtures) and any(mx is None for mx in prob.mixtures)
+    rays32 = make_rays(prob, n)
+    orc = _oracle(prob)
+    ref = orc.cast(rays32, per_ray=True, threads=8)
+    det = np.array([prob.xe[0] + 0.37 * (prob.xe[-1] - prob.xe[0]), prob.ye[0] + 0.61 * (prob.ye[-1] - prob.ye[0]),
+                    prob.ze[0] + 0.55 * (prob.ze[-1] - prob.ze[0])])
+    ne = orc.next_event(rays32, det)
+    with _mr(prob, precision) as m:
+        rays = rays32.astype(m.ray_dtype)
+        m.cast_rays(rays)
+        got = m.read_tally()
+        st = m.get_stats()
+        nseg, hsh, _, _ = m.trace_rays(rays)
+        m.load_detectors(det)
+        m.cast_next_event(rays)
+        dsum = m.read_detectors()
+    assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+    assert np.array_equal(nseg, ref.nseg) and np.array_equal(hsh, ref.hash)
+    _close(got, ref.tally, precision, "tally")
+    _close(dsum, [ne.det_sum], precision, "detector sum")
+
+
+def test_nuclide_call_order_and_replacement():
+    from paper_1706_07476_b200 import MonteRay, MonteRayError
+    from workloads import add_nuclides
+
+    base = make_problem(1)
+    prob = add_nuclides(base, n_nuclides=4)
+    rays = make_rays(base, 5000)
+    ref_mix = _oracle(prob).cast(rays)
+    ref_own = _oracle(base).cast(rays)
+    with MonteRay(0, 0) as m:
+        m.load_mesh(base.xe, base.ye, base.ze)
+        with pytest.raises(MonteRayError) as e:
+            m.define_material(1, [0], [1.0])
+        assert e.value.status == 2                                     # materials first
+        m.load_materials(base.density, base.cell_mat, base.cell_frac)
+        m.load_xs(0, *base.xs[0])
+        ids, w = prob.mixtures[1]
+        with pytest.raises(MonteRayError):
+            m.define_material(1, [99], [1.0])                          # nuclide index out of range
+        with pytest.raises(MonteRayError):
+            m.define_material(1, ids, -w)                              # negative weight
+        m.define_material(1, ids, w)
+        with pytest.raises(MonteRayError) as e:
+            m.cast_rays(rays)
+        assert e.value.status == 2 and "nuclide" in str(e.value)      # a named nuclide has no table yet
+        for q, (en, sg) in enumerate(prob.nuclide_xs):
+            m.load_nuclide_xs(q, en, sg)
+        m.cast_rays(rays)
+        _close(m.read_tally(), ref_mix.tally, 0, "mixture")
+        m.load_xs(1, *base.xs[1])                                      # a table of its own replaces the mixture
+        m.clear_tally()
+        m.cast_rays(rays)
+        _close(m.read_tally(), ref_own.tally, 0, "own table again")
