@@ -29,6 +29,10 @@
  * inverse-square law, fine-step quadrature of Sigma_t along the line (detectors inside and outside
  * the mesh), brute-force crossing lists for the cell sequence, detectors on planes / lattice
  * points, reciprocity tau(a->b) = tau(b->a), linearity in W, every rejection rule.
+ * The R-Z mesh walk (vrc_cast_rz, steps Z1..Z5) is pinned in tests/test_oracle_rz_pins.py: crossing lists from
+ * numpy.roots, mid-point membership by numpy.searchsorted on (rho, z), an independent exit distance, the
+ * homogeneous closed form, the collision-probability invariant, rotation invariance, quadrature.
+ * Multi-nuclide materials (vrc_sigma) are pinned in tests/test_oracle_nuclide_pins.py.
  * Nothing in this file is "parity unpinned".
  */
 #include <math.h>
@@ -423,6 +427,169 @@ int vrc_next_event(const vrc_problem *p, int64_t n, const double *rays, const do
         total += s;
     }
     if (det_sum) *det_sum += total;
+    if (counts) *counts = cnt;
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * R-Z (2-D cylindrical) tally mesh -- SURVEY.md §8(f) NEXT-4; "It must support ... 2-D
+ * cylindrical (R-Z) meshes".  The paper gives no algorithm; the estimator is unchanged (Eqs. 1-4), only the
+ * cells differ: cell (ir, iz) = { r_ir <= rho < r_{ir+1},  z_iz <= z < z_{iz+1} },  rho = sqrt(x^2 + y^2),
+ * r_0 = 0, linear index c = ir + nr*iz.  Rays stay 3-D.
+ *
+ * Steps (all IEEE double, one rounding per written operation, no contraction):
+ *   Z1 reject: non-finite field, E <= 0, no axis can move, rho0^2 = ox*ox + oy*oy >= r_nr*r_nr, z outside [z_0, z_nz)
+ *   Z2 sigma_m(E) as O2
+ *   Z3 start cell: ir = #{p in 0..nr : r_p*r_p <= rho0^2} - 1;  iz = upper_bound(z, oz) - 1
+ *   Z4 radial crossings.  a = dx*dx + dy*dy, b = ox*dx + oy*dy, inv_a = 1/a; if a == 0 or inv_a is not finite
+ *      the ray never crosses a cylinder.  For cylinder p:  cc_p = rho0^2 - r_p*r_p,  D_p = b*b - a*cc_p,
+ *        t_in(p)  = max(0, (-b - sqrt(D_p)) * inv_a)     entering cylinder p  (shell p -> shell p-1; needs b < 0, D_p > 0)
+ *        t_out(p) = max(0, (-b + sqrt(D_p)) * inv_a)     leaving cylinder p   (shell p-1 -> shell p)
+ *      In shell ir the pending radial crossing is t_in(ir) while the ray still moves inward (b < 0, ir >= 1,
+ *      D_ir > 0, and it has not yet turned outward), else t_out(ir+1); once outward, always outward.
+ *      Axial crossings as O4:  t_z(p) = (z_p - oz) * (1/dz).
+ *   Z5 walk: the pending crossing with the smaller parameter, ties radial before axial; l = t - t_cur; score as O5;
+ *      an outward step from shell nr-1 or an axial step out of [0, nz) ends the ray.
+ * Pins: tests/test_oracle_rz_pins.py.
+ * ------------------------------------------------------------------------------------------------ */
+typedef struct {
+    int32_t nr, nz;
+    const double *re, *ze;      /* nr+1 radii (re[0] == 0, strictly increasing), nz+1 planes */
+} vrc_rz_mesh;
+
+static int cast_one_rz(const vrc_problem *p, const vrc_rz_mesh *g, const double *ray, double *tally,
+                       const vrc_diag *dg, int64_t r, int64_t *segments_out)
+{
+    const double ox = ray[0], oy = ray[1], oz = ray[2], dx = ray[3], dy = ray[4], dz = ray[5];
+    const double E = ray[6], W = ray[7];
+    const int32_t nr = g->nr, nz = g->nz;
+    uint32_t nseg = 0;
+    uint64_t hash = FNV_BASIS;
+    double sum_l = 0.0, tau = 0.0, sum_score = 0.0, sum_sig_score = 0.0, t_cur = 0.0;
+    int accepted = 1;
+
+    /* Z1 */
+    for (int f = 0; f < 8; ++f) if (!isfinite(ray[f])) accepted = 0;
+    if (!(E > 0.0)) accepted = 0;
+    const double rho2 = ox * ox + oy * oy;
+    const double a = dx * dx + dy * dy;
+    const double inv_a = (a != 0.0) ? 1.0 / a : 0.0;
+    const int radial = (a != 0.0) && isfinite(inv_a) && isfinite(a);
+    const double inv_z = (dz != 0.0) ? 1.0 / dz : 0.0;
+    const int axial = (dz != 0.0) && isfinite(inv_z);
+    if (!radial && !axial) accepted = 0;
+    if (accepted && !(rho2 < g->re[nr] * g->re[nr])) accepted = 0;
+    if (accepted && !(oz >= g->ze[0] && oz < g->ze[nz])) accepted = 0;
+
+    if (accepted) {
+        double sig[64];
+        for (int32_t m = 0; m < p->M; ++m) sig[m] = vrc_sigma(p, m, E);         /* Z2 */
+        /* Z3 */
+        int32_t ir = -1;
+        for (int32_t q = 0; q <= nr; ++q) if (g->re[q] * g->re[q] <= rho2) ir = q;
+        int32_t iz = (int32_t)(upper_bound(g->ze, nz + 1, oz) - 1);
+        /* Z4 */
+        const double b = ox * dx + oy * dy;
+        int inward = 0;
+        double t_r = INFINITY, t_z = INFINITY;
+        int32_t pz = 0, stepz = 0;
+        if (radial) {
+            if (b < 0.0 && ir >= 1) {
+                double cc = rho2 - g->re[ir] * g->re[ir];
+                double D = b * b - a * cc;
+                if (D > 0.0) { inward = 1; t_r = fmax(0.0, (-b - sqrt(D)) * inv_a); }
+            }
+            if (!inward) {
+                double cc = rho2 - g->re[ir + 1] * g->re[ir + 1];
+                double D = b * b - a * cc;
+                t_r = fmax(0.0, (-b + sqrt(D)) * inv_a);
+            }
+        }
+        if (axial) {
+            stepz = dz > 0.0 ? 1 : -1;
+            pz = dz > 0.0 ? iz + 1 : iz;
+            t_z = (g->ze[pz] - oz) * inv_z;
+        }
+        /* Z5 */
+        for (;;) {
+            const int ax = (t_z < t_r) ? 1 : 0;            /* ties: radial first */
+            const double tn = ax ? t_z : t_r;
+            double l = tn - t_cur;
+            int64_t c = (int64_t)ir + (int64_t)nr * (int64_t)iz;
+            double S = 0.0;
+            for (int32_t k = 0; k < p->K; ++k) {
+                int32_t m = p->cell_mat[c * p->K + k];
+                if (m >= 0) S += (p->cell_frac[c * p->K + k] * p->density[m]) * sig[m];
+            }
+            double x = S * l;
+            double score = W * exp(-tau) * (x > 0.0 ? -expm1(-x) / S : l);
+            if (tally) tally[c] += score;
+            if (dg && dg->cap > 0 && (int64_t)nseg < dg->cap) {
+                if (dg->cells) dg->cells[r * dg->cap + nseg] = (int32_t)c;
+                if (dg->lens) dg->lens[r * dg->cap + nseg] = l;
+                if (dg->scores) dg->scores[r * dg->cap + nseg] = score;
+            }
+            for (int q = 0; q < 4; ++q) {
+                hash ^= (uint64_t)(((uint32_t)c >> (8 * q)) & 0xffu);
+                hash *= FNV_PRIME;
+            }
+            nseg += 1;
+            sum_l += l;
+            sum_score += score;
+            sum_sig_score += S * score;
+            tau += x;
+            t_cur = tn;
+            if (ax) {
+                iz += stepz;
+                if (iz < 0 || iz >= nz) break;
+                pz += stepz;
+                t_z = (g->ze[pz] - oz) * inv_z;
+            } else if (inward) {
+                ir -= 1;
+                inward = 0;
+                if (ir >= 1) {
+                    double cc = rho2 - g->re[ir] * g->re[ir];
+                    double D = b * b - a * cc;
+                    if (D > 0.0) { inward = 1; t_r = fmax(0.0, (-b - sqrt(D)) * inv_a); }
+                }
+                if (!inward) {
+                    double cc = rho2 - g->re[ir + 1] * g->re[ir + 1];
+                    double D = b * b - a * cc;
+                    t_r = fmax(0.0, (-b + sqrt(D)) * inv_a);
+                }
+            } else {
+                ir += 1;
+                if (ir >= nr) break;
+                double cc = rho2 - g->re[ir + 1] * g->re[ir + 1];
+                double D = b * b - a * cc;
+                t_r = fmax(0.0, (-b + sqrt(D)) * inv_a);
+            }
+        }
+    }
+    if (dg) {
+        if (dg->nseg) dg->nseg[r] = nseg;
+        if (dg->hash) dg->hash[r] = accepted ? hash : 0;
+        if (dg->sum_l) dg->sum_l[r] = sum_l;
+        if (dg->t_exit) dg->t_exit[r] = t_cur;
+        if (dg->tau_exit) dg->tau_exit[r] = tau;
+        if (dg->sum_score) dg->sum_score[r] = sum_score;
+        if (dg->sum_sig_score) dg->sum_sig_score[r] = sum_sig_score;
+    }
+    *segments_out += nseg;
+    return accepted;
+}
+
+/* n rays on the R-Z mesh g; p supplies materials and tables (p->nx, ny, nz, xe, ye, ze are ignored; cell_mat and
+ * cell_frac hold nr*nz cells).  Single thread, ray order. */
+int vrc_cast_rz(const vrc_problem *p, const vrc_rz_mesh *g, int64_t n, const double *rays, double *tally,
+                const vrc_diag *dg, vrc_counts *counts)
+{
+    if (p->M > 64 || g->nr < 1 || g->nz < 1 || g->re[0] != 0.0) return -1;
+    vrc_counts cnt = {0, 0, 0};
+    for (int64_t r = 0; r < n; ++r) {
+        if (cast_one_rz(p, g, rays + 8 * r, tally, dg, r, &cnt.segments)) cnt.rays_accepted++;
+        else cnt.rays_rejected++;
+    }
     if (counts) *counts = cnt;
     return 0;
 }

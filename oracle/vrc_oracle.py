@@ -47,6 +47,10 @@ class _Counts(C.Structure):
     _fields_ = [("rays_accepted", C.c_int64), ("rays_rejected", C.c_int64), ("segments", C.c_int64)]
 
 
+class _RzMesh(C.Structure):
+    _fields_ = [("nr", C.c_int32), ("nz", C.c_int32), ("re", C.c_void_p), ("ze", C.c_void_p)]
+
+
 class _NeDiag(C.Structure):
     _fields_ = [("nseg", C.c_void_p), ("hash", C.c_void_p), ("tau", C.c_void_p), ("score", C.c_void_p)]
 
@@ -71,6 +75,9 @@ def _load():
         _lib.vrc_next_event.restype = C.c_int
         _lib.vrc_next_event.argtypes = [C.POINTER(_Problem), C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
                                         C.c_void_p, C.c_void_p]
+        _lib.vrc_cast_rz.restype = C.c_int
+        _lib.vrc_cast_rz.argtypes = [C.POINTER(_Problem), C.POINTER(_RzMesh), C.c_int64, C.c_void_p, C.c_void_p,
+                                     C.c_void_p, C.c_void_p]
         _lib.vrc_fnv1a_cells.restype = C.c_uint64
         _lib.vrc_fnv1a_cells.argtypes = [C.c_void_p, C.c_int64]
         _lib.vrc_max_threads.restype = C.c_int
@@ -227,6 +234,37 @@ class Oracle:
             raise RuntimeError(f"oracle error {rc}")
         res.rays_accepted, res.rays_rejected, res.segments, res.threads = (
             int(cnt.rays_accepted), int(cnt.rays_rejected), int(cnt.segments), int(used))
+        return res
+
+    def cast_rz(self, rays, re, ze, *, per_ray: bool = True, cap: int = 0) -> CastResult:
+        """Cast `rays` on the R-Z mesh (re: nr+1 radii from 0, ze: nz+1 planes); the problem's cell arrays hold
+        nr*nz cells, c = ir + nr*iz (steps Z1..Z5 of vrc_oracle.c).  Single thread."""
+        r = np.ascontiguousarray(np.asarray(rays, dtype=np.float64).reshape(-1, 8))
+        n = r.shape[0]
+        re = np.ascontiguousarray(re, dtype=np.float64)
+        ze = np.ascontiguousarray(ze, dtype=np.float64)
+        nr, nz = len(re) - 1, len(ze) - 1
+        assert nr * nz == self.ncell, "the problem's cell arrays must hold nr*nz cells"
+        tally = np.zeros(self.ncell, dtype=np.float64)
+        res = CastResult(tally, 0, 0, 0, 1)
+        res.nseg = np.zeros(n, dtype=np.uint32)
+        res.hash = np.zeros(n, dtype=np.uint64)
+        for nm in ("sum_l", "t_exit", "tau_exit", "sum_score", "sum_sig_score"):
+            setattr(res, nm, np.zeros(n, dtype=np.float64))
+        dg = _Diag(res.nseg.ctypes.data, res.hash.ctypes.data, res.sum_l.ctypes.data, res.t_exit.ctypes.data,
+                   res.tau_exit.ctypes.data, res.sum_score.ctypes.data, res.sum_sig_score.ctypes.data, None, None, None, 0)
+        if cap > 0:
+            res.cells = np.full((n, cap), -1, dtype=np.int32)
+            res.lens = np.zeros((n, cap), dtype=np.float64)
+            res.scores = np.zeros((n, cap), dtype=np.float64)
+            dg.cells, dg.lens, dg.scores, dg.cap = res.cells.ctypes.data, res.lens.ctypes.data, res.scores.ctypes.data, cap
+        g = _RzMesh(nr, nz, re.ctypes.data, ze.ctypes.data)
+        cnt = _Counts()
+        rc = self.lib.vrc_cast_rz(C.byref(self._p), C.byref(g), n, r.ctypes.data, tally.ctypes.data,
+                                  C.cast(C.byref(dg), C.c_void_p), C.cast(C.byref(cnt), C.c_void_p))
+        if rc < 0:
+            raise RuntimeError(f"oracle error {rc}")
+        res.rays_accepted, res.rays_rejected, res.segments = int(cnt.rays_accepted), int(cnt.rays_rejected), int(cnt.segments)
         return res
 
     def next_event(self, rays, det) -> NextEventResult:

@@ -60,3 +60,36 @@ def tiny_rays(prob, seed, n, axis_aligned_share=0.0, e_lo=5e-4, e_hi=20.0, dtype
     w = 0.5 + g.random(n)
     rays = np.concatenate([pos, d, e[:, None], w[:, None]], axis=1)
     return np.ascontiguousarray(rays.astype(dtype))
+
+
+def tiny_rz_problem(seed, nr=5, nz=4, M=3, K=2, n_e=17, uniform=False, void=False, homogeneous=False):
+    """A tiny R-Z problem: tiny_problem's materials and tables on nr radial shells (from r = 0) x nz axial slabs.
+    Returned with nx = nr, ny = 1 (cell c = ir + nr*iz) and the extra fields re, ze, nr."""
+    prob = tiny_problem(seed, nx=nr, ny=1, nz=nz, M=M, K=K, n_e=n_e, uniform=uniform, void=void, homogeneous=homogeneous)
+    g = np.random.default_rng(seed + 1000)
+    prob.re = 0.5 * np.arange(nr + 1) if uniform else np.concatenate([[0.0], np.cumsum(0.15 + 0.6 * g.random(nr))])
+    prob.nr = nr
+    prob.xe, prob.ye = prob.re, np.array([0.0, 1.0])
+    return prob
+
+
+def tiny_rz_rays(prob, seed, n, axis_parallel_share=0.0, through_axis_share=0.0, e_lo=5e-4, e_hi=20.0, dtype=np.float32):
+    g = np.random.default_rng(seed)
+    R = prob.re[-1]
+    rho = R * np.sqrt(0.999 * g.random(n))
+    phi = 2 * np.pi * g.random(n)
+    z = prob.ze[0] + (0.001 + 0.998 * g.random(n)) * (prob.ze[-1] - prob.ze[0])
+    pos = np.stack([rho * np.cos(phi), rho * np.sin(phi), z], axis=1)
+    d = g.normal(size=(n, 3))
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    k = int(axis_parallel_share * n)
+    d[:k, :2] = 0.0
+    d[:k, 2] = np.where(g.random(k) < 0.5, -1.0, 1.0)
+    j = int(through_axis_share * n)
+    for r in range(k, k + j):      # aimed exactly at the axis in the xy plane (in fp32 inputs: nearly)
+        s = -pos[r, :2] / max(np.linalg.norm(pos[r, :2]), 1e-30)
+        d[r, :2] = s * np.linalg.norm(d[r, :2])
+    e = e_lo * (e_hi / e_lo) ** g.random(n)
+    w = 0.5 + g.random(n)
+    rays = np.concatenate([pos, d, e[:, None], w[:, None]], axis=1)
+    return np.ascontiguousarray(rays.astype(dtype))
