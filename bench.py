@@ -382,6 +382,30 @@ def main():
             "producer_wait_ms_per_step": (rs["producer_wait_ms"] - w0) / reps,
             "device_only_ms_per_step": ms_total / args.steps,
             "h2d_bytes_per_step": int(rays.nbytes), "d2h_bytes_per_step": int(prob.ncell * 8)}
+        # NEXT-4: the same estimator on an R-Z (cylindrical) pin-cell mesh, its own context
+        from workloads import make_rz_problem, make_rz_rays
+
+        rzp = make_rz_problem(256, 2048)
+        rz_rays = torch.from_numpy(make_rz_rays(rzp, 4_000_000)).to(dev)
+        with MonteRay(local_rank, 0) as mz:
+            mz.load_problem(rzp)
+            for _ in range(3):
+                mz.cast_rays(rz_rays)
+            barrier()
+            z0 = mz.get_stats()
+            a0.record()
+            for _ in range(reps):
+                mz.cast_rays(rz_rays)
+            a1.record()
+            barrier()
+            ms = a0.elapsed_time(a1) / reps
+            rz_seg = (mz.get_stats().segments - z0.segments) // reps
+        rz_bytes = rz_seg * (16 + 5 * rzp.K) + rz_rays.shape[0] * (32 + 16 * rzp.M)
+        next_rows["rz_cast"] = {
+            "value": rz_seg / (ms * 1e-3), "unit": UNIT, "rays_per_sec": rz_rays.shape[0] / (ms * 1e-3), "ms_per_step": ms,
+            "workload": rzp.name, "rays": int(rz_rays.shape[0]), "segments_per_step": int(rz_seg),
+            "roofline": {"bound": "hbm", "achieved": rz_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": rz_bytes / (ms * 1e-3) / 1e9 / peak}}
     total_launches = m.get_stats().kernel_launches
 
     # ---------------------------------------------------------------- CPU oracle beside it (rank 0, N = 1)

@@ -118,6 +118,16 @@ MR_API const char *mr_last_error(mr_ctx *ctx);
  * any material map loaded before.  Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA. */
 MR_API int mr_load_mesh(mr_ctx *ctx, int nx, int ny, int nz, const double *xe, const double *ye, const double *ze);
 
+/* R-Z (2-D cylindrical) tally mesh: nr radial shells re[0] = 0 < ... < re[nr]
+ * about the z axis and nz axial slabs ze[0..nz]; cell (ir, iz) = { re[ir] <= sqrt(x^2+y^2) < re[ir+1], ze[iz] <= z <
+ * ze[iz+1] }, linear index c = ir + nr*iz (ncell = nr*nz).  Rays stay 3-D records; everything else (materials,
+ * tables, mr_cast_rays, mr_trace_rays, moments, the producer ring) works as on a Cartesian mesh, with the walk of
+ * radial crossings from the quadratic (ox+t dx)^2 + (oy+t dy)^2 = r_p^2, ties radial before
+ * axial; a ray is rejected if x^2+y^2 >= re[nr]^2 or z is outside [ze[0], ze[nz]).  The ordering pre-pass and the
+ * next-event cast are not available on R-Z meshes (MR_ERR_UNSUPPORTED for the latter).  Replaces any mesh loaded
+ * before.  Errors: INVALID_ARG (re[0] != 0, not increasing), UNSUPPORTED, OOM, CUDA. */
+MR_API int mr_load_mesh_rz(mr_ctx *ctx, int nr, int nz, const double *re, const double *ze);
+
 /* Materials and per-cell composition.  density[M] g/cc (finite, >= 0); K slots per cell;
  * cell_mat[ncell*K] material index per slot, -1 = empty slot; cell_frac[ncell*K] volume
  * fractions (finite, >= 0; ignored for empty slots).  Slot k of cell c is element c*K+k.

@@ -85,6 +85,7 @@ struct mr_ctx {
     // mesh + tally
     int nx = 0, ny = 0, nz = 0, nedges = 0;
     long long ncell = 0;
+    bool mesh_rz = false;              // R-Z mesh (mr_load_mesh_rz): nx = nr radial shells, ny = 1, x planes = radii
     bool mesh_arith = false;           // every plane position equals fma(p, h, e0) bit for bit
     double mesh_e0[3] = {0, 0, 0}, mesh_h[3] = {0, 0, 0};
     double *d_edges = nullptr;
@@ -385,7 +386,7 @@ constexpr long long kSortMinRays = 1 << 14;   // below this a batch is a handful
 int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm_out, int nsec = 0, int det_first = 0)
 {
     *perm_out = nullptr;
-    if (!c->sort_rays || n < kSortMinRays || n > 0xffffffffLL || edges_smem_bytes(c) > kEdgesSmemMax) return MR_OK;
+    if (!c->sort_rays || c->mesh_rz || n < kSortMinRays || n > 0xffffffffLL || edges_smem_bytes(c) > kEdgesSmemMax) return MR_OK;
     const int sections = std::max(nsec, 1);
     const int nlen = 128;
     const int zdiv = (c->nz + 255) / 256;
@@ -434,6 +435,36 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
     return MR_OK;
 }
 
+template <typename Real, typename Rec, bool TRACE>
+int launch_rz_t(mr_ctx *c, const RzParams &Q, int block)
+{
+    const size_t smem = edges_smem_bytes(c) + (TRACE ? 0 : (size_t)(c->M + c->N) * block * sizeof(Real));
+    if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "rz mesh: planes and materials exceed shared memory");
+    const long long grid = (Q.c.n + block - 1) / block;
+    if (grid > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
+    if (int rc = set_smem(c, rz_kernel<Real, Rec, TRACE>, smem)) return rc;
+    rz_kernel<Real, Rec, TRACE><<<(unsigned)grid, block, smem, c->stream>>>(Q);
+    c->launches += 1;
+    MR_CUDA(c, cudaGetLastError());
+    return MR_OK;
+}
+
+int launch_rz_cast(mr_ctx *c, const CastParams &P)
+{
+    RzParams Q{};
+    Q.c = P;
+    const int block = c->block_threads;
+    if (c->precision == MR_PRECISION_DOUBLE) return launch_rz_t<double, CellRecGeneric<double>, false>(c, Q, block);
+    switch (c->layout) {
+    case LAYOUT_K1: return launch_rz_t<float, CellRec<LAYOUT_K1>, false>(c, Q, block);
+    case LAYOUT_K2: return launch_rz_t<float, CellRec<LAYOUT_K2>, false>(c, Q, block);
+    case LAYOUT_K3: return launch_rz_t<float, CellRec<LAYOUT_K3>, false>(c, Q, block);
+    case LAYOUT_K4: return launch_rz_t<float, CellRec<LAYOUT_K4>, false>(c, Q, block);
+    case LAYOUT_D8: return launch_rz_t<float, CellRec<LAYOUT_D8>, false>(c, Q, block);
+    default: return launch_rz_t<float, CellRecGeneric<float>, false>(c, Q, block);
+    }
+}
+
 // Queue the cast of n device-resident rays on the context's stream.
 int cast_device(mr_ctx *c, long long n, const void *d_rays)
 {
@@ -462,7 +493,8 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     }
     MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->stream));
     int rc;
-    if (c->precision == MR_PRECISION_DOUBLE) rc = launch_cast_t<double, CellRecGeneric<double>>(c, P);
+    if (c->mesh_rz) rc = launch_rz_cast(c, P);
+    else if (c->precision == MR_PRECISION_DOUBLE) rc = launch_cast_t<double, CellRecGeneric<double>>(c, P);
     else switch (c->layout) {
     case LAYOUT_K1: rc = launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P); break;
     case LAYOUT_K2: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
@@ -651,9 +683,12 @@ int mr_set_stream(mr_ctx *c, void *cuda_stream)
 
 const char *mr_last_error(mr_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
 
-int mr_load_mesh(mr_ctx *c, int nx, int ny, int nz, const double *xe, const double *ye, const double *ze)
+}  // extern "C"
+
+namespace {
+
+int load_mesh_common(mr_ctx *c, bool rz, int nx, int ny, int nz, const double *xe, const double *ye, const double *ze)
 {
-    MR_ENTER(c);
     if (nx < 1 || ny < 1 || nz < 1 || !xe || !ye || !ze) return c->fail(MR_ERR_INVALID_ARG, "mesh: bad size or NULL edge array");
     const long long ncell = (long long)nx * ny * nz;
     if ((long long)nx * ny > 0x7fffffffLL || ncell >= 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "mesh: nx*ny*nz must be < 2^31");
@@ -685,6 +720,7 @@ int mr_load_mesh(mr_ctx *c, int nx, int ny, int nz, const double *xe, const doub
         return c->fail(MR_ERR_OOM, "device allocation failed (mesh / tally)");
     }
     c->nx = nx; c->ny = ny; c->nz = nz; c->nedges = ne; c->ncell = ncell;
+    c->mesh_rz = rz;
     {   // arithmetic mesh?  (uniform spacing reproduced exactly by one fma per plane, checked plane by plane)
         const double *ax[3] = {xe, ye, ze};
         const int na[3] = {nx, ny, nz};
@@ -695,12 +731,32 @@ int mr_load_mesh(mr_ctx *c, int nx, int ny, int nz, const double *xe, const doub
             for (int p = 0; p <= na[a] && c->mesh_arith; ++p)
                 c->mesh_arith = (std::fma((double)p, c->mesh_h[a], c->mesh_e0[a]) == ax[a][p]);
         }
+        if (rz) c->mesh_arith = false;   // the R-Z walker reads its radii and planes from the table
     }
     MR_CUDA(c, cudaMemcpyAsync(c->d_edges, h.data(), sizeof(double) * ne, cudaMemcpyHostToDevice, c->stream));
     MR_CUDA(c, cudaMemsetAsync(c->d_tally, 0, sizeof(double) * ncell, c->stream));
     MR_CUDA(c, cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
     return MR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mr_load_mesh(mr_ctx *c, int nx, int ny, int nz, const double *xe, const double *ye, const double *ze)
+{
+    MR_ENTER(c);
+    return load_mesh_common(c, false, nx, ny, nz, xe, ye, ze);
+}
+
+int mr_load_mesh_rz(mr_ctx *c, int nr, int nz, const double *re, const double *ze)
+{
+    MR_ENTER(c);
+    if (nr < 1 || !re) return c->fail(MR_ERR_INVALID_ARG, "rz mesh: bad size or NULL radius array");
+    if (re[0] != 0.0) return c->fail(MR_ERR_INVALID_ARG, "rz mesh: the first radius must be 0");
+    const double ye[2] = {0.0, 1.0};
+    return load_mesh_common(c, true, nr, 1, nz, re, ye, ze);
 }
 
 int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int32_t *cell_mat, const double *cell_frac)
@@ -1117,7 +1173,15 @@ int mr_trace_rays(mr_ctx *c, int64_t n, const void *rays, int where, uint32_t *n
     // cells/lens beyond nseg stay as the caller left them: seed the device copies from the host arrays
     if (e == cudaSuccess && d_cells) e = cudaMemcpyAsync(d_cells, cells, (size_t)n * cap * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess && d_lens) e = cudaMemcpyAsync(d_lens, lens, (size_t)n * cap * 8, cudaMemcpyHostToDevice, c->stream);
-    if (e == cudaSuccess) {
+    if (e == cudaSuccess && c->mesh_rz) {
+        RzParams Q{};
+        Q.c.mesh = mesh_dev(c);
+        Q.c.rays = d_rays;
+        Q.c.n = n;
+        Q.nseg = d_nseg; Q.hash = d_hash; Q.cells = d_cells; Q.lens = d_lens; Q.cap = cap;
+        Q.ray_is_double = c->precision == MR_PRECISION_DOUBLE ? 1 : 0;
+        if (launch_rz_t<float, CellRecGeneric<float>, true>(c, Q, 256) != MR_OK) { cleanup(); return MR_ERR_CUDA; }
+    } else if (e == cudaSuccess) {
         TraceParams P{mesh_dev(c), d_rays, n, d_nseg, d_hash, d_cells, d_lens, cap, c->precision == MR_PRECISION_DOUBLE ? 1 : 0};
         const int block = 256;
         const unsigned grid = (unsigned)((n + block - 1) / block);
@@ -1343,6 +1407,7 @@ int mr_cast_next_event(mr_ctx *c, int64_t n, const void *rays, int where)
         return c->fail(MR_ERR_INVALID_ARG, "next_event: bad count, NULL buffer or unknown location");
     if (int rc = ready_to_cast(c)) return rc;
     if (!c->ndet) return c->fail(MR_ERR_STATE, "no detectors loaded");
+    if (c->mesh_rz) return c->fail(MR_ERR_UNSUPPORTED, "the next-event cast is not implemented on R-Z meshes");
     if (n == 0) return MR_OK;
     if (int rc = upload_xs_desc(c)) return rc;
     return run_batch(c, n, rays, where, [c](long long count, const void *d_rays) { return next_event_device(c, count, d_rays); });
@@ -1376,6 +1441,7 @@ int mr_trace_next_event(mr_ctx *c, int64_t n, const void *rays, int where, int d
     if (int rc = ready_to_cast(c)) return rc;
     if (!c->ndet) return c->fail(MR_ERR_STATE, "no detectors loaded");
     if (det < 0 || det >= c->ndet) return c->fail(MR_ERR_INVALID_ARG, "trace_next_event: detector index out of range");
+    if (c->mesh_rz) return c->fail(MR_ERR_UNSUPPORTED, "the next-event cast is not implemented on R-Z meshes");
     if (n == 0) return MR_OK;
     if (int rc = upload_xs_desc(c)) return rc;
     const size_t rb = c->ray_bytes();

@@ -672,6 +672,169 @@ __global__ void __launch_bounds__(256) trace_kernel(const __grid_constant__ Trac
 }
 
 // ------------------------------------------------------------------------------------------------
+// R-Z (2-D cylindrical) tally mesh, SURVEY.md §8(f) NEXT-4.  Cell (ir, iz), c = ir + nr*iz, radii
+// re[0] = 0 < ... < re[nr], planes ze[0..nz]; MeshDev carries nx = nr, ny = 1, nz and edges = re | (1 pad) | ze laid
+// out like a Cartesian mesh with ny = 1 (x planes = radii, z planes = ze).  Steps Z1-Z5 of DESIGN.md §10.6, every
+// trace-determining operation written with a rounding-explicit intrinsic (no contraction):
+//   rho0^2 = ox*ox + oy*oy,  a = dx*dx + dy*dy,  b = ox*dx + oy*dy,  inv_a = 1/a
+//   cylinder p:  cc = rho0^2 - r_p*r_p,  D = b*b - a*cc,  t_in/out = max(0, (-b -/+ sqrt(D)) * inv_a)
+//   plane p:     t_z = (z_p - oz) * (1/dz);  ties: radial before axial
+// One thread per ray; TRACE = the test entry (per-ray count / hash / lists, no cross sections, no tally).
+//   dynamic shared memory: [edges] [sigma: (M+N) x blockDim Real]
+// ------------------------------------------------------------------------------------------------
+struct RzParams {
+    CastParams c;            // mesh (nx = nr, ny = 1), records, tables, rays, tally, counters
+    uint32_t *nseg;          // TRACE outputs, any may be null
+    unsigned long long *hash;
+    int32_t *cells;
+    double *lens;
+    long long cap;
+    int ray_is_double;
+};
+
+__device__ __forceinline__ double rz_t_radial(double b, double a, double inv_a, double rho2, double rp, bool outward)
+{
+    const double cc = __dsub_rn(rho2, __dmul_rn(rp, rp));
+    const double D = __dsub_rn(__dmul_rn(b, b), __dmul_rn(a, cc));
+    const double sq = __dsqrt_rn(D);
+    const double num = outward ? __dadd_rn(-b, sq) : __dsub_rn(-b, sq);
+    return fmax(0.0, __dmul_rn(num, inv_a));
+}
+
+template <typename Real, typename Rec, bool TRACE>
+__global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParams Q)
+{
+    const CastParams &P = Q.c;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int stride = blockDim.x;
+    const int nr = P.mesh.nx, nz = P.mesh.nz;
+    double *s_edges = reinterpret_cast<double *>(smem_raw);
+    Real *sig = reinterpret_cast<Real *>(smem_raw + edges_smem_bytes_for(P.mesh.nedges)) + threadIdx.x;
+    for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
+    __syncthreads();
+    const double *re = s_edges, *ze = s_edges + nr + 3;        // Cartesian layout with ny = 1: x | y (2 planes) | z
+
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = r < P.n;
+    bool accepted = false;
+    unsigned nseg = 0;
+    unsigned long long h = 0;
+    if (live) {
+        double ox, oy, oz, dx, dy, dz, W;
+        Real E;
+        bool fin;
+        if (sizeof(Real) == 8 || (TRACE && Q.ray_is_double)) {
+            const Ray<double> R = load_ray_f64(P.rays, r);
+            ox = R.o[0]; oy = R.o[1]; oz = R.o[2]; dx = R.d[0]; dy = R.d[1]; dz = R.d[2]; W = R.W; E = (Real)R.E; fin = R.finite && R.E > 0.0;
+        } else {
+            const Ray<float> R = load_ray_f32(P.rays, r);
+            ox = R.o[0]; oy = R.o[1]; oz = R.o[2]; dx = R.d[0]; dy = R.d[1]; dz = R.d[2]; W = R.W; E = (Real)R.E; fin = R.finite && R.E > 0.0f;
+        }
+        // Z1
+        const double rho2 = __dadd_rn(__dmul_rn(ox, ox), __dmul_rn(oy, oy));
+        const double a = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+        const double inv_a = (a != 0.0) ? __drcp_rn(a) : 0.0;
+        const bool radial = (a != 0.0) && isfinite(inv_a) && isfinite(a);
+        const double inv_z = (dz != 0.0) ? __drcp_rn(dz) : 0.0;
+        const bool axial = (dz != 0.0) && isfinite(inv_z);
+        accepted = fin && (radial || axial) && (rho2 < __dmul_rn(re[nr], re[nr])) && (oz >= ze[0] && oz < ze[nz]);
+        if (accepted) {
+            if (!TRACE) sigma_all<Real>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, E, sig, stride);   // Z2
+            // Z3: ir = #{p : r_p^2 <= rho0^2} - 1 (r_p^2 is non-decreasing in p), iz by comparisons
+            int lo = 0, hi = nr + 1;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (__dmul_rn(re[mid], re[mid]) <= rho2) lo = mid + 1; else hi = mid;
+            }
+            int ir = lo - 1;
+            int iz = upper_bound_edges(ze, nz + 1, oz) - 1;
+            // Z4
+            const double b = __dadd_rn(__dmul_rn(ox, dx), __dmul_rn(oy, dy));
+            const double inf = __longlong_as_double(0x7ff0000000000000LL);
+            bool inward = false;
+            double t_r = inf, t_z = inf, t_cur = 0.0;
+            int pz = 0, stepz = 0;
+            auto next_radial = [&](bool may_go_in) {
+                inward = false;
+                if (may_go_in && b < 0.0 && ir >= 1) {
+                    const double cc = __dsub_rn(rho2, __dmul_rn(re[ir], re[ir]));
+                    const double D = __dsub_rn(__dmul_rn(b, b), __dmul_rn(a, cc));
+                    if (D > 0.0) { inward = true; t_r = fmax(0.0, __dmul_rn(__dsub_rn(-b, __dsqrt_rn(D)), inv_a)); }
+                }
+                if (!inward) t_r = rz_t_radial(b, a, inv_a, rho2, re[ir + 1], true);
+            };
+            if (radial) next_radial(true);
+            if (axial) {
+                stepz = dz > 0.0 ? 1 : -1;
+                pz = dz > 0.0 ? iz + 1 : iz;
+                t_z = __dmul_rn(__dsub_rn(ze[pz], oz), inv_z);
+            }
+            if (TRACE) h = 0xcbf29ce484222325ULL;
+            double wa = W;
+            Rec rec;
+            if (!TRACE) rec.reset();
+            // Z5
+            for (;;) {
+                const bool ax = t_z < t_r;                      // ties: radial first
+                const double tn = ax ? t_z : t_r;
+                const double len = __dsub_rn(tn, t_cur);
+                const int cell = ir + nr * iz;
+                if (TRACE) {
+                    if ((long long)nseg < Q.cap) {
+                        if (Q.cells) Q.cells[r * Q.cap + nseg] = cell;
+                        if (Q.lens) Q.lens[r * Q.cap + nseg] = len;
+                    }
+                    const unsigned cu = (unsigned)cell;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        h ^= (unsigned long long)((cu >> (8 * q)) & 0xffu);
+                        h *= 0x100000001b3ULL;
+                    }
+                } else {
+                    rec.load(P.recs, P.ids, P.K, cell);
+                    const double S = (double)Rec::sigma(rec.value(), sig, stride, P.K);
+                    double g, ex;
+                    score_terms<sizeof(Real) == 8>(S, len, g, ex);
+                    if (len > 0.0) red_add_f64(P.tally + cell, wa * g);
+                    wa *= ex;
+                }
+                ++nseg;
+                t_cur = tn;
+                if (ax) {
+                    iz += stepz;
+                    if (iz < 0 || iz >= nz) break;
+                    pz += stepz;
+                    t_z = __dmul_rn(__dsub_rn(ze[pz], oz), inv_z);
+                } else if (inward) {
+                    ir -= 1;
+                    next_radial(true);
+                } else {
+                    ir += 1;
+                    if (ir >= nr) break;
+                    t_r = rz_t_radial(b, a, inv_a, rho2, re[ir + 1], true);
+                }
+            }
+        }
+        if (TRACE) {
+            if (Q.nseg) Q.nseg[r] = nseg;
+            if (Q.hash) Q.hash[r] = h;
+        }
+    }
+    if (!TRACE) {
+        const unsigned full = 0xffffffffu;
+        const unsigned acc = __popc(__ballot_sync(full, accepted));
+        const unsigned rej = __popc(__ballot_sync(full, live && !accepted));
+        unsigned long long segs = nseg;
+        for (int o = 16; o > 0; o >>= 1) segs += __shfl_xor_sync(full, segs, o);
+        if ((threadIdx.x & 31) == 0) {
+            if (acc) atomicAdd(P.counters + 0, (unsigned long long)acc);
+            if (rej) atomicAdd(P.counters + 1, (unsigned long long)rej);
+            if (segs) atomicAdd(P.counters + 2, segs);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Next-event (point-detector) estimator, SURVEY.md §8(f) NEXT-3 ("requires a ray-cast from
 // each source and collision event to the estimator location").  One thread per (event, detector): the same
 // S1 look-up and S2/S3 walker, with the UNNORMALISED direction d = det - o so that the crossing parameter

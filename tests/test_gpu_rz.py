@@ -1,0 +1,132 @@
+"""GPU parity on R-Z (cylindrical) meshes, through the C ABI against the
+oracle's vrc_cast_rz on the same seeded inputs: traces (count, hash, full cell and length lists) bit-exact,
+counters exact, tallies within the parity tolerances of DESIGN.md §5."""
+import numpy as np
+import pytest
+
+from tests.tiny import tiny_rz_problem, tiny_rz_rays
+
+pytestmark = pytest.mark.gpu
+
+
+def _check(prob, rays32, precision, cap):
+    from oracle.vrc_oracle import Oracle
+    from paper_1706_07476_b200 import MonteRay
+
+    ref = Oracle(prob).cast_rz(rays32, prob.re, prob.ze, cap=cap)
+    with MonteRay(0, precision) as m:
+        m.load_problem(prob)
+        rays = rays32.astype(m.ray_dtype)
+        assert m.cast_rays(rays) == len(rays32)
+        got = m.read_tally()
+        st = m.get_stats()
+        nseg, hsh, cells, lens = m.trace_rays(rays, cap=cap)
+    assert np.array_equal(nseg, ref.nseg), "segment counts differ"
+    assert np.array_equal(hsh, ref.hash), "cell-sequence hashes differ"
+    assert np.array_equal(cells, ref.cells), "cell traces differ"
+    assert np.array_equal(lens, ref.lens), "segment lengths differ (must be bitwise equal)"
+    assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+    d = np.abs(got - ref.tally)
+    bound = (1e-4 * np.abs(ref.tally) + 1e-7 * ref.tally.max()) if precision == 0 else (1e-10 * np.abs(ref.tally) + 1e-290)
+    assert np.all(d <= bound)
+    return ref
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("seed,K,M,uniform", [(401, 1, 2, False), (402, 3, 4, True), (403, 4, 5, False), (404, 8, 8, False)])
+def test_rz_tiny_problems(seed, K, M, uniform, precision):
+    """Every record layout; rays parallel to the axis, aimed at the axis, chords that miss inner cylinders;
+    4001 rays = several CTAs and a ragged last warp."""
+    prob = tiny_rz_problem(seed, nr=7, nz=6, M=M, K=K, n_e=33, uniform=uniform)
+    rays = tiny_rz_rays(prob, seed, 4001, axis_parallel_share=0.05, through_axis_share=0.05)
+    ref = _check(prob, rays, precision, cap=32)
+    assert ref.nseg.max() <= 32
+
+
+def test_rz_exact_geometry_cases_and_rejections():
+    prob = tiny_rz_problem(409, nr=4, nz=3, uniform=True)       # radii 0.5 k (R = 2), planes -1 + 0.75 k
+    ok = [0.3, 0.2, 0.0, 0.6, 0.0, 0.8, 1.0, 1.0]
+    rows = [ok, [0.0, 0.0, -1.0, 0.0, 0.0, 1.0, 1.0, 1.0],     # on the axis, on the lower plane
+            [1.5, 0.0, 0.5, -1.0, 0.0, 0.0, 1.0, 1.0],          # on a cylinder, through the axis
+            [1.0, 0.0, 0.5, 0.0, 1.0, 0.0, 1.0, 1.0],           # on a cylinder, tangent direction
+            [0.5, 0.5, -1.0, 1.0, 1.0, 1.0, 1.0, 1.0]]
+    for f, v in ((0, np.nan), (6, 0.0), (7, np.inf), (0, 2.0), (2, 1.25), (2, -1.0000001)):
+        b = list(ok)
+        b[f] = v
+        rows.append(b)
+    rows.append([0.3, 0.2, 0.0, 0.0, 0.0, -0.0, 1.0, 1.0])      # zero direction
+    rays = np.array(rows * 30, dtype=np.float32)
+    for precision in (0, 1):
+        ref = _check(prob, rays, precision, cap=16)
+        assert ref.rays_rejected == 30 * 7
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_rz_larger_mesh_with_batches_ring_and_moments(precision):
+    """A 300 x 400 R-Z mesh (120 000 cells): host batch, producer ring and per-batch moments work unchanged."""
+    from oracle.vrc_oracle import Oracle
+    from paper_1706_07476_b200 import MonteRay
+
+    prob = tiny_rz_problem(410, nr=300, nz=400, M=4, K=3, n_e=500)
+    rays32 = tiny_rz_rays(prob, 410, 40_000)
+    ref = Oracle(prob).cast_rz(rays32, prob.re, prob.ze)
+    with MonteRay(0, precision) as m:
+        m.load_problem(prob)
+        rays = np.ascontiguousarray(rays32.astype(m.ray_dtype))
+        m.cast_rays(rays[:15_000])
+        m.end_batch()
+        m.ring_open(2, 4096)
+        m.ring_push(rays[15_000:])
+        m.ring_close()
+        m.end_batch()
+        got = m.read_tally()
+        st = m.get_stats()
+        s1, s2, nb = m.read_moments()
+    assert nb == 2 and np.array_equal(s1, got)
+    assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+    d = np.abs(got - ref.tally)
+    bound = (1e-4 * np.abs(ref.tally) + 1e-7 * ref.tally.max()) if precision == 0 else (1e-10 * np.abs(ref.tally) + 1e-290)
+    assert np.all(d <= bound)
+
+
+def test_rz_argument_errors_and_unsupported_paths():
+    from paper_1706_07476_b200 import MonteRay, MonteRayError
+
+    prob = tiny_rz_problem(411, nr=4, nz=3)
+    with MonteRay(0, 0) as m:
+        with pytest.raises(MonteRayError):
+            m.load_mesh_rz([0.1, 1.0], [0.0, 1.0])               # first radius must be 0
+        with pytest.raises(MonteRayError):
+            m.load_mesh_rz([0.0, 1.0, 1.0], [0.0, 1.0])           # not strictly increasing
+        m.load_problem(prob)
+        m.load_detectors([[0.1, 0.1, 0.1]])
+        with pytest.raises(MonteRayError) as e:
+            m.cast_next_event(tiny_rz_rays(prob, 1, 10))
+        assert e.value.status == 5                                # MR_ERR_UNSUPPORTED
+        # a Cartesian mesh loaded afterwards replaces the R-Z one
+        m.load_mesh([0.0, 1.0], [0.0, 1.0], [0.0, 1.0])
+        assert m.ncell == 1
+
+
+def test_rz_pin_cell_workload_in_bench_configuration():
+    """The R-Z row bench.py times (pin cell, 256 x 2048 shells x slabs) on a sample of its rays: every ray's
+    trace hash, counters and the whole tally against the oracle."""
+    import torch
+
+    from oracle.vrc_oracle import Oracle
+    from paper_1706_07476_b200 import MonteRay
+    from workloads import make_rz_problem, make_rz_rays
+
+    prob = make_rz_problem(256, 2048)
+    rays = make_rz_rays(prob, 300_000)
+    ref = Oracle(prob).cast_rz(rays, prob.re, prob.ze)
+    with MonteRay(0, 0) as m:
+        m.load_problem(prob)
+        d = torch.from_numpy(rays).cuda()
+        m.cast_rays(d)
+        got = m.read_tally()
+        st = m.get_stats()
+        nseg, hsh, _, _ = m.trace_rays(d)
+    assert np.array_equal(nseg, ref.nseg) and np.array_equal(hsh, ref.hash)
+    assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+    assert np.all(np.abs(got - ref.tally) <= 1e-4 * np.abs(ref.tally) + 1e-7 * ref.tally.max())

@@ -12,5 +12,7 @@ from .configs import (  # noqa: F401
     add_nuclides,
     make_problem,
     make_rays,
+    make_rz_problem,
+    make_rz_rays,
     rng_for,
 )

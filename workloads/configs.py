@@ -373,3 +373,36 @@ def add_nuclides(prob, n_nuclides: int = 6, max_per_material: int = 4, keep_dire
         q.mixtures.append((ids, f32r(w / w.sum())))
         q.xs[m] = None
     return q
+
+
+# --------------------------------------------------------------------------- R-Z pin-cell-like problem (NEXT-4)
+def make_rz_problem(nr: int = 256, nz: int = 512, n_e: int = 20_000):
+    """One fuel-pin cell seen as an R-Z mesh: UO2 to r = 0.41 cm, zircaloy to 0.475 cm, borated water out to the
+    equivalent-cell radius 0.7135 cm (pitch/sqrt(pi)), 365.76 cm high; nr equal shells, nz equal slabs, K = 1.
+    Stands in for the paper's wish for 2-D cylindrical meshes; inputs only."""
+    from types import SimpleNamespace
+
+    names = ["uo2", "zircaloy", "borated_water"]
+    r_out = PWR_PITCH / np.sqrt(np.pi)
+    re = r_out * np.arange(nr + 1) / nr
+    ze = PWR_HEIGHT * np.arange(nz + 1) / nz
+    rc = 0.5 * (re[1:] + re[:-1])
+    shell_mat = np.where(rc < PWR_R_PELLET, 0, np.where(rc < PWR_R_CLAD, 1, 2)).astype(np.int32)
+    cell_mat = np.tile(shell_mat, nz).reshape(-1, 1)
+    return SimpleNamespace(config=3, name=f"rz_pin_cell_{nr}x{nz}", nx=nr, ny=1, nz=nz, nr=nr, re=re, ze=ze, xe=re,
+                           ye=np.array([0.0, 1.0]), density=_densities(names), K=1, cell_mat=cell_mat,
+                           cell_frac=np.ones((nr * nz, 1)), xs=_tables(3, names, n_e, 50), M=3, ncell=nr * nz,
+                           material_names=names)
+
+
+def make_rz_rays(prob, n: int, batch: int = 0) -> np.ndarray:
+    """Rays born uniformly in the fuel (rho < 0.41 cm), isotropic, Watt energies; float32 [n, 8]."""
+    g = rng_for(3, 11, batch)
+    rho = PWR_R_PELLET * np.sqrt(g.random(n))
+    phi = 2.0 * np.pi * g.random(n)
+    z = prob.ze[0] + g.random(n) * (prob.ze[-1] - prob.ze[0])
+    pos = np.stack([rho * np.cos(phi), rho * np.sin(phi), z], axis=1)
+    d = _isotropic(g, n)
+    rays = np.concatenate([pos, d, _watt(g, n)[:, None], (0.5 + g.random(n))[:, None]], axis=1).astype(np.float32)
+    rays[:, 2] = np.clip(rays[:, 2], np.float32(prob.ze[0]), np.nextafter(np.float32(prob.ze[-1]), np.float32(0)))
+    return np.ascontiguousarray(rays)
