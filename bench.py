@@ -191,6 +191,7 @@ def main():
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--sort", type=int, default=-1, help="override MR_OPT_SORT_RAYS (default: library default)")
     ap.add_argument("--opt", action="append", default=[], help="library option as ID=VALUE (MR_OPT_* of include/monteray.h), repeatable")
+    ap.add_argument("--pre-opt", action="append", default=[], help="like --opt, but set BEFORE the problem is loaded (options read by mr_load_materials)")
     ap.add_argument("--stage-rays", type=int, default=0, help="override MR_OPT_STAGE_RAYS (rays per H2D chunk of a host batch)")
     args = ap.parse_args()
     prob_kw = {}
@@ -216,6 +217,9 @@ def main():
     prob = make_problem(args.config, **prob_kw)
     rays = make_rays(prob, n_rays, batch=rank)  # every rank its own batch: weak scaling
     m = MonteRay(local_rank, 0)
+    for kv in args.pre_opt:
+        k, v = kv.split("=")
+        m.set_option(int(k), int(v))
     m.load_problem(prob)
     if args.block_threads:
         m.set_option(MR_OPT_BLOCK_THREADS, args.block_threads)

@@ -296,9 +296,13 @@ enum {
     MR_OPT_STAGE_RAYS = 3,    /* rays per staging chunk for host batches (H2D of chunk i+1 overlaps the cast of chunk i) */
     MR_OPT_COPY_THREADS = 4,  /* host threads that copy a PAGEABLE batch into the pinned ring (a pinned batch is DMA'd directly) */
     MR_OPT_PAIR_RECORDS = 5,  /* 1: 16-byte cell records (K = 2, 3, MIXED) are fetched as 32-byte pairs kept in registers; 0: one by one */
-    MR_OPT_ORDER_MODE = 6     /* key of the MR_OPT_SORT_RAYS pre-pass: 1 = (start z-slab, length): CTAs resident together work in the
+    MR_OPT_ORDER_MODE = 6,    /* key of the MR_OPT_SORT_RAYS pre-pass: 1 = (start z-slab, length): CTAs resident together work in the
                                  same slabs (L2 reuse); 2 = longest rays first: no tail; 0 = auto: 2 when tally + cell records fit
                                  in half the L2, else 1 */
+    MR_OPT_FUSED_TALLY = 7    /* read by mr_load_materials.  K = 4 records (MIXED) have 8 spare bytes: 1 = the cast kernel accumulates
+                                 each cell's score THERE (the load and the atomic of a segment then share one DRAM sector) and the sums
+                                 are moved into the contiguous tally whenever it is looked at (mr_read_tally, mr_tally_device_ptr,
+                                 mr_end_batch, mr_clear_tally); 0 = never; 2 (default) = when ncell * 40 bytes exceed twice the L2 */
 };
 MR_API int mr_set_option(mr_ctx *ctx, int option, int64_t value);
 MR_API int mr_get_option(mr_ctx *ctx, int option, int64_t *value);

@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     LIB_PATH,
     MR_OPT_BLOCK_THREADS,
     MR_OPT_COPY_THREADS,
+    MR_OPT_FUSED_TALLY,
     MR_OPT_ORDER_MODE,
     MR_OPT_PAIR_RECORDS,
     MR_OPT_SORT_RAYS,

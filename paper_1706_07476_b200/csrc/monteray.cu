@@ -155,6 +155,9 @@ struct mr_ctx {
     long long hist_cap = 0;
 
     int order_mode = 0;              // option MR_OPT_ORDER_MODE: 0 auto, 1 slab-major, 2 longest first
+    int fused_opt = 2;               // option MR_OPT_FUSED_TALLY: 0 off, 1 on, 2 auto (decided by mr_load_materials)
+    bool fused = false;              // LAYOUT_K4 records carry the score accumulators (LAYOUT_K4F in the cast kernel)
+    bool fused_dirty = false;        // in-record sums not yet moved into d_tally
     size_t l2_bytes = 0;             // device L2 size
     size_t rec_bytes_per_cell = 0;
     size_t resident_bytes() const { return (size_t)ncell * (8 + rec_bytes_per_cell); }   // tally + cell records
@@ -206,8 +209,23 @@ struct mr_ctx {
 
 namespace {
 
+// LAYOUT_K4F: bring d_tally up to date (queued on the stream).  No-op unless in-record sums are pending.
+cudaError_t flush_fused(mr_ctx *c)
+{
+    if (!c->fused || !c->fused_dirty || !c->d_recs || !c->d_tally) return cudaSuccess;
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    const unsigned grid = (unsigned)std::min<long long>((c->ncell + 255) / 256, (long long)sms * 16);
+    flush_fused_kernel<<<grid, 256, 0, c->stream>>>(c->d_recs, c->d_tally, c->ncell);
+    c->launches += 1;
+    c->fused_dirty = false;
+    return cudaGetLastError();
+}
+
 void free_materials(mr_ctx *c)
 {
+    if (flush_fused(c) == cudaSuccess) cudaStreamSynchronize(c->stream);   // the sums live in the records about to go
+    c->fused = false;
     c->dev_free(c->d_recs);
     c->dev_free(c->d_ids);
     c->d_recs = nullptr;
@@ -499,7 +517,10 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     case LAYOUT_K1: rc = launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P); break;
     case LAYOUT_K2: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
     case LAYOUT_K3: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K3P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P); break;
-    case LAYOUT_K4: rc = launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P); break;
+    case LAYOUT_K4:
+        if (c->fused) { rc = launch_cast_t<float, CellRec<LAYOUT_K4F>>(c, P); c->fused_dirty = true; }
+        else rc = launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P);
+        break;
     case LAYOUT_D8: rc = launch_cast_t<float, CellRec<LAYOUT_D8>>(c, P); break;
     default: rc = launch_cast_t<float, CellRecGeneric<float>>(c, P);
     }
@@ -833,6 +854,9 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
     c->d_ids = ids;
     c->layout = layout;
     c->rec_bytes_per_cell = rec_bytes + id_bytes;
+    c->fused = layout == LAYOUT_K4 && !c->mesh_rz &&
+               (c->fused_opt == 1 || (c->fused_opt == 2 && (size_t)c->ncell * 40 > 2 * c->l2_bytes));
+    c->fused_dirty = false;
     c->K = K;
     if (M != c->M || (int)c->xs_n.size() != M) {
         c->M = M;
@@ -1073,6 +1097,7 @@ int mr_read_tally(mr_ctx *c, double *out)
     MR_ENTER(c);
     if (!out) return c->fail(MR_ERR_INVALID_ARG, "read_tally: out is NULL");
     if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    MR_CUDA(c, flush_fused(c));
     MR_CUDA(c, cudaMemcpyAsync(out, c->d_tally, sizeof(double) * c->ncell, cudaMemcpyDeviceToHost, c->stream));
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
     return MR_OK;
@@ -1082,6 +1107,7 @@ int mr_clear_tally(mr_ctx *c)
 {
     MR_ENTER(c);
     if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    MR_CUDA(c, flush_fused(c));      // empties the in-record accumulators
     MR_CUDA(c, cudaMemsetAsync(c->d_tally, 0, sizeof(double) * c->ncell, c->stream));
     MR_CUDA(c, cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
     if (c->d_prev) {   // the batch moments restart with the tally
@@ -1131,6 +1157,7 @@ int mr_tally_device_ptr(mr_ctx *c, double **out)
     MR_ENTER(c);
     if (!out) return c->fail(MR_ERR_INVALID_ARG, "tally_device_ptr: out is NULL");
     if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    MR_CUDA(c, flush_fused(c));
     *out = c->d_tally;
     return MR_OK;
 }
@@ -1317,6 +1344,7 @@ int mr_end_batch(mr_ctx *c)
         MR_CUDA(c, cudaMemsetAsync(c->d_prev, 0, sizeof(double) * c->ncell, c->stream));
         MR_CUDA(c, cudaMemsetAsync(c->d_s2, 0, sizeof(double) * c->ncell, c->stream));
     }
+    MR_CUDA(c, flush_fused(c));
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
     const long long want = (c->ncell / 2 + 255) / 256 + 1;
@@ -1726,6 +1754,10 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "pair-records option is 0 or 1");
         c->pair_records = (int)value;
         return MR_OK;
+    case MR_OPT_FUSED_TALLY:
+        if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "fused-tally option is 0 (off), 1 (on) or 2 (auto)");
+        c->fused_opt = (int)value;
+        return MR_OK;
     case MR_OPT_ORDER_MODE:
         if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "order mode is 0 (auto), 1 (slab-major) or 2 (longest first)");
         c->order_mode = (int)value;
@@ -1749,6 +1781,7 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     case MR_OPT_COPY_THREADS: *value = c->copy_threads; return MR_OK;
     case MR_OPT_PAIR_RECORDS: *value = c->pair_records; return MR_OK;
     case MR_OPT_ORDER_MODE: *value = c->order_mode; return MR_OK;
+    case MR_OPT_FUSED_TALLY: *value = c->fused_opt; return MR_OK;
     }
     return c->fail(MR_ERR_INVALID_ARG, "unknown option");
 }

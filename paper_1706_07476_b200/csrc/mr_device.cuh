@@ -30,6 +30,7 @@ enum CellLayout : int {
     LAYOUT_K3 = 3,         // 16 B {float r0,r1,r2; u32 ids}
     LAYOUT_K4 = 4,         // 32 B {float r0..r3; u32 ids; u32 pad[3]}
     LAYOUT_D8 = 8,         // 32 B {float r[8]}  dense: slot k holds material k
+    LAYOUT_K4F = 14,       // kernel-side only: LAYOUT_K4 record whose 8 spare bytes (offset 24) hold the cell's score accumulator
     LAYOUT_K2P = 12,       // kernel-side only: LAYOUT_K2 / LAYOUT_K3 records fetched as 32-byte pairs
     LAYOUT_K3P = 13,
     LAYOUT_GENERIC = 100   // coef[ncell*K] (float or double) + ids[ncell*K] (u8, 0xff = empty)
@@ -361,7 +362,12 @@ __device__ __forceinline__ bool walker_step(Walker &w, const AxisF *axf, int str
 //   sigma(value, sig, stride, K) Sigma_t of that cell
 template <int LAYOUT> struct CellRec;
 
-template <> struct CellRec<LAYOUT_K1> {
+// where a cell's score goes: the contiguous fp64 tally, unless the record type keeps the accumulator inside the record
+struct PlainTally {
+    static __device__ __forceinline__ double *tally_at(double *tally, const void *, int cell) { return tally + cell; }
+};
+
+template <> struct CellRec<LAYOUT_K1> : PlainTally {
     typedef uint2 Value;
     uint2 v;
     __device__ __forceinline__ void reset() {}
@@ -395,7 +401,7 @@ struct SingleRec {
     __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c) { v = ldg_u4(reinterpret_cast<const uint4 *>(recs) + c); }
     __device__ __forceinline__ uint4 value() const { return v; }
 };
-template <typename Fetch> struct RecK2 : Fetch {
+template <typename Fetch> struct RecK2 : Fetch, PlainTally {
     typedef uint4 Value;
     static __device__ __forceinline__ float sigma(const Value &v, const float *sig, int stride, int)
     {
@@ -403,7 +409,7 @@ template <typename Fetch> struct RecK2 : Fetch {
         return fmaf(__uint_as_float(v.y), sig[((v.z >> 8) & 0xffu) * stride], s);
     }
 };
-template <typename Fetch> struct RecK3 : Fetch {
+template <typename Fetch> struct RecK3 : Fetch, PlainTally {
     typedef uint4 Value;
     static __device__ __forceinline__ float sigma(const Value &v, const float *sig, int stride, int)
     {
@@ -416,7 +422,7 @@ template <> struct CellRec<LAYOUT_K2> : RecK2<SingleRec> {};
 template <> struct CellRec<LAYOUT_K3> : RecK3<SingleRec> {};
 template <> struct CellRec<LAYOUT_K2P> : RecK2<PairRec> {};
 template <> struct CellRec<LAYOUT_K3P> : RecK3<PairRec> {};
-template <> struct CellRec<LAYOUT_K4> {
+template <> struct CellRec<LAYOUT_K4> : PlainTally {
     struct Value { uint4 v; uint32_t ids; };
     Value q;
     __device__ __forceinline__ void reset() {}
@@ -435,7 +441,38 @@ template <> struct CellRec<LAYOUT_K4> {
         return fmaf(__uint_as_float(q.v.w), sig[(q.ids >> 24) * stride], s);
     }
 };
-template <> struct CellRec<LAYOUT_D8> {
+// LAYOUT_K4 with the score accumulator INSIDE the record (bytes 24..31 of the 32-byte record are spare): on a mesh far
+// larger than L2 every segment costs one DRAM fetch for the record and another for the tally sector; with the
+// accumulator in the record's own sector the RED that follows the load hits L2.  The whole record is
+// read with one plain (coherent) 32-byte load -- not ld.global.nc: the sector is written by the REDs of this kernel.
+// flush_fused_kernel moves the in-record sums into the contiguous tally whenever the tally is looked at.
+template <> struct CellRec<LAYOUT_K4F> {
+    struct Value { uint4 v; uint32_t ids; };
+    Value q;
+    __device__ __forceinline__ void reset() {}
+    __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c)
+    {
+        uint4 lo, hi;
+        asm volatile("ld.global.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=r"(lo.x), "=r"(lo.y), "=r"(lo.z), "=r"(lo.w), "=r"(hi.x), "=r"(hi.y), "=r"(hi.z), "=r"(hi.w)
+                     : "l"(reinterpret_cast<const uint4 *>(recs) + 2 * (size_t)c));
+        q.v = lo;
+        q.ids = hi.x;
+    }
+    __device__ __forceinline__ Value value() const { return q; }
+    static __device__ __forceinline__ float sigma(const Value &q, const float *sig, int stride, int)
+    {
+        float s = __uint_as_float(q.v.x) * sig[(q.ids & 0xffu) * stride];
+        s = fmaf(__uint_as_float(q.v.y), sig[((q.ids >> 8) & 0xffu) * stride], s);
+        s = fmaf(__uint_as_float(q.v.z), sig[((q.ids >> 16) & 0xffu) * stride], s);
+        return fmaf(__uint_as_float(q.v.w), sig[(q.ids >> 24) * stride], s);
+    }
+    static __device__ __forceinline__ double *tally_at(double *, const void *recs, int cell)
+    {
+        return reinterpret_cast<double *>(reinterpret_cast<uintptr_t>(recs) + 32 * (size_t)cell + 24);
+    }
+};
+template <> struct CellRec<LAYOUT_D8> : PlainTally {
     struct Value { float4 a, b; };
     Value q;
     __device__ __forceinline__ void reset() {}
@@ -461,7 +498,7 @@ template <> struct CellRec<LAYOUT_D8> {
 };
 
 // Generic layout, either precision: nothing is prefetched, the slots are read in sigma().
-template <typename Real> struct CellRecGeneric {
+template <typename Real> struct CellRecGeneric : PlainTally {
     struct Value { const Real *coef; const uint8_t *ids; };
     Value q;
     __device__ __forceinline__ void reset() {}
@@ -578,6 +615,16 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
 
             double wa = R.W;   // W * exp(-tau), a running product of exp(-x)
             double *const tally = P.tally;
+            // S4 + S5 + S6 for one segment: score = W e^{-tau} (1 - e^{-x}) / Sigma, x = Sigma * len (Eq. (4));
+            // a zero-length segment scores exactly 0: nothing to add
+            auto score = [&](const typename Rec::Value &cur, int cell, double len) {
+                const double S = (double)Rec::sigma(cur, sig, stride, P.K);
+                double g, ex;
+                score_terms<sizeof(Real) == 8>(S, len, g, ex);
+                if (len > 0.0) red_add_f64(Rec::tally_at(tally, P.recs, cell), wa * g);
+                wa *= ex;
+                ++nseg;
+            };
             Rec rec;
             rec.reset();
             rec.load(P.recs, P.ids, P.K, w.c);
@@ -587,14 +634,7 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
                 const bool leave = walker_step<EDGE_MODE>(w, axf, stride, P.mesh, e, cell, len);
                 const typename Rec::Value cur = rec.value();
                 if (!leave) rec.load(P.recs, P.ids, P.K, w.c);   // next cell's record: in flight during the score
-                // S4 + S5 (Eq. (4)): score = W e^{-tau} (1 - e^{-x}) / Sigma,  x = Sigma * len
-                const double S = (double)Rec::sigma(cur, sig, stride, P.K);
-                double g, ex;
-                score_terms<sizeof(Real) == 8>(S, len, g, ex);
-                // S6 (a zero-length segment scores exactly 0: nothing to add)
-                if (len > 0.0) red_add_f64(tally + cell, wa * g);
-                wa *= ex;
-                ++nseg;
+                score(cur, cell, len);
                 if (leave) break;
             }
         }
@@ -1002,6 +1042,20 @@ __global__ void __launch_bounds__(256) fold_batch_kernel(const double *__restric
             const double t = tally[c], x = t - prev[c];
             s2[c] = fma(x, x, s2[c]);
             prev[c] = t;
+        }
+    }
+}
+
+// LAYOUT_K4F: move the in-record score sums into the contiguous tally (tally[c] += acc; acc = 0)
+__global__ void __launch_bounds__(256) flush_fused_kernel(void *recs, double *__restrict__ tally, long long ncell)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += stride) {
+        double *acc = reinterpret_cast<double *>(reinterpret_cast<char *>(recs) + 32 * c + 24);
+        const double v = *acc;
+        if (v != 0.0) {
+            tally[c] += v;
+            *acc = 0.0;
         }
     }
 }

@@ -321,3 +321,39 @@ def test_order_modes_give_the_same_result():
         from paper_1706_07476_b200 import MonteRayError
         with pytest.raises(MonteRayError):
             m.set_option(MR_OPT_ORDER_MODE, 3)
+
+
+@pytest.mark.parametrize("fused", [1, 0])
+def test_fused_in_record_tally_for_k4(fused):
+    """MR_OPT_FUSED_TALLY: K = 4 records carry the score accumulators; every call that looks at the tally
+    (read, device pointer / tensor view, end_batch, clear) first moves the in-record sums into the contiguous
+    tally, so nothing observable changes.  Includes a materials reload between two casts (the sums survive)."""
+    from paper_1706_07476_b200 import MR_OPT_FUSED_TALLY, MonteRay
+
+    prob = make_problem(4, n=48, n_e=3000)
+    rays = make_rays(prob, 40_001)
+    ref = _oracle(prob).cast(rays, threads=_threads())
+    with MonteRay(0, 0) as m:
+        m.set_option(MR_OPT_FUSED_TALLY, fused)
+        m.load_problem(prob)
+        m.cast_rays(rays[:10_000])
+        m.end_batch()
+        m.cast_rays(rays[10_000:25_000])
+        t_view = m.tally_tensor().cpu().numpy().copy()          # device view is up to date
+        part = _oracle(prob).cast(rays[:25_000], threads=_threads())
+        assert_tally(t_view, part.tally, 0)
+        m.load_materials(prob.density, prob.cell_mat, prob.cell_frac)   # new records: pending sums must not be lost
+        for k, (e, s) in enumerate(prob.xs):
+            m.load_xs(k, e, s)
+        m.cast_rays(rays[25_000:])
+        m.end_batch()
+        got = m.read_tally()
+        s1, s2, nb = m.read_moments()
+        st = m.get_stats()
+        m.clear_tally()
+        assert not m.read_tally().any()
+        m.cast_rays(rays[:100])
+        assert m.read_tally().any()
+    assert nb == 2 and np.array_equal(s1, got)
+    assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+    assert_tally(got, ref.tally, 0)
