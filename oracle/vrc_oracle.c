@@ -455,6 +455,9 @@ int vrc_next_event(const vrc_problem *p, int64_t n, const double *rays, const do
 typedef struct {
     int32_t nr, nz;
     const double *re, *ze;      /* nr+1 radii (re[0] == 0, strictly increasing), nz+1 planes */
+    int32_t spherical;          /* 1: 1-D spherical shells about the origin ("1-D spherical meshes"):
+                                 *    rho0^2 = ox*ox + oy*oy + oz*oz, a = dx*dx + dy*dy + dz*dz, b = ox*dx + oy*dy + oz*dz,
+                                 *    no axial crossings, nz = 1 and ze is not read; everything else as Z1-Z5 */
 } vrc_rz_mesh;
 
 static int cast_one_rz(const vrc_problem *p, const vrc_rz_mesh *g, const double *ray, double *tally,
@@ -471,15 +474,16 @@ static int cast_one_rz(const vrc_problem *p, const vrc_rz_mesh *g, const double 
     /* Z1 */
     for (int f = 0; f < 8; ++f) if (!isfinite(ray[f])) accepted = 0;
     if (!(E > 0.0)) accepted = 0;
-    const double rho2 = ox * ox + oy * oy;
-    const double a = dx * dx + dy * dy;
+    const int sph = g->spherical != 0;
+    const double rho2 = sph ? ox * ox + oy * oy + oz * oz : ox * ox + oy * oy;
+    const double a = sph ? dx * dx + dy * dy + dz * dz : dx * dx + dy * dy;
     const double inv_a = (a != 0.0) ? 1.0 / a : 0.0;
     const int radial = (a != 0.0) && isfinite(inv_a) && isfinite(a);
     const double inv_z = (dz != 0.0) ? 1.0 / dz : 0.0;
-    const int axial = (dz != 0.0) && isfinite(inv_z);
+    const int axial = !sph && (dz != 0.0) && isfinite(inv_z);
     if (!radial && !axial) accepted = 0;
     if (accepted && !(rho2 < g->re[nr] * g->re[nr])) accepted = 0;
-    if (accepted && !(oz >= g->ze[0] && oz < g->ze[nz])) accepted = 0;
+    if (accepted && !sph && !(oz >= g->ze[0] && oz < g->ze[nz])) accepted = 0;
 
     if (accepted) {
         double sig[64];
@@ -487,9 +491,9 @@ static int cast_one_rz(const vrc_problem *p, const vrc_rz_mesh *g, const double 
         /* Z3 */
         int32_t ir = -1;
         for (int32_t q = 0; q <= nr; ++q) if (g->re[q] * g->re[q] <= rho2) ir = q;
-        int32_t iz = (int32_t)(upper_bound(g->ze, nz + 1, oz) - 1);
+        int32_t iz = sph ? 0 : (int32_t)(upper_bound(g->ze, nz + 1, oz) - 1);
         /* Z4 */
-        const double b = ox * dx + oy * dy;
+        const double b = sph ? ox * dx + oy * dy + oz * dz : ox * dx + oy * dy;
         int inward = 0;
         double t_r = INFINITY, t_z = INFINITY;
         int32_t pz = 0, stepz = 0;
@@ -584,7 +588,7 @@ static int cast_one_rz(const vrc_problem *p, const vrc_rz_mesh *g, const double 
 int vrc_cast_rz(const vrc_problem *p, const vrc_rz_mesh *g, int64_t n, const double *rays, double *tally,
                 const vrc_diag *dg, vrc_counts *counts)
 {
-    if (p->M > 64 || g->nr < 1 || g->nz < 1 || g->re[0] != 0.0) return -1;
+    if (p->M > 64 || g->nr < 1 || g->nz < 1 || g->re[0] != 0.0 || (g->spherical && g->nz != 1)) return -1;
     vrc_counts cnt = {0, 0, 0};
     for (int64_t r = 0; r < n; ++r) {
         if (cast_one_rz(p, g, rays + 8 * r, tally, dg, r, &cnt.segments)) cnt.rays_accepted++;

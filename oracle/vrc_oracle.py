@@ -48,7 +48,7 @@ class _Counts(C.Structure):
 
 
 class _RzMesh(C.Structure):
-    _fields_ = [("nr", C.c_int32), ("nz", C.c_int32), ("re", C.c_void_p), ("ze", C.c_void_p)]
+    _fields_ = [("nr", C.c_int32), ("nz", C.c_int32), ("re", C.c_void_p), ("ze", C.c_void_p), ("spherical", C.c_int32)]
 
 
 class _NeDiag(C.Structure):
@@ -236,7 +236,11 @@ class Oracle:
             int(cnt.rays_accepted), int(cnt.rays_rejected), int(cnt.segments), int(used))
         return res
 
-    def cast_rz(self, rays, re, ze, *, per_ray: bool = True, cap: int = 0) -> CastResult:
+    def cast_sphere(self, rays, re, *, cap: int = 0) -> CastResult:
+        """Cast `rays` on 1-D spherical shells (re: nr+1 radii from 0 about the origin); cell c = ir."""
+        return self.cast_rz(rays, re, np.array([0.0, 1.0]), cap=cap, spherical=True)
+
+    def cast_rz(self, rays, re, ze, *, per_ray: bool = True, cap: int = 0, spherical: bool = False) -> CastResult:
         """Cast `rays` on the R-Z mesh (re: nr+1 radii from 0, ze: nz+1 planes); the problem's cell arrays hold
         nr*nz cells, c = ir + nr*iz (steps Z1..Z5 of vrc_oracle.c).  Single thread."""
         r = np.ascontiguousarray(np.asarray(rays, dtype=np.float64).reshape(-1, 8))
@@ -258,7 +262,7 @@ class Oracle:
             res.lens = np.zeros((n, cap), dtype=np.float64)
             res.scores = np.zeros((n, cap), dtype=np.float64)
             dg.cells, dg.lens, dg.scores, dg.cap = res.cells.ctypes.data, res.lens.ctypes.data, res.scores.ctypes.data, cap
-        g = _RzMesh(nr, nz, re.ctypes.data, ze.ctypes.data)
+        g = _RzMesh(nr, nz, re.ctypes.data, ze.ctypes.data, 1 if spherical else 0)
         cnt = _Counts()
         rc = self.lib.vrc_cast_rz(C.byref(self._p), C.byref(g), n, r.ctypes.data, tally.ctypes.data,
                                   C.cast(C.byref(dg), C.c_void_p), C.cast(C.byref(cnt), C.c_void_p))

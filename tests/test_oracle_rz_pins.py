@@ -150,3 +150,60 @@ def test_rejections():
     res = Oracle(prob).cast_rz(np.array(rows), prob.re, prob.ze)
     assert res.rays_accepted == 2 and res.rays_rejected == 7
     assert res.nseg[-1] == 3 and not res.nseg[1:-1].any()
+
+
+# ----------------------------------------------------------------------------- 1-D spherical shells
+def test_sphere_trace_equals_brute_force_roots_and_closed_forms():
+    """Spherical shells ("1-D spherical meshes"): crossings from numpy.roots of |o + t d|^2 = r_p^2,
+    shell of each segment mid-point by searchsorted on |x|, exit = outer sphere; homogeneous closed form."""
+    from tests.tiny import tiny_sphere_problem, tiny_sphere_rays
+
+    for seed, uniform in ((11, False), (12, True)):
+        prob = tiny_sphere_problem(seed, nr=7, uniform=uniform, homogeneous=True)
+        rays = tiny_sphere_rays(prob, seed, 300, through_centre_share=0.05).astype(np.float64)
+        res = Oracle(prob).cast_sphere(rays, prob.re, cap=20)
+        assert res.rays_accepted == 300
+        for r in range(len(rays)):
+            o, d = rays[r, :3], rays[r, 3:6]
+            ts = []
+            for p in range(1, prob.nr + 1):
+                for t in np.roots([d @ d, 2 * (o @ d), o @ o - prob.re[p] ** 2]):
+                    if abs(t.imag) < 1e-9 and t.real > 1e-12:
+                        ts.append(float(t.real))
+            ts = np.array(sorted(ts))
+            t_out = (-(o @ d) + np.sqrt((o @ d) ** 2 - (d @ d) * (o @ o - prob.re[-1] ** 2))) / (d @ d)
+            ts = ts[ts <= t_out * (1 + 1e-12)]
+            n = int(res.nseg[r])
+            if r >= 15:                                   # (the rays aimed exactly at the centre have double roots)
+                assert n == len(ts), (seed, r, n, len(ts))
+                bounds = np.concatenate([[0.0], ts])
+                np.testing.assert_allclose(res.lens[r, :n], np.diff(bounds), rtol=1e-8, atol=1e-11)
+                mids = o[None, :] + (0.5 * (bounds[1:] + bounds[:-1]))[:, None] * d[None, :]
+                shells = np.searchsorted(prob.re, np.linalg.norm(mids, axis=1), side="right") - 1
+                assert np.array_equal(res.cells[r, :n], shells)
+            assert res.t_exit[r] == pytest.approx(t_out, rel=1e-12)
+            S = prob.density[0] * np.interp(float(rays[r, 6]), *prob.xs[0])
+            assert res.sum_score[r] == pytest.approx(float(rays[r, 7]) / S * -np.expm1(-S * t_out), rel=1e-11)
+    # through the centre from shell 3 of uniform shells 0.5 k: 3,2,1,0,1,2,...,6 with lengths 0.2, 0.5, 0.5, 1.0, 0.5...
+    prob = tiny_sphere_problem(13, nr=7, uniform=True)
+    res = Oracle(prob).cast_sphere(np.array([[0.0, 1.7, 0.0, 0, -1, 0, 1.0, 1.0]]), prob.re, cap=12)
+    assert list(res.cells[0, : res.nseg[0]]) == [3, 2, 1, 0, 1, 2, 3, 4, 5, 6]
+    np.testing.assert_allclose(res.lens[0, :10], [0.2, 0.5, 0.5, 1.0] + [0.5] * 6, rtol=1e-13, atol=1e-15)
+
+
+def test_sphere_rotation_invariance_and_rejections():
+    from tests.tiny import tiny_sphere_problem, tiny_sphere_rays
+
+    prob = tiny_sphere_problem(14, nr=6, K=2, M=3)
+    rays = tiny_sphere_rays(prob, 14, 400).astype(np.float64)
+    a = Oracle(prob).cast_sphere(rays, prob.re).tally
+    q, _ = np.linalg.qr(np.random.default_rng(1).normal(size=(3, 3)))     # any orthogonal map leaves shells invariant
+    rot = rays.copy()
+    rot[:, :3] = rays[:, :3] @ q.T
+    rot[:, 3:6] = rays[:, 3:6] @ q.T
+    np.testing.assert_allclose(Oracle(prob).cast_sphere(rot, prob.re).tally, a, rtol=1e-9, atol=1e-12 * a.max())
+    R = prob.re[-1]
+    rows = [[0.1, 0.1, 0.1, 0, 0, 1, 1.0, 1.0], [R, 0, 0, 1, 0, 0, 1.0, 1.0], [0.1, 0, 0, 0, 0, 0, 1.0, 1.0],
+            [0.1, 0, 0, 0, 0, 1, -1.0, 1.0], [0.0, 0.0, 0.0, 0, 0, 1, 1.0, 1.0]]
+    res = Oracle(prob).cast_sphere(np.array(rows), prob.re)
+    assert res.rays_accepted == 2 and res.rays_rejected == 3 and res.nseg[4] == prob.nr

@@ -93,3 +93,30 @@ def tiny_rz_rays(prob, seed, n, axis_parallel_share=0.0, through_axis_share=0.0,
     w = 0.5 + g.random(n)
     rays = np.concatenate([pos, d, e[:, None], w[:, None]], axis=1)
     return np.ascontiguousarray(rays.astype(dtype))
+
+
+def tiny_sphere_problem(seed, nr=6, M=3, K=2, n_e=17, uniform=False, homogeneous=False):
+    """Tiny 1-D spherical problem: nr shells about the origin (cell c = ir); fields re, nr, sphere=True."""
+    prob = tiny_problem(seed, nx=nr, ny=1, nz=1, M=M, K=K, n_e=n_e, uniform=uniform, homogeneous=homogeneous)
+    g = np.random.default_rng(seed + 2000)
+    prob.re = 0.5 * np.arange(nr + 1) if uniform else np.concatenate([[0.0], np.cumsum(0.15 + 0.6 * g.random(nr))])
+    prob.nr = nr
+    prob.sphere = True
+    prob.xe, prob.ye, prob.ze = prob.re, np.array([0.0, 1.0]), np.array([0.0, 1.0])
+    return prob
+
+
+def tiny_sphere_rays(prob, seed, n, through_centre_share=0.0, e_lo=5e-4, e_hi=20.0, dtype=np.float32):
+    g = np.random.default_rng(seed)
+    R = prob.re[-1]
+    u = g.normal(size=(n, 3))
+    u /= np.linalg.norm(u, axis=1, keepdims=True)
+    pos = u * (R * np.cbrt(0.999 * g.random(n)))[:, None]
+    d = g.normal(size=(n, 3))
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    k = int(through_centre_share * n)
+    d[:k] = -pos[:k] / np.maximum(np.linalg.norm(pos[:k], axis=1, keepdims=True), 1e-30)
+    e = e_lo * (e_hi / e_lo) ** g.random(n)
+    w = 0.5 + g.random(n)
+    rays = np.concatenate([pos, d, e[:, None], w[:, None]], axis=1)
+    return np.ascontiguousarray(rays.astype(dtype))
