@@ -128,6 +128,12 @@ MR_API int mr_load_mesh(mr_ctx *ctx, int nx, int ny, int nz, const double *xe, c
  * before.  Errors: INVALID_ARG (re[0] != 0, not increasing), UNSUPPORTED, OOM, CUDA. */
 MR_API int mr_load_mesh_rz(mr_ctx *ctx, int nr, int nz, const double *re, const double *ze);
 
+/* 1-D spherical tally mesh ("1-D spherical meshes"): nr shells re[0] = 0 < ... < re[nr] about the origin,
+ * cell c = ir = the shell that holds sqrt(x^2+y^2+z^2) (ncell = nr).  The walk is the radial part of the R-Z walk with
+ * rho0^2 = |o|^2, a = |d|^2, b = o.d and no axial crossings; a ray is rejected if |o|^2 >= re[nr]^2.  Same
+ * restrictions as mr_load_mesh_rz.  Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA. */
+MR_API int mr_load_mesh_sphere(mr_ctx *ctx, int nr, const double *re);
+
 /* Materials and per-cell composition.  density[M] g/cc (finite, >= 0); K slots per cell;
  * cell_mat[ncell*K] material index per slot, -1 = empty slot; cell_frac[ncell*K] volume
  * fractions (finite, >= 0; ignored for empty slots).  Slot k of cell c is element c*K+k.

@@ -29,7 +29,7 @@ EXPORTS = [
     "mr_create", "mr_create_ex", "mr_destroy", "mr_set_stream", "mr_last_error", "mr_load_mesh",
     "mr_load_materials", "mr_load_xs", "mr_cast_rays", "mr_read_tally", "mr_clear_tally", "mr_sync",
     "mr_get_stats", "mr_tally_device_ptr", "mr_trace_rays", "mr_set_option", "mr_get_option",
-    "mr_end_batch", "mr_read_moments", "mr_read_mean_sigma", "mr_load_nuclide_xs", "mr_define_material", "mr_load_mesh_rz",
+    "mr_end_batch", "mr_read_moments", "mr_read_mean_sigma", "mr_load_nuclide_xs", "mr_define_material", "mr_load_mesh_rz", "mr_load_mesh_sphere",
     "mr_ring_open", "mr_ring_push", "mr_ring_flush", "mr_ring_close", "mr_ring_get_stats",
     "mr_load_detectors", "mr_cast_next_event", "mr_read_detectors", "mr_clear_detectors", "mr_trace_next_event",
 ]
@@ -80,6 +80,7 @@ def load_library() -> C.CDLL:
         "mr_set_stream": [vp, vp],
         "mr_load_mesh": [vp, i32, i32, i32, vp, vp, vp],
         "mr_load_mesh_rz": [vp, i32, i32, vp, vp],
+        "mr_load_mesh_sphere": [vp, i32, vp],
         "mr_load_materials": [vp, i32, vp, i32, vp, vp],
         "mr_load_xs": [vp, i32, i64, vp, vp],
         "mr_cast_rays": [vp, i64, vp, i32],
@@ -230,6 +231,11 @@ class MonteRay:
         self._check(self.lib.mr_load_mesh_rz(self._h, len(re) - 1, len(ze) - 1, re.ctypes.data, ze.ctypes.data))
         self.ncell = (len(re) - 1) * (len(ze) - 1)
 
+    def load_mesh_sphere(self, re):
+        re = _f64(re)
+        self._check(self.lib.mr_load_mesh_sphere(self._h, len(re) - 1, re.ctypes.data))
+        self.ncell = len(re) - 1
+
     def load_materials(self, density, cell_mat, cell_frac):
         density = _f64(density)
         cell_mat = np.ascontiguousarray(cell_mat, dtype=np.int32)
@@ -261,7 +267,9 @@ class MonteRay:
 
     def load_problem(self, prob):
         """Convenience: mesh + materials + all tables (and nuclide mixtures) of a workloads.Problem-like object."""
-        if getattr(prob, "re", None) is not None:
+        if getattr(prob, "sphere", False):
+            self.load_mesh_sphere(prob.re)
+        elif getattr(prob, "re", None) is not None:
             self.load_mesh_rz(prob.re, prob.ze)
         else:
             self.load_mesh(prob.xe, prob.ye, prob.ze)

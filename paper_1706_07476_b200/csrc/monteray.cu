@@ -86,6 +86,7 @@ struct mr_ctx {
     int nx = 0, ny = 0, nz = 0, nedges = 0;
     long long ncell = 0;
     bool mesh_rz = false;              // R-Z mesh (mr_load_mesh_rz): nx = nr radial shells, ny = 1, x planes = radii
+    bool mesh_sphere = false;          // with mesh_rz: 1-D spherical shells (mr_load_mesh_sphere), nz = 1
     bool mesh_arith = false;           // every plane position equals fma(p, h, e0) bit for bit
     double mesh_e0[3] = {0, 0, 0}, mesh_h[3] = {0, 0, 0};
     double *d_edges = nullptr;
@@ -471,6 +472,7 @@ int launch_rz_cast(mr_ctx *c, const CastParams &P)
 {
     RzParams Q{};
     Q.c = P;
+    Q.spherical = c->mesh_sphere ? 1 : 0;
     const int block = c->block_threads;
     if (c->precision == MR_PRECISION_DOUBLE) return launch_rz_t<double, CellRecGeneric<double>, false>(c, Q, block);
     switch (c->layout) {
@@ -742,6 +744,7 @@ int load_mesh_common(mr_ctx *c, bool rz, int nx, int ny, int nz, const double *x
     }
     c->nx = nx; c->ny = ny; c->nz = nz; c->nedges = ne; c->ncell = ncell;
     c->mesh_rz = rz;
+    c->mesh_sphere = false;
     {   // arithmetic mesh?  (uniform spacing reproduced exactly by one fma per plane, checked plane by plane)
         const double *ax[3] = {xe, ye, ze};
         const int na[3] = {nx, ny, nz};
@@ -778,6 +781,17 @@ int mr_load_mesh_rz(mr_ctx *c, int nr, int nz, const double *re, const double *z
     if (re[0] != 0.0) return c->fail(MR_ERR_INVALID_ARG, "rz mesh: the first radius must be 0");
     const double ye[2] = {0.0, 1.0};
     return load_mesh_common(c, true, nr, 1, nz, re, ye, ze);
+}
+
+int mr_load_mesh_sphere(mr_ctx *c, int nr, const double *re)
+{
+    MR_ENTER(c);
+    if (nr < 1 || !re) return c->fail(MR_ERR_INVALID_ARG, "spherical mesh: bad size or NULL radius array");
+    if (re[0] != 0.0) return c->fail(MR_ERR_INVALID_ARG, "spherical mesh: the first radius must be 0");
+    const double one[2] = {0.0, 1.0};
+    if (int rc = load_mesh_common(c, true, nr, 1, 1, re, one, one)) return rc;
+    c->mesh_sphere = true;
+    return MR_OK;
 }
 
 int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int32_t *cell_mat, const double *cell_frac)
@@ -1207,6 +1221,7 @@ int mr_trace_rays(mr_ctx *c, int64_t n, const void *rays, int where, uint32_t *n
         Q.c.n = n;
         Q.nseg = d_nseg; Q.hash = d_hash; Q.cells = d_cells; Q.lens = d_lens; Q.cap = cap;
         Q.ray_is_double = c->precision == MR_PRECISION_DOUBLE ? 1 : 0;
+        Q.spherical = c->mesh_sphere ? 1 : 0;
         if (launch_rz_t<float, CellRecGeneric<float>, true>(c, Q, 256) != MR_OK) { cleanup(); return MR_ERR_CUDA; }
     } else if (e == cudaSuccess) {
         TraceParams P{mesh_dev(c), d_rays, n, d_nseg, d_hash, d_cells, d_lens, cap, c->precision == MR_PRECISION_DOUBLE ? 1 : 0};

@@ -730,6 +730,7 @@ struct RzParams {
     double *lens;
     long long cap;
     int ray_is_double;
+    int spherical;           // 1: 1-D spherical shells about the origin (no axial crossings; nz = 1)
 };
 
 __device__ __forceinline__ double rz_t_radial(double b, double a, double inv_a, double rho2, double rp, bool outward)
@@ -771,13 +772,18 @@ __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParam
             ox = R.o[0]; oy = R.o[1]; oz = R.o[2]; dx = R.d[0]; dy = R.d[1]; dz = R.d[2]; W = R.W; E = (Real)R.E; fin = R.finite && R.E > 0.0f;
         }
         // Z1
-        const double rho2 = __dadd_rn(__dmul_rn(ox, ox), __dmul_rn(oy, oy));
-        const double a = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+        const bool sph = Q.spherical != 0;
+        double rho2 = __dadd_rn(__dmul_rn(ox, ox), __dmul_rn(oy, oy));
+        double a = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+        if (sph) {
+            rho2 = __dadd_rn(rho2, __dmul_rn(oz, oz));
+            a = __dadd_rn(a, __dmul_rn(dz, dz));
+        }
         const double inv_a = (a != 0.0) ? __drcp_rn(a) : 0.0;
         const bool radial = (a != 0.0) && isfinite(inv_a) && isfinite(a);
         const double inv_z = (dz != 0.0) ? __drcp_rn(dz) : 0.0;
-        const bool axial = (dz != 0.0) && isfinite(inv_z);
-        accepted = fin && (radial || axial) && (rho2 < __dmul_rn(re[nr], re[nr])) && (oz >= ze[0] && oz < ze[nz]);
+        const bool axial = !sph && (dz != 0.0) && isfinite(inv_z);
+        accepted = fin && (radial || axial) && (rho2 < __dmul_rn(re[nr], re[nr])) && (sph || (oz >= ze[0] && oz < ze[nz]));
         if (accepted) {
             if (!TRACE) sigma_all<Real>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, E, sig, stride);   // Z2
             // Z3: ir = #{p : r_p^2 <= rho0^2} - 1 (r_p^2 is non-decreasing in p), iz by comparisons
@@ -787,9 +793,10 @@ __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParam
                 if (__dmul_rn(re[mid], re[mid]) <= rho2) lo = mid + 1; else hi = mid;
             }
             int ir = lo - 1;
-            int iz = upper_bound_edges(ze, nz + 1, oz) - 1;
+            int iz = sph ? 0 : upper_bound_edges(ze, nz + 1, oz) - 1;
             // Z4
-            const double b = __dadd_rn(__dmul_rn(ox, dx), __dmul_rn(oy, dy));
+            double b = __dadd_rn(__dmul_rn(ox, dx), __dmul_rn(oy, dy));
+            if (sph) b = __dadd_rn(b, __dmul_rn(oz, dz));
             const double inf = __longlong_as_double(0x7ff0000000000000LL);
             bool inward = false;
             double t_r = inf, t_z = inf, t_cur = 0.0;

@@ -130,3 +130,35 @@ def test_rz_pin_cell_workload_in_bench_configuration():
     assert np.array_equal(nseg, ref.nseg) and np.array_equal(hsh, ref.hash)
     assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
     assert np.all(np.abs(got - ref.tally) <= 1e-4 * np.abs(ref.tally) + 1e-7 * ref.tally.max())
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+@pytest.mark.parametrize("seed,K,M,uniform,nr", [(421, 1, 2, False, 9), (422, 3, 4, True, 40), (423, 8, 8, False, 300)])
+def test_spherical_shell_mesh(seed, K, M, uniform, nr, precision):
+    """1-D spherical shells (mr_load_mesh_sphere): traces (cells and lengths) bit-exact, counters
+    exact, tallies in tolerance; rays aimed at the centre, rejected rays (outside the sphere, zero direction)."""
+    from oracle.vrc_oracle import Oracle
+    from paper_1706_07476_b200 import MonteRay
+    from tests.tiny import tiny_sphere_problem, tiny_sphere_rays
+
+    prob = tiny_sphere_problem(seed, nr=nr, M=M, K=K, n_e=65, uniform=uniform)
+    rays32 = tiny_sphere_rays(prob, seed, 5003, through_centre_share=0.05)
+    rays32[7, :3] = [1.5 * prob.re[-1], 0.0, 0.0]    # outside the sphere: rejected
+    rays32[9, 3:6] = 0.0                             # zero direction: rejected
+    cap = 2 * nr + 1 if nr <= 40 else 0
+    ref = Oracle(prob).cast_sphere(rays32, prob.re, cap=cap)
+    assert ref.rays_rejected == 2
+    with MonteRay(0, precision) as m:
+        m.load_problem(prob)
+        rays = rays32.astype(m.ray_dtype)
+        m.cast_rays(rays)
+        got = m.read_tally()
+        st = m.get_stats()
+        nseg, hsh, cells, lens = m.trace_rays(rays, cap=cap)
+    assert np.array_equal(nseg, ref.nseg) and np.array_equal(hsh, ref.hash)
+    if cap:
+        assert np.array_equal(cells, ref.cells) and np.array_equal(lens, ref.lens)
+    assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+    d = np.abs(got - ref.tally)
+    bound = (1e-4 * np.abs(ref.tally) + 1e-7 * ref.tally.max()) if precision == 0 else (1e-10 * np.abs(ref.tally) + 1e-290)
+    assert np.all(d <= bound)
