@@ -847,19 +847,29 @@ __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParam
                 }
                 ++nseg;
                 t_cur = tn;
-                if (ax) {
-                    iz += stepz;
-                    if (iz < 0 || iz >= nz) break;
-                    pz += stepz;
-                    t_z = __dmul_rn(__dsub_rn(ze[pz], oz), inv_z);
-                } else if (inward) {
-                    ir -= 1;
-                    next_radial(true);
-                } else {
-                    ir += 1;
-                    if (ir >= nr) break;
-                    t_r = rz_t_radial(b, a, inv_a, rho2, re[ir + 1], true);
-                }
+                // One instruction stream for the three kinds of step (axial, inward, outward): the next crossing of
+                // BOTH families is evaluated and the one that applies is selected, never branched on, so the lanes
+                // of a warp do not serialise (15 of 32 lanes were active with a three-way branch here).  The values
+                // that are kept come from exactly the operations of Z4.
+                const int iz_n = ax ? iz + stepz : iz;
+                const int ir_n = ax ? ir : (inward ? ir - 1 : ir + 1);
+                if (iz_n < 0 || iz_n >= nz || ir_n >= nr) break;
+                iz = iz_n;
+                ir = ir_n;
+                const int pz_n = pz + stepz;
+                const double tz_new = __dmul_rn(__dsub_rn(ze[min(max(pz_n, 0), nz)], oz), inv_z);
+                pz = ax ? pz_n : pz;
+                t_z = ax ? tz_new : t_z;
+                const double r_in = re[ir], r_out = re[ir + 1];
+                const double bb = __dmul_rn(b, b);
+                const double D_in = __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, __dmul_rn(r_in, r_in))));
+                const double D_out = __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, __dmul_rn(r_out, r_out))));
+                const bool go_in = !ax && inward && ir >= 1 && D_in > 0.0;      // inward implies b < 0
+                const double sq = __dsqrt_rn(go_in ? D_in : D_out);
+                const double num = go_in ? __dsub_rn(-b, sq) : __dadd_rn(-b, sq);
+                const double tr_new = fmax(0.0, __dmul_rn(num, inv_a));
+                t_r = ax ? t_r : tr_new;
+                inward = ax ? inward : go_in;
             }
         }
         if (TRACE) {
