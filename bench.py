@@ -420,8 +420,11 @@ def main():
         threads = max(1, min(max_threads(), len(os.sched_getaffinity(0))))
         n_s = min(args.cpu_sample_rays, n_rays)
         rate, segs, dt, used = cpu_oracle_rate(prob, rays[:n_s], threads)
+        n_1 = max(1000, n_s // 10)                  # the oracle on ONE thread beside the all-cores figure
+        rate1, segs1, dt1, _ = cpu_oracle_rate(prob, rays[:n_1], 1)
         cpu = {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle",
-               "sample": f"first {n_s} rays of the batch ({segs} segments), {dt:.1f} s wall on {used} threads"}
+               "sample": f"first {n_s} rays of the batch ({segs} segments), {dt:.1f} s wall on {used} threads",
+               "single_thread": {"value": rate1, "unit": UNIT, "sample": f"first {n_1} rays ({segs1} segments), {dt1:.1f} s wall"}}
 
     if rank == 0:
         out = {
