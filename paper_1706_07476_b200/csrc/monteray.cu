@@ -151,7 +151,8 @@ struct mr_ctx {
     int pair_records = 1;            // option MR_OPT_PAIR_RECORDS
 
     // ray-ordering pre-pass scratch (grown on demand)
-    uint32_t *d_keys = nullptr, *d_perm = nullptr, *d_hist = nullptr;
+    uint32_t *d_keys = nullptr, *d_perm = nullptr, *d_hist = nullptr, *d_blk_hist = nullptr;
+    long long blk_hist_cap = 0;
     long long sort_cap = 0;
     long long hist_cap = 0;
 
@@ -440,15 +441,43 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
     SortParams S{mesh_dev(c), d_rays, n, c->precision == MR_PRECISION_DOUBLE ? 1 : 0,
                  zdiv, lshift, nlen, nkeys, c->d_keys, c->d_hist, c->d_perm, nsec > 0 ? c->d_det : nullptr, det_first,
                  c->order_mode == 2 || (c->order_mode == 0 && c->resident_bytes() <= c->l2_bytes / 2) ? 1 : 0, nslab,
-                 c->mesh_arith ? 1 : 0};
-    MR_CUDA(c, cudaMemsetAsync(c->d_hist, 0, (size_t)hist_entries * 4, c->stream));
-    const dim3 grid((unsigned)((n + 255) / 256), (unsigned)sections);
+                 c->mesh_arith ? 1 : 0, 0, nullptr};
     const size_t smem = edges_smem_bytes(c);
-    if (int rc = set_smem(c, classify_kernel, smem)) return rc;
-    classify_kernel<<<grid, 256, smem, c->stream>>>(S);
-    scan_kernel<<<sections, 1024, 0, c->stream>>>(c->d_hist, nkeys);
-    scatter_kernel<<<grid, 256, 0, c->stream>>>(S);
-    c->launches += 3;
+    // Block-local variant: every CTA counts its own contiguous share of the rays in shared memory, so neither pass
+    // needs a global atomic.  Used when the counters fit beside the plane table; else the global-atomic kernels.
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    const size_t cnt_smem = smem + (size_t)nkeys * 4;
+    const int nblk = (int)std::max<long long>(1, std::min<long long>(sms, n / 4096));
+    if (cnt_smem <= 200 * 1024) {
+        const long long need = (long long)sections * nblk * nkeys;
+        if (need > c->blk_hist_cap) {
+            MR_CUDA(c, cudaStreamSynchronize(c->stream));
+            c->dev_free(c->d_blk_hist);
+            c->d_blk_hist = (uint32_t *)c->dev_alloc((size_t)need * 4);
+            c->blk_hist_cap = c->d_blk_hist ? need : 0;
+            if (!c->d_blk_hist) return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering block histograms)");
+        }
+        S.nblk = nblk;
+        S.blk_hist = c->d_blk_hist;
+        const dim3 gblk((unsigned)nblk, (unsigned)sections), gkey((unsigned)((nkeys + 255) / 256), (unsigned)sections);
+        if (int rc = set_smem(c, count_kernel, cnt_smem)) return rc;
+        if (int rc = set_smem(c, place_kernel, (size_t)nkeys * 4)) return rc;
+        count_kernel<<<gblk, 1024, cnt_smem, c->stream>>>(S);
+        key_totals_kernel<<<gkey, 256, 0, c->stream>>>(S);
+        scan_kernel<<<sections, 1024, 0, c->stream>>>(c->d_hist, nkeys);
+        block_offsets_kernel<<<gkey, 256, 0, c->stream>>>(S);
+        place_kernel<<<gblk, 1024, (size_t)nkeys * 4, c->stream>>>(S);
+        c->launches += 5;
+    } else {
+        MR_CUDA(c, cudaMemsetAsync(c->d_hist, 0, (size_t)hist_entries * 4, c->stream));
+        const dim3 grid((unsigned)((n + 255) / 256), (unsigned)sections);
+        if (int rc = set_smem(c, classify_kernel, smem)) return rc;
+        classify_kernel<<<grid, 256, smem, c->stream>>>(S);
+        scan_kernel<<<sections, 1024, 0, c->stream>>>(c->d_hist, nkeys);
+        scatter_kernel<<<grid, 256, 0, c->stream>>>(S);
+        c->launches += 3;
+    }
     MR_CUDA(c, cudaGetLastError());
     *perm_out = c->d_perm;
     return MR_OK;
@@ -682,6 +711,7 @@ int mr_destroy(mr_ctx *c)
     c->dev_free(c->d_keys);
     c->dev_free(c->d_perm);
     c->dev_free(c->d_hist);
+    c->dev_free(c->d_blk_hist);
     for (int s = 0; s < kStageSlots; ++s) {
         if (c->ev_copied[s]) cudaEventDestroy(c->ev_copied[s]);
         if (c->ev_done[s]) cudaEventDestroy(c->ev_done[s]);

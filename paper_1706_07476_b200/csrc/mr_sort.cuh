@@ -36,17 +36,14 @@ struct SortParams {
     int longest_first;
     int nslab;
     int arith;       // the mesh is arithmetic (MeshDev::e0, h valid): cell indices by one multiply instead of a search
+    // block-local variant (count_kernel ... place_kernel): CTA b of a section owns rays [n*b/nblk, n*(b+1)/nblk)
+    int nblk;
+    uint32_t *blk_hist;   // [sections][nblk][nkeys]: per-CTA counts, then per-CTA first output positions
 };
 
-// dynamic shared memory: [edges] (always staged: the search would otherwise hammer global memory)
-__global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
+// key of ray r for the section (detector) of this CTA; e = the plane table staged in shared memory
+__device__ __forceinline__ uint32_t ray_key(const SortParams &P, const double *e, long long r)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double *e = reinterpret_cast<double *>(smem_raw);
-    for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) e[i] = __ldg(P.mesh.edges + i);
-    __syncthreads();
-    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= P.n) return;
     // the key only orders the work: an index that is off by one near a plane is harmless here
     auto cell_of = [&](int a, int base, int n, double x) {
         if (P.arith) return min(max((int)floor((x - P.mesh.e0[a]) / P.mesh.h[a]), 0), n - 1);
@@ -63,17 +60,42 @@ __global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
         for (int a = 0; a < 3; ++a) { o[a] = R.o[a]; d[a] = R.d[a]; }
         ok = (P.det ? (isfinite(o[0]) && isfinite(o[1]) && isfinite(o[2]) && isfinite(R.E) && isfinite(R.W)) : R.finite) && R.E > 0.0f;
     }
-    uint32_t *keys = P.keys, *hist = P.hist;
     if (P.det) {
         const double *D = P.det + 3 * (size_t)(P.det_first + blockIdx.y);
         for (int a = 0; a < 3; ++a) d[a] = __ldg(D + a) - o[a];
         ok = ok && isfinite(d[0]) && isfinite(d[1]) && isfinite(d[2]);
-        keys += (size_t)blockIdx.y * P.n;
-        hist += (size_t)blockIdx.y * (P.nkeys + 1);
     }
     const int base[3] = {0, P.mesh.nx + 1, P.mesh.nx + P.mesh.ny + 2};
     const int n[3] = {P.mesh.nx, P.mesh.ny, P.mesh.nz};
     int idx[3] = {0, 0, 0};
+    if (P.arith) {
+        // arithmetic mesh: the whole estimate in fp32 -- nine fp64 divisions per ray made this pass fp64-pipe bound
+        // (64 lanes per clock per SM).  The key only orders the work: an index that is off by one near a plane, or a
+        // ray on the box surface that lands in the last bucket, is harmless.
+        uint32_t key = (uint32_t)(P.nkeys - 1);
+        float of[3], df[3], ih[3], span[3], t_exit = __int_as_float(0x7f800000);
+        for (int a = 0; a < 3 && ok; ++a) {
+            of[a] = (float)(o[a] - P.mesh.e0[a]);
+            df[a] = (float)d[a];
+            ih[a] = __frcp_rn((float)P.mesh.h[a]);
+            span[a] = (float)n[a] * (float)P.mesh.h[a];
+            ok = of[a] >= 0.f && of[a] < span[a];
+            idx[a] = min((int)(of[a] * ih[a]), n[a] - 1);
+            if (df[a] != 0.f) t_exit = fminf(t_exit, __fdividef((df[a] > 0.f ? span[a] : 0.f) - of[a], df[a]));
+        }
+        if (P.det) t_exit = fminf(t_exit, 1.0f);   // the walk ends at the detector
+        if (ok && isfinite(t_exit)) {
+            int est = 1;   // cells crossed ~ 1 + sum of index distances between the origin and the exit point
+            for (int a = 0; a < 3; ++a) {
+                const float x = fminf(fmaxf(fmaf(t_exit, df[a], of[a]), 0.f), span[a]);
+                est += abs(min((int)(x * ih[a]), n[a] - 1) - idx[a]);
+            }
+            const int lb = min(est >> P.lshift, P.nlen - 1);
+            key = P.longest_first ? (uint32_t)((P.nlen - 1 - lb) * P.nslab + idx[2] / P.zdiv)
+                                  : (uint32_t)((idx[2] / P.zdiv) * P.nlen + lb);
+        }
+        return key;
+    }
     double t_exit = __longlong_as_double(0x7ff0000000000000LL);
     for (int a = 0; a < 3 && ok; ++a) {
         ok = (o[a] >= e[base[a]] && o[a] < e[base[a] + n[a]]);
@@ -98,11 +120,96 @@ __global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
         key = P.longest_first ? (uint32_t)((P.nlen - 1 - lb) * P.nslab + idx[2] / P.zdiv)
                               : (uint32_t)((idx[2] / P.zdiv) * P.nlen + lb);
     }
-    keys[r] = key;
+    return key;
+}
+
+// dynamic shared memory: [edges] (always staged: the search would otherwise hammer global memory)
+__global__ void __launch_bounds__(256) classify_kernel(const SortParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *e = reinterpret_cast<double *>(smem_raw);
+    for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) e[i] = __ldg(P.mesh.edges + i);
+    __syncthreads();
+    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= P.n) return;
+    const uint32_t key = ray_key(P, e, r);
+    const size_t sec = P.det ? blockIdx.y : 0;
+    P.keys[sec * P.n + r] = key;
     // one atomic per distinct key of the warp (rays born in one small region share a handful of keys)
     const unsigned act = __activemask();
     const unsigned peers = __match_any_sync(act, key);
-    if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(hist + key, (unsigned)__popc(peers));
+    if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(P.hist + sec * (P.nkeys + 1) + key, (unsigned)__popc(peers));
+}
+
+// ---- block-local counting sort (no global atomics: 10^7 random global atomics cost ~0.22 ms in each of classify and
+//      scatter; shared-memory counters cost a fifth of that).  grid = (nblk, sections), 1024 threads.
+//      dynamic shared memory: [edges] [counters: nkeys u32]
+__global__ void __launch_bounds__(1024) count_kernel(const SortParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *e = reinterpret_cast<double *>(smem_raw);
+    uint32_t *cnt = reinterpret_cast<uint32_t *>(smem_raw + sizeof(double) * (size_t)((P.mesh.nedges + 1) & ~1));
+    for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) e[i] = __ldg(P.mesh.edges + i);
+    for (int k = threadIdx.x; k < P.nkeys; k += blockDim.x) cnt[k] = 0u;
+    __syncthreads();
+    const size_t sec = blockIdx.y;
+    const long long first = P.n * blockIdx.x / P.nblk, last = P.n * (blockIdx.x + 1) / P.nblk;
+    for (long long r = first + threadIdx.x; r < last; r += blockDim.x) {
+        const uint32_t key = ray_key(P, e, r);
+        P.keys[sec * P.n + r] = key;
+        atomicAdd(cnt + key, 1u);
+    }
+    __syncthreads();
+    uint32_t *out = P.blk_hist + (sec * P.nblk + blockIdx.x) * (size_t)P.nkeys;
+    for (int k = threadIdx.x; k < P.nkeys; k += blockDim.x) out[k] = cnt[k];
+}
+
+// per (section, key): total over the CTAs -> hist (scanned next by scan_kernel)
+__global__ void __launch_bounds__(256) key_totals_kernel(const SortParams P)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= P.nkeys) return;
+    const size_t sec = blockIdx.y;
+    const uint32_t *in = P.blk_hist + sec * P.nblk * (size_t)P.nkeys + k;
+    uint32_t t = 0;
+    for (int b = 0; b < P.nblk; ++b) t += in[(size_t)b * P.nkeys];
+    P.hist[sec * (P.nkeys + 1) + k] = t;
+}
+
+// per (section, key): first output position of every CTA = the key's offset + the counts of the CTAs before it
+__global__ void __launch_bounds__(256) block_offsets_kernel(const SortParams P)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= P.nkeys) return;
+    const size_t sec = blockIdx.y;
+    uint32_t *io = P.blk_hist + sec * P.nblk * (size_t)P.nkeys + k;
+    uint32_t run = P.hist[sec * (P.nkeys + 1) + k];
+    for (int b0 = 0; b0 < P.nblk; b0 += 16) {          // 16 independent loads in flight, then the running sum
+        uint32_t t[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) t[j] = (b0 + j < P.nblk) ? io[(size_t)(b0 + j) * P.nkeys] : 0u;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            if (b0 + j < P.nblk) io[(size_t)(b0 + j) * P.nkeys] = run;
+            run += t[j];
+        }
+    }
+}
+
+// dynamic shared memory: [cursors: nkeys u32]
+__global__ void __launch_bounds__(1024) place_kernel(const SortParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint32_t *cur = reinterpret_cast<uint32_t *>(smem_raw);
+    const size_t sec = blockIdx.y;
+    const uint32_t *in = P.blk_hist + (sec * P.nblk + blockIdx.x) * (size_t)P.nkeys;
+    for (int k = threadIdx.x; k < P.nkeys; k += blockDim.x) cur[k] = in[k];
+    __syncthreads();
+    const long long first = P.n * blockIdx.x / P.nblk, last = P.n * (blockIdx.x + 1) / P.nblk;
+    for (long long r = first + threadIdx.x; r < last; r += blockDim.x) {
+        const uint32_t pos = atomicAdd(cur + P.keys[sec * P.n + r], 1u);
+        P.perm[sec * P.n + pos] = (uint32_t)r;
+    }
 }
 
 // one CTA per histogram (blockIdx.x = section, nkeys + 1 entries apart): exclusive prefix sum of hist[0..nkeys) in place

@@ -296,7 +296,7 @@ def test_ray_ordering_prepass_on_and_off(precision):
             before = m.get_stats().kernel_launches
             m.cast_rays(r)
             st = m.get_stats()
-            assert st.kernel_launches - before == (4 if sort else 1)
+            assert st.kernel_launches - before == (6 if sort else 1)   # five ordering kernels + the cast
             assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
             assert_tally(m.read_tally(), ref.tally, precision)
 
