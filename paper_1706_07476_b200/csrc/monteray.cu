@@ -488,9 +488,13 @@ int launch_rz_t(mr_ctx *c, const RzParams &Q, int block)
 {
     const size_t smem = edges_smem_bytes(c) + (TRACE ? 0 : (size_t)(c->M + c->N) * block * sizeof(Real));
     if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "rz mesh: planes and materials exceed shared memory");
-    const long long grid = (Q.c.n + block - 1) / block;
-    if (grid > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
     if (int rc = set_smem(c, rz_kernel<Real, Rec, TRACE>, smem)) return rc;
+    // persistent kernel: as many CTAs as can be resident; lanes pull rays from counters[3]
+    int sms = 148, per_sm = 1;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    MR_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rz_kernel<Real, Rec, TRACE>, block, smem));
+    const long long grid = std::max<long long>(1, std::min<long long>((Q.c.n + block - 1) / block, (long long)sms * std::max(per_sm, 1)));
+    MR_CUDA(c, cudaMemsetAsync(c->d_counters + 3, 0, sizeof(unsigned long long), c->stream));
     rz_kernel<Real, Rec, TRACE><<<(unsigned)grid, block, smem, c->stream>>>(Q);
     c->launches += 1;
     MR_CUDA(c, cudaGetLastError());
@@ -1249,6 +1253,7 @@ int mr_trace_rays(mr_ctx *c, int64_t n, const void *rays, int where, uint32_t *n
         Q.c.mesh = mesh_dev(c);
         Q.c.rays = d_rays;
         Q.c.n = n;
+        Q.c.counters = c->d_counters;     // only the work counter [3] is used by a trace launch
         Q.nseg = d_nseg; Q.hash = d_hash; Q.cells = d_cells; Q.lens = d_lens; Q.cap = cap;
         Q.ray_is_double = c->precision == MR_PRECISION_DOUBLE ? 1 : 0;
         Q.spherical = c->mesh_sphere ? 1 : 0;

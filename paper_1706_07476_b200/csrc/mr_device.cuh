@@ -742,6 +742,13 @@ __device__ __forceinline__ double rz_t_radial(double b, double a, double inv_a, 
     return fmax(0.0, __dmul_rn(num, inv_a));
 }
 
+// Ray lengths on these meshes vary by about 2x around their mean (17.8 of 32 lanes were active with one ray per
+// thread, and ordering the rays by length makes neighbouring lanes hammer the same ring-shaped cells), so the kernel
+// is PERSISTENT: a lane that finishes its ray takes the next one from a global counter (P.counters[3], zeroed before
+// the launch); refills are batched (at least kRefillLanes idle lanes, or nothing left to do) to keep the divergent
+// per-ray set-up rare.
+constexpr int kRefillLanes = 8;
+
 template <typename Real, typename Rec, bool TRACE>
 __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParams Q)
 {
@@ -754,136 +761,181 @@ __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParam
     for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
     __syncthreads();
     const double *re = s_edges, *ze = s_edges + nr + 3;        // Cartesian layout with ny = 1: x | y (2 planes) | z
+    const bool sph = Q.spherical != 0;
+    const unsigned full = 0xffffffffu;
+    const unsigned lane = threadIdx.x & 31;
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
 
-    const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = r < P.n;
-    bool accepted = false;
+    // per-lane ray state
+    long long r = -1;
+    bool active = false, inward = false;
+    double oz = 0.0, rho2 = 0.0, a = 0.0, b = 0.0, inv_a = 0.0, inv_z = 0.0, t_r = inf, t_z = inf, t_cur = 0.0, wa = 0.0;
+    int ir = 0, iz = 0, pz = 0, stepz = 0;
     unsigned nseg = 0;
     unsigned long long h = 0;
-    if (live) {
-        double ox, oy, oz, dx, dy, dz, W;
-        Real E;
-        bool fin;
-        if (sizeof(Real) == 8 || (TRACE && Q.ray_is_double)) {
-            const Ray<double> R = load_ray_f64(P.rays, r);
-            ox = R.o[0]; oy = R.o[1]; oz = R.o[2]; dx = R.d[0]; dy = R.d[1]; dz = R.d[2]; W = R.W; E = (Real)R.E; fin = R.finite && R.E > 0.0;
-        } else {
-            const Ray<float> R = load_ray_f32(P.rays, r);
-            ox = R.o[0]; oy = R.o[1]; oz = R.o[2]; dx = R.d[0]; dy = R.d[1]; dz = R.d[2]; W = R.W; E = (Real)R.E; fin = R.finite && R.E > 0.0f;
-        }
-        // Z1
-        const bool sph = Q.spherical != 0;
-        double rho2 = __dadd_rn(__dmul_rn(ox, ox), __dmul_rn(oy, oy));
-        double a = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
-        if (sph) {
-            rho2 = __dadd_rn(rho2, __dmul_rn(oz, oz));
-            a = __dadd_rn(a, __dmul_rn(dz, dz));
-        }
-        const double inv_a = (a != 0.0) ? __drcp_rn(a) : 0.0;
-        const bool radial = (a != 0.0) && isfinite(inv_a) && isfinite(a);
-        const double inv_z = (dz != 0.0) ? __drcp_rn(dz) : 0.0;
-        const bool axial = !sph && (dz != 0.0) && isfinite(inv_z);
-        accepted = fin && (radial || axial) && (rho2 < __dmul_rn(re[nr], re[nr])) && (sph || (oz >= ze[0] && oz < ze[nz]));
-        if (accepted) {
-            if (!TRACE) sigma_all<Real>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, E, sig, stride);   // Z2
-            // Z3: ir = #{p : r_p^2 <= rho0^2} - 1 (r_p^2 is non-decreasing in p), iz by comparisons
-            int lo = 0, hi = nr + 1;
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (__dmul_rn(re[mid], re[mid]) <= rho2) lo = mid + 1; else hi = mid;
-            }
-            int ir = lo - 1;
-            int iz = sph ? 0 : upper_bound_edges(ze, nz + 1, oz) - 1;
-            // Z4
-            double b = __dadd_rn(__dmul_rn(ox, dx), __dmul_rn(oy, dy));
-            if (sph) b = __dadd_rn(b, __dmul_rn(oz, dz));
-            const double inf = __longlong_as_double(0x7ff0000000000000LL);
-            bool inward = false;
-            double t_r = inf, t_z = inf, t_cur = 0.0;
-            int pz = 0, stepz = 0;
-            auto next_radial = [&](bool may_go_in) {
-                inward = false;
-                if (may_go_in && b < 0.0 && ir >= 1) {
-                    const double cc = __dsub_rn(rho2, __dmul_rn(re[ir], re[ir]));
-                    const double D = __dsub_rn(__dmul_rn(b, b), __dmul_rn(a, cc));
-                    if (D > 0.0) { inward = true; t_r = fmax(0.0, __dmul_rn(__dsub_rn(-b, __dsqrt_rn(D)), inv_a)); }
-                }
-                if (!inward) t_r = rz_t_radial(b, a, inv_a, rho2, re[ir + 1], true);
-            };
-            if (radial) next_radial(true);
-            if (axial) {
-                stepz = dz > 0.0 ? 1 : -1;
-                pz = dz > 0.0 ? iz + 1 : iz;
-                t_z = __dmul_rn(__dsub_rn(ze[pz], oz), inv_z);
-            }
-            if (TRACE) h = 0xcbf29ce484222325ULL;
-            double wa = W;
-            Rec rec;
-            if (!TRACE) rec.reset();
-            // Z5
-            for (;;) {
-                const bool ax = t_z < t_r;                      // ties: radial first
-                const double tn = ax ? t_z : t_r;
-                const double len = __dsub_rn(tn, t_cur);
-                const int cell = ir + nr * iz;
-                if (TRACE) {
-                    if ((long long)nseg < Q.cap) {
-                        if (Q.cells) Q.cells[r * Q.cap + nseg] = cell;
-                        if (Q.lens) Q.lens[r * Q.cap + nseg] = len;
+    Rec rec;
+    // per-lane totals for the counters
+    unsigned n_acc = 0, n_rej = 0;
+    unsigned long long n_seg = 0;
+    bool exhausted = false;                                     // warp-uniform: the ray counter has run past P.n
+
+    for (;;) {
+        const unsigned idle = __ballot_sync(full, !active);
+        if (!exhausted && idle && (__popc(idle) >= kRefillLanes || idle == full)) {
+            unsigned long long base = 0;
+            if (lane == 0) base = atomicAdd(P.counters + 3, (unsigned long long)__popc(idle));
+            base = __shfl_sync(full, base, 0);
+            exhausted = (long long)(base + __popc(idle)) >= P.n;
+            if (!active) {
+                r = (long long)base + __popc(idle & ((1u << lane) - 1u));
+                if (r < P.n) {
+                    double ox, oy, dx, dy, dz, W;
+                    Real E;
+                    bool fin;
+                    if (sizeof(Real) == 8 || (TRACE && Q.ray_is_double)) {
+                        const Ray<double> R = load_ray_f64(P.rays, r);
+                        ox = R.o[0]; oy = R.o[1]; oz = R.o[2]; dx = R.d[0]; dy = R.d[1]; dz = R.d[2]; W = R.W; E = (Real)R.E; fin = R.finite && R.E > 0.0;
+                    } else {
+                        const Ray<float> R = load_ray_f32(P.rays, r);
+                        ox = R.o[0]; oy = R.o[1]; oz = R.o[2]; dx = R.d[0]; dy = R.d[1]; dz = R.d[2]; W = R.W; E = (Real)R.E; fin = R.finite && R.E > 0.0f;
                     }
-                    const unsigned cu = (unsigned)cell;
+                    // Z1
+                    rho2 = __dadd_rn(__dmul_rn(ox, ox), __dmul_rn(oy, oy));
+                    a = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+                    if (sph) {
+                        rho2 = __dadd_rn(rho2, __dmul_rn(oz, oz));
+                        a = __dadd_rn(a, __dmul_rn(dz, dz));
+                    }
+                    inv_a = (a != 0.0) ? __drcp_rn(a) : 0.0;
+                    const bool radial = (a != 0.0) && isfinite(inv_a) && isfinite(a);
+                    inv_z = (dz != 0.0) ? __drcp_rn(dz) : 0.0;
+                    const bool axial = !sph && (dz != 0.0) && isfinite(inv_z);
+                    const bool accepted = fin && (radial || axial) && (rho2 < __dmul_rn(re[nr], re[nr])) &&
+                                          (sph || (oz >= ze[0] && oz < ze[nz]));
+                    nseg = 0;
+                    h = 0;
+                    if (accepted) {
+                        if (!TRACE) sigma_all<Real>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, E, sig, stride);   // Z2
+                        // Z3: ir = #{p : r_p^2 <= rho0^2} - 1 (r_p^2 is non-decreasing in p), iz by comparisons
+                        int lo = 0, hi = nr + 1;
+                        while (lo < hi) {
+                            const int mid = (lo + hi) >> 1;
+                            if (__dmul_rn(re[mid], re[mid]) <= rho2) lo = mid + 1; else hi = mid;
+                        }
+                        ir = lo - 1;
+                        iz = sph ? 0 : upper_bound_edges(ze, nz + 1, oz) - 1;
+                        // Z4
+                        b = __dadd_rn(__dmul_rn(ox, dx), __dmul_rn(oy, dy));
+                        if (sph) b = __dadd_rn(b, __dmul_rn(oz, dz));
+                        inward = false;
+                        t_r = inf; t_z = inf; t_cur = 0.0; pz = 0; stepz = 0;
+                        if (radial) {
+                            if (b < 0.0 && ir >= 1) {
+                                const double cc = __dsub_rn(rho2, __dmul_rn(re[ir], re[ir]));
+                                const double D = __dsub_rn(__dmul_rn(b, b), __dmul_rn(a, cc));
+                                if (D > 0.0) { inward = true; t_r = fmax(0.0, __dmul_rn(__dsub_rn(-b, __dsqrt_rn(D)), inv_a)); }
+                            }
+                            if (!inward) t_r = rz_t_radial(b, a, inv_a, rho2, re[ir + 1], true);
+                        }
+                        if (axial) {
+                            stepz = dz > 0.0 ? 1 : -1;
+                            pz = dz > 0.0 ? iz + 1 : iz;
+                            t_z = __dmul_rn(__dsub_rn(ze[pz], oz), inv_z);
+                        }
+                        if (TRACE) h = 0xcbf29ce484222325ULL;
+                        wa = W;
+                        if (!TRACE) rec.reset();
+                        active = true;
+                        ++n_acc;
+                    } else {
+                        ++n_rej;
+                        if (TRACE) {
+                            if (Q.nseg) Q.nseg[r] = 0;
+                            if (Q.hash) Q.hash[r] = 0;
+                        }
+                    }
+                }
+            }
+        }
+        if (__ballot_sync(full, active) == 0) {
+            if (exhausted) break;
+            continue;
+        }
+        if (active) {
+            // Z5: one segment
+            const bool ax = t_z < t_r;                      // ties: radial first
+            const double tn = ax ? t_z : t_r;
+            const double len = __dsub_rn(tn, t_cur);
+            const int cell = ir + nr * iz;
+            if (TRACE) {
+                if ((long long)nseg < Q.cap) {
+                    if (Q.cells) Q.cells[r * Q.cap + nseg] = cell;
+                    if (Q.lens) Q.lens[r * Q.cap + nseg] = len;
+                }
+                const unsigned cu = (unsigned)cell;
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        h ^= (unsigned long long)((cu >> (8 * q)) & 0xffu);
-                        h *= 0x100000001b3ULL;
-                    }
-                } else {
-                    rec.load(P.recs, P.ids, P.K, cell);
-                    const double S = (double)Rec::sigma(rec.value(), sig, stride, P.K);
-                    double g, ex;
-                    score_terms<sizeof(Real) == 8>(S, len, g, ex);
-                    if (len > 0.0) red_add_f64(P.tally + cell, wa * g);
-                    wa *= ex;
+                for (int q = 0; q < 4; ++q) {
+                    h ^= (unsigned long long)((cu >> (8 * q)) & 0xffu);
+                    h *= 0x100000001b3ULL;
                 }
-                ++nseg;
-                t_cur = tn;
-                // One instruction stream for the three kinds of step (axial, inward, outward): the next crossing of
-                // BOTH families is evaluated and the one that applies is selected, never branched on, so the lanes
-                // of a warp do not serialise (15 of 32 lanes were active with a three-way branch here).  The values
-                // that are kept come from exactly the operations of Z4.
-                const int iz_n = ax ? iz + stepz : iz;
-                const int ir_n = ax ? ir : (inward ? ir - 1 : ir + 1);
-                if (iz_n < 0 || iz_n >= nz || ir_n >= nr) break;
+            } else {
+                rec.load(P.recs, P.ids, P.K, cell);
+                const double S = (double)Rec::sigma(rec.value(), sig, stride, P.K);
+                double g, ex;
+                score_terms<sizeof(Real) == 8>(S, len, g, ex);
+                if (len > 0.0) red_add_f64(P.tally + cell, wa * g);
+                wa *= ex;
+            }
+            ++nseg;
+            t_cur = tn;
+            // One instruction stream for the three kinds of step (axial, inward, outward): the next crossing of BOTH
+            // families is evaluated and the one that applies is selected, never branched on.  The values that are kept
+            // come from exactly the operations of Z4.
+            const int iz_n = ax ? iz + stepz : iz;
+            const int ir_n = ax ? ir : (inward ? ir - 1 : ir + 1);
+            if (iz_n < 0 || iz_n >= nz || ir_n >= nr) {
+                active = false;                             // the ray has left the mesh
+                n_seg += nseg;
+                if (TRACE) {
+                    if (Q.nseg) Q.nseg[r] = nseg;
+                    if (Q.hash) Q.hash[r] = h;
+                }
+            } else {
                 iz = iz_n;
                 ir = ir_n;
-                const int pz_n = pz + stepz;
-                const double tz_new = __dmul_rn(__dsub_rn(ze[min(max(pz_n, 0), nz)], oz), inv_z);
-                pz = ax ? pz_n : pz;
-                t_z = ax ? tz_new : t_z;
-                const double r_in = re[ir], r_out = re[ir + 1];
+                if (ax) {                                   // predicated: lanes on a radial step read nothing here
+                    pz += stepz;
+                    t_z = __dmul_rn(__dsub_rn(ze[pz], oz), inv_z);
+                }
+                // one radius per step (the kernel is bound by shared-memory wavefronts: lanes read different shells):
+                // the inner cylinder while the ray may still go inward, else the outer one; only at the turning point
+                // (inner cylinder missed, once per ray) is the outer radius read as well
+                const bool may_in = !ax && inward && ir >= 1;               // inward implies b < 0
+                const double rp = re[may_in ? ir : ir + 1];
                 const double bb = __dmul_rn(b, b);
-                const double D_in = __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, __dmul_rn(r_in, r_in))));
-                const double D_out = __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, __dmul_rn(r_out, r_out))));
-                const bool go_in = !ax && inward && ir >= 1 && D_in > 0.0;      // inward implies b < 0
-                const double sq = __dsqrt_rn(go_in ? D_in : D_out);
+                double D = __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, __dmul_rn(rp, rp))));
+                bool go_in = may_in && D > 0.0;
+                if (may_in && !go_in) {
+                    const double ro = re[ir + 1];
+                    D = __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, __dmul_rn(ro, ro))));
+                }
+                const double sq = __dsqrt_rn(D);
                 const double num = go_in ? __dsub_rn(-b, sq) : __dadd_rn(-b, sq);
                 const double tr_new = fmax(0.0, __dmul_rn(num, inv_a));
                 t_r = ax ? t_r : tr_new;
                 inward = ax ? inward : go_in;
             }
         }
-        if (TRACE) {
-            if (Q.nseg) Q.nseg[r] = nseg;
-            if (Q.hash) Q.hash[r] = h;
-        }
     }
     if (!TRACE) {
-        const unsigned full = 0xffffffffu;
-        const unsigned acc = __popc(__ballot_sync(full, accepted));
-        const unsigned rej = __popc(__ballot_sync(full, live && !accepted));
-        unsigned long long segs = nseg;
-        for (int o = 16; o > 0; o >>= 1) segs += __shfl_xor_sync(full, segs, o);
-        if ((threadIdx.x & 31) == 0) {
+        unsigned acc = n_acc, rej = n_rej;
+        unsigned long long segs = n_seg;
+        for (int o = 16; o > 0; o >>= 1) {
+            acc += __shfl_xor_sync(full, acc, o);
+            rej += __shfl_xor_sync(full, rej, o);
+            segs += __shfl_xor_sync(full, segs, o);
+        }
+        if (lane == 0) {
             if (acc) atomicAdd(P.counters + 0, (unsigned long long)acc);
             if (rej) atomicAdd(P.counters + 1, (unsigned long long)rej);
             if (segs) atomicAdd(P.counters + 2, segs);
