@@ -36,6 +36,38 @@ def main():
         for c in range(0, 1000, 111):
             f.write(f"cell {c} tally {float(res.tally[c]).hex()}\n")
     print("wrote", out)
+    write_extensions()
+
+
+def write_extensions():
+    """tests/golden/extensions_oracle.txt: regression lock on the oracle's next-event, nuclide-mixture, R-Z and
+    spherical paths; same rule: written from the oracle alone."""
+    from tests.tiny import tiny_rz_problem, tiny_rz_rays, tiny_sphere_problem, tiny_sphere_rays
+    from workloads import add_nuclides
+
+    out = os.path.join(os.path.dirname(os.path.abspath(__file__)), "extensions_oracle.txt")
+    with open(out, "w") as f:
+        f.write("# oracle/vrc_oracle.c, IEEE double; written by tests/golden/make_golden.py; C99 hex floats\n")
+        prob = make_problem(1)
+        rays = make_rays(prob, 2000)
+        ne = Oracle(prob).next_event(rays, [5.0, 5.0, 5.0])
+        f.write(f"next_event config1 2000 det 5,5,5 segments {ne.segments} hash_xor {int(np.bitwise_xor.reduce(ne.hash)):#018x} "
+                f"det_sum {ne.det_sum.hex()} tau17 {float(ne.tau[17]).hex()}\n")
+        mix = add_nuclides(prob, n_nuclides=5)
+        rm = Oracle(mix).cast(rays, per_ray=True)
+        f.write(f"nuclides config1 2000 segments {rm.segments} tally_sum {float(rm.tally.sum()).hex()} "
+                f"sum_score17 {float(rm.sum_score[17]).hex()}\n")
+        rz = tiny_rz_problem(7, nr=6, nz=5, K=2, M=3)
+        rr = tiny_rz_rays(rz, 7, 500)
+        zr = Oracle(rz).cast_rz(rr, rz.re, rz.ze)
+        f.write(f"rz tiny7 500 segments {zr.segments} hash_xor {int(np.bitwise_xor.reduce(zr.hash)):#018x} "
+                f"tally_sum {float(zr.tally.sum()).hex()} t_exit3 {float(zr.t_exit[3]).hex()}\n")
+        sp = tiny_sphere_problem(14, nr=6, K=2, M=3)
+        sr = tiny_sphere_rays(sp, 14, 500)
+        ss = Oracle(sp).cast_sphere(sr, sp.re)
+        f.write(f"sphere tiny14 500 segments {ss.segments} hash_xor {int(np.bitwise_xor.reduce(ss.hash)):#018x} "
+                f"tally_sum {float(ss.tally.sum()).hex()} t_exit3 {float(ss.t_exit[3]).hex()}\n")
+    print("wrote", out)
 
 
 if __name__ == "__main__":
