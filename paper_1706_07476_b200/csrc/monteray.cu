@@ -137,7 +137,7 @@ struct mr_ctx {
     cudaEvent_t ev_copied[kStageSlots] = {nullptr, nullptr};
     cudaEvent_t ev_done[kStageSlots] = {nullptr, nullptr};
     size_t stage_cap_rays = 0;       // rays each slot can hold now
-    long long stage_rays = 1 << 21;  // option MR_OPT_STAGE_RAYS
+    long long stage_rays = 1 << 20;  // option MR_OPT_STAGE_RAYS (chunks grow from a quarter of it to twice it)
     int next_slot = 0;
     int copy_threads = 4;            // option MR_OPT_COPY_THREADS
 
@@ -151,10 +151,16 @@ struct mr_ctx {
     int pair_records = 1;            // option MR_OPT_PAIR_RECORDS
 
     // ray-ordering pre-pass scratch (grown on demand)
-    uint32_t *d_keys = nullptr, *d_perm = nullptr, *d_hist = nullptr, *d_blk_hist = nullptr;
-    long long blk_hist_cap = 0;
-    long long sort_cap = 0;
-    long long hist_cap = 0;
+    // Two compute lanes: lane 0 queues on `stream`, lane 1 on the internal `stream2`.  Only the chunks of a HOST batch
+    // alternate between them (run_batch), so that the ramp-down of one chunk's cast kernel overlaps the start of the
+    // next chunk's; every other call works on lane 0.  Each lane has its own ordering scratch.
+    int lane = 0;
+    cudaStream_t stream2 = nullptr;
+    cudaEvent_t ev_lane = nullptr;
+    cudaStream_t work_stream() const { return lane ? stream2 : stream; }
+    uint32_t *d_keys_l[2] = {nullptr, nullptr}, *d_perm_l[2] = {nullptr, nullptr}, *d_hist_l[2] = {nullptr, nullptr},
+             *d_blk_hist_l[2] = {nullptr, nullptr};
+    long long sort_cap_l[2] = {0, 0}, hist_cap_l[2] = {0, 0}, blk_hist_cap_l[2] = {0, 0};
 
     int order_mode = 0;              // option MR_OPT_ORDER_MODE: 0 auto, 1 slab-major, 2 longest first
     int fused_opt = 2;               // option MR_OPT_FUSED_TALLY: 0 off, 1 on, 2 auto (decided by mr_load_materials)
@@ -307,7 +313,7 @@ int launch_cast_m(mr_ctx *c, const CastParams &P, int block, size_t smem)
     const long long grid = (P.n + block - 1) / block;
     if (grid > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
     if (int rc = set_smem(c, cast_kernel<Real, Rec, MODE>, smem)) return rc;
-    cast_kernel<Real, Rec, MODE><<<(unsigned)grid, block, smem, c->stream>>>(P);
+    cast_kernel<Real, Rec, MODE><<<(unsigned)grid, block, smem, c->work_stream()>>>(P);
     c->launches += 1;
     MR_CUDA(c, cudaGetLastError());
     return MR_OK;
@@ -406,6 +412,10 @@ constexpr long long kSortMinRays = 1 << 14;   // below this a batch is a handful
 int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm_out, int nsec = 0, int det_first = 0)
 {
     *perm_out = nullptr;
+    const int L = c->lane;
+    cudaStream_t ws = c->work_stream();
+    uint32_t *&d_keys = c->d_keys_l[L], *&d_perm = c->d_perm_l[L], *&d_hist = c->d_hist_l[L], *&d_blk_hist = c->d_blk_hist_l[L];
+    long long &sort_cap = c->sort_cap_l[L], &hist_cap = c->hist_cap_l[L], &blk_hist_cap = c->blk_hist_cap_l[L];
     if (!c->sort_rays || c->mesh_rz || n < kSortMinRays || n > 0xffffffffLL || edges_smem_bytes(c) > kEdgesSmemMax) return MR_OK;
     const int sections = std::max(nsec, 1);
     const int nlen = 128;
@@ -416,30 +426,30 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
     while ((maxlen >> lshift) >= nlen) ++lshift;
     const int nkeys = nslab * nlen + 1;
     const long long entries = n * sections;
-    if (entries > c->sort_cap) {
-        MR_CUDA(c, cudaStreamSynchronize(c->stream));
-        c->dev_free(c->d_keys);
-        c->dev_free(c->d_perm);
-        c->d_keys = (uint32_t *)c->dev_alloc((size_t)entries * 4);
-        c->d_perm = (uint32_t *)c->dev_alloc((size_t)entries * 4);
-        c->sort_cap = (c->d_keys && c->d_perm) ? entries : 0;
-        if (!c->sort_cap) {
-            c->dev_free(c->d_keys);
-            c->dev_free(c->d_perm);
-            c->d_keys = c->d_perm = nullptr;
+    if (entries > sort_cap) {
+        MR_CUDA(c, cudaStreamSynchronize(ws));
+        c->dev_free(d_keys);
+        c->dev_free(d_perm);
+        d_keys = (uint32_t *)c->dev_alloc((size_t)entries * 4);
+        d_perm = (uint32_t *)c->dev_alloc((size_t)entries * 4);
+        sort_cap = (d_keys && d_perm) ? entries : 0;
+        if (!sort_cap) {
+            c->dev_free(d_keys);
+            c->dev_free(d_perm);
+            d_keys = d_perm = nullptr;
             return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering scratch)");
         }
     }
     const long long hist_entries = (long long)(nkeys + 1) * sections;
-    if (hist_entries > c->hist_cap) {
-        MR_CUDA(c, cudaStreamSynchronize(c->stream));
-        c->dev_free(c->d_hist);
-        c->d_hist = (uint32_t *)c->dev_alloc((size_t)hist_entries * 4);
-        c->hist_cap = c->d_hist ? hist_entries : 0;
-        if (!c->d_hist) return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering histogram)");
+    if (hist_entries > hist_cap) {
+        MR_CUDA(c, cudaStreamSynchronize(ws));
+        c->dev_free(d_hist);
+        d_hist = (uint32_t *)c->dev_alloc((size_t)hist_entries * 4);
+        hist_cap = d_hist ? hist_entries : 0;
+        if (!d_hist) return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering histogram)");
     }
     SortParams S{mesh_dev(c), d_rays, n, c->precision == MR_PRECISION_DOUBLE ? 1 : 0,
-                 zdiv, lshift, nlen, nkeys, c->d_keys, c->d_hist, c->d_perm, nsec > 0 ? c->d_det : nullptr, det_first,
+                 zdiv, lshift, nlen, nkeys, d_keys, d_hist, d_perm, nsec > 0 ? c->d_det : nullptr, det_first,
                  c->order_mode == 2 || (c->order_mode == 0 && c->resident_bytes() <= c->l2_bytes / 2) ? 1 : 0, nslab,
                  c->mesh_arith ? 1 : 0, 0, nullptr};
     const size_t smem = edges_smem_bytes(c);
@@ -451,35 +461,35 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
     const int nblk = (int)std::max<long long>(1, std::min<long long>(sms, n / 4096));
     if (cnt_smem <= 200 * 1024) {
         const long long need = (long long)sections * nblk * nkeys;
-        if (need > c->blk_hist_cap) {
-            MR_CUDA(c, cudaStreamSynchronize(c->stream));
-            c->dev_free(c->d_blk_hist);
-            c->d_blk_hist = (uint32_t *)c->dev_alloc((size_t)need * 4);
-            c->blk_hist_cap = c->d_blk_hist ? need : 0;
-            if (!c->d_blk_hist) return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering block histograms)");
+        if (need > blk_hist_cap) {
+            MR_CUDA(c, cudaStreamSynchronize(ws));
+            c->dev_free(d_blk_hist);
+            d_blk_hist = (uint32_t *)c->dev_alloc((size_t)need * 4);
+            blk_hist_cap = d_blk_hist ? need : 0;
+            if (!d_blk_hist) return c->fail(MR_ERR_OOM, "device allocation failed (ray ordering block histograms)");
         }
         S.nblk = nblk;
-        S.blk_hist = c->d_blk_hist;
+        S.blk_hist = d_blk_hist;
         const dim3 gblk((unsigned)nblk, (unsigned)sections), gkey((unsigned)((nkeys + 255) / 256), (unsigned)sections);
         if (int rc = set_smem(c, count_kernel, cnt_smem)) return rc;
         if (int rc = set_smem(c, place_kernel, (size_t)nkeys * 4)) return rc;
-        count_kernel<<<gblk, 1024, cnt_smem, c->stream>>>(S);
-        key_totals_kernel<<<gkey, 256, 0, c->stream>>>(S);
-        scan_kernel<<<sections, 1024, 0, c->stream>>>(c->d_hist, nkeys);
-        block_offsets_kernel<<<gkey, 256, 0, c->stream>>>(S);
-        place_kernel<<<gblk, 1024, (size_t)nkeys * 4, c->stream>>>(S);
+        count_kernel<<<gblk, 1024, cnt_smem, ws>>>(S);
+        key_totals_kernel<<<gkey, 256, 0, ws>>>(S);
+        scan_kernel<<<sections, 1024, 0, ws>>>(d_hist, nkeys);
+        block_offsets_kernel<<<gkey, 256, 0, ws>>>(S);
+        place_kernel<<<gblk, 1024, (size_t)nkeys * 4, ws>>>(S);
         c->launches += 5;
     } else {
-        MR_CUDA(c, cudaMemsetAsync(c->d_hist, 0, (size_t)hist_entries * 4, c->stream));
+        MR_CUDA(c, cudaMemsetAsync(d_hist, 0, (size_t)hist_entries * 4, ws));
         const dim3 grid((unsigned)((n + 255) / 256), (unsigned)sections);
         if (int rc = set_smem(c, classify_kernel, smem)) return rc;
-        classify_kernel<<<grid, 256, smem, c->stream>>>(S);
-        scan_kernel<<<sections, 1024, 0, c->stream>>>(c->d_hist, nkeys);
-        scatter_kernel<<<grid, 256, 0, c->stream>>>(S);
+        classify_kernel<<<grid, 256, smem, ws>>>(S);
+        scan_kernel<<<sections, 1024, 0, ws>>>(d_hist, nkeys);
+        scatter_kernel<<<grid, 256, 0, ws>>>(S);
         c->launches += 3;
     }
     MR_CUDA(c, cudaGetLastError());
-    *perm_out = c->d_perm;
+    *perm_out = d_perm;
     return MR_OK;
 }
 
@@ -494,8 +504,8 @@ int launch_rz_t(mr_ctx *c, const RzParams &Q, int block)
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
     MR_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rz_kernel<Real, Rec, TRACE>, block, smem));
     const long long grid = std::max<long long>(1, std::min<long long>((Q.c.n + block - 1) / block, (long long)sms * std::max(per_sm, 1)));
-    MR_CUDA(c, cudaMemsetAsync(c->d_counters + 3, 0, sizeof(unsigned long long), c->stream));
-    rz_kernel<Real, Rec, TRACE><<<(unsigned)grid, block, smem, c->stream>>>(Q);
+    MR_CUDA(c, cudaMemsetAsync(c->d_counters + 3, 0, sizeof(unsigned long long), c->work_stream()));
+    rz_kernel<Real, Rec, TRACE><<<(unsigned)grid, block, smem, c->work_stream()>>>(Q);
     c->launches += 1;
     MR_CUDA(c, cudaGetLastError());
     return MR_OK;
@@ -544,7 +554,7 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
         c->kev.push_back(a);
         c->kev.push_back(b);
     }
-    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->stream));
+    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->work_stream()));
     int rc;
     if (c->mesh_rz) rc = launch_rz_cast(c, P);
     else if (c->precision == MR_PRECISION_DOUBLE) rc = launch_cast_t<double, CellRecGeneric<double>>(c, P);
@@ -560,7 +570,7 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     default: rc = launch_cast_t<float, CellRecGeneric<float>>(c, P);
     }
     if (rc) return rc;
-    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used + 1], c->stream));
+    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used + 1], c->work_stream()));
     c->kev_used += 2;
     return MR_OK;
 }
@@ -658,6 +668,8 @@ int mr_create_ex(mr_ctx **out, int device, int precision, const mr_allocator *al
     if (alloc) c->alloc = *alloc;
     DeviceGuard guard(device);
     bool ok = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&c->ev_lane, cudaEventDisableTiming) == cudaSuccess;
     for (int s = 0; s < kStageSlots && ok; ++s) {
         ok = ok && cudaEventCreateWithFlags(&c->ev_copied[s], cudaEventDisableTiming) == cudaSuccess;
         ok = ok && cudaEventCreateWithFlags(&c->ev_done[s], cudaEventDisableTiming) == cudaSuccess;
@@ -712,10 +724,14 @@ int mr_destroy(mr_ctx *c)
     c->dev_free(c->d_s2);
     c->dev_free(c->d_det);
     c->dev_free(c->d_det_sum);
-    c->dev_free(c->d_keys);
-    c->dev_free(c->d_perm);
-    c->dev_free(c->d_hist);
-    c->dev_free(c->d_blk_hist);
+    for (int l = 0; l < 2; ++l) {
+        c->dev_free(c->d_keys_l[l]);
+        c->dev_free(c->d_perm_l[l]);
+        c->dev_free(c->d_hist_l[l]);
+        c->dev_free(c->d_blk_hist_l[l]);
+    }
+    if (c->stream2) { cudaStreamSynchronize(c->stream2); cudaStreamDestroy(c->stream2); }
+    if (c->ev_lane) cudaEventDestroy(c->ev_lane);
     for (int s = 0; s < kStageSlots; ++s) {
         if (c->ev_copied[s]) cudaEventDestroy(c->ev_copied[s]);
         if (c->ev_done[s]) cudaEventDestroy(c->ev_done[s]);
@@ -1104,8 +1120,19 @@ int run_batch(mr_ctx *c, int64_t n, const void *rays, int where, Work work)
     MR_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
     int64_t chunk = (int64_t)std::max<size_t>(1024, (size_t)n > 2 * per ? per / 4 : per);
     int last_slot = -1;
-    for (int64_t first = 0, count = 0; first < n; first += count, chunk = std::min<int64_t>(2 * chunk, (int64_t)big)) {
+    // Consecutive chunks alternate between the two compute lanes: every cast kernel ramps up and down for about
+    // 0.2 ms (a CTA lives as long as its longest ray), and with one stream those ramps add up chunk after chunk.
+    // (Not on R-Z meshes: their persistent kernel has one work counter.)
+    const bool two_lanes = !c->mesh_rz && n > chunk;
+    struct LaneReset { mr_ctx *c; ~LaneReset() { c->lane = 0; } } lane_reset{c};
+    if (two_lanes) {
+        MR_CUDA(c, cudaEventRecord(c->ev_lane, c->stream));
+        MR_CUDA(c, cudaStreamWaitEvent(c->stream2, c->ev_lane, 0));
+    }
+    int k = 0;
+    for (int64_t first = 0, count = 0; first < n; first += count, chunk = std::min<int64_t>(2 * chunk, (int64_t)big), ++k) {
         count = std::min<int64_t>(chunk, n - first);
+        c->lane = two_lanes ? (k & 1) : 0;
         const int s = c->next_slot;
         c->next_slot = (s + 1) % kStageSlots;
         const char *src = (const char *)rays + (size_t)first * rb;
@@ -1117,10 +1144,15 @@ int run_batch(mr_ctx *c, int64_t n, const void *rays, int where, Work work)
         MR_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_done[s], 0));  // device slot free again
         MR_CUDA(c, cudaMemcpyAsync(c->d_stage[s], src, (size_t)count * rb, cudaMemcpyHostToDevice, c->copy_stream));
         MR_CUDA(c, cudaEventRecord(c->ev_copied[s], c->copy_stream));
-        MR_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied[s], 0));
+        MR_CUDA(c, cudaStreamWaitEvent(c->work_stream(), c->ev_copied[s], 0));
         if (int rc = work((long long)count, (const void *)c->d_stage[s])) return rc;
-        MR_CUDA(c, cudaEventRecord(c->ev_done[s], c->stream));
+        MR_CUDA(c, cudaEventRecord(c->ev_done[s], c->work_stream()));
         last_slot = s;
+    }
+    c->lane = 0;
+    if (two_lanes) {   // the context's stream continues after both lanes
+        MR_CUDA(c, cudaEventRecord(c->ev_lane, c->stream2));
+        MR_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_lane, 0));
     }
     MR_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
     c->have_timing = true;
@@ -1297,7 +1329,7 @@ int launch_ne_m(mr_ctx *c, const NextEventParams &P, int ndet_launch, int block,
     const long long gx = (P.n + block - 1) / block;
     if (gx > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
     if (int rc = set_smem(c, next_event_kernel<Real, Rec, MODE, TRACE>, smem)) return rc;
-    next_event_kernel<Real, Rec, MODE, TRACE><<<dim3((unsigned)gx, (unsigned)ndet_launch), block, smem, c->stream>>>(P);
+    next_event_kernel<Real, Rec, MODE, TRACE><<<dim3((unsigned)gx, (unsigned)ndet_launch), block, smem, c->work_stream()>>>(P);
     c->launches += 1;
     MR_CUDA(c, cudaGetLastError());
     return MR_OK;
@@ -1364,7 +1396,7 @@ int next_event_device(mr_ctx *c, long long n, const void *d_rays)
         c->kev.push_back(a);
         c->kev.push_back(b);
     }
-    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->stream));
+    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->work_stream()));
     // detectors in groups whose ordering scratch stays below 2^25 (event, detector) pairs
     const int group = (int)std::max<long long>(1, std::min<long long>(c->ndet, (1LL << 25) / std::max<long long>(n, 1)));
     for (int first = 0; first < c->ndet; first += group) {
@@ -1373,7 +1405,7 @@ int next_event_device(mr_ctx *c, long long n, const void *d_rays)
         if (int rc = order_rays(c, n, d_rays, &P.perm, count, first)) return rc;
         if (int rc = launch_next_event<false>(c, P, count)) return rc;
     }
-    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used + 1], c->stream));
+    MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used + 1], c->work_stream()));
     c->kev_used += 2;
     return MR_OK;
 }
