@@ -21,7 +21,9 @@
  *     has finished (stream order, or mr_sync).
  *   - outputs are caller-allocated host arrays.
  *   - one context is used by one host thread at a time.  All device work of a context is
- *     queued on ONE CUDA stream (mr_set_stream; default: the legacy default stream).
+ *     ordered on ONE CUDA stream (mr_set_stream; default: the legacy default stream): the
+ *     library's internal copy and compute streams fork from it and join it again before a
+ *     call returns, so work the caller queues on that stream afterwards sees the results.
  *   - cell linear index c = ix + nx*(iy + ny*iz), x fastest.
  *   - units: cm, MeV, g/cc, cm^2/g; the tally is raw weight*cm sums (no volume or source
  *     normalisation: that is host-side bookkeeping, off the hot path).
@@ -299,7 +301,8 @@ MR_API int mr_trace_rays(mr_ctx *ctx, int64_t n, const void *rays, int where, ui
 enum {
     MR_OPT_BLOCK_THREADS = 1, /* threads per CTA of the cast kernel (multiple of 32, <= 256) */
     MR_OPT_SORT_RAYS = 2,     /* 0: cast in buffer order; 1: bin rays by start slab and length first */
-    MR_OPT_STAGE_RAYS = 3,    /* rays per staging chunk for host batches (H2D of chunk i+1 overlaps the cast of chunk i) */
+    MR_OPT_STAGE_RAYS = 3,    /* base chunk size (rays) for host batches: chunks grow from a quarter of it to twice it; the H2D copy of
+                                 chunk i+1 overlaps the cast of chunk i, and consecutive casts run on two internal lanes */
     MR_OPT_COPY_THREADS = 4,  /* host threads that copy a PAGEABLE batch into the pinned ring (a pinned batch is DMA'd directly) */
     MR_OPT_PAIR_RECORDS = 5,  /* 1: 16-byte cell records (K = 2, 3, MIXED) are fetched as 32-byte pairs kept in registers; 0: one by one */
     MR_OPT_ORDER_MODE = 6,    /* key of the MR_OPT_SORT_RAYS pre-pass: 1 = (start z-slab, length): CTAs resident together work in the
