@@ -187,6 +187,7 @@ def main():
     ap.add_argument("--ne-detectors", type=int, default=4)
     ap.add_argument("--producers", type=int, default=4, help="host threads feeding the producer ring")
     ap.add_argument("--ring-slots", type=int, default=4)
+    ap.add_argument("--push-rays", type=int, default=8192, help="rays per mr_ring_push call of a producer (a burst of collision events)")
     ap.add_argument("--ring-slot-rays", type=int, default=1 << 20)
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--sort", type=int, default=-1, help="override MR_OPT_SORT_RAYS (default: library default)")
@@ -350,7 +351,7 @@ def main():
         # NEXT-1 (Fig. 4): P host threads push the batch piecewise into the producer ring; buffers ship as they fill
         P = max(1, args.producers)
         bounds = np.linspace(0, n_rays, P + 1).astype(np.int64)
-        piece = 8192                      # rays per push: a burst of collision events
+        piece = max(1, args.push_rays)    # rays per push: a burst of collision events
 
         def produce(lo, hi):
             i = lo
