@@ -182,6 +182,8 @@ def main():
     ap.add_argument("--cpu-sample-rays", type=int, default=1_000_000, help="rays of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--double", action="store_true", help="all-double mode (MR_PRECISION_DOUBLE, 64-byte ray records): a context line, "
+                    "not the headline; the roofline then uses B_seg = 16 + 9K, B_ray = 64 + 32M (SURVEY.md 8(d)); implies --no-next")
     ap.add_argument("--no-next", action="store_true", help="skip the SURVEY 8(f) rows (next-event cast, batch-moment fold)")
     ap.add_argument("--ne-rays", type=int, default=2_000_000, help="events per next-event step")
     ap.add_argument("--ne-detectors", type=int, default=4)
@@ -217,7 +219,10 @@ def main():
 
     prob = make_problem(args.config, **prob_kw)
     rays = make_rays(prob, n_rays, batch=rank)  # every rank its own batch: weak scaling
-    m = MonteRay(local_rank, 0)
+    if args.double:
+        args.no_next = True
+        rays = rays.astype(np.float64)
+    m = MonteRay(local_rank, 1 if args.double else 0)
     for kv in args.pre_opt:
         k, v = kv.split("=")
         m.set_option(int(k), int(v))
@@ -274,6 +279,8 @@ def main():
     peak, peak_src = measured_peak()
     dense = prob.config == 5
     alg_bytes = algorithmic_bytes(prob, seg_step, n_rays, dense)
+    if args.double:
+        alg_bytes = seg_step * (16 + 9 * prob.K) + n_rays * (64 + 32 * prob.M)
     achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
     traffic = committed_traffic(CONFIG_NAMES[args.config])
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
@@ -434,7 +441,7 @@ def main():
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": CONFIG_NAMES[args.config], "mesh": [prob.nx, prob.ny, prob.nz], "K": prob.K, "M": prob.M,
                        "rays_per_step_per_gpu": n_rays, "segments_per_step_per_gpu": int(seg_step),
-                       "precision": "mixed (fp32 tables/rays/coefficients, fp64 walk/score/tally)",
+                       "precision": "double (everything fp64)" if args.double else "mixed (fp32 tables/rays/coefficients, fp64 walk/score/tally)",
                        "parallelism": f"replicas x{world}" if world > 1 else "1 GPU",
                        "l2": "inputs larger than L2 (rays 320 MB + cell records 139 MB + tally 69 MB), no flush"
                        if args.config == 3 else "no flush"},

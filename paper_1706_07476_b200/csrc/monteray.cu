@@ -517,7 +517,9 @@ int launch_rz_cast(mr_ctx *c, const CastParams &P)
     Q.c = P;
     Q.spherical = c->mesh_sphere ? 1 : 0;
     const int block = c->block_threads;
-    if (c->precision == MR_PRECISION_DOUBLE) return launch_rz_t<double, CellRecGeneric<double>, false>(c, Q, block);
+    if (c->precision == MR_PRECISION_DOUBLE)
+        return c->layout == LAYOUT_DK3 ? launch_rz_t<double, CellRec<LAYOUT_DK3>, false>(c, Q, block)
+                                       : launch_rz_t<double, CellRecGeneric<double>, false>(c, Q, block);
     switch (c->layout) {
     case LAYOUT_K1: return launch_rz_t<float, CellRec<LAYOUT_K1>, false>(c, Q, block);
     case LAYOUT_K2: return launch_rz_t<float, CellRec<LAYOUT_K2>, false>(c, Q, block);
@@ -557,7 +559,8 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->work_stream()));
     int rc;
     if (c->mesh_rz) rc = launch_rz_cast(c, P);
-    else if (c->precision == MR_PRECISION_DOUBLE) rc = launch_cast_t<double, CellRecGeneric<double>>(c, P);
+    else if (c->precision == MR_PRECISION_DOUBLE)
+        rc = c->layout == LAYOUT_DK3 ? launch_cast_t<double, CellRec<LAYOUT_DK3>>(c, P) : launch_cast_t<double, CellRecGeneric<double>>(c, P);
     else switch (c->layout) {
     case LAYOUT_K1: rc = launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P); break;
     case LAYOUT_K2: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
@@ -859,6 +862,7 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
 
     const bool dbl = c->precision == MR_PRECISION_DOUBLE;
     int layout = LAYOUT_GENERIC;
+    if (dbl && K <= 3) layout = LAYOUT_DK3;
     if (!dbl) {
         if (K <= 4) layout = K;  // LAYOUT_K1..K4
         if (K == 8 && M == 8) {  // dense: every cell lists materials 0..7 in order (ids implicit)
@@ -871,7 +875,7 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
     switch (layout) {
     case LAYOUT_K1: rec_bytes = 8; break;
     case LAYOUT_K2: case LAYOUT_K3: rec_bytes = 16; break;
-    case LAYOUT_K4: case LAYOUT_D8: rec_bytes = 32; break;
+    case LAYOUT_K4: case LAYOUT_D8: case LAYOUT_DK3: rec_bytes = 32; break;
     default: rec_bytes = (size_t)K * (dbl ? 8 : 4); id_bytes = (size_t)K;
     }
     const long long chunk = std::min<long long>(c->ncell, 1LL << 22);
@@ -1353,7 +1357,9 @@ int launch_ne_t(mr_ctx *c, const NextEventParams &P, int ndet_launch)
 template <bool TRACE>
 int launch_next_event(mr_ctx *c, const NextEventParams &P, int ndet_launch)
 {
-    if (c->precision == MR_PRECISION_DOUBLE) return launch_ne_t<double, CellRecGeneric<double>, TRACE>(c, P, ndet_launch);
+    if (c->precision == MR_PRECISION_DOUBLE)
+        return c->layout == LAYOUT_DK3 ? launch_ne_t<double, CellRec<LAYOUT_DK3>, TRACE>(c, P, ndet_launch)
+                                       : launch_ne_t<double, CellRecGeneric<double>, TRACE>(c, P, ndet_launch);
     switch (c->layout) {
     case LAYOUT_K1: return launch_ne_t<float, CellRec<LAYOUT_K1>, TRACE>(c, P, ndet_launch);
     case LAYOUT_K2: return c->pair_records ? launch_ne_t<float, CellRec<LAYOUT_K2P>, TRACE>(c, P, ndet_launch) : launch_ne_t<float, CellRec<LAYOUT_K2>, TRACE>(c, P, ndet_launch);

@@ -30,6 +30,7 @@ enum CellLayout : int {
     LAYOUT_K3 = 3,         // 16 B {float r0,r1,r2; u32 ids}
     LAYOUT_K4 = 4,         // 32 B {float r0..r3; u32 ids; u32 pad[3]}
     LAYOUT_D8 = 8,         // 32 B {float r[8]}  dense: slot k holds material k
+    LAYOUT_DK3 = 23,       // DOUBLE mode, K <= 3: 32 B {double r0,r1,r2; u32 ids; u32 pad}, one LDG.E.256 per cell
     LAYOUT_K4F = 14,       // kernel-side only: LAYOUT_K4 record whose 8 spare bytes (offset 24) hold the cell's score accumulator
     LAYOUT_K2P = 12,       // kernel-side only: LAYOUT_K2 / LAYOUT_K3 records fetched as 32-byte pairs
     LAYOUT_K3P = 13,
@@ -494,6 +495,31 @@ template <> struct CellRec<LAYOUT_D8> : PlainTally {
         s = fmaf(q.b.y, sig[5 * stride], s);
         s = fmaf(q.b.z, sig[6 * stride], s);
         return fmaf(q.b.w, sig[7 * stride], s);
+    }
+};
+
+// DOUBLE mode, K <= 3: the whole record in one 32-byte load (the generic layout costs 2K uncoalesced loads per cell).
+// An empty slot packs as r = 0, id = 0 and adds +0 in the same slot order, like the fp32 records.
+template <> struct CellRec<LAYOUT_DK3> : PlainTally {
+    struct Value { double r0, r1, r2; uint32_t ids; };
+    Value q;
+    __device__ __forceinline__ void reset() {}
+    __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c)
+    {
+        uint4 lo, hi;
+        ldg_256(reinterpret_cast<const uint4 *>(recs) + 2 * (size_t)c, lo, hi);
+        q.r0 = __hiloint2double((int)lo.y, (int)lo.x);
+        q.r1 = __hiloint2double((int)lo.w, (int)lo.z);
+        q.r2 = __hiloint2double((int)hi.y, (int)hi.x);
+        q.ids = hi.z;
+    }
+    __device__ __forceinline__ Value value() const { return q; }
+    static __device__ __forceinline__ double sigma(const Value &q, const double *sig, int stride, int)
+    {
+        double s = q.r0 * sig[(q.ids & 0xffu) * stride];
+        s += q.r1 * sig[((q.ids >> 8) & 0xffu) * stride];
+        s += q.r2 * sig[((q.ids >> 16) & 0xffu) * stride];
+        return s;
     }
 };
 
@@ -1199,6 +1225,14 @@ __global__ void pack_cells_kernel(const PackParams P)
         uint4 *p = reinterpret_cast<uint4 *>(P.recs) + 2 * c;
         p[0] = make_uint4(__float_as_uint(rf[0]), __float_as_uint(rf[1]), __float_as_uint(rf[2]), __float_as_uint(rf[3]));
         p[1] = make_uint4(pid(0) | (pid(1) << 8) | (pid(2) << 16) | (pid(3) << 24), 0u, 0u, 0u);
+        break;
+    }
+    case LAYOUT_DK3: {
+        double *p = reinterpret_cast<double *>(P.recs) + 4 * c;
+        p[0] = rd[0];
+        p[1] = P.K > 1 ? rd[1] : 0.0;
+        p[2] = P.K > 2 ? rd[2] : 0.0;
+        reinterpret_cast<uint2 *>(p + 3)[0] = make_uint2(pid(0) | ((P.K > 1 ? pid(1) : 0u) << 8) | ((P.K > 2 ? pid(2) : 0u) << 16), 0u);
         break;
     }
     case LAYOUT_D8: {
