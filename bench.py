@@ -310,114 +310,117 @@ def main():
                "d2h_bytes_per_step": int(prob.ncell * 8), "ms_per_step": 1e3 * dt / args.steps}
     # ---------------------------------------------------------------- next-event cast, batch-moment fold
     next_rows = None
-    if not args.no_next:
+    if not args.no_next and world == 1:   # context rows, single GPU only; never allowed to cost the headline line
         next_rows = {}
-        lo = np.array([prob.xe[0], prob.ye[0], prob.ze[0]])
-        hi = np.array([prob.xe[-1], prob.ye[-1], prob.ze[-1]])
-        g = np.random.default_rng(7)
-        dets = lo + (0.05 + 0.9 * g.random((args.ne_detectors, 3))) * (hi - lo)   # detector points inside the mesh
-        n_ne = min(args.ne_rays, n_rays)
-        m.load_detectors(dets)
-        d_ev = d_rays[:n_ne]
-        for _ in range(3):
-            m.cast_next_event(d_ev)
-        barrier()
-        s0 = m.get_stats()
-        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        reps = max(3, min(args.steps, 10))
-        a0.record()
-        for _ in range(reps):
-            m.cast_next_event(d_ev)
-        a1.record()
-        barrier()
-        ms = a0.elapsed_time(a1) / reps
-        s1 = m.get_stats()
-        ne_seg = (s1.ne_segments - s0.ne_segments) // reps
-        ne_bytes = ne_seg * (4 if dense else 5) * prob.K + n_ne * args.ne_detectors * (32 + 16 * prob.M)
-        next_rows["next_event"] = {
-            "value": ne_seg / (ms * 1e-3), "unit": "segments/s", "pairs_per_sec": n_ne * args.ne_detectors / (ms * 1e-3),
-            "ms_per_step": ms, "events": n_ne, "detectors": args.ne_detectors, "segments_per_step": int(ne_seg),
-            "roofline": {"bound": "hbm", "achieved": ne_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                         "frac": ne_bytes / (ms * 1e-3) / 1e9 / peak,
-                         "algorithmic_bytes": "5K (4K dense) per segment + (32 + 16 M) per (event, detector) pair"}}
-        for _ in range(3):
-            m.end_batch()
-        barrier()
-        a0.record()
-        for _ in range(reps):
-            m.end_batch()
-        a1.record()
-        barrier()
-        ms = a0.elapsed_time(a1) / reps
-        fold_bytes = prob.ncell * 40
-        next_rows["end_batch"] = {
-            "value": prob.ncell / (ms * 1e-3), "unit": "cells/s", "ms_per_step": ms,
-            "roofline": {"bound": "hbm", "achieved": fold_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                         "frac": fold_bytes / (ms * 1e-3) / 1e9 / peak,
-                         "algorithmic_bytes": "40 per cell (read tally, read+write previous total and sum of squares)"}}
-        # NEXT-1 (Fig. 4): P host threads push the batch piecewise into the producer ring; buffers ship as they fill
-        P = max(1, args.producers)
-        bounds = np.linspace(0, n_rays, P + 1).astype(np.int64)
-        piece = max(1, args.push_rays)    # rays per push: a burst of collision events
-
-        def produce(lo, hi):
-            i = lo
-            while i < hi:
-                j = min(hi, i + piece)
-                m.ring_push(rays[i:j])
-                i = j
-
-        def ring_step():
-            ts = [threading.Thread(target=produce, args=(int(bounds[k]), int(bounds[k + 1]))) for k in range(P)]
-            for t in ts:
-                t.start()
-            for t in ts:
-                t.join()
-            m.ring_flush()
-            m.read_tally_into(h_tally.data_ptr())
-
-        m.ring_open(args.ring_slots, min(args.ring_slot_rays, max(1024, n_rays)))
-        ring_step()
-        w0 = m.ring_stats()["producer_wait_ms"]
-        barrier()
-        reps = max(2, min(args.steps, 5))
-        t0 = time.perf_counter()
-        for _ in range(reps):
-            ring_step()
-        torch.cuda.synchronize()
-        dt = (time.perf_counter() - t0) / reps
-        rs = m.ring_stats()
-        m.ring_close()
-        next_rows["producer_ring"] = {
-            "value": seg_step / dt, "unit": UNIT, "ms_per_step": 1e3 * dt, "producers": P, "rays_per_push": piece,
-            "slots": args.ring_slots, "rays_per_slot": min(args.ring_slot_rays, max(1024, n_rays)),
-            "producer_wait_ms_per_step": (rs["producer_wait_ms"] - w0) / reps,
-            "device_only_ms_per_step": ms_total / args.steps,
-            "h2d_bytes_per_step": int(rays.nbytes), "d2h_bytes_per_step": int(prob.ncell * 8)}
-        # NEXT-4: the same estimator on an R-Z (cylindrical) pin-cell mesh, its own context
-        from workloads import make_rz_problem, make_rz_rays
-
-        rzp = make_rz_problem(256, 2048)
-        rz_rays = torch.from_numpy(make_rz_rays(rzp, 4_000_000)).to(dev)
-        with MonteRay(local_rank, 0) as mz:
-            mz.load_problem(rzp)
+        try:
+            lo = np.array([prob.xe[0], prob.ye[0], prob.ze[0]])
+            hi = np.array([prob.xe[-1], prob.ye[-1], prob.ze[-1]])
+            g = np.random.default_rng(7)
+            dets = lo + (0.05 + 0.9 * g.random((args.ne_detectors, 3))) * (hi - lo)   # detector points inside the mesh
+            n_ne = min(args.ne_rays, n_rays)
+            m.load_detectors(dets)
+            d_ev = d_rays[:n_ne]
             for _ in range(3):
-                mz.cast_rays(rz_rays)
+                m.cast_next_event(d_ev)
             barrier()
-            z0 = mz.get_stats()
+            s0 = m.get_stats()
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = max(3, min(args.steps, 10))
             a0.record()
             for _ in range(reps):
-                mz.cast_rays(rz_rays)
+                m.cast_next_event(d_ev)
             a1.record()
             barrier()
             ms = a0.elapsed_time(a1) / reps
-            rz_seg = (mz.get_stats().segments - z0.segments) // reps
-        rz_bytes = rz_seg * (16 + 5 * rzp.K) + rz_rays.shape[0] * (32 + 16 * rzp.M)
-        next_rows["rz_cast"] = {
-            "value": rz_seg / (ms * 1e-3), "unit": UNIT, "rays_per_sec": rz_rays.shape[0] / (ms * 1e-3), "ms_per_step": ms,
-            "workload": rzp.name, "rays": int(rz_rays.shape[0]), "segments_per_step": int(rz_seg),
-            "roofline": {"bound": "hbm", "achieved": rz_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                         "frac": rz_bytes / (ms * 1e-3) / 1e9 / peak}}
+            s1 = m.get_stats()
+            ne_seg = (s1.ne_segments - s0.ne_segments) // reps
+            ne_bytes = ne_seg * (4 if dense else 5) * prob.K + n_ne * args.ne_detectors * (32 + 16 * prob.M)
+            next_rows["next_event"] = {
+                "value": ne_seg / (ms * 1e-3), "unit": "segments/s", "pairs_per_sec": n_ne * args.ne_detectors / (ms * 1e-3),
+                "ms_per_step": ms, "events": n_ne, "detectors": args.ne_detectors, "segments_per_step": int(ne_seg),
+                "roofline": {"bound": "hbm", "achieved": ne_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                             "frac": ne_bytes / (ms * 1e-3) / 1e9 / peak,
+                             "algorithmic_bytes": "5K (4K dense) per segment + (32 + 16 M) per (event, detector) pair"}}
+            for _ in range(3):
+                m.end_batch()
+            barrier()
+            a0.record()
+            for _ in range(reps):
+                m.end_batch()
+            a1.record()
+            barrier()
+            ms = a0.elapsed_time(a1) / reps
+            fold_bytes = prob.ncell * 40
+            next_rows["end_batch"] = {
+                "value": prob.ncell / (ms * 1e-3), "unit": "cells/s", "ms_per_step": ms,
+                "roofline": {"bound": "hbm", "achieved": fold_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                             "frac": fold_bytes / (ms * 1e-3) / 1e9 / peak,
+                             "algorithmic_bytes": "40 per cell (read tally, read+write previous total and sum of squares)"}}
+            # NEXT-1 (Fig. 4): P host threads push the batch piecewise into the producer ring; buffers ship as they fill
+            P = max(1, args.producers)
+            bounds = np.linspace(0, n_rays, P + 1).astype(np.int64)
+            piece = max(1, args.push_rays)    # rays per push: a burst of collision events
+
+            def produce(lo, hi):
+                i = lo
+                while i < hi:
+                    j = min(hi, i + piece)
+                    m.ring_push(rays[i:j])
+                    i = j
+
+            def ring_step():
+                ts = [threading.Thread(target=produce, args=(int(bounds[k]), int(bounds[k + 1]))) for k in range(P)]
+                for t in ts:
+                    t.start()
+                for t in ts:
+                    t.join()
+                m.ring_flush()
+                m.read_tally_into(h_tally.data_ptr())
+
+            m.ring_open(args.ring_slots, min(args.ring_slot_rays, max(1024, n_rays)))
+            ring_step()
+            w0 = m.ring_stats()["producer_wait_ms"]
+            barrier()
+            reps = max(2, min(args.steps, 5))
+            t0 = time.perf_counter()
+            for _ in range(reps):
+                ring_step()
+            torch.cuda.synchronize()
+            dt = (time.perf_counter() - t0) / reps
+            rs = m.ring_stats()
+            m.ring_close()
+            next_rows["producer_ring"] = {
+                "value": seg_step / dt, "unit": UNIT, "ms_per_step": 1e3 * dt, "producers": P, "rays_per_push": piece,
+                "slots": args.ring_slots, "rays_per_slot": min(args.ring_slot_rays, max(1024, n_rays)),
+                "producer_wait_ms_per_step": (rs["producer_wait_ms"] - w0) / reps,
+                "device_only_ms_per_step": ms_total / args.steps,
+                "h2d_bytes_per_step": int(rays.nbytes), "d2h_bytes_per_step": int(prob.ncell * 8)}
+            # NEXT-4: the same estimator on an R-Z (cylindrical) pin-cell mesh, its own context
+            from workloads import make_rz_problem, make_rz_rays
+
+            rzp = make_rz_problem(256, 2048)
+            rz_rays = torch.from_numpy(make_rz_rays(rzp, 4_000_000)).to(dev)
+            with MonteRay(local_rank, 0) as mz:
+                mz.load_problem(rzp)
+                for _ in range(3):
+                    mz.cast_rays(rz_rays)
+                barrier()
+                z0 = mz.get_stats()
+                a0.record()
+                for _ in range(reps):
+                    mz.cast_rays(rz_rays)
+                a1.record()
+                barrier()
+                ms = a0.elapsed_time(a1) / reps
+                rz_seg = (mz.get_stats().segments - z0.segments) // reps
+            rz_bytes = rz_seg * (16 + 5 * rzp.K) + rz_rays.shape[0] * (32 + 16 * rzp.M)
+            next_rows["rz_cast"] = {
+                "value": rz_seg / (ms * 1e-3), "unit": UNIT, "rays_per_sec": rz_rays.shape[0] / (ms * 1e-3), "ms_per_step": ms,
+                "workload": rzp.name, "rays": int(rz_rays.shape[0]), "segments_per_step": int(rz_seg),
+                "roofline": {"bound": "hbm", "achieved": rz_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                             "frac": rz_bytes / (ms * 1e-3) / 1e9 / peak}}
+        except Exception as e:  # noqa: BLE001 -- report, do not lose the JSON line
+            next_rows["error"] = repr(e)
     total_launches = m.get_stats().kernel_launches
 
     # ---------------------------------------------------------------- CPU oracle beside it (rank 0, N = 1)
