@@ -308,10 +308,14 @@ enum {
     MR_OPT_ORDER_MODE = 6,    /* key of the MR_OPT_SORT_RAYS pre-pass: 1 = (start z-slab, length): CTAs resident together work in the
                                  same slabs (L2 reuse); 2 = longest rays first: no tail; 0 = auto: 2 when tally + cell records fit
                                  in half the L2, else 1 */
-    MR_OPT_FUSED_TALLY = 7    /* read by mr_load_materials.  K = 4 records (MIXED) have 8 spare bytes: 1 = the cast kernel accumulates
+    MR_OPT_FUSED_TALLY = 7,   /* read by mr_load_materials.  K = 4 records (MIXED) have 8 spare bytes: 1 = the cast kernel accumulates
                                  each cell's score THERE (the load and the atomic of a segment then share one DRAM sector) and the sums
                                  are moved into the contiguous tally whenever it is looked at (mr_read_tally, mr_tally_device_ptr,
                                  mr_end_batch, mr_clear_tally); 0 = never; 2 (default) = when ncell * 40 bytes exceed twice the L2 */
+    MR_OPT_TILED_INDEX = 8    /* 1 (default): when a mesh (K <= 3, MIXED, Cartesian) holds at most 1024 DISTINCT cell records,
+                                 mr_load_materials also builds a dictionary of them and a 2-byte index per cell in 32-byte tiles of
+                                 4 x 4 (x, y) cells, and mr_cast_rays walks those (a step inside a tile needs no load); 0: never.
+                                 Setting 0 after the load makes the cast use the plain records again */
 };
 MR_API int mr_set_option(mr_ctx *ctx, int option, int64_t value);
 MR_API int mr_get_option(mr_ctx *ctx, int option, int64_t *value);

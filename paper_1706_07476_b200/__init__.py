@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     MR_OPT_PAIR_RECORDS,
     MR_OPT_SORT_RAYS,
     MR_OPT_STAGE_RAYS,
+    MR_OPT_TILED_INDEX,
     MR_PRECISION_DOUBLE,
     MR_PRECISION_MIXED,
     MR_WHERE_DEVICE,

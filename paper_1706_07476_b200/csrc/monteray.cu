@@ -17,6 +17,7 @@
 #include <cstring>
 #include <string>
 #include <thread>
+#include <unordered_map>
 #include <vector>
 
 #define MR_PACK_MAX_SLOTS MR_MAX_SLOTS
@@ -163,6 +164,13 @@ struct mr_ctx {
     long long sort_cap_l[2] = {0, 0}, hist_cap_l[2] = {0, 0}, blk_hist_cap_l[2] = {0, 0};
 
     int order_mode = 0;              // option MR_OPT_ORDER_MODE: 0 auto, 1 slab-major, 2 longest first
+    // Tiled mixture index (K <= 3, MIXED, Cartesian): the distinct cell records as a small dictionary (shared memory in the
+    // cast kernel) and a 2-byte index per cell stored in 4 x 4 (x, y) tiles of 32 bytes -- built by mr_load_materials when
+    // the mesh has at most kDictMax distinct records (option MR_OPT_TILED_INDEX).
+    int tiled_opt = 1;
+    uint4 *d_dict = nullptr;
+    uint4 *d_tiles = nullptr;
+    int ndict = 0, ntx = 0, nty = 0;
     int fused_opt = 2;               // option MR_OPT_FUSED_TALLY: 0 off, 1 on, 2 auto (decided by mr_load_materials)
     bool fused = false;              // LAYOUT_K4 records carry the score accumulators (LAYOUT_K4F in the cast kernel)
     bool fused_dirty = false;        // in-record sums not yet moved into d_tally
@@ -236,8 +244,12 @@ void free_materials(mr_ctx *c)
     c->fused = false;
     c->dev_free(c->d_recs);
     c->dev_free(c->d_ids);
+    c->dev_free(c->d_dict);
+    c->dev_free(c->d_tiles);
     c->d_recs = nullptr;
     c->d_ids = nullptr;
+    c->d_dict = c->d_tiles = nullptr;
+    c->ndict = 0;
     c->layout = 0;
     c->K = 0;
 }
@@ -273,6 +285,75 @@ void free_stage(mr_ctx *c)
         c->d_stage[s] = nullptr;
     }
     c->stage_cap_rays = 0;
+}
+
+constexpr int kDictMax = 1024;   // distinct cell records the cast kernel keeps in shared memory (16 KB)
+
+// Dictionary + tiled 2-byte index of the cell records (see mr_ctx::d_dict).  The records are formed exactly as
+// pack_cells_kernel forms them (r = (float)(frac * density), empty slot = {0, id 0}), in the K = 3 encoding whatever K <= 3 is.
+// Gives up (leaves ndict = 0) as soon as more than kDictMax distinct records have been seen.
+int build_tiled_index(mr_ctx *c, int M, const double *density, int K, const int32_t *cell_mat, const double *cell_frac)
+{
+    c->ndict = 0;
+    if (!c->tiled_opt || c->precision != MR_PRECISION_MIXED || K > 3 || c->mesh_rz) return MR_OK;
+    struct Key {
+        uint32_t w[4];
+        bool operator==(const Key &o) const { return std::memcmp(w, o.w, 16) == 0; }
+    };
+    struct Hash {
+        size_t operator()(const Key &k) const
+        {
+            uint64_t h = 0xcbf29ce484222325ULL;
+            for (int i = 0; i < 4; ++i) h = (h ^ k.w[i]) * 0x100000001b3ULL;
+            return (size_t)h;
+        }
+    };
+    std::unordered_map<Key, uint16_t, Hash> dict;
+    std::vector<Key> entries;
+    const int nx = c->nx, ny = c->ny, nz = c->nz;
+    const int ntx = (nx + 3) / 4, nty = (ny + 3) / 4;
+    std::vector<uint16_t> tiles((size_t)ntx * nty * nz * 16, 0);
+    for (long long cell = 0; cell < c->ncell; ++cell) {
+        Key k{{0u, 0u, 0u, 0u}};
+        for (int s = 0; s < K; ++s) {
+            const int m = cell_mat[cell * K + s];
+            if (m < 0) continue;                              // empty slot: r = 0, id = 0
+            const float r = (float)(cell_frac[cell * K + s] * density[m]);
+            std::memcpy(&k.w[s], &r, 4);
+            k.w[3] |= (uint32_t)m << (8 * s);
+        }
+        auto it = dict.find(k);
+        if (it == dict.end()) {
+            if ((int)entries.size() >= kDictMax) return MR_OK;   // too many distinct records: keep the plain layout
+            it = dict.emplace(k, (uint16_t)entries.size()).first;
+            entries.push_back(k);
+        }
+        const int ix = (int)(cell % nx), iy = (int)((cell / nx) % ny), iz = (int)(cell / ((long long)nx * ny));
+        const size_t tile = (size_t)(ix >> 2) + (size_t)ntx * ((size_t)(iy >> 2) + (size_t)nty * iz);
+        tiles[tile * 16 + (size_t)((iy & 3) * 4 + (ix & 3))] = it->second;
+    }
+    (void)M;
+    uint4 *d_dict = (uint4 *)c->dev_alloc(sizeof(uint4) * kDictMax);
+    uint4 *d_tiles = (uint4 *)c->dev_alloc(tiles.size() * 2);
+    if (!d_dict || !d_tiles) {
+        c->dev_free(d_dict);
+        c->dev_free(d_tiles);
+        return c->fail(MR_ERR_OOM, "device allocation failed (tiled mixture index)");
+    }
+    cudaError_t e = cudaMemcpyAsync(d_dict, entries.data(), entries.size() * 16, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_tiles, tiles.data(), tiles.size() * 2, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) {
+        c->dev_free(d_dict);
+        c->dev_free(d_tiles);
+        return c->fail_cuda(e, "mr_load_materials (tiled index)");
+    }
+    c->d_dict = d_dict;
+    c->d_tiles = d_tiles;
+    c->ndict = (int)entries.size();
+    c->ntx = ntx;
+    c->nty = nty;
+    return MR_OK;
 }
 
 bool finite_increasing(const double *a, int n)
@@ -323,7 +404,8 @@ template <typename Real, typename Rec>
 int launch_cast_t(mr_ctx *c, const CastParams &P)
 {
     const int block = c->block_threads;
-    const size_t per_block = walker_smem_bytes(block) + (size_t)(c->M + c->N) * block * sizeof(Real);
+    const size_t per_block = walker_smem_bytes(block) + (size_t)(c->M + c->N) * block * sizeof(Real) +
+                             (Rec::kTiled ? (size_t)c->ndict * sizeof(uint4) : 0);
     const int mode = edge_mode(c, per_block);
     const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
     if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "materials x block threads exceed shared memory; lower MR_OPT_BLOCK_THREADS");
@@ -561,7 +643,14 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     if (c->mesh_rz) rc = launch_rz_cast(c, P);
     else if (c->precision == MR_PRECISION_DOUBLE)
         rc = c->layout == LAYOUT_DK3 ? launch_cast_t<double, CellRec<LAYOUT_DK3>>(c, P) : launch_cast_t<double, CellRecGeneric<double>>(c, P);
-    else switch (c->layout) {
+    else if (c->ndict > 0 && c->tiled_opt && c->layout >= LAYOUT_K1 && c->layout <= LAYOUT_K3) {
+        P.dict = c->d_dict;
+        P.tiles = c->d_tiles;
+        P.ndict = c->ndict;
+        P.ntx = c->ntx;
+        P.nty = c->nty;
+        rc = launch_cast_t<float, CellRec<LAYOUT_T3>>(c, P);
+    } else switch (c->layout) {
     case LAYOUT_K1: rc = launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P); break;
     case LAYOUT_K2: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
     case LAYOUT_K3: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K3P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P); break;
@@ -926,6 +1015,7 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
                (c->fused_opt == 1 || (c->fused_opt == 2 && (size_t)c->ncell * 40 > 2 * c->l2_bytes));
     c->fused_dirty = false;
     c->K = K;
+    if (int rc = build_tiled_index(c, M, density, K, cell_mat, cell_frac)) return rc;
     if (M != c->M || (int)c->xs_n.size() != M) {
         c->M = M;
         c->mix.assign(M, {});
@@ -1846,6 +1936,10 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "pair-records option is 0 or 1");
         c->pair_records = (int)value;
         return MR_OK;
+    case MR_OPT_TILED_INDEX:
+        if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "tiled-index option is 0 or 1");
+        c->tiled_opt = (int)value;
+        return MR_OK;
     case MR_OPT_FUSED_TALLY:
         if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "fused-tally option is 0 (off), 1 (on) or 2 (auto)");
         c->fused_opt = (int)value;
@@ -1874,6 +1968,7 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     case MR_OPT_PAIR_RECORDS: *value = c->pair_records; return MR_OK;
     case MR_OPT_ORDER_MODE: *value = c->order_mode; return MR_OK;
     case MR_OPT_FUSED_TALLY: *value = c->fused_opt; return MR_OK;
+    case MR_OPT_TILED_INDEX: *value = c->tiled_opt; return MR_OK;
     }
     return c->fail(MR_ERR_INVALID_ARG, "unknown option");
 }
