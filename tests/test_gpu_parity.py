@@ -357,3 +357,34 @@ def test_fused_in_record_tally_for_k4(fused):
     assert nb == 2 and np.array_equal(s1, got)
     assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
     assert_tally(got, ref.tally, 0)
+
+
+def test_tiled_mixture_index_on_off_and_fallback():
+    """MR_OPT_TILED_INDEX: the dictionary + tiled 2-byte index path and the plain-record path give the same counters
+    and tallies within tolerance of the oracle; meshes whose sides are not multiples of the 4 x 4 tile; a mesh with
+    more than 1024 distinct records falls back to the plain records by itself."""
+    from paper_1706_07476_b200 import MR_OPT_TILED_INDEX, MonteRay
+
+    for seed, dims, K in ((601, (7, 5, 6), 1), (602, (9, 6, 5), 2), (603, (13, 11, 4), 3), (604, (12, 10, 9), 2)):
+        prob = tiny_problem(seed, nx=dims[0], ny=dims[1], nz=dims[2], M=4, K=K, n_e=33)
+        if seed == 603:      # few distinct records: a repeating pattern, as in a lattice
+            prob.cell_mat[:] = prob.cell_mat[np.arange(prob.ncell) % 7]
+            prob.cell_frac[:] = prob.cell_frac[np.arange(prob.ncell) % 7]
+        rays = tiny_rays(prob, seed, 20_000, axis_aligned_share=0.05)
+        ref = _oracle(prob).cast(rays, threads=_threads())
+        tallies = []
+        for tiled in (1, 0):
+            with MonteRay(0, 0) as m:
+                m.set_option(MR_OPT_TILED_INDEX, tiled)
+                m.load_problem(prob)
+                m.cast_rays(rays)
+                st = m.get_stats()
+                assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+                tallies.append(m.read_tally())
+                assert_tally(tallies[-1], ref.tally, 0)
+                if tiled:            # switching the option off after the load goes back to the plain records
+                    m.set_option(MR_OPT_TILED_INDEX, 0)
+                    m.clear_tally()
+                    m.cast_rays(rays)
+                    assert_tally(m.read_tally(), ref.tally, 0)
+        np.testing.assert_allclose(tallies[0], tallies[1], rtol=1e-9, atol=1e-12 * ref.tally.max())
