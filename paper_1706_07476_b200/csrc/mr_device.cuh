@@ -241,7 +241,7 @@ __device__ __forceinline__ void sigma_all(const XsDesc *xs, int M, int N, const 
 // axis one packed word (next plane | exit plane << 16) and the signed cell-index increment live in
 // registers; the per-axis doubles (o_a, inv_a) sit in shared memory, [axis][thread], 16 B each, so a
 // warp's LDS.128 is bank-conflict free whatever axis each lane picks.  The kernel is bound by
-// L1TEX data-pipe wavefronts (two uncoalesced global accesses per segment), so shared-memory
+// per-request units (LSU wavefronts, the SM->L2 request port, L2 tag look-ups: DESIGN.md §4.3, §4.6), so shared-memory
 // traffic per step is kept to that one LDS.128 (+ the sigma reads); when the mesh is arithmetic
 // (EDGES_ARITH) the plane position is recomputed with one I2F + DFMA instead of a table read.
 // ------------------------------------------------------------------------------------------------
@@ -401,7 +401,7 @@ template <> struct CellRec<LAYOUT_K1> : PlainTally {
 
 // 16-byte records (K = 2, 3) are fetched as 32-byte aligned PAIRS (cells 2j, 2j+1: x neighbours) with one
 // LDG.E.256 and the pair is kept in registers: a step in x that stays inside the pair (about a quarter of
-// all steps on a mesh with square xy cells) needs no load at all.  The kernel is bound by L1TEX wavefronts
+// all steps on a mesh with square xy cells) needs no load at all.  The kernel is bound by per-request units
 // (one per lane for an uncoalesced access), so every load not issued is time saved.
 struct PairRec {
     uint4 a, b;
@@ -472,7 +472,7 @@ template <> struct CellRec<LAYOUT_K4> : PlainTally {
 // Few distinct records (a lattice of pins, a room of air and concrete): the records live in a shared-memory dictionary
 // and the mesh holds a 2-byte index per cell in 32-byte tiles of 4 x 4 (x, y) cells, kept in registers.  A step in x or
 // y that stays inside the tile needs no global load: 0.29 loads per segment on the PWR-like mesh against 0.65 with
-// record pairs -- the cast kernel is bound by L2 tag look-ups, one per request (DESIGN.md §4.3).
+// record pairs -- the cast kernel is bound by L2 tag look-ups, one per request (DESIGN.md §4.6).
 template <> struct CellRec<LAYOUT_T3> : PlainTally {
     static constexpr bool kTiled = true;
     typedef uint4 Value;
