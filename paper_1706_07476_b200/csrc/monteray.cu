@@ -170,7 +170,7 @@ struct mr_ctx {
     int tiled_opt = 1;
     uint4 *d_dict = nullptr;
     uint4 *d_tiles = nullptr;
-    int ndict = 0, ntx = 0, nty = 0;
+    int ndict = 0, ntx = 0, nty = 0, tile_bits = 16;
     int fused_opt = 2;               // option MR_OPT_FUSED_TALLY: 0 off, 1 on, 2 auto (decided by mr_load_materials)
     bool fused = false;              // LAYOUT_K4 records carry the score accumulators (LAYOUT_K4F in the cast kernel)
     bool fused_dirty = false;        // in-record sums not yet moved into d_tally
@@ -310,9 +310,7 @@ int build_tiled_index(mr_ctx *c, int M, const double *density, int K, const int3
     };
     std::unordered_map<Key, uint16_t, Hash> dict;
     std::vector<Key> entries;
-    const int nx = c->nx, ny = c->ny, nz = c->nz;
-    const int ntx = (nx + 3) / 4, nty = (ny + 3) / 4;
-    std::vector<uint16_t> tiles((size_t)ntx * nty * nz * 16, 0);
+    std::vector<uint16_t> id_of((size_t)c->ncell);
     for (long long cell = 0; cell < c->ncell; ++cell) {
         Key k{{0u, 0u, 0u, 0u}};
         for (int s = 0; s < K; ++s) {
@@ -328,20 +326,31 @@ int build_tiled_index(mr_ctx *c, int M, const double *density, int K, const int3
             it = dict.emplace(k, (uint16_t)entries.size()).first;
             entries.push_back(k);
         }
+        id_of[(size_t)cell] = it->second;
+    }
+    // index width by dictionary size: 4 bits (tiles of 8 x 8 cells), 8 bits (8 x 4), 16 bits (4 x 4); 32 bytes per tile
+    const int bits = entries.size() <= 16 ? 4 : (entries.size() <= 256 ? 8 : 16);
+    const int xs = bits == 16 ? 2 : 3, ys = bits == 4 ? 3 : 2;
+    const int nx = c->nx, ny = c->ny, nz = c->nz;
+    const int ntx = (nx + (1 << xs) - 1) >> xs, nty = (ny + (1 << ys) - 1) >> ys;
+    std::vector<uint32_t> tiles((size_t)ntx * nty * nz * 8, 0u);
+    for (long long cell = 0; cell < c->ncell; ++cell) {
         const int ix = (int)(cell % nx), iy = (int)((cell / nx) % ny), iz = (int)(cell / ((long long)nx * ny));
-        const size_t tile = (size_t)(ix >> 2) + (size_t)ntx * ((size_t)(iy >> 2) + (size_t)nty * iz);
-        tiles[tile * 16 + (size_t)((iy & 3) * 4 + (ix & 3))] = it->second;
+        const size_t tile = (size_t)(ix >> xs) + (size_t)ntx * ((size_t)(iy >> ys) + (size_t)nty * iz);
+        const int e = ((iy & ((1 << ys) - 1)) << xs) | (ix & ((1 << xs) - 1));
+        const int bit = e * bits;
+        tiles[tile * 8 + (size_t)(bit >> 5)] |= (uint32_t)id_of[(size_t)cell] << (bit & 31);
     }
     (void)M;
     uint4 *d_dict = (uint4 *)c->dev_alloc(sizeof(uint4) * kDictMax);
-    uint4 *d_tiles = (uint4 *)c->dev_alloc(tiles.size() * 2);
+    uint4 *d_tiles = (uint4 *)c->dev_alloc(tiles.size() * 4);
     if (!d_dict || !d_tiles) {
         c->dev_free(d_dict);
         c->dev_free(d_tiles);
         return c->fail(MR_ERR_OOM, "device allocation failed (tiled mixture index)");
     }
     cudaError_t e = cudaMemcpyAsync(d_dict, entries.data(), entries.size() * 16, cudaMemcpyHostToDevice, c->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_tiles, tiles.data(), tiles.size() * 2, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_tiles, tiles.data(), tiles.size() * 4, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) {
         c->dev_free(d_dict);
@@ -353,6 +362,7 @@ int build_tiled_index(mr_ctx *c, int M, const double *density, int K, const int3
     c->ndict = (int)entries.size();
     c->ntx = ntx;
     c->nty = nty;
+    c->tile_bits = bits;
     return MR_OK;
 }
 
@@ -649,7 +659,8 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
         P.ndict = c->ndict;
         P.ntx = c->ntx;
         P.nty = c->nty;
-        rc = launch_cast_t<float, CellRec<LAYOUT_T3>>(c, P);
+        rc = c->tile_bits == 4 ? launch_cast_t<float, TiledRec<4>>(c, P)
+           : c->tile_bits == 8 ? launch_cast_t<float, TiledRec<8>>(c, P) : launch_cast_t<float, TiledRec<16>>(c, P);
     } else switch (c->layout) {
     case LAYOUT_K1: rc = launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P); break;
     case LAYOUT_K2: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;

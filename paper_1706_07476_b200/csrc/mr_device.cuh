@@ -470,20 +470,23 @@ template <> struct CellRec<LAYOUT_K4> : PlainTally {
 // read with one plain (coherent) 32-byte load -- not ld.global.nc: the sector is written by the REDs of this kernel.
 // flush_fused_kernel moves the in-record sums into the contiguous tally whenever the tally is looked at.
 // Few distinct records (a lattice of pins, a room of air and concrete): the records live in a shared-memory dictionary
-// and the mesh holds a 2-byte index per cell in 32-byte tiles of 4 x 4 (x, y) cells, kept in registers.  A step in x or
-// y that stays inside the tile needs no global load: 0.29 loads per segment on the PWR-like mesh against 0.65 with
+// and the mesh holds a small index per cell in 32-byte tiles of (x, y) cells, kept in registers.  A step in x or
+// y that stays inside the tile needs no global load (2-byte indices, 4 x 4 tiles): 0.29 loads per segment on the PWR-like mesh against 0.65 with
 // record pairs -- the cast kernel is bound by L2 tag look-ups, one per request.
-template <> struct CellRec<LAYOUT_T3> : PlainTally {
+// BITS = index width: 16 (tiles of 4 x 4 cells, up to 1024 records), 8 (8 x 4, up to 256), 4 (8 x 8, up to 16).
+template <int BITS> struct TiledRec : PlainTally {
     static constexpr bool kTiled = true;
+    static constexpr int kXs = BITS == 16 ? 2 : 3;     // log2 of the tile's x extent
+    static constexpr int kYs = BITS == 4 ? 3 : 2;      // log2 of the tile's y extent
     typedef uint4 Value;
     uint4 a, b;
     int tag;       // resident tile, -1: none
-    int e;         // entry of the current cell inside the tile: (iy & 3) * 4 + (ix & 3)
+    int e;         // entry of the current cell inside the tile: (iy & (ty - 1)) * tx + (ix & (tx - 1))
     __device__ __forceinline__ void reset() { tag = -1; }
     __device__ __forceinline__ void load_tiled(const uint4 *tiles, int ntx, int nty, int ix, int iy, int iz)
     {
-        const int t = (ix >> 2) + ntx * ((iy >> 2) + nty * iz);
-        e = ((iy & 3) << 2) | (ix & 3);
+        const int t = (ix >> kXs) + ntx * ((iy >> kYs) + nty * iz);
+        e = ((iy & ((1 << kYs) - 1)) << kXs) | (ix & ((1 << kXs) - 1));
         if (t != tag) {
             tag = t;
             ldg_256(tiles + 2 * (size_t)t, a, b);
@@ -491,11 +494,12 @@ template <> struct CellRec<LAYOUT_T3> : PlainTally {
     }
     __device__ __forceinline__ Value value(const uint4 *s_dict) const
     {
-        const int r = e >> 1;
+        const int bit = e * BITS;
+        const int r = bit >> 5;
         const uint32_t lo4 = (r & 2) ? ((r & 1) ? a.w : a.z) : ((r & 1) ? a.y : a.x);
         const uint32_t hi4 = (r & 2) ? ((r & 1) ? b.w : b.z) : ((r & 1) ? b.y : b.x);
         const uint32_t w = (r & 4) ? hi4 : lo4;
-        return s_dict[(e & 1) ? (w >> 16) : (w & 0xffffu)];
+        return s_dict[(w >> (bit & 31)) & ((1u << BITS) - 1u)];
     }
     static __device__ __forceinline__ float sigma(const Value &v, const float *sig, int stride, int K)
     {
