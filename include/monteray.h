@@ -312,10 +312,13 @@ enum {
                                  each cell's score THERE (the load and the atomic of a segment then share one DRAM sector) and the sums
                                  are moved into the contiguous tally whenever it is looked at (mr_read_tally, mr_tally_device_ptr,
                                  mr_end_batch, mr_clear_tally); 0 = never; 2 (default) = when ncell * 40 bytes exceed twice the L2 */
-    MR_OPT_TILED_INDEX = 8    /* 1 (default): when a mesh (K <= 3, MIXED, Cartesian) holds at most 1024 DISTINCT cell records,
+    MR_OPT_TILED_INDEX = 8,   /* 1 (default): when a mesh (K <= 3, MIXED, Cartesian) holds at most 1024 DISTINCT cell records,
                                  mr_load_materials also builds a dictionary of them and a 2-byte index per cell in 32-byte tiles of
                                  4 x 4 (x, y) cells, and mr_cast_rays walks those (a step inside a tile needs no load); 0: never.
                                  Setting 0 after the load makes the cast use the plain records again */
+    MR_OPT_AGGREGATE_FIRST = 9 /* n >= 0: the tally atomics of the first n segments of every ray are warp-aggregated (lanes that score
+                                 into the same cell are found with match.any and one of them adds the sum): for batches born in a
+                                 region of a few cells, where same-address atomics serialise in L2.  Default 2; 0 = off */
 };
 MR_API int mr_set_option(mr_ctx *ctx, int option, int64_t value);
 MR_API int mr_get_option(mr_ctx *ctx, int option, int64_t *value);

@@ -7,6 +7,7 @@ does, and fails loudly if it has not been built.  There is no CPU fallback.
 from .binding import (  # noqa: F401
     EXPORTS,
     LIB_PATH,
+    MR_OPT_AGGREGATE_FIRST,
     MR_OPT_BLOCK_THREADS,
     MR_OPT_COPY_THREADS,
     MR_OPT_FUSED_TALLY,

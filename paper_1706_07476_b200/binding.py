@@ -24,6 +24,7 @@ MR_OPT_BLOCK_THREADS, MR_OPT_SORT_RAYS, MR_OPT_STAGE_RAYS, MR_OPT_COPY_THREADS, 
 MR_OPT_ORDER_MODE = 6
 MR_OPT_FUSED_TALLY = 7
 MR_OPT_TILED_INDEX = 8
+MR_OPT_AGGREGATE_FIRST = 9
 _STATUS = {1: "MR_ERR_INVALID_ARG", 2: "MR_ERR_STATE", 3: "MR_ERR_CUDA", 4: "MR_ERR_OOM", 5: "MR_ERR_UNSUPPORTED"}
 
 EXPORTS = [

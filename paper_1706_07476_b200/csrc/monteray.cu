@@ -171,6 +171,7 @@ struct mr_ctx {
     uint4 *d_dict = nullptr;
     uint4 *d_tiles = nullptr;
     int ndict = 0, ntx = 0, nty = 0, tile_bits = 16;
+    int agg_first = 2;               // option MR_OPT_AGGREGATE_FIRST
     int fused_opt = 2;               // option MR_OPT_FUSED_TALLY: 0 off, 1 on, 2 auto (decided by mr_load_materials)
     bool fused = false;              // LAYOUT_K4 records carry the score accumulators (LAYOUT_K4F in the cast kernel)
     bool fused_dirty = false;        // in-record sums not yet moved into d_tally
@@ -639,6 +640,7 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     P.rays = d_rays;
     if (int rc = order_rays(c, n, d_rays, &P.perm)) return rc;
     P.n = n;
+    P.agg_first = c->agg_first;
     P.tally = c->d_tally;
     P.counters = c->d_counters;
     if (c->kev_used + 2 > c->kev.size()) {
@@ -1947,6 +1949,10 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "pair-records option is 0 or 1");
         c->pair_records = (int)value;
         return MR_OK;
+    case MR_OPT_AGGREGATE_FIRST:
+        if (value < 0 || value > 1 << 20) return c->fail(MR_ERR_INVALID_ARG, "aggregate-first option is a segment count >= 0");
+        c->agg_first = (int)value;
+        return MR_OK;
     case MR_OPT_TILED_INDEX:
         if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "tiled-index option is 0 or 1");
         c->tiled_opt = (int)value;
@@ -1980,6 +1986,7 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     case MR_OPT_ORDER_MODE: *value = c->order_mode; return MR_OK;
     case MR_OPT_FUSED_TALLY: *value = c->fused_opt; return MR_OK;
     case MR_OPT_TILED_INDEX: *value = c->tiled_opt; return MR_OK;
+    case MR_OPT_AGGREGATE_FIRST: *value = c->agg_first; return MR_OK;
     }
     return c->fail(MR_ERR_INVALID_ARG, "unknown option");
 }

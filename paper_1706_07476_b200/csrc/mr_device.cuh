@@ -66,6 +66,7 @@ struct CastParams {
     const void *rays;      // 8 floats (mixed) or 8 doubles per ray
     const uint32_t *perm;  // optional processing order (ray index per work item), may be null
     long long n;
+    int agg_first;         // warp-aggregate the tally atomics of the first agg_first segments of every ray (0: never)
     double *tally;
     unsigned long long *counters;  // [0] accepted [1] rejected [2] segments
 };
@@ -712,11 +713,27 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
             double *const tally = P.tally;
             // S4 + S5 + S6 for one segment: score = W e^{-tau} (1 - e^{-x}) / Sigma, x = Sigma * len (Eq. (4));
             // a zero-length segment scores exactly 0: nothing to add
-            auto score = [&](const typename Rec::Value &cur, int cell, double len) {
+            auto score = [&](const typename Rec::Value &cur, int cell, double len, const bool aggregate) {
                 const double S = (double)Rec::sigma(cur, sig, stride, P.K);
                 double g, ex;
                 score_terms<sizeof(Real) == 8>(S, len, g, ex);
-                if (len > 0.0) red_add_f64(Rec::tally_at(tally, P.recs, cell), wa * g);
+                double v = wa * g;
+                bool add = len > 0.0;
+                // Warp-aggregated atomics for the first P.agg_first segments of a ray: rays born in one small region (a
+                // source volume of a few cells) hit the same cells in their first steps, and same-address REDs serialise
+                // in L2.  Lanes of the warp that score into the same cell are found with match.any; the lowest adds the sum.
+                if (aggregate) {
+                    const unsigned act = __activemask();
+                    const unsigned peers = __match_any_sync(act, add ? cell : -1 - (int)(threadIdx.x & 31));
+                    if (peers & (peers - 1)) {                       // somebody shares this cell
+                        const int me = threadIdx.x & 31, leader = __ffs(peers) - 1;
+                        double sum = 0.0;
+                        for (unsigned rest = peers; rest; rest &= rest - 1) sum += __shfl_sync(peers, v, __ffs(rest) - 1);
+                        v = sum;
+                        add = add && me == leader;
+                    }
+                }
+                if (add) red_add_f64(Rec::tally_at(tally, P.recs, cell), v);
                 wa *= ex;
                 ++nseg;
             };
@@ -731,7 +748,8 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
                     rec.load(P.recs, P.ids, P.K, w.c);
             };
             fetch();
-            for (;;) {
+            // one segment; returns true when the ray has left the mesh
+            auto segment = [&](const bool aggregate) {
                 int cell;
                 double len;
                 const bool leave = walker_step<EDGE_MODE>(w, axf, stride, P.mesh, e, cell, len);
@@ -739,9 +757,13 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
                 if constexpr (Rec::kTiled) cur = rec.value(s_dict);
                 else cur = rec.value();
                 if (!leave) fetch();                              // next cell's record: in flight during the score
-                score(cur, cell, len);
-                if (leave) break;
-            }
+                score(cur, cell, len, aggregate);
+                return leave;
+            };
+            // the first P.agg_first segments with warp-aggregated atomics, the rest (the hot loop) without the test
+            bool left = false;
+            for (int k = 0; k < P.agg_first && !left; ++k) left = segment(true);
+            while (!left) left = segment(false);
         }
     }
     // per-warp totals -> three global counters

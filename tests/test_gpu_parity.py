@@ -388,3 +388,27 @@ def test_tiled_mixture_index_on_off_and_fallback():
                     m.cast_rays(rays)
                     assert_tally(m.read_tally(), ref.tally, 0)
         np.testing.assert_allclose(tallies[0], tallies[1], rtol=1e-9, atol=1e-12 * ref.tally.max())
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_warp_aggregated_atomics_for_the_first_segments(precision):
+    """MR_OPT_AGGREGATE_FIRST: lanes of a warp that score into the same cell during a ray's first segments add one
+    sum instead of many atomics (config 5's shape: every ray starts in a 4 x 4 x 4-cell region).  Counters and
+    tallies are unchanged for 0, the default and a value larger than any ray."""
+    from paper_1706_07476_b200 import MR_OPT_AGGREGATE_FIRST, MonteRay
+
+    prob = make_problem(5, n=24, n_e=4000, n_res=50)
+    rays = make_rays(prob, 60_000)
+    rays[::97, 6] = -1.0                                   # rejected rays inside warps that aggregate
+    ref = _oracle(prob).cast(rays, threads=_threads())
+    with MonteRay(0, precision) as m:
+        m.load_problem(prob)
+        assert m.get_option(MR_OPT_AGGREGATE_FIRST) == 2
+        r = rays.astype(m.ray_dtype)
+        for a in (0, 2, 1000):
+            m.set_option(MR_OPT_AGGREGATE_FIRST, a)
+            m.clear_tally()
+            m.cast_rays(r)
+            st = m.get_stats()
+            assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+            assert_tally(m.read_tally(), ref.tally, precision)
