@@ -66,3 +66,18 @@ def test_product_does_not_import_oracle(repo_root):
             text = open(os.path.join(repo_root, "oracle", f)).read()
             assert "import paper_1706_07476_b200" not in text and "from paper_1706_07476_b200" not in text
             assert "monteray.h" not in text and "mr_device" not in text
+
+
+def test_option_and_limit_constants_match_the_header(repo_root):
+    """binding.py restates the MR_OPT_* / precision / location constants of monteray.h: keep them in step."""
+    import paper_1706_07476_b200.binding as b
+
+    text = open(os.path.join(repo_root, "include", "monteray.h")).read()
+    found = dict(re.findall(r"\b(MR_(?:OPT|PRECISION|WHERE)_\w+)\s*=\s*(\d+)", text))
+    assert len([k for k in found if k.startswith("MR_OPT_")]) >= 9
+    for name, value in found.items():
+        assert hasattr(b, name), f"{name} is in monteray.h but not in binding.py"
+        assert getattr(b, name) == int(value), name
+    status = dict(re.findall(r"\b(MR_(?:OK|ERR_\w+))\s*=\s*(\d+)", text))
+    for name, value in status.items():
+        assert getattr(b, name) == int(value), name
