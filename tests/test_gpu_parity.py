@@ -179,6 +179,36 @@ def test_full_size_configs_in_bench_configuration(cfg):
     assert_tally(got, ref.tally, 0)
 
 
+@pytest.mark.slow
+def test_config4_batches_0_1_99_on_the_full_mesh():
+    """BASELINE.json config 4 is 10^8 rays in 100 batches of 10^6 on the 512^3 mesh.  The oracle needs about
+    3.4e8 segments per batch on the host cores, so parity covers 3 OF THE 100 BATCHES -- the first two and the
+    last (every batch has its own seeded stream, SeedSequence([.., 4, 9, batch])) -- each against its own oracle
+    tally, then the three together (the resident tally is the running sum over batches)."""
+    import torch
+
+    prob = make_problem(4)
+    orc = _oracle(prob)
+    total = np.zeros(prob.ncell)
+    with _mr(prob, 0) as m:
+        seg = 0
+        for batch in (0, 1, 99):
+            rays = make_rays(prob, 1_000_000, batch=batch)
+            ref = orc.cast(rays, per_ray=True, threads=_threads())
+            d_rays = torch.from_numpy(rays).cuda()
+            before = m.read_tally()
+            m.cast_rays(d_rays)
+            got = m.read_tally()
+            nseg, hsh, _, _ = m.trace_rays(d_rays)
+            assert np.array_equal(nseg, ref.nseg) and np.array_equal(hsh, ref.hash), f"batch {batch}: traces differ"
+            assert_tally(got - before, ref.tally, 0)
+            total += ref.tally
+            seg += ref.segments
+        st = m.get_stats()
+        assert (st.rays_accepted, st.rays_rejected, st.segments) == (3_000_000, 0, seg)
+        assert_tally(m.read_tally(), total, 0)
+
+
 # ------------------------------------------------------------------------------------- API behaviour
 def test_host_device_and_chunked_staging_agree():
     import torch

@@ -62,10 +62,11 @@ def tiny_rays(prob, seed, n, axis_aligned_share=0.0, e_lo=5e-4, e_hi=20.0, dtype
     return np.ascontiguousarray(rays.astype(dtype))
 
 
-def tiny_rz_problem(seed, nr=5, nz=4, M=3, K=2, n_e=17, uniform=False, void=False, homogeneous=False):
+def tiny_rz_problem(seed, nr=5, nz=4, M=3, K=2, n_e=17, uniform=False, void=False, homogeneous=False, fp32_values=True):
     """A tiny R-Z problem: tiny_problem's materials and tables on nr radial shells (from r = 0) x nz axial slabs.
     Returned with nx = nr, ny = 1 (cell c = ir + nr*iz) and the extra fields re, ze, nr."""
-    prob = tiny_problem(seed, nx=nr, ny=1, nz=nz, M=M, K=K, n_e=n_e, uniform=uniform, void=void, homogeneous=homogeneous)
+    prob = tiny_problem(seed, nx=nr, ny=1, nz=nz, M=M, K=K, n_e=n_e, uniform=uniform, void=void, homogeneous=homogeneous,
+                        fp32_values=fp32_values)
     g = np.random.default_rng(seed + 1000)
     prob.re = 0.5 * np.arange(nr + 1) if uniform else np.concatenate([[0.0], np.cumsum(0.15 + 0.6 * g.random(nr))])
     prob.nr = nr
@@ -95,9 +96,10 @@ def tiny_rz_rays(prob, seed, n, axis_parallel_share=0.0, through_axis_share=0.0,
     return np.ascontiguousarray(rays.astype(dtype))
 
 
-def tiny_sphere_problem(seed, nr=6, M=3, K=2, n_e=17, uniform=False, homogeneous=False):
+def tiny_sphere_problem(seed, nr=6, M=3, K=2, n_e=17, uniform=False, homogeneous=False, fp32_values=True):
     """Tiny 1-D spherical problem: nr shells about the origin (cell c = ir); fields re, nr, sphere=True."""
-    prob = tiny_problem(seed, nx=nr, ny=1, nz=1, M=M, K=K, n_e=n_e, uniform=uniform, homogeneous=homogeneous)
+    prob = tiny_problem(seed, nx=nr, ny=1, nz=1, M=M, K=K, n_e=n_e, uniform=uniform, homogeneous=homogeneous,
+                        fp32_values=fp32_values)
     g = np.random.default_rng(seed + 2000)
     prob.re = 0.5 * np.arange(nr + 1) if uniform else np.concatenate([[0.0], np.cumsum(0.15 + 0.6 * g.random(nr))])
     prob.nr = nr

@@ -57,9 +57,14 @@ def rng_for(config: int, stream: int, batch: int = 0) -> np.random.Generator:
     )
 
 
+_ROUND_FP32 = True  # False only inside make_problem(..., double_inputs=True)
+
+
 def f32r(a) -> np.ndarray:
-    """Round to the nearest fp32 value, return as float64."""
-    return np.asarray(a, dtype=np.float64).astype(np.float32).astype(np.float64)
+    """Round to the nearest fp32 value, return as float64 (reading Q2).  Inside make_problem(double_inputs=True)
+    nothing is rounded: the all-double mode is then fed values that are NOT fp32-representable."""
+    a = np.asarray(a, dtype=np.float64)
+    return a.astype(np.float32).astype(np.float64) if _ROUND_FP32 else a.copy()
 
 
 @dataclass
@@ -256,8 +261,15 @@ def config5(n: int = 64, n_e: int = 200_000, n_res: int = 2000) -> Problem:
     return Problem(5, CONFIG_NAMES[5], n, n, n, ed.copy(), ed.copy(), ed.copy(), names, density, K, ids, frac, xs)
 
 
-def make_problem(config: int, **kw) -> Problem:
-    return {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}[config](**kw)
+def make_problem(config: int, double_inputs: bool = False, **kw) -> Problem:
+    """double_inputs=True: tables, densities and fractions keep their full double values (inputs for the all-double
+    mode only; the mixed library would round them and no longer read the oracle's numbers)."""
+    global _ROUND_FP32
+    _ROUND_FP32 = not double_inputs
+    try:
+        return {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}[config](**kw)
+    finally:
+        _ROUND_FP32 = True
 
 
 # --------------------------------------------------------------------------- rays
@@ -281,23 +293,26 @@ def _watt(g, n, a=0.988, b=2.249):
     return np.clip(e, E_LO, E_HI)
 
 
-def _pack(pos, d, e, w, lo, hi) -> np.ndarray:
-    """Round to fp32 and keep origins inside the half-open box [lo, hi) after rounding."""
-    rays = np.empty((len(e), 8), dtype=np.float32)
+def _pack(pos, d, e, w, lo, hi, dtype=np.float32) -> np.ndarray:
+    """Round to `dtype` (fp32: the mixed-mode record; fp64: nothing is rounded) and keep origins inside the
+    half-open box [lo, hi) after rounding."""
+    ft = np.dtype(dtype).type
+    rays = np.empty((len(e), 8), dtype=dtype)
     rays[:, 0:3] = pos
     for a in range(3):
-        hi32 = np.nextafter(np.float32(hi[a]), np.float32(-np.inf)) if np.float32(hi[a]) >= hi[a] else np.float32(hi[a])
-        lo32 = np.nextafter(np.float32(lo[a]), np.float32(np.inf)) if np.float32(lo[a]) < lo[a] else np.float32(lo[a])
-        rays[:, a] = np.clip(rays[:, a], lo32, hi32)
+        hi_t = np.nextafter(ft(hi[a]), ft(-np.inf)) if ft(hi[a]) >= hi[a] else ft(hi[a])
+        lo_t = np.nextafter(ft(lo[a]), ft(np.inf)) if ft(lo[a]) < lo[a] else ft(lo[a])
+        rays[:, a] = np.clip(rays[:, a], lo_t, hi_t)
     rays[:, 3:6] = d
     rays[:, 6] = e
-    rays[:, 6] = np.clip(rays[:, 6], np.float32(E_LO), np.float32(E_HI))
+    rays[:, 6] = np.clip(rays[:, 6], ft(E_LO), ft(E_HI))
     rays[:, 7] = w
     return rays
 
 
-def make_rays(prob: Problem, n: int, batch: int = 0) -> np.ndarray:
-    """float32 [n, 8] ray records for problem `prob` (shape rules per config)."""
+def make_rays(prob: Problem, n: int, batch: int = 0, dtype=np.float32) -> np.ndarray:
+    """[n, 8] ray records for problem `prob` (shape rules per config): float32 (the mixed-mode
+    record, reading Q2) or, for the all-double mode, float64 with nothing rounded."""
     c = prob.config
     g = rng_for(c, 9, batch)
     lo = (prob.xe[0], prob.ye[0], prob.ze[0])
@@ -343,7 +358,7 @@ def make_rays(prob: Problem, n: int, batch: int = 0) -> np.ndarray:
         raise ValueError(c)
     d = _isotropic(g, n)
     w = 0.5 + g.random(n)
-    return _pack(pos, d, e, w, lo, hi)
+    return _pack(pos, d, e, w, lo, hi, dtype)
 
 
 # --------------------------------------------------------------------------- multi-nuclide materials (NEXT-4)
@@ -376,7 +391,16 @@ def add_nuclides(prob, n_nuclides: int = 6, max_per_material: int = 4, keep_dire
 
 
 # --------------------------------------------------------------------------- R-Z pin-cell-like problem (NEXT-4)
-def make_rz_problem(nr: int = 256, nz: int = 512, n_e: int = 20_000):
+def make_rz_problem(nr: int = 256, nz: int = 512, n_e: int = 20_000, double_inputs: bool = False):
+    global _ROUND_FP32
+    _ROUND_FP32 = not double_inputs
+    try:
+        return _make_rz_problem(nr, nz, n_e)
+    finally:
+        _ROUND_FP32 = True
+
+
+def _make_rz_problem(nr: int, nz: int, n_e: int):
     """One fuel-pin cell seen as an R-Z mesh: UO2 to r = 0.41 cm, zircaloy to 0.475 cm, borated water out to the
     equivalent-cell radius 0.7135 cm (pitch/sqrt(pi)), 365.76 cm high; nr equal shells, nz equal slabs, K = 1.
     Stands in for the paper's wish for 2-D cylindrical meshes; inputs only."""
@@ -395,14 +419,15 @@ def make_rz_problem(nr: int = 256, nz: int = 512, n_e: int = 20_000):
                            material_names=names)
 
 
-def make_rz_rays(prob, n: int, batch: int = 0) -> np.ndarray:
-    """Rays born uniformly in the fuel (rho < 0.41 cm), isotropic, Watt energies; float32 [n, 8]."""
+def make_rz_rays(prob, n: int, batch: int = 0, dtype=np.float32) -> np.ndarray:
+    """Rays born uniformly in the fuel (rho < 0.41 cm), isotropic, Watt energies; [n, 8] float32 (or float64, unrounded)."""
     g = rng_for(3, 11, batch)
     rho = PWR_R_PELLET * np.sqrt(g.random(n))
     phi = 2.0 * np.pi * g.random(n)
     z = prob.ze[0] + g.random(n) * (prob.ze[-1] - prob.ze[0])
     pos = np.stack([rho * np.cos(phi), rho * np.sin(phi), z], axis=1)
     d = _isotropic(g, n)
-    rays = np.concatenate([pos, d, _watt(g, n)[:, None], (0.5 + g.random(n))[:, None]], axis=1).astype(np.float32)
-    rays[:, 2] = np.clip(rays[:, 2], np.float32(prob.ze[0]), np.nextafter(np.float32(prob.ze[-1]), np.float32(0)))
+    ft = np.dtype(dtype).type
+    rays = np.concatenate([pos, d, _watt(g, n)[:, None], (0.5 + g.random(n))[:, None]], axis=1).astype(dtype)
+    rays[:, 2] = np.clip(rays[:, 2], ft(prob.ze[0]), np.nextafter(ft(prob.ze[-1]), ft(0)))
     return np.ascontiguousarray(rays)
