@@ -316,9 +316,51 @@ enum {
                                  mr_load_materials also builds a dictionary of them and a 2-byte index per cell in 32-byte tiles of
                                  4 x 4 (x, y) cells, and mr_cast_rays walks those (a step inside a tile needs no load); 0: never.
                                  Setting 0 after the load makes the cast use the plain records again */
+    MR_OPT_COARSE_RECORDS = 10, /* read by mr_load_materials and mr_cast_rays.  1 (default): when every aligned block of 2^s cells per axis
+                                 (largest s in 1..5; MIXED, K <= 4, Cartesian, no dictionary path) holds ONE composition -- a material map
+                                 coarser than the tally mesh -- mr_load_materials also stores one record per BLOCK and mr_cast_rays reads
+                                 those: the table stays in L2 where per-cell records of a mesh far larger than L2 cost a DRAM line per
+                                 segment, and a step inside a block needs no load.  0: never (after the load: use the per-cell records) */
+    MR_OPT_DEFERRED_TALLY = 11, /* the two-phase tally for meshes far larger than L2 (MIXED, Cartesian; coarse-record or K = 4 record path):
+                                 phase A walks and scores but appends (cell, score) pairs to the bin of the cell's tally REGION (a range
+                                 of the linear cell index worth at most L2/8 of tally), phase B adds the pairs bin after bin, while the
+                                 region is in L2.  tally[c] receives the same scores in another order.  0 = never, 1 = whenever the
+                                 path allows, 2 (default) = coarse-record path on a mesh whose tally exceeds twice the L2 */
+    MR_OPT_DEFER_POOL_ENTRIES = 12, /* size of the deferred tally's pool in (cell, score) pairs (12 bytes each); 0 (default) = sized from the batch
+                                 (rays x (nx+ny+nz)/3, at most 24 GB; batches that need more are cast in pieces) and grown when a cast ran
+                                 out.  A pool that is too small is never an error: the pairs that do not fit are added straight to the tally */
+    MR_OPT_DEFER_REGION_SHIFT = 13, /* s: the deferred tally's regions are 2^s cells of the linear cell index (at most 64 regions: s is raised
+                                 until they cover the mesh); 0 (default) = the largest s with 8 * 2^s bytes <= L2/8 */
     MR_OPT_AGGREGATE_FIRST = 9 /* n >= 0: the tally atomics of the first n segments of every ray are warp-aggregated (lanes that score
                                  into the same cell are found with match.any and one of them adds the sum): for batches born in a
                                  region of a few cells, where same-address atomics serialise in L2.  Default 2; 0 = off */
+};
+/* Read-only facts about the resident problem, through mr_get_option (mr_set_option refuses them). */
+enum {
+    MR_INFO_RECORD_PATH = 100,     /* which cell-record path (S4) mr_cast_rays takes now: one of MR_PATH_* */
+    MR_INFO_DISTINCT_RECORDS = 101,/* size of the dictionary of distinct cell records (0: none was built) */
+    MR_INFO_COARSE_SHIFT = 102,    /* s of MR_OPT_COARSE_RECORDS (blocks of 2^s cells per axis; 0: none) */
+    MR_INFO_DEFERRED = 103,        /* 1 if mr_cast_rays uses the deferred tally now (MR_OPT_DEFERRED_TALLY) */
+    MR_INFO_DEFER_DIRECT_PAIRS = 104 /* (cell, score) pairs the deferred tally had to add directly because its pool was full */
+};
+enum {
+    MR_PATH_NONE = 0,          /* no materials loaded */
+    MR_PATH_K1 = 1,            /* MIXED, 8-byte records {r, id} */
+    MR_PATH_K2 = 2,            /* MIXED, 16-byte records, one load per cell */
+    MR_PATH_K3 = 3,
+    MR_PATH_K4 = 4,            /* MIXED, 32-byte records */
+    MR_PATH_K2_PAIRS = 5,      /* MIXED, 16-byte records fetched as 32-byte x-neighbour pairs (MR_OPT_PAIR_RECORDS) */
+    MR_PATH_K3_PAIRS = 6,
+    MR_PATH_K4_FUSED = 7,      /* MIXED, 32-byte records that also hold the cell's score accumulator (MR_OPT_FUSED_TALLY) */
+    MR_PATH_DENSE8 = 8,        /* MIXED, K = M = 8, ids implicit */
+    MR_PATH_GENERIC = 9,       /* MIXED, coefficient + id arrays */
+    MR_PATH_TILED4 = 10,       /* MIXED, dictionary + tiled index, 4-bit / 8-bit / 16-bit indices (MR_OPT_TILED_INDEX) */
+    MR_PATH_TILED8 = 11,
+    MR_PATH_TILED16 = 12,
+    MR_PATH_COARSE = 13,       /* MIXED, one record per block of cells (MR_OPT_COARSE_RECORDS) */
+    MR_PATH_DOUBLE_K3 = 14,    /* DOUBLE, K <= 3, 32-byte records */
+    MR_PATH_DOUBLE_GENERIC = 15,
+    MR_PATH_RZ = 16            /* R-Z / spherical mesh kernel (per-cell records of the layouts above) */
 };
 MR_API int mr_set_option(mr_ctx *ctx, int option, int64_t value);
 MR_API int mr_get_option(mr_ctx *ctx, int option, int64_t *value);

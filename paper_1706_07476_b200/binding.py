@@ -25,6 +25,15 @@ MR_OPT_ORDER_MODE = 6
 MR_OPT_FUSED_TALLY = 7
 MR_OPT_TILED_INDEX = 8
 MR_OPT_AGGREGATE_FIRST = 9
+MR_OPT_COARSE_RECORDS = 10
+MR_OPT_DEFERRED_TALLY = 11
+MR_OPT_DEFER_POOL_ENTRIES = 12
+MR_OPT_DEFER_REGION_SHIFT = 13
+MR_INFO_RECORD_PATH, MR_INFO_DISTINCT_RECORDS, MR_INFO_COARSE_SHIFT = 100, 101, 102
+MR_INFO_DEFERRED, MR_INFO_DEFER_DIRECT_PAIRS = 103, 104
+MR_PATH_NAMES = {0: "none", 1: "k1", 2: "k2", 3: "k3", 4: "k4", 5: "k2_pairs", 6: "k3_pairs", 7: "k4_fused", 8: "dense8",
+                 9: "generic", 10: "tiled4", 11: "tiled8", 12: "tiled16", 13: "coarse_blocks", 14: "double_k3",
+                 15: "double_generic", 16: "rz"}
 _STATUS = {1: "MR_ERR_INVALID_ARG", 2: "MR_ERR_STATE", 3: "MR_ERR_CUDA", 4: "MR_ERR_OOM", 5: "MR_ERR_UNSUPPORTED"}
 
 EXPORTS = [
@@ -433,6 +442,10 @@ class MonteRay:
         self._check(self.lib.mr_trace_next_event(self._h, n, C.c_void_p(ptr), where, det, nseg.ctypes.data,
                                                  hsh.ctypes.data, tau.ctypes.data, score.ctypes.data))
         return nseg, hsh, tau, score
+
+    def record_path(self) -> str:
+        """Name of the cell-record path mr_cast_rays takes for the resident problem (MR_INFO_RECORD_PATH)."""
+        return MR_PATH_NAMES[self.get_option(MR_INFO_RECORD_PATH)]
 
     def set_option(self, option: int, value: int):
         self._check(self.lib.mr_set_option(self._h, option, value))

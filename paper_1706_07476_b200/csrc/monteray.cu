@@ -23,6 +23,7 @@
 #define MR_PACK_MAX_SLOTS MR_MAX_SLOTS
 #include "mr_device.cuh"
 #include "mr_sort.cuh"
+#include "mr_defer.cuh"
 
 using namespace mr;
 
@@ -164,6 +165,7 @@ struct mr_ctx {
     long long sort_cap_l[2] = {0, 0}, hist_cap_l[2] = {0, 0}, blk_hist_cap_l[2] = {0, 0};
 
     int order_mode = 0;              // option MR_OPT_ORDER_MODE: 0 auto, 1 slab-major, 2 longest first
+    bool order_longest_auto = false; // set by cast_device: the deferred tally needs no slab locality, only a short tail
     // Tiled mixture index (K <= 3, MIXED, Cartesian): the distinct cell records as a small dictionary (shared memory in the
     // cast kernel) and a 2-byte index per cell stored in 4 x 4 (x, y) tiles of 32 bytes -- built by mr_load_materials when
     // the mesh has at most kDictMax distinct records (option MR_OPT_TILED_INDEX).
@@ -171,6 +173,27 @@ struct mr_ctx {
     uint4 *d_dict = nullptr;
     uint4 *d_tiles = nullptr;
     int ndict = 0, ntx = 0, nty = 0, tile_bits = 16;
+    // Block-constant compositions (MIXED, K <= 4, Cartesian): one LAYOUT_K4 record per aligned block of 2^cshift cells per axis,
+    // built by mr_load_materials when every such block holds one record (option MR_OPT_COARSE_RECORDS); cshift = 0: none
+    int coarse_opt = 1;
+    void *d_crecs = nullptr;
+    int cshift = 0, cnx = 0, cny = 0, cnz = 0;
+    // Deferred tally (mr_defer.cuh; option MR_OPT_DEFERRED_TALLY: 0 off, 1 on, 2 auto = coarse-record path on a mesh whose
+    // tally exceeds twice the L2): pool of (cell, score) chunks, per-bin chunk table and the control words
+    // ctl[0..63] bin cursors | ctl[64] chunks handed out | ctl[65] phase-A work counter | ctl[66] pairs added directly (cumulative) | ctl[67] phase-B work counter
+    int defer_opt = 2;
+    uint32_t *d_defer_cells = nullptr;
+    double *d_defer_scores = nullptr;
+    int *d_defer_table = nullptr;
+    unsigned long long *d_defer_ctl = nullptr;
+    unsigned long long *h_defer_ctl = nullptr;     // pinned: {chunks handed out, work, direct} after the last deferred cast
+    cudaEvent_t ev_defer = nullptr;
+    bool defer_pending = false;                    // h_defer_ctl is being written by the stream
+    unsigned long long defer_direct_seen = 0;
+    int defer_pool_chunks = 0, defer_max_chunks = 0;
+    double defer_entries_per_ray = 0.0;            // sizing estimate; grows when a cast ran out of pool
+    long long defer_pool_fixed = 0;                // option MR_OPT_DEFER_POOL_ENTRIES (0: sized by the estimate)
+    int defer_shift_fixed = 0;                     // option MR_OPT_DEFER_REGION_SHIFT (0: from the L2 size)
     int agg_first = 2;               // option MR_OPT_AGGREGATE_FIRST
     int fused_opt = 2;               // option MR_OPT_FUSED_TALLY: 0 off, 1 on, 2 auto (decided by mr_load_materials)
     bool fused = false;              // LAYOUT_K4 records carry the score accumulators (LAYOUT_K4F in the cast kernel)
@@ -247,9 +270,12 @@ void free_materials(mr_ctx *c)
     c->dev_free(c->d_ids);
     c->dev_free(c->d_dict);
     c->dev_free(c->d_tiles);
+    c->dev_free(c->d_crecs);
     c->d_recs = nullptr;
     c->d_ids = nullptr;
     c->d_dict = c->d_tiles = nullptr;
+    c->d_crecs = nullptr;
+    c->cshift = 0;
     c->ndict = 0;
     c->layout = 0;
     c->K = 0;
@@ -275,6 +301,20 @@ void free_tables(mr_ctx *c)
     c->dev_free(c->d_xs);
     c->d_xs = nullptr;
     c->xs_dirty = true;
+}
+
+void free_defer(mr_ctx *c)
+{
+    c->dev_free(c->d_defer_cells);
+    c->dev_free(c->d_defer_scores);
+    c->dev_free(c->d_defer_table);
+    c->dev_free(c->d_defer_ctl);
+    c->d_defer_cells = nullptr;
+    c->d_defer_scores = nullptr;
+    c->d_defer_table = nullptr;
+    c->d_defer_ctl = nullptr;
+    c->defer_pool_chunks = c->defer_max_chunks = 0;
+    c->defer_pending = false;
 }
 
 void free_stage(mr_ctx *c)
@@ -364,6 +404,87 @@ int build_tiled_index(mr_ctx *c, int M, const double *density, int K, const int3
     c->ntx = ntx;
     c->nty = nty;
     c->tile_bits = bits;
+    return MR_OK;
+}
+
+constexpr int kCoarseMaxShift = 5;        // blocks of up to 32^3 cells
+constexpr long long kCoarseMinCells = 1 << 15;
+
+// Coarse-grid records (see mr_ctx::d_crecs).  A cell whose coordinates share exactly l low zero bits (l < kCoarseMaxShift)
+// is compared with the cell whose coordinates have the low l+1 bits cleared; a difference rules out every block size
+// 2^j, j > l.  If no comparison at levels 1..s fails, every aligned 2^s block holds one composition (by induction up the
+// chain of those parents).  Compared are the caller's (material, fraction) slots, bit for bit.
+int build_coarse_records(mr_ctx *c, const double *density, int K, const int32_t *cell_mat, const double *cell_frac)
+{
+    c->cshift = 0;
+    if (!c->coarse_opt || c->precision != MR_PRECISION_MIXED || K > 4 || c->mesh_rz || c->ncell < kCoarseMinCells) return MR_OK;
+    const int nx = c->nx, ny = c->ny, nz = c->nz;
+    std::atomic<int> fail_mask{0};           // bit j: some 2^j block is not constant
+    auto same = [&](long long a, long long b) {
+        for (int k = 0; k < K; ++k) {
+            const int ma = cell_mat[a * K + k], mb = cell_mat[b * K + k];
+            if (ma != mb) return false;
+            if (ma >= 0 && std::memcmp(&cell_frac[a * K + k], &cell_frac[b * K + k], 8) != 0) return false;
+        }
+        return true;
+    };
+    auto scan = [&](int z0, int z1) {
+        int local = 0;
+        for (int iz = z0; iz < z1; ++iz) {
+            if (fail_mask.load(std::memory_order_relaxed) & 2) return;      // not even 2^3-cell blocks: give up
+            for (int iy = 0; iy < ny; ++iy)
+                for (int ix = 0; ix < nx; ++ix) {
+                    const unsigned bits = (unsigned)(ix | iy | iz) | (1u << kCoarseMaxShift);
+                    const int l = __builtin_ctz(bits);
+                    if (l >= kCoarseMaxShift || (local >> (l + 1)) & 1) continue;
+                    const int m = ~((2 << l) - 1);
+                    const long long me = ix + (long long)nx * (iy + (long long)ny * iz);
+                    const long long pa = (ix & m) + (long long)nx * ((iy & m) + (long long)ny * (iz & m));
+                    if (!same(me, pa)) {
+                        local |= 1 << (l + 1);
+                        fail_mask.fetch_or(1 << (l + 1), std::memory_order_relaxed);
+                    }
+                }
+        }
+    };
+    {
+        const int T = (int)std::max(1u, std::min(16u, std::min(std::thread::hardware_concurrency(), (unsigned)nz)));
+        std::vector<std::thread> pool;
+        for (int t = 1; t < T; ++t) pool.emplace_back(scan, (int)((long long)nz * t / T), (int)((long long)nz * (t + 1) / T));
+        scan(0, (int)((long long)nz / T));
+        for (std::thread &th : pool) th.join();
+    }
+    int s = 0;
+    while (s < kCoarseMaxShift && !((fail_mask.load() >> (s + 1)) & 1)) ++s;
+    if (s == 0) return MR_OK;
+    const int cnx = (nx + (1 << s) - 1) >> s, cny = (ny + (1 << s) - 1) >> s, cnz = (nz + (1 << s) - 1) >> s;
+    std::vector<uint32_t> recs((size_t)cnx * cny * cnz * 8, 0u);
+    for (int bz = 0; bz < cnz; ++bz)
+        for (int by = 0; by < cny; ++by)
+            for (int bx = 0; bx < cnx; ++bx) {
+                const long long cell = ((long long)bx << s) + (long long)nx * (((long long)by << s) + (long long)ny * ((long long)bz << s));
+                uint32_t *r = &recs[((size_t)bx + (size_t)cnx * ((size_t)by + (size_t)cny * bz)) * 8];
+                for (int k = 0; k < K; ++k) {
+                    const int m = cell_mat[cell * K + k];
+                    if (m < 0) continue;                              // empty slot: r = 0, id = 0
+                    const float v = (float)(cell_frac[cell * K + k] * density[m]);
+                    std::memcpy(&r[k], &v, 4);
+                    r[4] |= (uint32_t)m << (8 * k);
+                }
+            }
+    void *d = c->dev_alloc(recs.size() * 4);
+    if (!d) return c->fail(MR_ERR_OOM, "device allocation failed (coarse cell records)");
+    cudaError_t e = cudaMemcpyAsync(d, recs.data(), recs.size() * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) {
+        c->dev_free(d);
+        return c->fail_cuda(e, "mr_load_materials (coarse records)");
+    }
+    c->d_crecs = d;
+    c->cshift = s;
+    c->cnx = cnx;
+    c->cny = cny;
+    c->cnz = cnz;
     return MR_OK;
 }
 
@@ -543,7 +664,7 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
     }
     SortParams S{mesh_dev(c), d_rays, n, c->precision == MR_PRECISION_DOUBLE ? 1 : 0,
                  zdiv, lshift, nlen, nkeys, d_keys, d_hist, d_perm, nsec > 0 ? c->d_det : nullptr, det_first,
-                 c->order_mode == 2 || (c->order_mode == 0 && c->resident_bytes() <= c->l2_bytes / 2) ? 1 : 0, nslab,
+                 c->order_mode == 2 || (c->order_mode == 0 && (c->resident_bytes() <= c->l2_bytes / 2 || c->order_longest_auto)) ? 1 : 0, nslab,
                  c->mesh_arith ? 1 : 0, 0, nullptr};
     const size_t smem = edges_smem_bytes(c);
     // Block-local variant: every CTA counts its own contiguous share of the rays in shared memory, so neither pass
@@ -623,6 +744,173 @@ int launch_rz_cast(mr_ctx *c, const CastParams &P)
     }
 }
 
+// ---- deferred tally (mr_defer.cuh) ----------------------------------------------------------------
+constexpr int kDeferCtlWords = 72;
+
+bool use_deferred(const mr_ctx *c, int path)
+{
+    if (c->precision != MR_PRECISION_MIXED || c->mesh_rz) return false;
+    if (path != MR_PATH_COARSE && path != MR_PATH_K4) return false;
+    if (c->defer_opt == 1) return true;
+    return c->defer_opt == 2 && path == MR_PATH_COARSE && (size_t)c->ncell * 8 > 2 * c->l2_bytes;
+}
+
+// region size: at most an eighth of the L2 of tally per bin, at most kDeferBins bins
+void defer_geometry(const mr_ctx *c, int *shift, int *nbin)
+{
+    int s = 10;
+    while (((size_t)8 << (s + 1)) <= std::max<size_t>(c->l2_bytes / 8, (size_t)1 << 13)) ++s;
+    if (c->defer_shift_fixed > 0) s = c->defer_shift_fixed;
+    while (((c->ncell + (1LL << s) - 1) >> s) > kDeferBins) ++s;
+    *shift = s;
+    *nbin = (int)((c->ncell + (1LL << s) - 1) >> s);
+}
+
+// (Re)allocates the pool for `entries` (cell, score) pairs.  The stream must be idle.
+int ensure_defer_pool(mr_ctx *c, long long entries)
+{
+    const long long max_chunks_total = (1LL << 20) - 1;                       // pool indices are 32-bit
+    int shift, nbin;
+    defer_geometry(c, &shift, &nbin);
+    long long chunks = (entries + kDeferChunk - 1) / kDeferChunk;
+    if (c->defer_pool_fixed == 0) {
+        // every resident warp may hold one partly filled range per bin (padded when the warp drains)
+        int sms = 148;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+        chunks += ((long long)sms * 32 * nbin * kDeferRange + kDeferChunk - 1) / kDeferChunk + nbin;
+    }
+    chunks = std::max<long long>(1, std::min(max_chunks_total, chunks));
+    if (c->defer_pool_fixed == 0 ? chunks <= c->defer_pool_chunks : (chunks == c->defer_pool_chunks && c->d_defer_table)) return MR_OK;
+    MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    free_defer(c);
+    if (!c->h_defer_ctl) {
+        MR_CUDA(c, cudaMallocHost((void **)&c->h_defer_ctl, 4 * sizeof(unsigned long long)));
+        std::memset(c->h_defer_ctl, 0, 4 * sizeof(unsigned long long));
+        MR_CUDA(c, cudaEventCreateWithFlags(&c->ev_defer, cudaEventDisableTiming));
+    }
+    const long long per_bin = std::min(chunks, 4 * chunks / std::max(nbin, 1) + 64);   // a bin may hold 4x its share
+    c->d_defer_cells = (uint32_t *)c->dev_alloc((size_t)chunks * kDeferChunk * 4);
+    c->d_defer_scores = (double *)c->dev_alloc((size_t)chunks * kDeferChunk * 8);
+    c->d_defer_table = (int *)c->dev_alloc((size_t)nbin * per_bin * 4);
+    c->d_defer_ctl = (unsigned long long *)c->dev_alloc(kDeferCtlWords * 8);
+    if (!c->d_defer_cells || !c->d_defer_scores || !c->d_defer_table || !c->d_defer_ctl) {
+        free_defer(c);
+        return c->fail(MR_ERR_OOM, "device allocation failed (deferred-tally pool)");
+    }
+    MR_CUDA(c, cudaMemsetAsync(c->d_defer_ctl, 0, kDeferCtlWords * 8, c->stream));
+    c->defer_pool_chunks = (int)chunks;
+    c->defer_max_chunks = (int)per_bin;
+    c->defer_direct_seen = 0;
+    return MR_OK;
+}
+
+template <typename Rec, int MODE>
+int launch_defer_m(mr_ctx *c, const CastParams &P, const DeferParams &D, size_t smem)
+{
+    const int block = 128;
+    if (int rc = set_smem(c, cast_defer_kernel<Rec, MODE>, smem)) return rc;
+    int sms = 148, per_sm = 1;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    MR_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cast_defer_kernel<Rec, MODE>, block, smem));
+    const long long grid = std::max<long long>(1, std::min<long long>((P.n + block - 1) / block, (long long)sms * std::max(per_sm, 1)));
+    cast_defer_kernel<Rec, MODE><<<(unsigned)grid, block, smem, c->work_stream()>>>(P, D);
+    c->launches += 1;
+    MR_CUDA(c, cudaGetLastError());
+    return MR_OK;
+}
+
+// The cast of P.n rays with the deferred tally: phase A (walk + score, pairs binned by tally region), phase B (bin
+// after bin into the tally), in sub-batches sized to the pool.
+template <typename Rec>
+int cast_deferred(mr_ctx *c, CastParams P)
+{
+    cudaStream_t ws = c->work_stream();
+    // did the previous deferred cast run out of pool?  (looked at without waiting)
+    if (c->defer_pending && cudaEventQuery(c->ev_defer) == cudaSuccess) {
+        c->defer_pending = false;
+        if (c->h_defer_ctl[2] > c->defer_direct_seen) {
+            c->defer_direct_seen = c->h_defer_ctl[2];
+            c->defer_entries_per_ray *= 1.5;
+        }
+    } else
+        cudaGetLastError();
+    if (c->defer_entries_per_ray <= 0.0) c->defer_entries_per_ray = (double)(c->nx + c->ny + c->nz) / 3.0 + 8.0;
+    const long long pool_cap_entries = (long long)((24ULL << 30) / 12);
+    const long long want = c->defer_pool_fixed > 0 ? c->defer_pool_fixed
+                         : std::max<long long>(1 << 20, std::min<long long>(pool_cap_entries, (long long)((double)P.n * c->defer_entries_per_ray)));
+    if (int rc = ensure_defer_pool(c, want)) return rc;
+    const long long pool_entries = std::max<long long>(kDeferChunk, std::min<long long>(want, (long long)c->defer_pool_chunks * kDeferChunk));
+    const long long sub = std::max<long long>(1024, (long long)((double)pool_entries / c->defer_entries_per_ray));
+
+    DeferParams D{};
+    defer_geometry(c, &D.bin_shift, &D.nbin);
+    D.max_chunks = c->defer_max_chunks;
+    D.pool_chunks = c->defer_pool_chunks;
+    D.cells = c->d_defer_cells;
+    D.scores = c->d_defer_scores;
+    D.table = c->d_defer_table;
+    D.cursor = c->d_defer_ctl;
+    D.pool_next = reinterpret_cast<unsigned int *>(c->d_defer_ctl + 64);
+    D.work = c->d_defer_ctl + 65;
+    D.direct = c->d_defer_ctl + 66;
+    D.queue = reinterpret_cast<unsigned int *>(c->d_defer_ctl + 67);
+
+    const int block = 128;
+    const size_t per_block = walker_smem_bytes(block) + (((size_t)(c->M + c->N) * block * sizeof(float) + 15) & ~(size_t)15) +
+                             (size_t)(block / 32) * defer_warp_smem_bytes(D.nbin);
+    const int mode = edge_mode(c, per_block);
+    const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
+    if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "deferred tally: materials and bins exceed shared memory");
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    const long long n_all = P.n;
+    const char *rays0 = (const char *)P.rays;
+    const uint32_t *perm0 = P.perm;
+    for (long long first = 0; first < n_all; first += sub) {
+        P.n = std::min(sub, n_all - first);
+        if (perm0) P.perm = perm0 + first;
+        else P.rays = rays0 + (size_t)first * c->ray_bytes();
+        MR_CUDA(c, cudaMemsetAsync(c->d_defer_ctl, 0, 66 * 8, ws));
+        MR_CUDA(c, cudaMemsetAsync(c->d_defer_ctl + 67, 0, 8, ws));
+        MR_CUDA(c, cudaMemsetAsync(c->d_defer_table, 0xff, (size_t)D.nbin * D.max_chunks * 4, ws));
+        int rc;
+        switch (mode) {
+        case EDGES_ARITH: rc = launch_defer_m<Rec, EDGES_ARITH>(c, P, D, smem); break;
+        case EDGES_SHARED: rc = launch_defer_m<Rec, EDGES_SHARED>(c, P, D, smem); break;
+        default: rc = launch_defer_m<Rec, EDGES_GLOBAL>(c, P, D, smem);
+        }
+        if (rc) return rc;
+        defer_scatter_kernel<<<(unsigned)(sms * 8), 256, 0, ws>>>(D, c->d_tally);
+        c->launches += 1;
+        MR_CUDA(c, cudaGetLastError());
+    }
+    if (!c->defer_pending && !c->ring) {     // (a producer ring ships from other threads: leave the feedback to the next plain call)
+        MR_CUDA(c, cudaMemcpyAsync(c->h_defer_ctl, c->d_defer_ctl + 64, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ws));
+        MR_CUDA(c, cudaEventRecord(c->ev_defer, ws));
+        c->defer_pending = true;
+    }
+    return MR_OK;
+}
+
+// Which cell-record path mr_cast_rays takes for the resident problem (MR_INFO_RECORD_PATH).
+int record_path(const mr_ctx *c)
+{
+    if (!c->d_recs) return MR_PATH_NONE;
+    if (c->mesh_rz) return MR_PATH_RZ;
+    if (c->precision == MR_PRECISION_DOUBLE) return c->layout == LAYOUT_DK3 ? MR_PATH_DOUBLE_K3 : MR_PATH_DOUBLE_GENERIC;
+    if (c->ndict > 0 && c->tiled_opt && c->layout >= LAYOUT_K1 && c->layout <= LAYOUT_K3)
+        return c->tile_bits == 4 ? MR_PATH_TILED4 : (c->tile_bits == 8 ? MR_PATH_TILED8 : MR_PATH_TILED16);
+    if (c->cshift > 0 && c->coarse_opt && c->layout >= LAYOUT_K1 && c->layout <= LAYOUT_K4) return MR_PATH_COARSE;
+    switch (c->layout) {
+    case LAYOUT_K1: return MR_PATH_K1;
+    case LAYOUT_K2: return c->pair_records ? MR_PATH_K2_PAIRS : MR_PATH_K2;
+    case LAYOUT_K3: return c->pair_records ? MR_PATH_K3_PAIRS : MR_PATH_K3;
+    case LAYOUT_K4: return (c->fused && c->defer_opt != 1) ? MR_PATH_K4_FUSED : MR_PATH_K4;
+    case LAYOUT_D8: return MR_PATH_DENSE8;
+    default: return MR_PATH_GENERIC;
+    }
+}
+
 // Queue the cast of n device-resident rays on the context's stream.
 int cast_device(mr_ctx *c, long long n, const void *d_rays)
 {
@@ -638,7 +926,10 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     P.mix_nuc = c->d_mix_nuc;
     P.mix_w = c->d_mix_w;
     P.rays = d_rays;
-    if (int rc = order_rays(c, n, d_rays, &P.perm)) return rc;
+    c->order_longest_auto = use_deferred(c, record_path(c));
+    const int rc_order = order_rays(c, n, d_rays, &P.perm);
+    c->order_longest_auto = false;
+    if (rc_order) return rc_order;
     P.n = n;
     P.agg_first = c->agg_first;
     P.tally = c->d_tally;
@@ -652,10 +943,11 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     }
     MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->work_stream()));
     int rc;
-    if (c->mesh_rz) rc = launch_rz_cast(c, P);
-    else if (c->precision == MR_PRECISION_DOUBLE)
-        rc = c->layout == LAYOUT_DK3 ? launch_cast_t<double, CellRec<LAYOUT_DK3>>(c, P) : launch_cast_t<double, CellRecGeneric<double>>(c, P);
-    else if (c->ndict > 0 && c->tiled_opt && c->layout >= LAYOUT_K1 && c->layout <= LAYOUT_K3) {
+    switch (record_path(c)) {
+    case MR_PATH_RZ: rc = launch_rz_cast(c, P); break;
+    case MR_PATH_DOUBLE_K3: rc = launch_cast_t<double, CellRec<LAYOUT_DK3>>(c, P); break;
+    case MR_PATH_DOUBLE_GENERIC: rc = launch_cast_t<double, CellRecGeneric<double>>(c, P); break;
+    case MR_PATH_TILED4: case MR_PATH_TILED8: case MR_PATH_TILED16:
         P.dict = c->d_dict;
         P.tiles = c->d_tiles;
         P.ndict = c->ndict;
@@ -663,15 +955,24 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
         P.nty = c->nty;
         rc = c->tile_bits == 4 ? launch_cast_t<float, TiledRec<4>>(c, P)
            : c->tile_bits == 8 ? launch_cast_t<float, TiledRec<8>>(c, P) : launch_cast_t<float, TiledRec<16>>(c, P);
-    } else switch (c->layout) {
-    case LAYOUT_K1: rc = launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P); break;
-    case LAYOUT_K2: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
-    case LAYOUT_K3: rc = c->pair_records ? launch_cast_t<float, CellRec<LAYOUT_K3P>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P); break;
-    case LAYOUT_K4:
-        if (c->fused) { rc = launch_cast_t<float, CellRec<LAYOUT_K4F>>(c, P); c->fused_dirty = true; }
-        else rc = launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P);
         break;
-    case LAYOUT_D8: rc = launch_cast_t<float, CellRec<LAYOUT_D8>>(c, P); break;
+    case MR_PATH_COARSE:
+        P.crecs = c->d_crecs;
+        P.cshift = c->cshift;
+        P.cnx = c->cnx;
+        P.cny = c->cny;
+        rc = use_deferred(c, MR_PATH_COARSE) ? cast_deferred<CellRec<LAYOUT_C4>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_C4>>(c, P);
+        break;
+    case MR_PATH_K1: rc = launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P); break;
+    case MR_PATH_K2: rc = launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
+    case MR_PATH_K3: rc = launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P); break;
+    case MR_PATH_K2_PAIRS: rc = launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P); break;
+    case MR_PATH_K3_PAIRS: rc = launch_cast_t<float, CellRec<LAYOUT_K3P>>(c, P); break;
+    case MR_PATH_K4_FUSED: rc = launch_cast_t<float, CellRec<LAYOUT_K4F>>(c, P); c->fused_dirty = true; break;
+    case MR_PATH_K4:
+        rc = use_deferred(c, MR_PATH_K4) ? cast_deferred<CellRec<LAYOUT_K4>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P);
+        break;
+    case MR_PATH_DENSE8: rc = launch_cast_t<float, CellRec<LAYOUT_D8>>(c, P); break;
     default: rc = launch_cast_t<float, CellRecGeneric<float>>(c, P);
     }
     if (rc) return rc;
@@ -825,6 +1126,9 @@ int mr_destroy(mr_ctx *c)
     c->dev_free(c->d_edges);
     c->dev_free(c->d_tally);
     c->dev_free(c->d_counters);
+    free_defer(c);
+    if (c->h_defer_ctl) cudaFreeHost(c->h_defer_ctl);
+    if (c->ev_defer) cudaEventDestroy(c->ev_defer);
     c->dev_free(c->d_prev);
     c->dev_free(c->d_s2);
     c->dev_free(c->d_det);
@@ -1029,6 +1333,10 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
     c->fused_dirty = false;
     c->K = K;
     if (int rc = build_tiled_index(c, M, density, K, cell_mat, cell_frac)) return rc;
+    if (c->ndict == 0) {
+        if (int rc = build_coarse_records(c, density, K, cell_mat, cell_frac)) return rc;
+    }
+    if (c->cshift > 0) c->fused = false;     // the records are no longer per cell: nowhere to keep a per-cell accumulator
     if (M != c->M || (int)c->xs_n.size() != M) {
         c->M = M;
         c->mix.assign(M, {});
@@ -1969,6 +2277,29 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         if (value < 1 || value > 64) return c->fail(MR_ERR_INVALID_ARG, "copy threads must be in [1, 64]");
         c->copy_threads = (int)value;
         return MR_OK;
+    case MR_OPT_COARSE_RECORDS:
+        if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "coarse-records option is 0 or 1");
+        c->coarse_opt = (int)value;
+        return MR_OK;
+    case MR_OPT_DEFER_POOL_ENTRIES:
+        if (value < 0 || value > (1LL << 32)) return c->fail(MR_ERR_INVALID_ARG, "deferred-tally pool size is 0 (auto) or a number of pairs up to 2^32");
+        MR_CUDA(c, cudaStreamSynchronize(c->stream));
+        free_defer(c);
+        c->defer_pool_fixed = value;
+        return MR_OK;
+    case MR_OPT_DEFER_REGION_SHIFT:
+        if (value != 0 && (value < 8 || value > 30)) return c->fail(MR_ERR_INVALID_ARG, "deferred-tally region shift is 0 (auto) or in [8, 30]");
+        MR_CUDA(c, cudaStreamSynchronize(c->stream));
+        free_defer(c);
+        c->defer_shift_fixed = (int)value;
+        return MR_OK;
+    case MR_OPT_DEFERRED_TALLY:
+        if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "deferred-tally option is 0 (off), 1 (on) or 2 (auto)");
+        if (value == 1 && c->fused && c->fused_dirty) {
+            MR_CUDA(c, flush_fused(c));
+        }
+        c->defer_opt = (int)value;
+        return MR_OK;
     }
     return c->fail(MR_ERR_INVALID_ARG, "unknown option");
 }
@@ -1987,6 +2318,23 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     case MR_OPT_FUSED_TALLY: *value = c->fused_opt; return MR_OK;
     case MR_OPT_TILED_INDEX: *value = c->tiled_opt; return MR_OK;
     case MR_OPT_AGGREGATE_FIRST: *value = c->agg_first; return MR_OK;
+    case MR_OPT_COARSE_RECORDS: *value = c->coarse_opt; return MR_OK;
+    case MR_INFO_RECORD_PATH: *value = record_path(c); return MR_OK;
+    case MR_INFO_DISTINCT_RECORDS: *value = c->ndict; return MR_OK;
+    case MR_INFO_COARSE_SHIFT: *value = c->cshift; return MR_OK;
+    case MR_OPT_DEFERRED_TALLY: *value = c->defer_opt; return MR_OK;
+    case MR_OPT_DEFER_POOL_ENTRIES: *value = c->defer_pool_fixed; return MR_OK;
+    case MR_OPT_DEFER_REGION_SHIFT: *value = c->defer_shift_fixed; return MR_OK;
+    case MR_INFO_DEFERRED: *value = use_deferred(c, record_path(c)) ? 1 : 0; return MR_OK;
+    case MR_INFO_DEFER_DIRECT_PAIRS: {
+        unsigned long long v = 0;
+        if (c->d_defer_ctl) {
+            MR_CUDA(c, cudaMemcpyAsync(&v, c->d_defer_ctl + 66, 8, cudaMemcpyDeviceToHost, c->stream));
+            MR_CUDA(c, cudaStreamSynchronize(c->stream));
+        }
+        *value = (int64_t)v;
+        return MR_OK;
+    }
     }
     return c->fail(MR_ERR_INVALID_ARG, "unknown option");
 }

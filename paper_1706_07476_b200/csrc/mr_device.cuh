@@ -35,6 +35,7 @@ enum CellLayout : int {
     LAYOUT_K4F = 14,       // kernel-side only: LAYOUT_K4 record whose 8 spare bytes (offset 24) hold the cell's score accumulator
     LAYOUT_K2P = 12,       // kernel-side only: LAYOUT_K2 / LAYOUT_K3 records fetched as 32-byte pairs
     LAYOUT_K3P = 13,
+    LAYOUT_C4 = 16,        // kernel-side only: block-constant compositions -- LAYOUT_K4 records on a coarse grid of 2^s-cell blocks
     LAYOUT_GENERIC = 100   // coef[ncell*K] (float or double) + ids[ncell*K] (u8, 0xff = empty)
 };
 
@@ -57,6 +58,8 @@ struct CastParams {
     const uint4 *dict;     // LAYOUT_T3: the distinct records (K = 3 encoding), ndict of them
     const uint4 *tiles;    // LAYOUT_T3: 32-byte tiles of 4 x 4 (x, y) 2-byte dictionary indices, ntx * nty * nz of them
     int ndict, ntx, nty;
+    const void *crecs;     // LAYOUT_C4: one LAYOUT_K4 record per block of 2^cshift cells per axis, cnx * cny * cnz of them
+    int cshift, cnx, cny;
     int K, M;
     const XsDesc *xs;      // [M + N]: materials (n = 0: a nuclide mixture), then nuclides
     int N;                 // nuclide descriptors (0: every material has a table of its own)
@@ -388,6 +391,7 @@ template <int LAYOUT> struct CellRec;
 // where a cell's score goes: the contiguous fp64 tally, unless the record type keeps the accumulator inside the record
 struct PlainTally {
     static constexpr bool kTiled = false;
+    static constexpr bool kCoarse = false;
     static __device__ __forceinline__ double *tally_at(double *tally, const void *, int cell) { return tally + cell; }
 };
 
@@ -513,6 +517,7 @@ template <int BITS> struct TiledRec : PlainTally {
 
 template <> struct CellRec<LAYOUT_K4F> {
     static constexpr bool kTiled = false;
+    static constexpr bool kCoarse = false;
     struct Value { uint4 v; uint32_t ids; };
     Value q;
     __device__ __forceinline__ void reset() {}
@@ -538,6 +543,38 @@ template <> struct CellRec<LAYOUT_K4F> {
         return reinterpret_cast<double *>(reinterpret_cast<uintptr_t>(recs) + 32 * (size_t)cell + 24);
     }
 };
+// Block-constant compositions (a material map coarser than the tally mesh: the usual case when a fine tally mesh is
+// laid over a geometry of larger bodies; config 4 assigns materials in 8^3-cell blocks): mr_load_materials finds the
+// largest s such that every aligned block of 2^s cells per axis holds ONE record, and stores one LAYOUT_K4 record per
+// block.  On a mesh far larger than L2 the per-cell records (4.3 GB at 512^3) cost a DRAM line per segment; the
+// coarse table (8 MB at s = 3) stays in L2, and a step that stays inside the block needs no load at all.
+template <> struct CellRec<LAYOUT_C4> : PlainTally {
+    static constexpr bool kCoarse = true;
+    struct Value { uint4 v; uint32_t ids; };
+    Value q;
+    int tag;       // resident block, -1: none
+    __device__ __forceinline__ void reset() { tag = -1; }
+    __device__ __forceinline__ void load_coarse(const void *crecs, int s, int cnx, int cny, int ix, int iy, int iz)
+    {
+        const int b = (ix >> s) + cnx * ((iy >> s) + cny * (iz >> s));
+        if (b != tag) {
+            tag = b;
+            uint4 lo, hi;
+            ldg_256(reinterpret_cast<const uint4 *>(crecs) + 2 * (size_t)b, lo, hi);
+            q.v = lo;
+            q.ids = hi.x;
+        }
+    }
+    __device__ __forceinline__ Value value() const { return q; }
+    static __device__ __forceinline__ float sigma(const Value &q, const float *sig, int stride, int)
+    {
+        float s = __uint_as_float(q.v.x) * sig[(q.ids & 0xffu) * stride];
+        s = fmaf(__uint_as_float(q.v.y), sig[((q.ids >> 8) & 0xffu) * stride], s);
+        s = fmaf(__uint_as_float(q.v.z), sig[((q.ids >> 16) & 0xffu) * stride], s);
+        return fmaf(__uint_as_float(q.v.w), sig[(q.ids >> 24) * stride], s);
+    }
+};
+
 template <> struct CellRec<LAYOUT_D8> : PlainTally {
     struct Value { float4 a, b; };
     Value q;
@@ -744,6 +781,9 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
                 if constexpr (Rec::kTiled)
                     rec.load_tiled(P.tiles, P.ntx, P.nty, walker_cell_index(w.pl0, w.dc0), walker_cell_index(w.pl1, w.dc1),
                                    walker_cell_index(w.pl2, w.dc2));
+                else if constexpr (Rec::kCoarse)
+                    rec.load_coarse(P.crecs, P.cshift, P.cnx, P.cny, walker_cell_index(w.pl0, w.dc0),
+                                    walker_cell_index(w.pl1, w.dc1), walker_cell_index(w.pl2, w.dc2));
                 else
                     rec.load(P.recs, P.ids, P.K, w.c);
             };

@@ -73,8 +73,10 @@ def test_option_and_limit_constants_match_the_header(repo_root):
     import paper_1706_07476_b200.binding as b
 
     text = open(os.path.join(repo_root, "include", "monteray.h")).read()
-    found = dict(re.findall(r"\b(MR_(?:OPT|PRECISION|WHERE)_\w+)\s*=\s*(\d+)", text))
-    assert len([k for k in found if k.startswith("MR_OPT_")]) >= 9
+    found = dict(re.findall(r"\b(MR_(?:OPT|INFO|PRECISION|WHERE)_\w+)\s*=\s*(\d+)", text))
+    assert len([k for k in found if k.startswith("MR_OPT_")]) >= 10
+    paths = dict(re.findall(r"\b(MR_PATH_\w+)\s*=\s*(\d+)", text))
+    assert sorted(int(v) for v in paths.values()) == sorted(b.MR_PATH_NAMES), "MR_PATH_* and binding.MR_PATH_NAMES differ"
     for name, value in found.items():
         assert hasattr(b, name), f"{name} is in monteray.h but not in binding.py"
         assert getattr(b, name) == int(value), name

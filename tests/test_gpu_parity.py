@@ -420,6 +420,116 @@ def test_tiled_mixture_index_on_off_and_fallback():
         np.testing.assert_allclose(tallies[0], tallies[1], rtol=1e-9, atol=1e-12 * ref.tally.max())
 
 
+def test_coarse_block_records_on_off_and_detection():
+    """MR_OPT_COARSE_RECORDS: compositions constant on aligned 2^s-cell blocks are read from one record per block.
+    Same counters and tallies (within tolerance of the oracle) with the option on and off; mesh sides that are not
+    multiples of the block; the block size found is the largest that holds; one odd cell anywhere lowers it."""
+    from paper_1706_07476_b200 import MR_INFO_COARSE_SHIFT, MR_OPT_COARSE_RECORDS, MR_OPT_TILED_INDEX, MonteRay
+
+    def blocky(seed, dims, block, K, M=5):
+        prob = tiny_problem(seed, nx=dims[0], ny=dims[1], nz=dims[2], M=M, K=K, n_e=33)
+        ix, iy, iz = np.meshgrid(np.arange(dims[0]), np.arange(dims[1]), np.arange(dims[2]), indexing="ij")
+        rep = ((ix // block) * block + dims[0] * ((iy // block) * block + dims[1] * ((iz // block) * block)))
+        rep = rep.transpose(2, 1, 0).reshape(-1)              # cell order: x fastest
+        prob.cell_mat[:] = prob.cell_mat[rep]
+        prob.cell_frac[:] = prob.cell_frac[rep]
+        return prob
+
+    cases = [(611, (40, 36, 32), 8, 4, 3), (612, (37, 41, 29), 4, 3, 2), (613, (64, 32, 16), 2, 1, 1), (614, (33, 33, 33), 16, 4, 4)]
+    for seed, dims, block, K, want_shift in cases:
+        prob = blocky(seed, dims, block, K)
+        rays = tiny_rays(prob, seed, 30_000, axis_aligned_share=0.05)
+        ref = _oracle(prob).cast(rays, threads=_threads())
+        for coarse in (1, 0):
+            with MonteRay(0, 0) as m:
+                m.set_option(MR_OPT_COARSE_RECORDS, coarse)
+                m.set_option(MR_OPT_TILED_INDEX, 0)            # else few distinct records would take the dictionary path
+                m.load_problem(prob)
+                assert m.get_option(MR_INFO_COARSE_SHIFT) == (want_shift if coarse else 0)
+                assert (m.record_path() == "coarse_blocks") == bool(coarse)
+                m.cast_rays(rays)
+                st = m.get_stats()
+                assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+                assert_tally(m.read_tally(), ref.tally, 0)
+                if coarse:                                     # option off after the load: back to the per-cell records
+                    m.set_option(MR_OPT_COARSE_RECORDS, 0)
+                    assert m.record_path() != "coarse_blocks"
+                    m.clear_tally()
+                    m.cast_rays(rays)
+                    assert_tally(m.read_tally(), ref.tally, 0)
+    # one odd cell inside an 8-block: blocks of 8 and 4 no longer hold, blocks of 2 still do unless the cell sits in one
+    prob = blocky(615, (40, 40, 32), 8, 4)
+    c = 5 + 40 * (6 + 40 * 7)
+    prob.cell_mat[c, 0] = (max(prob.cell_mat[c, 0], 0) + 1) % 5      # another material in slot 0 of that one cell
+    with MonteRay(0, 0) as m:
+        m.load_problem(prob)
+        assert m.get_option(MR_INFO_COARSE_SHIFT) == 0
+        rays = tiny_rays(prob, 615, 20_000)
+        m.cast_rays(rays)
+        assert_tally(m.read_tally(), _oracle(prob).cast(rays, threads=_threads()).tally, 0)
+
+
+@pytest.mark.parametrize("coarse", [1, 0])
+def test_deferred_tally_on_off_small_pool_and_pieces(coarse):
+    """MR_OPT_DEFERRED_TALLY: phase A bins (cell, score) pairs by tally region, phase B adds them bin after bin.  Forced
+    on a small mesh (auto needs a tally beyond twice the L2): same counters, tally within tolerance of the oracle, on
+    the coarse-record and on the K = 4 record path; rejected rays, ragged batch sizes, a batch smaller than a warp; a
+    pool far too small (most pairs take the direct path, counted by MR_INFO_DEFER_DIRECT_PAIRS) and a pool that makes
+    the library cast the batch in several pieces; moments and the producer ring on top."""
+    from paper_1706_07476_b200 import (MR_INFO_DEFER_DIRECT_PAIRS, MR_INFO_DEFERRED, MR_OPT_COARSE_RECORDS,
+                                       MR_OPT_DEFER_POOL_ENTRIES, MR_OPT_DEFER_REGION_SHIFT, MR_OPT_DEFERRED_TALLY,
+                                       MonteRay)
+
+    prob = make_problem(4, n=64, n_e=3000)
+    rays = make_rays(prob, 60_013)
+    rays[::997, 6] = -1.0
+    ref = _oracle(prob).cast(rays, threads=_threads())
+    with MonteRay(0, 0) as m:
+        m.set_option(MR_OPT_COARSE_RECORDS, coarse)
+        m.load_problem(prob)
+        assert m.get_option(MR_INFO_DEFERRED) == 0                  # auto: the tally fits in L2 many times over
+        assert m.record_path() == ("coarse_blocks" if coarse else "k4")
+        m.set_option(MR_OPT_DEFERRED_TALLY, 1)
+        assert m.get_option(MR_INFO_DEFERRED) == 1
+        seen = 0
+        # regions of 2^12 cells (64 bins) with the pool sized by the library, then far too small (most pairs take the
+        # direct path); regions of 2^15 cells (8 bins) and a pool that makes the library cast the batch in pieces; one region
+        for shift, pool in ((12, 0), (12, 4096), (15, 1_800_000), (0, 0)):
+            m.set_option(MR_OPT_DEFER_REGION_SHIFT, shift)
+            m.set_option(MR_OPT_DEFER_POOL_ENTRIES, pool)
+            m.clear_tally()
+            m.cast_rays(rays)
+            st = m.get_stats()
+            assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+            assert_tally(m.read_tally(), ref.tally, 0)
+            direct = m.get_option(MR_INFO_DEFER_DIRECT_PAIRS)
+            if pool == 0:
+                assert direct == 0
+            if pool == 4096:
+                assert direct > ref.segments // 2
+        m.set_option(MR_OPT_DEFER_REGION_SHIFT, 12)
+        m.set_option(MR_OPT_DEFER_POOL_ENTRIES, 0)
+        # tiny batches, additivity, moments, the ring
+        m.clear_tally()
+        m.cast_rays(rays[:7])
+        m.cast_rays(rays[7:20_000])
+        m.end_batch()
+        m.ring_open(2, 16384)
+        m.ring_push(rays[20_000:])
+        m.ring_close()
+        m.end_batch()
+        got = m.read_tally()
+        s1, s2, nb = m.read_moments()
+        st = m.get_stats()
+        assert nb == 2 and np.array_equal(s1, got)
+        assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+        assert_tally(got, ref.tally, 0)
+        m.set_option(MR_OPT_DEFERRED_TALLY, 0)
+        m.clear_tally()
+        m.cast_rays(rays)
+        assert_tally(m.read_tally(), ref.tally, 0)
+
+
 @pytest.mark.parametrize("precision", [0, 1])
 def test_warp_aggregated_atomics_for_the_first_segments(precision):
     """MR_OPT_AGGREGATE_FIRST: lanes of a warp that score into the same cell during a ray's first segments add one
