@@ -11,9 +11,15 @@ workload is BASELINE.json configs[2], the PWR 17x17-like lattice (170x170x300 ce
   value   : whole-job ray-cell segments/s with the ray batch already resident in HBM
   e2e     : the same metric through the C ABI with HOST buffers: each step copies the batch from
             pinned host memory (mr_cast_rays, where = host) and reads the tally back (mr_read_tally)
-  roofline: algorithmic bytes (31 B/segment + 96 B/ray on this config) / cast-kernel time, against
-            the measured copy bandwidth in MEASURED_PEAKS.json
+  roofline: ALGORITHMIC bytes (31 B/segment + 96 B/ray on this config) / cast-kernel time, against
+            the measured copy bandwidth in MEASURED_PEAKS.json.  `achieved` is that algorithmic rate, NOT DRAM traffic
+            (the working set is L2-resident): the DRAM rate from the committed ncu capture, the unit that really
+            limits the kernel, the measured L2 fp64-atomic ceiling and the whole-step fraction (ordering pre-pass
+            included) are reported beside it, and `roofline_plain_records` repeats the figure with the dictionary /
+            tiled-index path switched off (what a mesh with many distinct cell records gets)
   cpu_baseline: the CPU oracle, as it stands, on the box's host cores over a bounded sample
+
+    python bench.py --microbench red     the L2 fp64-atomic micro-benchmark alone (mr_microbench_red)
 
 N > 1 (torchrun, one rank per GPU): every rank holds the whole problem and casts its own batches
 (weak scaling, no data-path collective); time = max over ranks.  --impl reference times the
@@ -54,16 +60,44 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def committed_traffic(workload: str):
-    """dram bytes per cast-kernel launch from the committed ncu capture (profiles/traffic.txt), or None."""
+def committed_profile(workload: str, kernel: str):
+    """(dram bytes per launch, limiter dict) of `kernel` on `workload` from the committed ncu captures
+    (profiles/traffic.txt: `workload kernel dram_bytes commit`; profiles/limiters.json), or (None, None)."""
+    traffic, limiter = None, None
     try:
         for line in open(os.path.join(ROOT, "profiles", "traffic.txt")):
             w = line.split()
-            if len(w) >= 2 and w[0] == workload:
-                return float(w[1])
+            if len(w) >= 3 and not line.startswith("#") and w[0] == workload and w[1] == kernel:
+                traffic = float(w[2])
     except OSError:
         pass
-    return None
+    try:
+        with open(os.path.join(ROOT, "profiles", "limiters.json")) as f:
+            limiter = json.load(f).get(f"{workload}:{kernel}")
+    except (OSError, ValueError):
+        pass
+    return traffic, limiter
+
+
+def run_microbench(args):
+    """--microbench red: random fp64 red.global.add into an array the size of the PWR tally (69 MB, L2-resident), alone
+    and paired with a 16- / 32-byte gather from the same cell, lanes in groups of 1/2/4/8 sharing consecutive cells."""
+    import torch
+
+    from paper_1706_07476_b200 import microbench_red
+
+    if not torch.cuda.is_available():
+        raise SystemExit("the micro-benchmark needs a CUDA device")
+    rows = []
+    for ncell in (8_670_000, 1_000_000, 134_217_728):
+        for gather in (0, 16, 32):
+            for group in (1, 2, 4, 8):
+                r = microbench_red(0, ncell, group, gather, 1 << 28, 5)
+                rows.append(r)
+                print(f"# ncell {ncell:>10} gather {gather:>2} B group {group}: {r['best_ms']:.3f} ms "
+                      f"{r['lane_ops_per_sec'] / 1e9:7.1f} G lane-ops/s", file=sys.stderr)
+    print(json.dumps({"microbench": "red", "unit": "lane-ops/s", "rows": rows}))
+    return 0
 
 
 class ClockSampler:
@@ -185,6 +219,9 @@ def main():
     ap.add_argument("--double", action="store_true", help="all-double mode (MR_PRECISION_DOUBLE, 64-byte ray records): a context line, "
                     "not the headline; the roofline then uses B_seg = 16 + 9K, B_ray = 64 + 32M (SURVEY.md 8(d)); implies --no-next")
     ap.add_argument("--no-next", action="store_true", help="skip the SURVEY 8(f) rows (next-event cast, batch-moment fold)")
+    ap.add_argument("--microbench", default="", choices=["", "red"], help="run a micro-benchmark alone and exit")
+    ap.add_argument("--no-plain", action="store_true", help="skip the second roofline with the dictionary / tiled-index path off")
+    ap.add_argument("--batches", type=int, default=0, help="distinct ray batches cycled through (default: 1; config 4: 8 of its 100)")
     ap.add_argument("--ne-rays", type=int, default=2_000_000, help="events per next-event step")
     ap.add_argument("--ne-detectors", type=int, default=4)
     ap.add_argument("--producers", type=int, default=4, help="host threads feeding the producer ring")
@@ -201,6 +238,8 @@ def main():
 
     if args.impl == "reference":
         return run_reference(args, prob_kw)
+    if args.microbench:
+        return run_microbench(args)
 
     import numpy as np
     import torch
@@ -217,11 +256,16 @@ def main():
         multi.init_process_group("nccl")
     n_rays = args.rays or FULL_RAYS[args.config]
 
-    prob = make_problem(args.config, **prob_kw)
-    rays = make_rays(prob, n_rays, batch=rank)  # every rank its own batch: weak scaling
+    # all-double mode: genuinely double inputs (nothing rounded to fp32), as tests/test_gpu_double_inputs.py checks
+    prob = make_problem(args.config, double_inputs=args.double, **prob_kw)
+    # distinct batches cycled through step by step (BASELINE.json config 4: "10^8 rays in 10^6-ray batches"; every
+    # rank its own batches: weak scaling)
+    nb = args.batches or (8 if args.config == 4 else 1)
+    dtype = np.float64 if args.double else np.float32
+    batches = [make_rays(prob, n_rays, batch=rank * nb + b, dtype=dtype) for b in range(nb)]
+    rays = batches[0]
     if args.double:
         args.no_next = True
-        rays = rays.astype(np.float64)
     m = MonteRay(local_rank, 1 if args.double else 0)
     for kv in args.pre_opt:
         k, v = kv.split("=")
@@ -236,8 +280,13 @@ def main():
     for kv in args.opt:
         k, v = kv.split("=")
         m.set_option(int(k), int(v))
-    d_rays = torch.from_numpy(rays).to(dev)
+    d_batches = [torch.from_numpy(b).to(dev) for b in batches]
+    d_rays = d_batches[0]
     h_rays = torch.from_numpy(rays).pin_memory()
+    record_path = m.record_path()
+    from paper_1706_07476_b200 import (MR_INFO_COARSE_SHIFT, MR_INFO_DEFERRED, MR_INFO_DISTINCT_RECORDS, MR_OPT_TILED_INDEX,
+                                       microbench_red)
+    deferred = bool(m.get_option(MR_INFO_DEFERRED))
     h_tally = torch.empty(prob.ncell, dtype=torch.float64).pin_memory()
     sampler = ClockSampler(local_rank) if rank == 0 else None
 
@@ -247,8 +296,8 @@ def main():
         torch.cuda.synchronize()
 
     # ---------------------------------------------------------------- device-resident steps (value)
-    for _ in range(max(args.warmup, 3)):
-        m.cast_rays(d_rays)
+    for i in range(max(args.warmup, 3)):
+        m.cast_rays(d_batches[i % nb])
     barrier()
     st0 = m.get_stats()
     if sampler:
@@ -256,37 +305,77 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record()
-    for _ in range(args.steps):
-        m.cast_rays(d_rays)
+    for i in range(args.steps):
+        m.cast_rays(d_batches[i % nb])
     e1.record()
     barrier()
     if sampler:
         sampler.active = False
     ms_total = multi.max_over_ranks(e0.elapsed_time(e1), dev)
     st1 = m.get_stats()
-    seg_step = (st1.segments - st0.segments) // args.steps
+    seg_step = (st1.segments - st0.segments) // args.steps          # mean over the batches of the timed steps
     launches = st1.kernel_launches - st0.kernel_launches
     seg_all = multi.sum_over_ranks(seg_step, dev)
     value = seg_all * args.steps / (ms_total * 1e-3)
     rays_all = n_rays * world
 
     # ---------------------------------------------------------------- dominant-kernel time (roofline)
-    kms = []
-    for _ in range(min(args.steps, 10)):
-        m.cast_rays(d_rays)
-        kms.append(m.get_stats().last_kernel_ms)
-    kernel_ms = statistics.mean(kms)
     peak, peak_src = measured_peak()
     dense = prob.config == 5
-    alg_bytes = algorithmic_bytes(prob, seg_step, n_rays, dense)
-    if args.double:
-        alg_bytes = seg_step * (16 + 9 * prob.K) + n_rays * (64 + 32 * prob.M)
-    achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
-    traffic = committed_traffic(CONFIG_NAMES[args.config])
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "peak_source": peak_src, "kernel": "mr::cast_kernel", "kernel_ms": kernel_ms,
-                "algorithmic_bytes_per_launch": alg_bytes,
-                "segments_per_sec_at_roofline": peak * 1e9 / (alg_bytes / seg_step)}
+    workload = CONFIG_NAMES[args.config]
+
+    def kernel_roofline(kernel_name):
+        """Algorithmic bytes of the launches just timed over the cast kernel's own CUDA-event time (the library records
+        events around every cast-kernel launch on the launching stream; the ordering pre-pass is NOT inside them)."""
+        kms, segs = [], []
+        for i in range(min(args.steps, 10)):
+            s0 = m.get_stats().segments
+            m.cast_rays(d_batches[i % nb])
+            st = m.get_stats()
+            kms.append(st.last_kernel_ms)
+            segs.append(st.segments - s0)
+        kernel_ms, seg_launch = statistics.mean(kms), statistics.mean(segs)
+        alg = algorithmic_bytes(prob, seg_launch, n_rays, dense)
+        if args.double:
+            alg = seg_launch * (16 + 9 * prob.K) + n_rays * (64 + 32 * prob.M)
+        achieved = alg / (kernel_ms * 1e-3) / 1e9
+        traffic, limiter = committed_profile(workload + ("_double" if args.double else ""), kernel_name)
+        return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                "achieved_is": "algorithmic bytes (SURVEY.md 8(d)) / cast-kernel time; not DRAM traffic",
+                "peak_source": peak_src, "kernel": kernel_name, "kernel_ms": kernel_ms,
+                "kernel_ms_excludes": "the ray-ordering pre-pass (5 small kernels per batch); see whole_step_frac",
+                "algorithmic_bytes_per_launch": alg, "segments_per_launch": seg_launch,
+                "segments_per_sec_at_roofline": peak * 1e9 / (alg / seg_launch),
+                "dram_GBps_from_committed_capture": (traffic / (kernel_ms * 1e-3) / 1e9) if traffic else None,
+                "limiter": limiter}
+
+    kname = {"coarse_blocks": "cast_defer_kernel+defer_scatter_kernel" if deferred else "cast_kernel<C4>"}.get(
+        record_path, f"cast_kernel<{record_path}>")
+    roofline = kernel_roofline(kname)
+    roofline["whole_step_frac"] = value / world / roofline["segments_per_sec_at_roofline"]
+    # the measured L2 fp64-atomic ceiling (one uncoalesced red per lane into an array of the tally's size), same run
+    try:
+        red = microbench_red(local_rank, prob.ncell, 1, 0, 1 << 27, 3)
+        gat = microbench_red(local_rank, prob.ncell, 1, 16, 1 << 27, 3)
+        kernel_red_rate = roofline["segments_per_launch"] / (roofline["kernel_ms"] * 1e-3)
+        roofline["atomic_ceiling"] = {
+            "red_per_sec": red["lane_ops_per_sec"], "red_plus_16B_gather_per_sec": gat["lane_ops_per_sec"],
+            "kernel_red_per_sec": kernel_red_rate, "frac_of_red_ceiling": kernel_red_rate / red["lane_ops_per_sec"],
+            "how": "mr_microbench_red: random red.global.add.f64 into ncell doubles, 2^27 lane-ops, best of 3"}
+    except Exception as e:  # noqa: BLE001
+        roofline["atomic_ceiling"] = {"error": repr(e)}
+    roofline_plain = None
+    if record_path.startswith("tiled") and not args.no_plain:
+        m.set_option(MR_OPT_TILED_INDEX, 0)
+        plain_path = m.record_path()
+        for _ in range(3):
+            m.cast_rays(d_rays)
+        roofline_plain = kernel_roofline(f"cast_kernel<{plain_path}>")
+        roofline_plain["cell_record_path"] = plain_path
+        roofline_plain["why"] = ("the headline runs the dictionary + tiled-index path (this mesh has "
+                                 f"{m.get_option(MR_INFO_DISTINCT_RECORDS)} distinct cell records); a mesh with more than 1024 "
+                                 "distinct records gets this path")
+        m.set_option(MR_OPT_TILED_INDEX, 1)
 
     # ---------------------------------------------------------------- end to end through the C ABI, host buffers
     e2e = None
@@ -297,6 +386,7 @@ def main():
         barrier()
         if sampler:
             sampler.active = True
+        s_e0 = m.get_stats().segments
         t0 = time.perf_counter()
         for _ in range(args.steps):
             m.cast_rays(h_rays)                    # H2D of the batch from pinned memory, inside the call
@@ -306,7 +396,8 @@ def main():
         if sampler:
             sampler.active = False
         dt = multi.max_over_ranks(dt, dev)
-        e2e = {"value": seg_all * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(rays.nbytes),
+        seg_e2e = multi.sum_over_ranks(m.get_stats().segments - s_e0, dev)
+        e2e = {"value": seg_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": int(rays.nbytes),
                "d2h_bytes_per_step": int(prob.ncell * 8), "ms_per_step": 1e3 * dt / args.steps}
     # ---------------------------------------------------------------- next-event cast, batch-moment fold
     next_rows = None
@@ -422,6 +513,18 @@ def main():
         except Exception as e:  # noqa: BLE001 -- report, do not lose the JSON line
             next_rows["error"] = repr(e)
     total_launches = m.get_stats().kernel_launches
+    m_info = {"distinct": m.get_option(MR_INFO_DISTINCT_RECORDS), "coarse_shift": m.get_option(MR_INFO_COARSE_SHIFT)}
+    # replicas are combined by ONE fp64 sum all-reduce of the tally when it is read: timed here, outside `value`
+    allreduce_ms = None
+    if world > 1:
+        t = m.tally_tensor()
+        barrier()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record()
+        multi.allreduce_sum_(t)
+        a1.record()
+        barrier()
+        allreduce_ms = multi.max_over_ranks(a0.elapsed_time(a1), dev)
 
     # ---------------------------------------------------------------- CPU oracle beside it (rank 0, N = 1)
     cpu = None
@@ -445,11 +548,15 @@ def main():
             "config": {"workload": CONFIG_NAMES[args.config], "mesh": [prob.nx, prob.ny, prob.nz], "K": prob.K, "M": prob.M,
                        "rays_per_step_per_gpu": n_rays, "segments_per_step_per_gpu": int(seg_step),
                        "precision": "double (everything fp64)" if args.double else "mixed (fp32 tables/rays/coefficients, fp64 walk/score/tally)",
+                       "cell_record_path": record_path, "deferred_tally": deferred,
+                       "distinct_cell_records": m_info["distinct"], "coarse_block_shift": m_info["coarse_shift"],
+                       "distinct_batches_cycled": nb,
                        "parallelism": f"replicas x{world}" if world > 1 else "1 GPU",
                        "l2": "inputs larger than L2 (rays 320 MB + cell records 139 MB + tally 69 MB), no flush"
                        if args.config == 3 else "no flush"},
             "rays_per_sec": rays_all * args.steps / (ms_total * 1e-3),
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "next_rows": next_rows,
+            "roofline": roofline, "roofline_plain_records": roofline_plain, "cpu_baseline": cpu, "e2e": e2e, "next_rows": next_rows,
+            "allreduce_ms": allreduce_ms,
             "gpu_launches": int(launches), "gpu_launches_total": int(total_launches),
             "clocks": sampler.report() if sampler else None,
         }

@@ -331,6 +331,12 @@ enum {
                                  out.  A pool that is too small is never an error: the pairs that do not fit are added straight to the tally */
     MR_OPT_DEFER_REGION_SHIFT = 13, /* s: the deferred tally's regions are 2^s cells of the linear cell index (at most 64 regions: s is raised
                                  until they cover the mesh); 0 (default) = the largest s with 8 * 2^s bytes <= L2/8 */
+    MR_OPT_COOP_FLUSH = 14,   /* 1: the cast kernel stages every lane's (cell, score) pairs for 8 steps in shared memory and the warp then
+                                 adds them TRANSPOSED, one instruction carrying 8 consecutive segments of each of 4 rays (consecutive
+                                 cells of a ray often share a 32-byte tally sector; cells of unrelated rays never do).  MIXED mode,
+                                 dictionary / K = 1 / K = 3 pairs / dense-8 record paths; elsewhere ignored.  0: one atomic per
+                                 segment straight from the walking lane.  2 (default) = auto: on when tally + cell records fit in
+                                 half the L2 (it wins there: contended, resident tallies), off when they stream through it */
     MR_OPT_AGGREGATE_FIRST = 9 /* n >= 0: the tally atomics of the first n segments of every ray are warp-aggregated (lanes that score
                                  into the same cell are found with match.any and one of them adds the sum): for batches born in a
                                  region of a few cells, where same-address atomics serialise in L2.  Default 2; 0 = off */
@@ -364,6 +370,18 @@ enum {
 };
 MR_API int mr_set_option(mr_ctx *ctx, int option, int64_t value);
 MR_API int mr_get_option(mr_ctx *ctx, int option, int64_t *value);
+
+/* ---- measurement aid ------------------------------------------------------------------------ */
+
+/* The L2 fp64-atomic ceiling the cast kernel is measured against ("L2 atomic throughput against a
+ * measured micro-benchmark").  Issues the cast kernel's per-segment memory pattern and nothing else: every lane adds into
+ * a pseudo-random cell of a scratch array of `ncell` doubles (red.global.add.f64), optionally after loading `gather_bytes`
+ * (0, 16 or 32) from a scratch record array at the same cell; lanes in groups of `group` (a power of two <= 32) take
+ * consecutive cells (group = 4: one 32-byte sector).  ceil(lane_ops / 8192) * 8192 lane operations per launch, two warm-up
+ * launches, then `reps` timed ones on the legacy default stream of `device`: *best_ms and *mean_ms (may be NULL) per launch.
+ * Needs no context; allocates and frees its own scratch.  Errors: INVALID_ARG, CUDA, OOM. */
+MR_API int mr_microbench_red(int device, int64_t ncell, int group, int gather_bytes, int64_t lane_ops, int reps,
+                             double *best_ms, double *mean_ms);
 
 #ifdef __cplusplus
 }

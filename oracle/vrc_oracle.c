@@ -33,6 +33,9 @@
  * numpy.roots, mid-point membership by numpy.searchsorted on (rho, z), an independent exit distance, the
  * homogeneous closed form, the collision-probability invariant, rotation invariance, quadrature.
  * Multi-nuclide materials (vrc_sigma) are pinned in tests/test_oracle_nuclide_pins.py.
+ * The next-event walk on R-Z / spherical meshes (vrc_next_event_rz, steps NZ1..NZ6) is pinned in
+ * tests/test_oracle_ne_rz_pins.py.  The "1/d_a not finite" branch of O1 / O4 is pinned in
+ * tests/test_oracle_subnormal_pins.py.
  * Nothing in this file is "parity unpinned".
  */
 #include <math.h>
@@ -594,6 +597,161 @@ int vrc_cast_rz(const vrc_problem *p, const vrc_rz_mesh *g, int64_t n, const dou
         if (cast_one_rz(p, g, rays + 8 * r, tally, dg, r, &cnt.segments)) cnt.rays_accepted++;
         else cnt.rays_rejected++;
     }
+    if (counts) *counts = cnt;
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * Next-event (point-detector) estimator on R-Z and spherical meshes -- the NEXT-3 x NEXT-4 cell of SURVEY.md §8(f)
+ * ("requires a ray-cast from each source and collision event to the estimator location"; PAPER.md:358
+ * "1-D spherical ... 2-D cylindrical (R-Z) meshes").  The estimator is that of vrc_next_event, the cells those of
+ * vrc_cast_rz; nothing new is read into the paper (readings N-Q1..N-Q6 and Z-Q1..Z-Q5 of DESIGN.md §10 apply).
+ *
+ * Steps (all IEEE double, one rounding per written operation):
+ *   NZ1 reject (count, no contribution) an event with non-finite x, y, z, E or W, E <= 0, rho0^2 >= r_nr^2, z outside
+ *       [z_0, z_nz) (R-Z only), or, with d = det - o (one subtract per axis), R2 = dx*dx + dy*dy + dz*dz not finite or
+ *       == 0, or no crossing family that can move (Z1: a == 0 or 1/a not finite, and dz == 0 or 1/dz not finite);
+ *       the direction fields of the record are ignored
+ *   NZ2 sigma_m(E) as O2;   NZ3 start cell as Z3
+ *   NZ4 crossing parameters as Z4 with the UNNORMALISED direction d, so that t = 1 is the detector, exactly
+ *   NZ5 walk as Z5 (ties radial before axial); a segment whose pending crossing has t >= 1 ends AT the detector
+ *       (l = 1 - t_cur) and is the last; a step that leaves the mesh is the last too (outside is void, N-Q2).
+ *       tau += Sigma_i * (l_i * R),  R = sqrt(R2)
+ *   NZ6 score = W * exp(-tau) / R2
+ * Pins: tests/test_oracle_ne_rz_pins.py (homogeneous closed form, void inverse-square law, numpy.roots crossing lists
+ * cut at t = 1, quadrature of Sigma_t along the line, detectors on cylinders / planes / the axis, reciprocity,
+ * rotation invariance, every rejection rule).
+ * ------------------------------------------------------------------------------------------------ */
+static int next_event_rz_one(const vrc_problem *p, const vrc_rz_mesh *g, const double *ray, const double *det,
+                             const vrc_ne_diag *dg, int64_t r, double *score_out, int64_t *segments_out)
+{
+    const double ox = ray[0], oy = ray[1], oz = ray[2];
+    const double E = ray[6], W = ray[7];
+    const int32_t nr = g->nr, nz = g->nz;
+    const int sph = g->spherical != 0;
+    uint32_t nseg = 0;
+    uint64_t hash = FNV_BASIS;
+    double tau = 0.0, score = 0.0;
+    int accepted = 1;
+
+    /* NZ1 */
+    if (!isfinite(ox) || !isfinite(oy) || !isfinite(oz) || !isfinite(E) || !isfinite(W) || !(E > 0.0)) accepted = 0;
+    const double dx = det[0] - ox, dy = det[1] - oy, dz = det[2] - oz;
+    const double R2 = dx * dx + dy * dy + dz * dz;
+    if (!isfinite(R2) || !(R2 > 0.0)) accepted = 0;
+    const double rho2 = sph ? ox * ox + oy * oy + oz * oz : ox * ox + oy * oy;
+    const double a = sph ? dx * dx + dy * dy + dz * dz : dx * dx + dy * dy;
+    const double inv_a = (a != 0.0) ? 1.0 / a : 0.0;
+    const int radial = (a != 0.0) && isfinite(inv_a) && isfinite(a);
+    const double inv_z = (dz != 0.0) ? 1.0 / dz : 0.0;
+    const int axial = !sph && (dz != 0.0) && isfinite(inv_z);
+    if (!radial && !axial) accepted = 0;
+    if (accepted && !(rho2 < g->re[nr] * g->re[nr])) accepted = 0;
+    if (accepted && !sph && !(oz >= g->ze[0] && oz < g->ze[nz])) accepted = 0;
+
+    if (accepted) {
+        const double R = sqrt(R2);
+        double sig[64];
+        for (int32_t m = 0; m < p->M; ++m) sig[m] = vrc_sigma(p, m, E);         /* NZ2 */
+        /* NZ3 */
+        int32_t ir = -1;
+        for (int32_t q = 0; q <= nr; ++q) if (g->re[q] * g->re[q] <= rho2) ir = q;
+        int32_t iz = sph ? 0 : (int32_t)(upper_bound(g->ze, nz + 1, oz) - 1);
+        /* NZ4 */
+        const double b = sph ? ox * dx + oy * dy + oz * dz : ox * dx + oy * dy;
+        int inward = 0;
+        double t_r = INFINITY, t_z = INFINITY, t_cur = 0.0;
+        int32_t pz = 0, stepz = 0;
+        if (radial) {
+            if (b < 0.0 && ir >= 1) {
+                double cc = rho2 - g->re[ir] * g->re[ir];
+                double D = b * b - a * cc;
+                if (D > 0.0) { inward = 1; t_r = fmax(0.0, (-b - sqrt(D)) * inv_a); }
+            }
+            if (!inward) {
+                double cc = rho2 - g->re[ir + 1] * g->re[ir + 1];
+                double D = b * b - a * cc;
+                t_r = fmax(0.0, (-b + sqrt(D)) * inv_a);
+            }
+        }
+        if (axial) {
+            stepz = dz > 0.0 ? 1 : -1;
+            pz = dz > 0.0 ? iz + 1 : iz;
+            t_z = (g->ze[pz] - oz) * inv_z;
+        }
+        /* NZ5 */
+        for (;;) {
+            const int ax = (t_z < t_r) ? 1 : 0;            /* ties: radial first */
+            const double tn = ax ? t_z : t_r;
+            const int last = tn >= 1.0;
+            const double l = (last ? 1.0 : tn) - t_cur;
+            int64_t c = (int64_t)ir + (int64_t)nr * (int64_t)iz;
+            double S = 0.0;
+            for (int32_t k = 0; k < p->K; ++k) {
+                int32_t m = p->cell_mat[c * p->K + k];
+                if (m >= 0) S += (p->cell_frac[c * p->K + k] * p->density[m]) * sig[m];
+            }
+            tau += S * (l * R);
+            for (int q = 0; q < 4; ++q) {
+                hash ^= (uint64_t)(((uint32_t)c >> (8 * q)) & 0xffu);
+                hash *= FNV_PRIME;
+            }
+            nseg += 1;
+            if (last) break;
+            t_cur = tn;
+            if (ax) {
+                iz += stepz;
+                if (iz < 0 || iz >= nz) break;
+                pz += stepz;
+                t_z = (g->ze[pz] - oz) * inv_z;
+            } else if (inward) {
+                ir -= 1;
+                inward = 0;
+                if (ir >= 1) {
+                    double cc = rho2 - g->re[ir] * g->re[ir];
+                    double D = b * b - a * cc;
+                    if (D > 0.0) { inward = 1; t_r = fmax(0.0, (-b - sqrt(D)) * inv_a); }
+                }
+                if (!inward) {
+                    double cc = rho2 - g->re[ir + 1] * g->re[ir + 1];
+                    double D = b * b - a * cc;
+                    t_r = fmax(0.0, (-b + sqrt(D)) * inv_a);
+                }
+            } else {
+                ir += 1;
+                if (ir >= nr) break;
+                double cc = rho2 - g->re[ir + 1] * g->re[ir + 1];
+                double D = b * b - a * cc;
+                t_r = fmax(0.0, (-b + sqrt(D)) * inv_a);
+            }
+        }
+        score = W * exp(-tau) / R2;                                              /* NZ6 */
+    }
+    if (dg) {
+        if (dg->nseg) dg->nseg[r] = nseg;
+        if (dg->hash) dg->hash[r] = accepted ? hash : 0;
+        if (dg->tau) dg->tau[r] = tau;
+        if (dg->score) dg->score[r] = score;
+    }
+    *score_out = score;
+    *segments_out += nseg;
+    return accepted;
+}
+
+/* n events against ONE detector point det[3] on the R-Z / spherical mesh g; *det_sum += sum of scores (event order). */
+int vrc_next_event_rz(const vrc_problem *p, const vrc_rz_mesh *g, int64_t n, const double *rays, const double *det,
+                      double *det_sum, const vrc_ne_diag *dg, vrc_counts *counts)
+{
+    if (p->M > 64 || g->nr < 1 || g->nz < 1 || g->re[0] != 0.0 || (g->spherical && g->nz != 1)) return -1;
+    vrc_counts cnt = {0, 0, 0};
+    double total = 0.0;
+    for (int64_t r = 0; r < n; ++r) {
+        double s;
+        if (next_event_rz_one(p, g, rays + 8 * r, det, dg, r, &s, &cnt.segments)) cnt.rays_accepted++;
+        else cnt.rays_rejected++;
+        total += s;
+    }
+    if (det_sum) *det_sum += total;
     if (counts) *counts = cnt;
     return 0;
 }

@@ -78,6 +78,9 @@ def _load():
         _lib.vrc_cast_rz.restype = C.c_int
         _lib.vrc_cast_rz.argtypes = [C.POINTER(_Problem), C.POINTER(_RzMesh), C.c_int64, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_void_p]
+        _lib.vrc_next_event_rz.restype = C.c_int
+        _lib.vrc_next_event_rz.argtypes = [C.POINTER(_Problem), C.POINTER(_RzMesh), C.c_int64, C.c_void_p, C.c_void_p,
+                                           C.c_void_p, C.c_void_p, C.c_void_p]
         _lib.vrc_fnv1a_cells.restype = C.c_uint64
         _lib.vrc_fnv1a_cells.argtypes = [C.c_void_p, C.c_int64]
         _lib.vrc_max_threads.restype = C.c_int
@@ -291,6 +294,39 @@ class Oracle:
             raise RuntimeError(f"oracle error {rc}")
         return NextEventResult(float(total.value), int(cnt.rays_accepted), int(cnt.rays_rejected), int(cnt.segments),
                                nseg, hsh, tau, score)
+
+
+    def _next_event_rz(self, rays, det, re, ze, spherical) -> NextEventResult:
+        r = np.ascontiguousarray(np.asarray(rays, dtype=np.float64).reshape(-1, 8))
+        n = r.shape[0]
+        d = np.ascontiguousarray(np.asarray(det, dtype=np.float64).reshape(3))
+        re = np.ascontiguousarray(re, dtype=np.float64)
+        ze = np.ascontiguousarray(ze, dtype=np.float64)
+        nr, nz = len(re) - 1, len(ze) - 1
+        assert nr * nz == self.ncell, "the problem's cell arrays must hold nr*nz cells"
+        nseg = np.zeros(n, dtype=np.uint32)
+        hsh = np.zeros(n, dtype=np.uint64)
+        tau = np.zeros(n, dtype=np.float64)
+        score = np.zeros(n, dtype=np.float64)
+        dg = _NeDiag(nseg.ctypes.data, hsh.ctypes.data, tau.ctypes.data, score.ctypes.data)
+        g = _RzMesh(nr, nz, re.ctypes.data, ze.ctypes.data, 1 if spherical else 0)
+        total = C.c_double(0.0)
+        cnt = _Counts()
+        rc = self.lib.vrc_next_event_rz(C.byref(self._p), C.byref(g), n, r.ctypes.data, d.ctypes.data,
+                                        C.cast(C.byref(total), C.c_void_p), C.cast(C.byref(dg), C.c_void_p),
+                                        C.cast(C.byref(cnt), C.c_void_p))
+        if rc < 0:
+            raise RuntimeError(f"oracle error {rc}")
+        return NextEventResult(float(total.value), int(cnt.rays_accepted), int(cnt.rays_rejected), int(cnt.segments),
+                               nseg, hsh, tau, score)
+
+    def next_event_rz(self, rays, det, re, ze) -> NextEventResult:
+        """Next-event estimator of `rays` for ONE detector point on the R-Z mesh (re, ze): steps NZ1..NZ6 of vrc_oracle.c."""
+        return self._next_event_rz(rays, det, re, ze, False)
+
+    def next_event_sphere(self, rays, det, re) -> NextEventResult:
+        """The same on 1-D spherical shells about the origin."""
+        return self._next_event_rz(rays, det, re, np.array([0.0, 1.0]), True)
 
 
 # ---------------------------------------------------------------------------------------------------

@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     MR_OPT_AGGREGATE_FIRST,
     MR_OPT_BLOCK_THREADS,
     MR_OPT_COARSE_RECORDS,
+    MR_OPT_COOP_FLUSH,
     MR_OPT_COPY_THREADS,
     MR_OPT_DEFERRED_TALLY,
     MR_OPT_DEFER_POOL_ENTRIES,
@@ -34,4 +35,5 @@ from .binding import (  # noqa: F401
     MonteRayError,
     Stats,
     load_library,
+    microbench_red,
 )

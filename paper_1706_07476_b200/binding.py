@@ -29,6 +29,7 @@ MR_OPT_COARSE_RECORDS = 10
 MR_OPT_DEFERRED_TALLY = 11
 MR_OPT_DEFER_POOL_ENTRIES = 12
 MR_OPT_DEFER_REGION_SHIFT = 13
+MR_OPT_COOP_FLUSH = 14
 MR_INFO_RECORD_PATH, MR_INFO_DISTINCT_RECORDS, MR_INFO_COARSE_SHIFT = 100, 101, 102
 MR_INFO_DEFERRED, MR_INFO_DEFER_DIRECT_PAIRS = 103, 104
 MR_PATH_NAMES = {0: "none", 1: "k1", 2: "k2", 3: "k3", 4: "k4", 5: "k2_pairs", 6: "k3_pairs", 7: "k4_fused", 8: "dense8",
@@ -43,6 +44,7 @@ EXPORTS = [
     "mr_end_batch", "mr_read_moments", "mr_read_mean_sigma", "mr_load_nuclide_xs", "mr_define_material", "mr_load_mesh_rz", "mr_load_mesh_sphere",
     "mr_ring_open", "mr_ring_push", "mr_ring_flush", "mr_ring_close", "mr_ring_get_stats",
     "mr_load_detectors", "mr_cast_next_event", "mr_read_detectors", "mr_clear_detectors", "mr_trace_next_event",
+    "mr_microbench_red",
 ]
 
 
@@ -118,6 +120,7 @@ def load_library() -> C.CDLL:
         "mr_read_detectors": [vp, vp],
         "mr_clear_detectors": [vp],
         "mr_trace_next_event": [vp, i64, vp, i32, i32, vp, vp, vp, vp],
+        "mr_microbench_red": [i32, i64, i32, i32, i64, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)],
     }
     for name, argtypes in sigs.items():
         fn = getattr(lib, name)
@@ -127,6 +130,18 @@ def load_library() -> C.CDLL:
     lib.mr_last_error.restype = C.c_char_p
     _lib = lib
     return lib
+
+
+def microbench_red(device: int, ncell: int, group: int = 1, gather_bytes: int = 0, lane_ops: int = 1 << 28, reps: int = 5):
+    """mr_microbench_red -> dict(lane_ops, best_ms, mean_ms, lane_ops_per_sec): the L2 fp64-atomic ceiling."""
+    lib = load_library()
+    best, mean = C.c_double(), C.c_double()
+    rc = lib.mr_microbench_red(device, ncell, group, gather_bytes, lane_ops, reps, C.byref(best), C.byref(mean))
+    if rc != MR_OK:
+        raise MonteRayError(rc, "mr_microbench_red failed")
+    ops = max(128, (lane_ops + 63) // 64 // 128 * 128) * 64
+    return {"ncell": int(ncell), "group": group, "gather_bytes": gather_bytes, "lane_ops": ops, "best_ms": best.value,
+            "mean_ms": mean.value, "lane_ops_per_sec": ops / (best.value * 1e-3)}
 
 
 class _TorchAllocator:

@@ -24,6 +24,7 @@
 #include "mr_device.cuh"
 #include "mr_sort.cuh"
 #include "mr_defer.cuh"
+#include "mr_microbench.cuh"
 
 using namespace mr;
 
@@ -194,6 +195,9 @@ struct mr_ctx {
     double defer_entries_per_ray = 0.0;            // sizing estimate; grows when a cast ran out of pool
     long long defer_pool_fixed = 0;                // option MR_OPT_DEFER_POOL_ENTRIES (0: sized by the estimate)
     int defer_shift_fixed = 0;                     // option MR_OPT_DEFER_REGION_SHIFT (0: from the L2 size)
+    int coop_opt = 2;                // option MR_OPT_COOP_FLUSH: cast_coop_kernel (transposed tally adds) on the paths built for it;
+                                     // 2 = auto: when tally + cell records fit in half the L2 (measured: config 5 6.05 -> 5.55 ms, config 2
+                                     // 0.590 -> 0.558 ms; config 3, whose slabs stream through L2, 6.38 -> 7.22 ms: off there)
     int agg_first = 2;               // option MR_OPT_AGGREGATE_FIRST
     int fused_opt = 2;               // option MR_OPT_FUSED_TALLY: 0 off, 1 on, 2 auto (decided by mr_load_materials)
     bool fused = false;              // LAYOUT_K4 records carry the score accumulators (LAYOUT_K4F in the cast kernel)
@@ -546,6 +550,42 @@ int launch_cast_t(mr_ctx *c, const CastParams &P)
     case EDGES_SHARED: return launch_cast_m<Real, Rec, EDGES_SHARED>(c, P, block, smem);
     default: return launch_cast_m<Real, Rec, EDGES_GLOBAL>(c, P, block, smem);
     }
+}
+
+template <typename Real, typename Rec, int MODE>
+int launch_coop_m(mr_ctx *c, const CastParams &P, int block, size_t smem)
+{
+    const long long grid = (P.n + block - 1) / block;
+    if (grid > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
+    if (int rc = set_smem(c, cast_coop_kernel<Real, Rec, MODE>, smem)) return rc;
+    cast_coop_kernel<Real, Rec, MODE><<<(unsigned)grid, block, smem, c->work_stream()>>>(P);
+    c->launches += 1;
+    MR_CUDA(c, cudaGetLastError());
+    return MR_OK;
+}
+
+// cast_coop_kernel (cooperative, transposed tally adds) for the record types it is built for
+template <typename Real, typename Rec>
+int launch_coop_t(mr_ctx *c, const CastParams &P)
+{
+    const int block = c->block_threads;
+    const size_t per_block = walker_smem_bytes(block) + (((size_t)(c->M + c->N) * block * sizeof(Real) + 15) & ~(size_t)15) +
+                             (Rec::kTiled ? (size_t)c->ndict * sizeof(uint4) : 0) + (size_t)(block / 32) * coop_warp_smem_bytes();
+    const int mode = edge_mode(c, per_block);
+    const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
+    if (smem > 227 * 1024) return launch_cast_t<Real, Rec>(c, P);
+    switch (mode) {
+    case EDGES_ARITH: return launch_coop_m<Real, Rec, EDGES_ARITH>(c, P, block, smem);
+    case EDGES_SHARED: return launch_coop_m<Real, Rec, EDGES_SHARED>(c, P, block, smem);
+    default: return launch_coop_m<Real, Rec, EDGES_GLOBAL>(c, P, block, smem);
+    }
+}
+
+template <typename Real, typename Rec>
+int launch_cast_or_coop(mr_ctx *c, const CastParams &P)
+{
+    const bool coop = c->coop_opt == 1 || (c->coop_opt == 2 && c->resident_bytes() <= c->l2_bytes / 2);
+    return coop ? launch_coop_t<Real, Rec>(c, P) : launch_cast_t<Real, Rec>(c, P);
 }
 
 int upload_xs_desc(mr_ctx *c)
@@ -953,8 +993,8 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
         P.ndict = c->ndict;
         P.ntx = c->ntx;
         P.nty = c->nty;
-        rc = c->tile_bits == 4 ? launch_cast_t<float, TiledRec<4>>(c, P)
-           : c->tile_bits == 8 ? launch_cast_t<float, TiledRec<8>>(c, P) : launch_cast_t<float, TiledRec<16>>(c, P);
+        rc = c->tile_bits == 4 ? launch_cast_or_coop<float, TiledRec<4>>(c, P)
+           : c->tile_bits == 8 ? launch_cast_or_coop<float, TiledRec<8>>(c, P) : launch_cast_or_coop<float, TiledRec<16>>(c, P);
         break;
     case MR_PATH_COARSE:
         P.crecs = c->d_crecs;
@@ -963,16 +1003,16 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
         P.cny = c->cny;
         rc = use_deferred(c, MR_PATH_COARSE) ? cast_deferred<CellRec<LAYOUT_C4>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_C4>>(c, P);
         break;
-    case MR_PATH_K1: rc = launch_cast_t<float, CellRec<LAYOUT_K1>>(c, P); break;
+    case MR_PATH_K1: rc = launch_cast_or_coop<float, CellRec<LAYOUT_K1>>(c, P); break;
     case MR_PATH_K2: rc = launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
     case MR_PATH_K3: rc = launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P); break;
     case MR_PATH_K2_PAIRS: rc = launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P); break;
-    case MR_PATH_K3_PAIRS: rc = launch_cast_t<float, CellRec<LAYOUT_K3P>>(c, P); break;
+    case MR_PATH_K3_PAIRS: rc = launch_cast_or_coop<float, CellRec<LAYOUT_K3P>>(c, P); break;
     case MR_PATH_K4_FUSED: rc = launch_cast_t<float, CellRec<LAYOUT_K4F>>(c, P); c->fused_dirty = true; break;
     case MR_PATH_K4:
         rc = use_deferred(c, MR_PATH_K4) ? cast_deferred<CellRec<LAYOUT_K4>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P);
         break;
-    case MR_PATH_DENSE8: rc = launch_cast_t<float, CellRec<LAYOUT_D8>>(c, P); break;
+    case MR_PATH_DENSE8: rc = launch_cast_or_coop<float, CellRec<LAYOUT_D8>>(c, P); break;
     default: rc = launch_cast_t<float, CellRecGeneric<float>>(c, P);
     }
     if (rc) return rc;
@@ -2277,6 +2317,10 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         if (value < 1 || value > 64) return c->fail(MR_ERR_INVALID_ARG, "copy threads must be in [1, 64]");
         c->copy_threads = (int)value;
         return MR_OK;
+    case MR_OPT_COOP_FLUSH:
+        if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "cooperative-flush option is 0 (off), 1 (on) or 2 (auto)");
+        c->coop_opt = (int)value;
+        return MR_OK;
     case MR_OPT_COARSE_RECORDS:
         if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "coarse-records option is 0 or 1");
         c->coarse_opt = (int)value;
@@ -2319,6 +2363,7 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     case MR_OPT_TILED_INDEX: *value = c->tiled_opt; return MR_OK;
     case MR_OPT_AGGREGATE_FIRST: *value = c->agg_first; return MR_OK;
     case MR_OPT_COARSE_RECORDS: *value = c->coarse_opt; return MR_OK;
+    case MR_OPT_COOP_FLUSH: *value = c->coop_opt; return MR_OK;
     case MR_INFO_RECORD_PATH: *value = record_path(c); return MR_OK;
     case MR_INFO_DISTINCT_RECORDS: *value = c->ndict; return MR_OK;
     case MR_INFO_COARSE_SHIFT: *value = c->cshift; return MR_OK;
@@ -2340,3 +2385,64 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
 }
 
 }  // extern "C"
+
+// =================================================================================================
+// Measurement aid: the L2 fp64-atomic ceiling (mr_microbench.cuh)
+// =================================================================================================
+extern "C" int mr_microbench_red(int device, int64_t ncell, int group, int gather_bytes, int64_t lane_ops, int reps,
+                                 double *best_ms, double *mean_ms)
+{
+    if (ncell < 1024 || ncell > 0xffffffffLL || group < 1 || group > 32 || (group & (group - 1)) || lane_ops < 1 || reps < 1 ||
+        (gather_bytes != 0 && gather_bytes != 16 && gather_bytes != 32) || !best_ms)
+        return MR_ERR_INVALID_ARG;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) {
+        cudaGetLastError();
+        return MR_ERR_CUDA;
+    }
+    DeviceGuard guard(device);
+    RedBenchParams P{};
+    P.ncell = (unsigned)ncell;
+    P.group = group;
+    P.gather_bytes = gather_bytes;
+    P.iters = 64;
+    const long long threads = std::max<long long>(128, (lane_ops + P.iters - 1) / P.iters / 128 * 128);
+    double *tally = nullptr;
+    uint4 *recs = nullptr;
+    unsigned *sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    auto done = [&](int code) {
+        cudaFree(tally);
+        cudaFree(recs);
+        cudaFree(sink);
+        if (e0) cudaEventDestroy(e0);
+        if (e1) cudaEventDestroy(e1);
+        cudaGetLastError();
+        return code;
+    };
+    if (cudaMalloc(&tally, (size_t)ncell * 8) != cudaSuccess || cudaMalloc(&sink, 4) != cudaSuccess ||
+        (gather_bytes && cudaMalloc(&recs, (size_t)ncell * gather_bytes) != cudaSuccess))
+        return done(MR_ERR_OOM);
+    cudaMemset(tally, 0, (size_t)ncell * 8);
+    if (recs) cudaMemset(recs, 0, (size_t)ncell * gather_bytes);
+    P.tally = tally;
+    P.recs = recs;
+    P.sink = sink;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return done(MR_ERR_CUDA);
+    double best = 1e300, sum = 0.0;
+    for (int r = -2; r < reps; ++r) {                       // two warm-up launches
+        cudaEventRecord(e0, 0);
+        red_bench_kernel<<<(unsigned)(threads / 128), 128>>>(P);
+        cudaEventRecord(e1, 0);
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) return done(MR_ERR_CUDA);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (r >= 0) {
+            best = std::min(best, (double)ms);
+            sum += ms;
+        }
+    }
+    *best_ms = best;
+    if (mean_ms) *mean_ms = sum / reps;
+    return done(MR_OK);
+}

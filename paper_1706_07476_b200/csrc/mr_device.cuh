@@ -820,6 +820,151 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
 }
 
 // ------------------------------------------------------------------------------------------------
+// The cast kernel with COOPERATIVE tally adds (north_star subsystem (4); option MR_OPT_COOP_FLUSH).
+//
+// cast_kernel issues one red.global.add.f64 per segment from lanes that are 32 unrelated rays: 32 sectors per
+// instruction, and the L2 atomic unit takes about 2.1e11 such sector-requests per second (mr_microbench_red) -- the
+// unit the kernel saturates.  The same unit takes twice as many lane-adds when pairs of lanes share a sector.  Lanes of
+// different rays never do; CONSECUTIVE segments of one ray often do (an x-step stays inside the 32-byte sector of four
+// cells three times out of four).  So every lane walks kCoopWindow steps, staging (cell, score) in its own
+// shared-memory column; then the warp adds the staged pairs TRANSPOSED: one instruction carries the kCoopWindow
+// consecutive segments of 32 / kCoopWindow rays.  Scores, cells and their order per ray are unchanged; tally[c]
+// receives the same values in another order (reading Q18).
+//   column layout: entry (lane, row) at lane * (kCoopWindow + 1) + row -- conflict-free for the lane-wise writes
+//   (9 is odd) and nearly so for the transposed reads.
+//   dynamic shared memory: as cast_kernel, then per warp 32 x 9 x (8 + 4) bytes.
+// ------------------------------------------------------------------------------------------------
+constexpr int kCoopWindow = 8;
+__host__ __device__ constexpr size_t coop_warp_smem_bytes() { return (size_t)32 * (kCoopWindow + 1) * 12; }
+
+template <typename Real, typename Rec, int EDGE_MODE>
+__global__ void __launch_bounds__(256) cast_coop_kernel(const __grid_constant__ CastParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int stride = blockDim.x;
+    unsigned char *sp = smem_raw;
+    double *s_edges = reinterpret_cast<double *>(sp);
+    if (EDGE_MODE == EDGES_SHARED) sp += edges_smem_bytes_for(P.mesh.nedges);
+    AxisF *axf = reinterpret_cast<AxisF *>(sp) + threadIdx.x;
+    sp += sizeof(AxisF) * 3 * stride;
+    Real *sig = reinterpret_cast<Real *>(sp) + threadIdx.x;
+    sp += (sizeof(Real) * (size_t)(P.M + P.N) * stride + 15) & ~(size_t)15;
+    uint4 *s_dict = reinterpret_cast<uint4 *>(sp);
+    if (Rec::kTiled) sp += sizeof(uint4) * (size_t)P.ndict;
+    double *c_score = reinterpret_cast<double *>(sp + (threadIdx.x >> 5) * coop_warp_smem_bytes());
+    unsigned *c_cell = reinterpret_cast<unsigned *>(c_score + 32 * (kCoopWindow + 1));
+    const double *e = (EDGE_MODE == EDGES_SHARED) ? s_edges : P.mesh.edges;
+    if (EDGE_MODE == EDGES_SHARED) {
+        for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
+    }
+    if (Rec::kTiled) {
+        for (int i = threadIdx.x; i < P.ndict; i += blockDim.x) s_dict[i] = __ldg(P.dict + i);
+    }
+    if (EDGE_MODE == EDGES_SHARED || Rec::kTiled) __syncthreads();
+
+    const unsigned full = 0xffffffffu;
+    const unsigned lane = threadIdx.x & 31;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = i < P.n;
+    bool accepted = false;
+    unsigned nseg = 0;
+    Walker w{};
+    Rec rec;
+    double wa = 0.0;
+    auto fetch = [&]() {
+        if constexpr (Rec::kTiled)
+            rec.load_tiled(P.tiles, P.ntx, P.nty, walker_cell_index(w.pl0, w.dc0), walker_cell_index(w.pl1, w.dc1),
+                           walker_cell_index(w.pl2, w.dc2));
+        else if constexpr (Rec::kCoarse)
+            rec.load_coarse(P.crecs, P.cshift, P.cnx, P.cny, walker_cell_index(w.pl0, w.dc0), walker_cell_index(w.pl1, w.dc1),
+                            walker_cell_index(w.pl2, w.dc2));
+        else
+            rec.load(P.recs, P.ids, P.K, w.c);
+    };
+    if (live) {
+        const long long r = P.perm ? (long long)__ldg(P.perm + i) : i;
+        const Ray<Real> R = load_ray<Real>(P.rays, r);
+        accepted = R.finite && (R.E > (Real)0) && walker_init<EDGE_MODE>(w, axf, stride, P.mesh, e, R.o, R.d);
+        if (accepted) {
+            sigma_all<Real>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, R.E, sig, stride);
+            wa = R.W;
+            rec.reset();
+            fetch();
+        }
+    }
+    bool left = !accepted;
+    // one segment: walk, record, Eq. (4); returns the score (0 for a zero-length segment) and the cell
+    auto segment = [&](int &cell, double &v) {
+        double len;
+        const bool leave = walker_step<EDGE_MODE>(w, axf, stride, P.mesh, e, cell, len);
+        typename Rec::Value cur;
+        if constexpr (Rec::kTiled) cur = rec.value(s_dict);
+        else cur = rec.value();
+        if (!leave) fetch();
+        const double S = (double)Rec::sigma(cur, sig, stride, P.K);
+        double g, ex;
+        score_terms<sizeof(Real) == 8>(S, len, g, ex);
+        v = wa * g;
+        wa *= ex;
+        ++nseg;
+        left = leave;
+        return len > 0.0;
+    };
+    // the first P.agg_first segments of a ray with warp-aggregated atomics (rays born in one small region, §4.7)
+    for (int k = 0; k < P.agg_first; ++k) {
+        if (!left) {
+            int cell;
+            double v;
+            bool add = segment(cell, v);
+            const unsigned act = __activemask();
+            const unsigned peers = __match_any_sync(act, add ? cell : -1 - (int)lane);
+            if (peers & (peers - 1)) {
+                const int leader = __ffs(peers) - 1;
+                double sum = 0.0;
+                for (unsigned rest = peers; rest; rest &= rest - 1) sum += __shfl_sync(peers, v, __ffs(rest) - 1);
+                v = sum;
+                add = add && (int)lane == leader;
+            }
+            if (add) red_add_f64(P.tally + cell, v);
+        }
+    }
+    // windows of kCoopWindow steps, then the transposed adds
+    while (__any_sync(full, !left)) {
+        int k = 0;
+#pragma unroll 1
+        for (int j = 0; j < kCoopWindow; ++j) {
+            if (!left) {
+                int cell;
+                double v;
+                if (segment(cell, v)) {
+                    c_cell[lane * (kCoopWindow + 1) + k] = (unsigned)cell;
+                    c_score[lane * (kCoopWindow + 1) + k] = v;
+                    ++k;
+                }
+            }
+        }
+        __syncwarp();
+        const int row = lane % kCoopWindow;
+#pragma unroll
+        for (int p = 0; p < kCoopWindow; ++p) {
+            const int src = p * (32 / kCoopWindow) + lane / kCoopWindow;
+            const int kk = __shfl_sync(full, k, src);
+            if (row < kk) red_add_f64(P.tally + c_cell[src * (kCoopWindow + 1) + row], c_score[src * (kCoopWindow + 1) + row]);
+        }
+        __syncwarp();
+    }
+    const unsigned acc = __popc(__ballot_sync(full, accepted));
+    const unsigned rej = __popc(__ballot_sync(full, live && !accepted));
+    unsigned long long segs = nseg;
+    for (int o = 16; o > 0; o >>= 1) segs += __shfl_xor_sync(full, segs, o);
+    if (lane == 0) {
+        if (acc) atomicAdd(P.counters + 0, (unsigned long long)acc);
+        if (rej) atomicAdd(P.counters + 1, (unsigned long long)rej);
+        if (segs) atomicAdd(P.counters + 2, segs);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // The trace kernel (test entry point mr_trace_rays): the same walker, no cross sections, no tally.
 //   dynamic shared memory: [edges (EDGES_SHARED only)] [walker: 3 x blockDim x 16 B]
 // ------------------------------------------------------------------------------------------------

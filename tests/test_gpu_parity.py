@@ -306,6 +306,38 @@ def test_tally_tensor_view_is_the_resident_tally():
         assert np.array_equal(t.cpu().numpy(), m.read_tally())
 
 
+def test_tally_tensor_all_reduce_in_a_world_of_one():
+    """The one collective of the multi-GPU row: an NCCL fp64 sum all-reduce of tally_tensor().  Only one
+    GPU is available here, so the group has ONE rank: this checks that the borrowed view is a tensor NCCL accepts and
+    that the reduced view is still the resident tally -- not that two replicas add up (that runs on gloo, on the CPU)."""
+    import torch
+    import torch.distributed as dist
+
+    if not dist.is_nccl_available():
+        pytest.skip("torch built without NCCL")
+    prob = make_problem(1)
+    rays = make_rays(prob, 5000)
+    created = False
+    if not dist.is_initialized():
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29537", rank=0, world_size=1)
+        created = True
+    try:
+        with _mr(prob, 0) as m:
+            m.cast_rays(rays)
+            before = m.read_tally()
+            t = m.tally_tensor()
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
+            torch.cuda.synchronize()
+            assert np.array_equal(t.cpu().numpy(), before)
+            assert np.array_equal(m.read_tally(), before)
+            m.cast_rays(rays)                                  # the view keeps following the resident tally
+            m.sync()
+            np.testing.assert_allclose(t.cpu().numpy(), 2.0 * before, rtol=1e-12)
+    finally:
+        if created:
+            dist.destroy_process_group()
+
+
 @pytest.mark.parametrize("precision", [0, 1])
 def test_ray_ordering_prepass_on_and_off(precision):
     """MR_OPT_SORT_RAYS only changes which thread walks which ray: same counters, tally within tolerance
@@ -467,6 +499,41 @@ def test_coarse_block_records_on_off_and_detection():
         rays = tiny_rays(prob, 615, 20_000)
         m.cast_rays(rays)
         assert_tally(m.read_tally(), _oracle(prob).cast(rays, threads=_threads()).tally, 0)
+
+
+def test_cooperative_transposed_tally_adds():
+    """MR_OPT_COOP_FLUSH: lanes stage (cell, score) for 8 steps, the warp adds them transposed (8 consecutive segments of
+    4 rays per instruction).  Same counters, tallies within tolerance of the oracle, on every record path the kernel is
+    built for (dictionary 4/8/16-bit, K = 1, K = 3 pairs, dense 8) and unchanged behaviour on the others; rejected rays,
+    rays shorter than a window, a ragged last warp."""
+    from paper_1706_07476_b200 import MR_OPT_COOP_FLUSH, MR_OPT_TILED_INDEX, MonteRay
+
+    cases = []
+    p3 = make_problem(3, nx=68, ny=68, nz=40, n_e=2000)
+    cases.append((p3, make_rays(p3, 50_001), 1, "tiled4"))
+    cases.append((p3, make_rays(p3, 50_001), 0, "k3_pairs"))
+    p2 = make_problem(2, nx=60, ny=60, nz=30, n_e=2000)
+    cases.append((p2, make_rays(p2, 40_003), 0, "k1"))
+    p5 = make_problem(5, n=24, n_e=4000, n_res=50)
+    cases.append((p5, make_rays(p5, 40_000), 1, "dense8"))
+    pt = tiny_problem(631, nx=9, ny=8, nz=7, M=4, K=2, n_e=33)             # some 500 distinct records: 16-bit tiles
+    cases.append((pt, tiny_rays(pt, 631, 20_001, axis_aligned_share=0.1), 1, "tiled16"))
+    pk4 = tiny_problem(632, nx=9, ny=8, nz=7, M=5, K=4, n_e=33)            # a path the kernel is not built for
+    cases.append((pk4, tiny_rays(pk4, 632, 10_001), 1, "k4"))
+    for prob, rays, tiled, path in cases:
+        rays[::501, 6] = -1.0
+        ref = _oracle(prob).cast(rays, threads=_threads())
+        with MonteRay(0, 0) as m:
+            m.set_option(MR_OPT_TILED_INDEX, tiled)
+            m.load_problem(prob)
+            assert m.record_path() == path
+            for coop in (1, 0):
+                m.set_option(MR_OPT_COOP_FLUSH, coop)
+                m.clear_tally()
+                m.cast_rays(rays)
+                st = m.get_stats()
+                assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+                assert_tally(m.read_tally(), ref.tally, 0)
 
 
 @pytest.mark.parametrize("coarse", [1, 0])
