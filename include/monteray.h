@@ -125,9 +125,9 @@ MR_API int mr_load_mesh(mr_ctx *ctx, int nx, int ny, int nz, const double *xe, c
  * ze[iz+1] }, linear index c = ir + nr*iz (ncell = nr*nz).  Rays stay 3-D records; everything else (materials,
  * tables, mr_cast_rays, mr_trace_rays, moments, the producer ring) works as on a Cartesian mesh, with the walk of
  * radial crossings from the quadratic (ox+t dx)^2 + (oy+t dy)^2 = r_p^2, ties radial before
- * axial; a ray is rejected if x^2+y^2 >= re[nr]^2 or z is outside [ze[0], ze[nz]).  The ordering pre-pass and the
- * next-event cast are not available on R-Z meshes (MR_ERR_UNSUPPORTED for the latter).  Replaces any mesh loaded
- * before.  Errors: INVALID_ARG (re[0] != 0, not increasing), UNSUPPORTED, OOM, CUDA. */
+ * axial; a ray is rejected if x^2+y^2 >= re[nr]^2 or z is outside [ze[0], ze[nz]).  mr_cast_next_event works too
+ * (steps NZ1-NZ6 of DESIGN.md section 10.7: the same radial / axial crossings with the unnormalised direction towards the
+ * detector).  Replaces any mesh loaded before.  Errors: INVALID_ARG (re[0] != 0, not increasing), UNSUPPORTED, OOM, CUDA. */
 MR_API int mr_load_mesh_rz(mr_ctx *ctx, int nr, int nz, const double *re, const double *ze);
 
 /* 1-D spherical tally mesh ("1-D spherical meshes"): nr shells re[0] = 0 < ... < re[nr] about the origin,
@@ -237,6 +237,9 @@ MR_API int mr_load_detectors(mr_ctx *ctx, int ndet, const double *xyz);
  * W must already carry the angular density p(Omega -> detector) of the event (reading N-Q1).
  * A pair is REJECTED (counted, no contribution) if x,y,z,E or W is not finite, E <= 0, the origin is outside
  * the half-open box, or R^2 is 0 or not finite.  Asynchronous like mr_cast_rays.  n = 0 is a no-op.
+ * On an R-Z or spherical mesh the cells between event and detector are those of the mesh's own walk (radial crossings
+ * from the quadratic in t, ties radial before axial), with the same unnormalised direction and the same end at t = 1; the
+ * origin test is the mesh's (x^2+y^2 < re[nr]^2, z inside; |o|^2 < re[nr]^2 on a spherical mesh).
  * Requires mesh, materials, all tables and detectors.  Errors: INVALID_ARG, STATE, OOM, CUDA. */
 MR_API int mr_cast_next_event(mr_ctx *ctx, int64_t n, const void *rays, int where);
 

@@ -784,6 +784,44 @@ int launch_rz_cast(mr_ctx *c, const CastParams &P)
     }
 }
 
+template <typename Real, typename Rec, bool TRACE>
+int launch_rz_ne_t(mr_ctx *c, const RzNextEventParams &Q, int block)
+{
+    const size_t smem = edges_smem_bytes(c) + (size_t)(c->M + c->N) * block * sizeof(Real);
+    if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "rz mesh: planes and materials exceed shared memory");
+    if (int rc = set_smem(c, rz_next_event_kernel<Real, Rec, TRACE>, smem)) return rc;
+    int sms = 148, per_sm = 1;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    MR_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rz_next_event_kernel<Real, Rec, TRACE>, block, smem));
+    const long long pairs = Q.c.n * Q.ndet;
+    const long long grid = std::max<long long>(1, std::min<long long>((pairs + block - 1) / block, (long long)sms * std::max(per_sm, 1)));
+    MR_CUDA(c, cudaMemsetAsync(Q.work, 0, sizeof(unsigned long long), c->work_stream()));
+    rz_next_event_kernel<Real, Rec, TRACE><<<(unsigned)grid, block, smem, c->work_stream()>>>(Q);
+    c->launches += 1;
+    MR_CUDA(c, cudaGetLastError());
+    return MR_OK;
+}
+
+// next-event cast on an R-Z / spherical mesh: n device-resident events against detectors det_first .. det_first + ndet - 1
+template <bool TRACE>
+int launch_rz_next_event(mr_ctx *c, RzNextEventParams Q)
+{
+    Q.spherical = c->mesh_sphere ? 1 : 0;
+    Q.work = c->d_counters + 3;
+    const int block = c->block_threads;
+    if (c->precision == MR_PRECISION_DOUBLE)
+        return c->layout == LAYOUT_DK3 ? launch_rz_ne_t<double, CellRec<LAYOUT_DK3>, TRACE>(c, Q, block)
+                                       : launch_rz_ne_t<double, CellRecGeneric<double>, TRACE>(c, Q, block);
+    switch (c->layout) {
+    case LAYOUT_K1: return launch_rz_ne_t<float, CellRec<LAYOUT_K1>, TRACE>(c, Q, block);
+    case LAYOUT_K2: return launch_rz_ne_t<float, CellRec<LAYOUT_K2>, TRACE>(c, Q, block);
+    case LAYOUT_K3: return launch_rz_ne_t<float, CellRec<LAYOUT_K3>, TRACE>(c, Q, block);
+    case LAYOUT_K4: return launch_rz_ne_t<float, CellRec<LAYOUT_K4>, TRACE>(c, Q, block);
+    case LAYOUT_D8: return launch_rz_ne_t<float, CellRec<LAYOUT_D8>, TRACE>(c, Q, block);
+    default: return launch_rz_ne_t<float, CellRecGeneric<float>, TRACE>(c, Q, block);
+    }
+}
+
 // ---- deferred tally (mr_defer.cuh) ----------------------------------------------------------------
 constexpr int kDeferCtlWords = 72;
 
@@ -1840,6 +1878,30 @@ NextEventParams ne_params(mr_ctx *c, long long n, const void *d_rays)
     return P;
 }
 
+RzNextEventParams rz_ne_params(mr_ctx *c, long long n, const void *d_rays, int det_first, int ndet, double *det_sum,
+                               unsigned long long *counters)
+{
+    RzNextEventParams Q{};
+    Q.c.mesh = mesh_dev(c);
+    Q.c.recs = c->d_recs;
+    Q.c.ids = c->d_ids;
+    Q.c.K = c->K;
+    Q.c.M = c->M;
+    Q.c.xs = c->d_xs;
+    Q.c.N = c->N;
+    Q.c.mix_off = c->d_mix_off;
+    Q.c.mix_nuc = c->d_mix_nuc;
+    Q.c.mix_w = c->d_mix_w;
+    Q.c.rays = d_rays;
+    Q.c.n = n;
+    Q.c.counters = counters;
+    Q.det = c->d_det;
+    Q.det_first = det_first;
+    Q.ndet = ndet;
+    Q.det_sum = det_sum;
+    return Q;
+}
+
 // all detectors against n device-resident events (grid.y = detectors, at most 65535 per launch)
 int next_event_device(mr_ctx *c, long long n, const void *d_rays)
 {
@@ -1854,6 +1916,12 @@ int next_event_device(mr_ctx *c, long long n, const void *d_rays)
         c->kev.push_back(b);
     }
     MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used], c->work_stream()));
+    if (c->mesh_rz) {      // R-Z / spherical mesh: one persistent launch over all (event, detector) pairs, no ordering pre-pass
+        if (int rc = launch_rz_next_event<false>(c, rz_ne_params(c, n, d_rays, 0, c->ndet, c->d_det_sum, c->d_counters + 4))) return rc;
+        MR_CUDA(c, cudaEventRecord(c->kev[c->kev_used + 1], c->work_stream()));
+        c->kev_used += 2;
+        return MR_OK;
+    }
     // detectors in groups whose ordering scratch stays below 2^25 (event, detector) pairs
     const int group = (int)std::max<long long>(1, std::min<long long>(c->ndet, (1LL << 25) / std::max<long long>(n, 1)));
     for (int first = 0; first < c->ndet; first += group) {
@@ -1978,7 +2046,6 @@ int mr_cast_next_event(mr_ctx *c, int64_t n, const void *rays, int where)
         return c->fail(MR_ERR_INVALID_ARG, "next_event: bad count, NULL buffer or unknown location");
     if (int rc = ready_to_cast(c)) return rc;
     if (!c->ndet) return c->fail(MR_ERR_STATE, "no detectors loaded");
-    if (c->mesh_rz) return c->fail(MR_ERR_UNSUPPORTED, "the next-event cast is not implemented on R-Z meshes");
     if (n == 0) return MR_OK;
     if (int rc = upload_xs_desc(c)) return rc;
     return run_batch(c, n, rays, where, [c](long long count, const void *d_rays) { return next_event_device(c, count, d_rays); });
@@ -2012,7 +2079,6 @@ int mr_trace_next_event(mr_ctx *c, int64_t n, const void *rays, int where, int d
     if (int rc = ready_to_cast(c)) return rc;
     if (!c->ndet) return c->fail(MR_ERR_STATE, "no detectors loaded");
     if (det < 0 || det >= c->ndet) return c->fail(MR_ERR_INVALID_ARG, "trace_next_event: detector index out of range");
-    if (c->mesh_rz) return c->fail(MR_ERR_UNSUPPORTED, "the next-event cast is not implemented on R-Z meshes");
     if (n == 0) return MR_OK;
     if (int rc = upload_xs_desc(c)) return rc;
     const size_t rb = c->ray_bytes();
@@ -2041,7 +2107,11 @@ int mr_trace_next_event(mr_ctx *c, int64_t n, const void *rays, int where, int d
         d_rays = const_cast<void *>(rays);
     }
     int rc = MR_OK;
-    if (e == cudaSuccess) {
+    if (e == cudaSuccess && c->mesh_rz) {
+        RzNextEventParams Q = rz_ne_params(c, n, d_rays, det, 1, nullptr, nullptr);
+        Q.nseg = d_nseg; Q.hash = d_hash; Q.tau = d_tau; Q.score = d_score;
+        rc = launch_rz_next_event<true>(c, Q);
+    } else if (e == cudaSuccess) {
         NextEventParams P = ne_params(c, n, d_rays);
         P.det_first = det;
         P.nseg = d_nseg; P.hash = d_hash; P.tau = d_tau; P.score = d_score;

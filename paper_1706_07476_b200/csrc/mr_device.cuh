@@ -1400,6 +1400,231 @@ __global__ void __launch_bounds__(256) next_event_kernel(const __grid_constant__
 }
 
 // ------------------------------------------------------------------------------------------------
+// Next-event estimator on R-Z and spherical meshes (the NEXT-3 x NEXT-4 cell of SURVEY.md §8(f)):
+// steps NZ1-NZ6 of DESIGN.md §10.7 -- the crossing families of rz_kernel (Z4) with the UNNORMALISED direction
+// d = det - o, so that t = 1 is the detector; a pending crossing with t >= 1 ends the walk AT the detector; only tau is
+// carried; score = W exp(-tau) / R^2.  Work items are (event, detector) pairs, detector-major; persistent lanes as in
+// rz_kernel.  A lane keeps the sum of its scores for the detector it is working on and adds it to the detector's
+// resident sum when it moves on to the next detector (work items come in detector order), so a launch issues about
+// (lanes x detectors) atomics, not one per pair.
+//   dynamic shared memory: [edges] [sigma: (M+N) x blockDim Real]
+// ------------------------------------------------------------------------------------------------
+struct RzNextEventParams {
+    CastParams c;                  // mesh (nx = nr, ny = 1), records, tables, rays (events), n; c.counters -> next-event counters
+    const double *det;             // [ndet*3] all detector points
+    int det_first, ndet;           // detectors of this launch
+    double *det_sum;               // resident sums (null in a trace launch)
+    unsigned long long *work;      // pair counter, zeroed before the launch
+    uint32_t *nseg;                // per-event outputs of the test entry (one detector per launch), any may be null
+    unsigned long long *hash;
+    double *tau;
+    double *score;
+    int spherical;
+};
+
+template <typename Real, typename Rec, bool TRACE>
+__global__ void __launch_bounds__(256) rz_next_event_kernel(const __grid_constant__ RzNextEventParams Q)
+{
+    const CastParams &P = Q.c;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int stride = blockDim.x;
+    const int nr = P.mesh.nx, nz = P.mesh.nz;
+    double *s_edges = reinterpret_cast<double *>(smem_raw);
+    Real *sig = reinterpret_cast<Real *>(smem_raw + edges_smem_bytes_for(P.mesh.nedges)) + threadIdx.x;
+    for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
+    __syncthreads();
+    const double *re = s_edges, *ze = s_edges + nr + 3;
+    const bool sph = Q.spherical != 0;
+    const unsigned full = 0xffffffffu;
+    const unsigned lane = threadIdx.x & 31;
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    const long long total = P.n * Q.ndet;
+
+    long long ev = -1;
+    bool active = false, inward = false;
+    double oz = 0.0, rho2 = 0.0, a = 0.0, b = 0.0, inv_a = 0.0, inv_z = 0.0, t_r = inf, t_z = inf, t_cur = 0.0;
+    double W = 0.0, R2 = 1.0, Rd = 0.0, tau = 0.0;
+    int ir = 0, iz = 0, pz = 0, stepz = 0;
+    unsigned nseg = 0;
+    unsigned long long h = 0;
+    Rec rec;
+    int my_det = -1;                 // detector of the lane's running sum
+    double my_sum = 0.0;
+    unsigned n_acc = 0, n_rej = 0;
+    unsigned long long n_seg = 0;
+    bool exhausted = false;
+
+    for (;;) {
+        const unsigned idle = __ballot_sync(full, !active);
+        if (!exhausted && idle && (__popc(idle) >= kRefillLanes || idle == full)) {
+            unsigned long long base = 0;
+            if (lane == 0) base = atomicAdd(Q.work, (unsigned long long)__popc(idle));
+            base = __shfl_sync(full, base, 0);
+            exhausted = (long long)(base + __popc(idle)) >= total;
+            if (!active) {
+                const long long q = (long long)base + __popc(idle & ((1u << lane) - 1u));
+                if (q < total) {
+                    const int j = (int)(q / P.n);
+                    ev = q - (long long)j * P.n;
+                    const int det = Q.det_first + j;
+                    if (det != my_det) {
+                        if (!TRACE && my_det >= 0 && my_sum != 0.0) red_add_f64(Q.det_sum + my_det, my_sum);
+                        my_det = det;
+                        my_sum = 0.0;
+                    }
+                    double ox, oy;
+                    Real E;
+                    bool fin;
+                    if (sizeof(Real) == 8) {
+                        const Ray<double> R = load_ray_f64(P.rays, ev);
+                        ox = R.o[0]; oy = R.o[1]; oz = R.o[2]; W = R.W; E = (Real)R.E;
+                        fin = isfinite(ox) && isfinite(oy) && isfinite(oz) && isfinite(R.E) && isfinite(W) && R.E > 0.0;
+                    } else {
+                        const Ray<float> R = load_ray_f32(P.rays, ev);
+                        ox = R.o[0]; oy = R.o[1]; oz = R.o[2]; W = R.W; E = (Real)R.E;
+                        fin = isfinite(ox) && isfinite(oy) && isfinite(oz) && isfinite((double)R.E) && isfinite(W) && R.E > 0.0f;
+                    }
+                    // NZ1
+                    const double dx = __dsub_rn(__ldg(Q.det + 3 * det), ox), dy = __dsub_rn(__ldg(Q.det + 3 * det + 1), oy),
+                                 dz = __dsub_rn(__ldg(Q.det + 3 * det + 2), oz);
+                    R2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                    rho2 = __dadd_rn(__dmul_rn(ox, ox), __dmul_rn(oy, oy));
+                    a = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+                    if (sph) {
+                        rho2 = __dadd_rn(rho2, __dmul_rn(oz, oz));
+                        a = __dadd_rn(a, __dmul_rn(dz, dz));
+                    }
+                    inv_a = (a != 0.0) ? __drcp_rn(a) : 0.0;
+                    const bool radial = (a != 0.0) && isfinite(inv_a) && isfinite(a);
+                    inv_z = (dz != 0.0) ? __drcp_rn(dz) : 0.0;
+                    const bool axial = !sph && (dz != 0.0) && isfinite(inv_z);
+                    const bool accepted = fin && isfinite(R2) && (R2 > 0.0) && (radial || axial) &&
+                                          (rho2 < __dmul_rn(re[nr], re[nr])) && (sph || (oz >= ze[0] && oz < ze[nz]));
+                    nseg = 0;
+                    h = 0;
+                    tau = 0.0;
+                    if (accepted) {
+                        Rd = sqrt(R2);
+                        sigma_all<Real>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, E, sig, stride);       // NZ2
+                        int lo = 0, hi = nr + 1;                                                              // NZ3
+                        while (lo < hi) {
+                            const int mid = (lo + hi) >> 1;
+                            if (__dmul_rn(re[mid], re[mid]) <= rho2) lo = mid + 1; else hi = mid;
+                        }
+                        ir = lo - 1;
+                        iz = sph ? 0 : upper_bound_edges(ze, nz + 1, oz) - 1;
+                        b = __dadd_rn(__dmul_rn(ox, dx), __dmul_rn(oy, dy));                                  // NZ4
+                        if (sph) b = __dadd_rn(b, __dmul_rn(oz, dz));
+                        inward = false;
+                        t_r = inf; t_z = inf; t_cur = 0.0; pz = 0; stepz = 0;
+                        if (radial) {
+                            if (b < 0.0 && ir >= 1) {
+                                const double cc = __dsub_rn(rho2, __dmul_rn(re[ir], re[ir]));
+                                const double D = __dsub_rn(__dmul_rn(b, b), __dmul_rn(a, cc));
+                                if (D > 0.0) { inward = true; t_r = fmax(0.0, __dmul_rn(__dsub_rn(-b, __dsqrt_rn(D)), inv_a)); }
+                            }
+                            if (!inward) t_r = rz_t_radial(b, a, inv_a, rho2, re[ir + 1], true);
+                        }
+                        if (axial) {
+                            stepz = dz > 0.0 ? 1 : -1;
+                            pz = dz > 0.0 ? iz + 1 : iz;
+                            t_z = __dmul_rn(__dsub_rn(ze[pz], oz), inv_z);
+                        }
+                        if (TRACE) h = 0xcbf29ce484222325ULL;
+                        rec.reset();
+                        active = true;
+                        ++n_acc;
+                    } else {
+                        ++n_rej;
+                        if (TRACE) {
+                            if (Q.nseg) Q.nseg[ev] = 0;
+                            if (Q.hash) Q.hash[ev] = 0;
+                            if (Q.tau) Q.tau[ev] = 0.0;
+                            if (Q.score) Q.score[ev] = 0.0;
+                        }
+                    }
+                }
+            }
+        }
+        if (__ballot_sync(full, active) == 0) {
+            if (exhausted) break;
+            continue;
+        }
+        if (active) {
+            // NZ5: one segment
+            const bool ax = t_z < t_r;                      // ties: radial first
+            const double tn = ax ? t_z : t_r;
+            const bool last = tn >= 1.0;                    // the walk ends AT the detector
+            const double len = __dsub_rn(last ? 1.0 : tn, t_cur);
+            const int cell = ir + nr * iz;
+            rec.load(P.recs, P.ids, P.K, cell);
+            const double S = (double)Rec::sigma(rec.value(), sig, stride, P.K);
+            tau = fma(S, len * Rd, tau);
+            if (TRACE) {
+                const unsigned cu = (unsigned)cell;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    h ^= (unsigned long long)((cu >> (8 * q)) & 0xffu);
+                    h *= 0x100000001b3ULL;
+                }
+            }
+            ++nseg;
+            t_cur = tn;
+            const int iz_n = ax ? iz + stepz : iz;
+            const int ir_n = ax ? ir : (inward ? ir - 1 : ir + 1);
+            if (last || iz_n < 0 || iz_n >= nz || ir_n >= nr) {
+                active = false;                             // at the detector, or out of the mesh (the rest is void)
+                n_seg += nseg;
+                const double sc = W * exp_neg(tau) / R2;    // NZ6
+                my_sum += sc;
+                if (TRACE) {
+                    if (Q.nseg) Q.nseg[ev] = nseg;
+                    if (Q.hash) Q.hash[ev] = h;
+                    if (Q.tau) Q.tau[ev] = tau;
+                    if (Q.score) Q.score[ev] = sc;
+                }
+            } else {
+                iz = iz_n;
+                ir = ir_n;
+                if (ax) {
+                    pz += stepz;
+                    t_z = __dmul_rn(__dsub_rn(ze[pz], oz), inv_z);
+                }
+                const bool may_in = !ax && inward && ir >= 1;
+                const double rp = re[may_in ? ir : ir + 1];
+                const double bb = __dmul_rn(b, b);
+                double D = __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, __dmul_rn(rp, rp))));
+                bool go_in = may_in && D > 0.0;
+                if (may_in && !go_in) {
+                    const double ro = re[ir + 1];
+                    D = __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, __dmul_rn(ro, ro))));
+                }
+                const double sq = __dsqrt_rn(D);
+                const double num = go_in ? __dsub_rn(-b, sq) : __dadd_rn(-b, sq);
+                const double tr_new = fmax(0.0, __dmul_rn(num, inv_a));
+                t_r = ax ? t_r : tr_new;
+                inward = ax ? inward : go_in;
+            }
+        }
+    }
+    if (!TRACE) {
+        if (my_det >= 0 && my_sum != 0.0) red_add_f64(Q.det_sum + my_det, my_sum);
+        unsigned acc = n_acc, rej = n_rej;
+        unsigned long long segs = n_seg;
+        for (int o = 16; o > 0; o >>= 1) {
+            acc += __shfl_xor_sync(full, acc, o);
+            rej += __shfl_xor_sync(full, rej, o);
+            segs += __shfl_xor_sync(full, segs, o);
+        }
+        if (lane == 0 && P.counters) {
+            if (acc) atomicAdd(P.counters + 0, (unsigned long long)acc);
+            if (rej) atomicAdd(P.counters + 1, (unsigned long long)rej);
+            if (segs) atomicAdd(P.counters + 2, segs);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Per-batch moments, SURVEY.md §8(f) NEXT-2 (Eq. (5): FOM = 1/(sigma^2 T), sigma the standard
 // deviation of the tally mean).  mr_end_batch folds the batch that just ended:
 //     x = tally[c] - prev[c];   s2[c] += x*x;   prev[c] = tally[c]
