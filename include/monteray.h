@@ -340,6 +340,8 @@ enum {
                                  dictionary / K = 1 / K = 3 pairs / dense-8 record paths; elsewhere ignored.  0: one atomic per
                                  segment straight from the walking lane.  2 (default) = auto: on when tally + cell records fit in
                                  half the L2 (it wins there: contended, resident tallies), off when they stream through it */
+    MR_OPT_RZ_BLOCK_THREADS = 15, /* threads per CTA of the R-Z / spherical cast kernel (multiple of 32, <= 256; default 256: every CTA stages
+                                 the mesh's radii and planes in shared memory) */
     MR_OPT_AGGREGATE_FIRST = 9 /* n >= 0: the tally atomics of the first n segments of every ray are warp-aggregated (lanes that score
                                  into the same cell are found with match.any and one of them adds the sum): for batches born in a
                                  region of a few cells, where same-address atomics serialise in L2.  Default 2; 0 = off */

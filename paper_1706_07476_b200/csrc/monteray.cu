@@ -150,6 +150,7 @@ struct mr_ctx {
     size_t kev_used = 0;
     long long launches = 0;
     int block_threads = 128;
+    int rz_block_threads = 256;      // R-Z / spherical cast kernel (option MR_OPT_RZ_BLOCK_THREADS)
     int sort_rays = 1;
     int pair_records = 1;            // option MR_OPT_PAIR_RECORDS
 
@@ -750,7 +751,8 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
 template <typename Real, typename Rec, bool TRACE>
 int launch_rz_t(mr_ctx *c, const RzParams &Q, int block)
 {
-    const size_t smem = edges_smem_bytes(c) + (TRACE ? 0 : (size_t)(c->M + c->N) * block * sizeof(Real));
+    const size_t smem = edges_smem_bytes(c) + (TRACE ? 0 : (((size_t)(c->M + c->N) * block * sizeof(Real) + 15) & ~(size_t)15) +
+                                                           (size_t)(block / 32) * coop_warp_smem_bytes());
     if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "rz mesh: planes and materials exceed shared memory");
     if (int rc = set_smem(c, rz_kernel<Real, Rec, TRACE>, smem)) return rc;
     // persistent kernel: as many CTAs as can be resident; lanes pull rays from counters[3]
@@ -770,14 +772,15 @@ int launch_rz_cast(mr_ctx *c, const CastParams &P)
     RzParams Q{};
     Q.c = P;
     Q.spherical = c->mesh_sphere ? 1 : 0;
-    const int block = c->block_threads;
+    // every CTA stages the radii and planes in shared memory: 256 threads amortise that table over twice the warps
+    const int block = c->rz_block_threads;
     if (c->precision == MR_PRECISION_DOUBLE)
         return c->layout == LAYOUT_DK3 ? launch_rz_t<double, CellRec<LAYOUT_DK3>, false>(c, Q, block)
                                        : launch_rz_t<double, CellRecGeneric<double>, false>(c, Q, block);
     switch (c->layout) {
-    case LAYOUT_K1: return launch_rz_t<float, CellRec<LAYOUT_K1>, false>(c, Q, block);
-    case LAYOUT_K2: return launch_rz_t<float, CellRec<LAYOUT_K2>, false>(c, Q, block);
-    case LAYOUT_K3: return launch_rz_t<float, CellRec<LAYOUT_K3>, false>(c, Q, block);
+    case LAYOUT_K1: return launch_rz_t<float, QuadRecK1, false>(c, Q, block);
+    case LAYOUT_K2: return launch_rz_t<float, CellRec<LAYOUT_K2P>, false>(c, Q, block);
+    case LAYOUT_K3: return launch_rz_t<float, CellRec<LAYOUT_K3P>, false>(c, Q, block);
     case LAYOUT_K4: return launch_rz_t<float, CellRec<LAYOUT_K4>, false>(c, Q, block);
     case LAYOUT_D8: return launch_rz_t<float, CellRec<LAYOUT_D8>, false>(c, Q, block);
     default: return launch_rz_t<float, CellRecGeneric<float>, false>(c, Q, block);
@@ -1363,7 +1366,7 @@ int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int3
     default: rec_bytes = (size_t)K * (dbl ? 8 : 4); id_bytes = (size_t)K;
     }
     const long long chunk = std::min<long long>(c->ncell, 1LL << 22);
-    void *recs = c->dev_alloc(rec_bytes * (c->ncell + 1));   // + 1: 16-byte records are read as aligned pairs
+    void *recs = c->dev_alloc(rec_bytes * (c->ncell + 4));   // + 4: 16-byte records are read as aligned pairs, 8-byte ones in fours
     uint8_t *ids = id_bytes ? (uint8_t *)c->dev_alloc(id_bytes * c->ncell) : nullptr;
     int32_t *s_mat = (int32_t *)c->dev_alloc(sizeof(int32_t) * chunk * K);
     double *s_frac = (double *)c->dev_alloc(sizeof(double) * chunk * K);
@@ -2355,6 +2358,10 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         if (value < 32 || value > 256 || (value & 31)) return c->fail(MR_ERR_INVALID_ARG, "block threads must be a multiple of 32 in [32, 256]");
         c->block_threads = (int)value;
         return MR_OK;
+    case MR_OPT_RZ_BLOCK_THREADS:
+        if (value < 32 || value > 256 || (value & 31)) return c->fail(MR_ERR_INVALID_ARG, "block threads must be a multiple of 32 in [32, 256]");
+        c->rz_block_threads = (int)value;
+        return MR_OK;
     case MR_OPT_SORT_RAYS:
         if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "sort option is 0 or 1");
         c->sort_rays = (int)value;
@@ -2425,6 +2432,7 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     switch (option) {
     case MR_OPT_BLOCK_THREADS: *value = c->block_threads; return MR_OK;
     case MR_OPT_SORT_RAYS: *value = c->sort_rays; return MR_OK;
+    case MR_OPT_RZ_BLOCK_THREADS: *value = c->rz_block_threads; return MR_OK;
     case MR_OPT_STAGE_RAYS: *value = c->stage_rays; return MR_OK;
     case MR_OPT_COPY_THREADS: *value = c->copy_threads; return MR_OK;
     case MR_OPT_PAIR_RECORDS: *value = c->pair_records; return MR_OK;

@@ -400,7 +400,34 @@ template <> struct CellRec<LAYOUT_K1> : PlainTally {
     uint2 v;
     __device__ __forceinline__ void reset() {}
     __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c) { v = ldg_u2(reinterpret_cast<const uint2 *>(recs) + c); }
+    // through L1: for walks whose consecutive cells are neighbours in memory (radial steps on an R-Z mesh)
+    __device__ __forceinline__ void load_cached(const void *recs, const uint8_t *, int, int c) { v = __ldg(reinterpret_cast<const uint2 *>(recs) + c); }
     __device__ __forceinline__ Value value() const { return v; }
+    static __device__ __forceinline__ float sigma(const Value &v, const float *sig, int stride, int) { return __uint_as_float(v.x) * sig[v.y * stride]; }
+};
+
+// 8-byte K = 1 records fetched as 32-byte aligned GROUPS OF FOUR (cells 4j .. 4j+3: neighbours along the fastest axis) and
+// kept in registers: on an R-Z mesh a ray's consecutive cells are mostly radial neighbours, so three steps out of four
+// need no load (the R-Z kernel is bound by L2 requests: one atomic and one record load per segment).
+struct QuadRecK1 : PlainTally {
+    typedef uint2 Value;
+    uint4 a, b;
+    int tag;       // index of the resident group, -1: none
+    int sel;       // which of the four the current cell is
+    __device__ __forceinline__ void reset() { tag = -1; }
+    __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c)
+    {
+        sel = c & 3;
+        if ((c >> 2) != tag) {
+            tag = c >> 2;
+            ldg_256(reinterpret_cast<const uint4 *>(recs) + 2 * (size_t)tag, a, b);
+        }
+    }
+    __device__ __forceinline__ Value value() const
+    {
+        const uint4 h = (sel & 2) ? b : a;
+        return (sel & 1) ? make_uint2(h.z, h.w) : make_uint2(h.x, h.y);
+    }
     static __device__ __forceinline__ float sigma(const Value &v, const float *sig, int stride, int) { return __uint_as_float(v.x) * sig[v.y * stride]; }
 };
 
@@ -427,6 +454,7 @@ struct SingleRec {
     uint4 v;
     __device__ __forceinline__ void reset() {}
     __device__ __forceinline__ void load(const void *recs, const uint8_t *, int, int c) { v = ldg_u4(reinterpret_cast<const uint4 *>(recs) + c); }
+    __device__ __forceinline__ void load_cached(const void *recs, const uint8_t *, int, int c) { v = __ldg(reinterpret_cast<const uint4 *>(recs) + c); }
     __device__ __forceinline__ uint4 value() const { return v; }
 };
 template <typename Fetch> struct RecK2 : Fetch, PlainTally {
@@ -646,6 +674,19 @@ template <typename Real> struct CellRecGeneric : PlainTally {
         return s;
     }
 };
+
+// rec.load_cached(...) where the record type has one (the load goes through L1), else rec.load(...)
+template <typename Rec>
+__device__ __forceinline__ auto load_record_cached(Rec &rec, const void *recs, const uint8_t *ids, int K, int c, int)
+    -> decltype(rec.load_cached(recs, ids, K, c), void())
+{
+    rec.load_cached(recs, ids, K, c);
+}
+template <typename Rec>
+__device__ __forceinline__ void load_record_cached(Rec &rec, const void *recs, const uint8_t *ids, int K, int c, long)
+{
+    rec.load(recs, ids, K, c);
+}
 
 // ------------------------------------------------------------------------------------------------
 // S5: the two factors of Eq. (4) for one segment, x = Sigma * len >= 0:
@@ -1062,7 +1103,7 @@ __device__ __forceinline__ double rz_t_radial(double b, double a, double inv_a, 
 constexpr int kRefillLanes = 8;
 
 template <typename Real, typename Rec, bool TRACE>
-__global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParams Q)
+__global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzParams Q)
 {
     const CastParams &P = Q.c;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -1070,6 +1111,10 @@ __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParam
     const int nr = P.mesh.nx, nz = P.mesh.nz;
     double *s_edges = reinterpret_cast<double *>(smem_raw);
     Real *sig = reinterpret_cast<Real *>(smem_raw + edges_smem_bytes_for(P.mesh.nedges)) + threadIdx.x;
+    // cast launches only: per warp 32 x 9 staged (score, cell) pairs behind the sigma columns
+    unsigned char *stage = smem_raw + edges_smem_bytes_for(P.mesh.nedges) + ((sizeof(Real) * (size_t)(P.M + P.N) * stride + 15) & ~(size_t)15);
+    double *c_score = reinterpret_cast<double *>(stage + (threadIdx.x >> 5) * coop_warp_smem_bytes());
+    unsigned *c_cell = reinterpret_cast<unsigned *>(c_score + 32 * (kCoopWindow + 1));
     for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
     __syncthreads();
     const double *re = s_edges, *ze = s_edges + nr + 3;        // Cartesian layout with ny = 1: x | y (2 planes) | z
@@ -1156,7 +1201,10 @@ __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParam
                         }
                         if (TRACE) h = 0xcbf29ce484222325ULL;
                         wa = W;
-                        if (!TRACE) rec.reset();
+                        if (!TRACE) {
+                            rec.reset();
+                            rec.load(P.recs, P.ids, P.K, ir + nr * iz);
+                        }
                         active = true;
                         ++n_acc;
                     } else {
@@ -1173,12 +1221,21 @@ __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParam
             if (exhausted) break;
             continue;
         }
+        // kCoopWindow steps per lane, every scored segment staged in the lane's shared-memory column, then the warp adds
+        // the staged pairs TRANSPOSED: one instruction carries 8 consecutive segments of each of 4 rays.  On an R-Z mesh
+        // consecutive cells of a ray are mostly radial neighbours, i.e. neighbours in the tally: 4 of them share a 32-byte
+        // sector, and the L2 request rate (1 atomic + 1 record load per segment) is what bounds this kernel.
+        int k = 0;
+#pragma unroll 1
+        for (int j = 0; j < (TRACE ? 1 : kCoopWindow); ++j)
         if (active) {
             // Z5: one segment
             const bool ax = t_z < t_r;                      // ties: radial first
             const double tn = ax ? t_z : t_r;
             const double len = __dsub_rn(tn, t_cur);
             const int cell = ir + nr * iz;
+            const int iz_n = ax ? iz + stepz : iz;
+            const int ir_n = ax ? ir : (inward ? ir - 1 : ir + 1);
             if (TRACE) {
                 if ((long long)nseg < Q.cap) {
                     if (Q.cells) Q.cells[r * Q.cap + nseg] = cell;
@@ -1191,11 +1248,18 @@ __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParam
                     h *= 0x100000001b3ULL;
                 }
             } else {
-                rec.load(P.recs, P.ids, P.K, cell);
-                const double S = (double)Rec::sigma(rec.value(), sig, stride, P.K);
+                // the record of `cell` was requested one step ago (or at the refill); the next cell's is requested now,
+                // before this segment is scored, so that its L2 latency hides behind the score and the next crossing
+                const typename Rec::Value cur = rec.value();
+                if (!(iz_n < 0 || iz_n >= nz || ir_n >= nr)) rec.load(P.recs, P.ids, P.K, ir_n + nr * iz_n);
+                const double S = (double)Rec::sigma(cur, sig, stride, P.K);
                 double g, ex;
                 score_terms<sizeof(Real) == 8>(S, len, g, ex);
-                if (len > 0.0) red_add_f64(P.tally + cell, wa * g);
+                if (len > 0.0) {
+                    c_cell[lane * (kCoopWindow + 1) + k] = (unsigned)cell;
+                    c_score[lane * (kCoopWindow + 1) + k] = wa * g;
+                    ++k;
+                }
                 wa *= ex;
             }
             ++nseg;
@@ -1203,8 +1267,6 @@ __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParam
             // One instruction stream for the three kinds of step (axial, inward, outward): the next crossing of BOTH
             // families is evaluated and the one that applies is selected, never branched on.  The values that are kept
             // come from exactly the operations of Z4.
-            const int iz_n = ax ? iz + stepz : iz;
-            const int ir_n = ax ? ir : (inward ? ir - 1 : ir + 1);
             if (iz_n < 0 || iz_n >= nz || ir_n >= nr) {
                 active = false;                             // the ray has left the mesh
                 n_seg += nseg;
@@ -1237,6 +1299,17 @@ __global__ void __launch_bounds__(256) rz_kernel(const __grid_constant__ RzParam
                 t_r = ax ? t_r : tr_new;
                 inward = ax ? inward : go_in;
             }
+        }
+        if (!TRACE) {
+            __syncwarp();
+            const int row = lane % kCoopWindow;
+#pragma unroll
+            for (int p = 0; p < kCoopWindow; ++p) {
+                const int src = p * (32 / kCoopWindow) + lane / kCoopWindow;
+                const int kk = __shfl_sync(full, k, src);
+                if (row < kk) red_add_f64(P.tally + c_cell[src * (kCoopWindow + 1) + row], c_score[src * (kCoopWindow + 1) + row]);
+            }
+            __syncwarp();
         }
     }
     if (!TRACE) {
