@@ -542,6 +542,7 @@ int launch_cast_t(mr_ctx *c, const CastParams &P)
 {
     const int block = c->block_threads;
     const size_t per_block = walker_smem_bytes(block) + (size_t)(c->M + c->N) * block * sizeof(Real) +
+                             (rec_per_entry<Rec>::value ? (size_t)kPerEntryMax * block * sizeof(Real) : 0) +
                              (Rec::kTiled ? (size_t)c->ndict * sizeof(uint4) : 0);
     const int mode = edge_mode(c, per_block);
     const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
@@ -571,6 +572,7 @@ int launch_coop_t(mr_ctx *c, const CastParams &P)
 {
     const int block = c->block_threads;
     const size_t per_block = walker_smem_bytes(block) + (((size_t)(c->M + c->N) * block * sizeof(Real) + 15) & ~(size_t)15) +
+                             (rec_per_entry<Rec>::value ? (size_t)kPerEntryMax * block * sizeof(Real) : 0) +
                              (Rec::kTiled ? (size_t)c->ndict * sizeof(uint4) : 0) + (size_t)(block / 32) * coop_warp_smem_bytes();
     const int mode = edge_mode(c, per_block);
     const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;

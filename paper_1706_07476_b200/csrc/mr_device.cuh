@@ -6,6 +6,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 
 namespace mr {
 
@@ -507,11 +508,16 @@ template <> struct CellRec<LAYOUT_K4> : PlainTally {
 // y that stays inside the tile needs no global load (2-byte indices, 4 x 4 tiles): 0.29 loads per segment on the PWR-like mesh against 0.65 with
 // record pairs -- the cast kernel is bound by L2 tag look-ups, one per request.
 // BITS = index width: 16 (tiles of 4 x 4 cells, up to 1024 records), 8 (8 x 4, up to 256), 4 (8 x 8, up to 16).
+//
+// BITS = 4 (kPerEntry): with at most 16 distinct records a ray evaluates Sigma_t of EVERY dictionary entry once, right after
+// S1 (same fmaf chain in slot order, so the values are those of the per-cell evaluation bit for bit), into its own
+// shared-memory column; a step then costs one 4-byte shared load instead of the 16-byte record and K sigma reads.
 template <int BITS> struct TiledRec : PlainTally {
     static constexpr bool kTiled = true;
+    static constexpr bool kPerEntry = BITS == 4;
     static constexpr int kXs = BITS == 16 ? 2 : 3;     // log2 of the tile's x extent
     static constexpr int kYs = BITS == 4 ? 3 : 2;      // log2 of the tile's y extent
-    typedef uint4 Value;
+    typedef typename std::conditional<BITS == 4, float, uint4>::type Value;   // kPerEntry: Sigma_t itself
     uint4 a, b;
     int tag;       // resident tile, -1: none
     int e;         // entry of the current cell inside the tile: (iy & (ty - 1)) * tx + (ix & (tx - 1))
@@ -525,23 +531,42 @@ template <int BITS> struct TiledRec : PlainTally {
             ldg_256(tiles + 2 * (size_t)t, a, b);
         }
     }
-    __device__ __forceinline__ Value value(const uint4 *s_dict) const
+    __device__ __forceinline__ int entry() const       // dictionary index of the current cell
     {
         const int bit = e * BITS;
         const int r = bit >> 5;
         const uint32_t lo4 = (r & 2) ? ((r & 1) ? a.w : a.z) : ((r & 1) ? a.y : a.x);
         const uint32_t hi4 = (r & 2) ? ((r & 1) ? b.w : b.z) : ((r & 1) ? b.y : b.x);
         const uint32_t w = (r & 4) ? hi4 : lo4;
-        return s_dict[(w >> (bit & 31)) & ((1u << BITS) - 1u)];
+        return (int)((w >> (bit & 31)) & ((1u << BITS) - 1u));
     }
-    static __device__ __forceinline__ float sigma(const Value &v, const float *sig, int stride, int K)
+    // sig_e: the thread's column of per-entry Sigma_t values (kPerEntry only)
+    __device__ __forceinline__ Value value(const uint4 *s_dict, const float *sig_e, int stride) const
+    {
+        if constexpr (kPerEntry) {
+            float v = sig_e[entry() * stride];
+            asm volatile("" : "+f"(v));        // read out of the resident tile BEFORE the next tile is requested (no register copy of the tile)
+            return v;
+        } else
+            return s_dict[entry()];
+    }
+    // Sigma_t of a dictionary record (K = 3 encoding), slots added in order
+    static __device__ __forceinline__ float sigma_rec(const uint4 &v, const float *sig, int stride, int K)
     {
         float s = __uint_as_float(v.x) * sig[(v.w & 0xffu) * stride];
         if (K > 1) s = fmaf(__uint_as_float(v.y), sig[((v.w >> 8) & 0xffu) * stride], s);
         if (K > 2) s = fmaf(__uint_as_float(v.z), sig[((v.w >> 16) & 0xffu) * stride], s);
         return s;
     }
+    static __device__ __forceinline__ float sigma(const Value &v, const float *sig, int stride, int K)
+    {
+        if constexpr (kPerEntry) return v;
+        else return sigma_rec(v, sig, stride, K);
+    }
 };
+constexpr int kPerEntryMax = 16;   // dictionary entries of the kPerEntry path (TiledRec<4>)
+template <typename Rec, typename = void> struct rec_per_entry { static constexpr bool value = false; };
+template <typename Rec> struct rec_per_entry<Rec, typename std::enable_if<Rec::kPerEntry>::type> { static constexpr bool value = true; };
 
 template <> struct CellRec<LAYOUT_K4F> {
     static constexpr bool kTiled = false;
@@ -765,6 +790,9 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
     sp += sizeof(AxisF) * 3 * stride;
     Real *sig = reinterpret_cast<Real *>(sp) + threadIdx.x;
     sp += sizeof(Real) * (size_t)(P.M + P.N) * stride;
+    constexpr bool kPerEntry = rec_per_entry<Rec>::value;
+    Real *sig_e = reinterpret_cast<Real *>(sp) + threadIdx.x;   // kPerEntry: Sigma_t of every dictionary entry for this thread's ray
+    if (kPerEntry) sp += sizeof(Real) * (size_t)kPerEntryMax * stride;
     uint4 *s_dict = reinterpret_cast<uint4 *>(sp);
     const double *e = (EDGE_MODE == EDGES_SHARED) ? s_edges : P.mesh.edges;
     if (EDGE_MODE == EDGES_SHARED) {
@@ -786,6 +814,8 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
         if (accepted) {
             // S1: every material's sigma at the ray's energy, kept in this thread's shared column
             sigma_all<Real>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, R.E, sig, stride);
+            if constexpr (kPerEntry)
+                for (int q = 0; q < P.ndict; ++q) sig_e[q * stride] = Rec::sigma_rec(s_dict[q], sig, stride, P.K);
 
             double wa = R.W;   // W * exp(-tau), a running product of exp(-x)
             double *const tally = P.tally;
@@ -835,7 +865,7 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
                 double len;
                 const bool leave = walker_step<EDGE_MODE>(w, axf, stride, P.mesh, e, cell, len);
                 typename Rec::Value cur;
-                if constexpr (Rec::kTiled) cur = rec.value(s_dict);
+                if constexpr (Rec::kTiled) cur = rec.value(s_dict, (const float *)sig_e, stride);
                 else cur = rec.value();
                 if (!leave) fetch();                              // next cell's record: in flight during the score
                 score(cur, cell, len, aggregate);
@@ -890,6 +920,9 @@ __global__ void __launch_bounds__(256) cast_coop_kernel(const __grid_constant__ 
     sp += sizeof(AxisF) * 3 * stride;
     Real *sig = reinterpret_cast<Real *>(sp) + threadIdx.x;
     sp += (sizeof(Real) * (size_t)(P.M + P.N) * stride + 15) & ~(size_t)15;
+    constexpr bool kPerEntry = rec_per_entry<Rec>::value;
+    Real *sig_e = reinterpret_cast<Real *>(sp) + threadIdx.x;
+    if (kPerEntry) sp += sizeof(Real) * (size_t)kPerEntryMax * stride;
     uint4 *s_dict = reinterpret_cast<uint4 *>(sp);
     if (Rec::kTiled) sp += sizeof(uint4) * (size_t)P.ndict;
     double *c_score = reinterpret_cast<double *>(sp + (threadIdx.x >> 5) * coop_warp_smem_bytes());
@@ -928,6 +961,8 @@ __global__ void __launch_bounds__(256) cast_coop_kernel(const __grid_constant__ 
         accepted = R.finite && (R.E > (Real)0) && walker_init<EDGE_MODE>(w, axf, stride, P.mesh, e, R.o, R.d);
         if (accepted) {
             sigma_all<Real>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, R.E, sig, stride);
+            if constexpr (kPerEntry)
+                for (int q = 0; q < P.ndict; ++q) sig_e[q * stride] = Rec::sigma_rec(s_dict[q], sig, stride, P.K);
             wa = R.W;
             rec.reset();
             fetch();
@@ -939,7 +974,7 @@ __global__ void __launch_bounds__(256) cast_coop_kernel(const __grid_constant__ 
         double len;
         const bool leave = walker_step<EDGE_MODE>(w, axf, stride, P.mesh, e, cell, len);
         typename Rec::Value cur;
-        if constexpr (Rec::kTiled) cur = rec.value(s_dict);
+        if constexpr (Rec::kTiled) cur = rec.value(s_dict, (const float *)sig_e, stride);
         else cur = rec.value();
         if (!leave) fetch();
         const double S = (double)Rec::sigma(cur, sig, stride, P.K);
