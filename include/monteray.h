@@ -198,7 +198,10 @@ MR_API int mr_sync(mr_ctx *ctx);
 MR_API int mr_get_stats(mr_ctx *ctx, mr_stats *out);
 
 /* Borrowed device pointer to the ncell fp64 tally (e.g. for a caller-side NCCL all-reduce
- * across replicas).  Valid until the next mr_load_mesh / mr_destroy. */
+ * across replicas).  Valid until the next mr_load_mesh / mr_destroy.  The call brings the array up to date
+ * (work queued on the context's stream) and, from then on until the next mr_load_mesh, every cast adds
+ * straight into it: the score accumulators of MR_OPT_FUSED_TALLY and MR_OPT_TILED_TALLY, which live outside
+ * this array, are no longer used, so a view the caller keeps goes on following the tally in stream order. */
 MR_API int mr_tally_device_ptr(mr_ctx *ctx, double **out);
 
 /* ---- per-batch moments (Eq. (5) FOM = 1/(sigma^2 T), "sigma the
@@ -342,6 +345,13 @@ enum {
                                  half the L2 (it wins there: contended, resident tallies), off when they stream through it */
     MR_OPT_RZ_BLOCK_THREADS = 15, /* threads per CTA of the R-Z / spherical cast kernel (multiple of 32, <= 256; default 256: every CTA stages
                                  the mesh's radii and planes in shared memory) */
+    MR_OPT_TILED_TALLY = 16,  /* 1: on the dictionary path (MR_OPT_TILED_INDEX) the cast kernel keeps the walk in tile coordinates
+                                 and adds the scores into TILE-ORDERED accumulators (one double per tile entry: consecutive cells of a ray
+                                 are neighbours in memory whichever of x and y the ray steps in), which are moved into the linear tally
+                                 whenever it is looked at (mr_read_tally, mr_tally_device_ptr, mr_end_batch, mr_clear_tally); with
+                                 MR_OPT_COOP_FLUSH the transposed adds then share 128-byte lines (L2 requests per segment 1.0 -> 0.45).
+                                 0 (default): the kernel adds straight into the linear tally -- measured faster on every config
+                                 (the kernel is bound by instruction issue once the requests are gone) */
     MR_OPT_AGGREGATE_FIRST = 9 /* n >= 0: the tally atomics of the first n segments of every ray are warp-aggregated (lanes that score
                                  into the same cell are found with match.any and one of them adds the sum): for batches born in a
                                  region of a few cells, where same-address atomics serialise in L2.  Default 2; 0 = off */

@@ -24,6 +24,7 @@
 #include "mr_device.cuh"
 #include "mr_sort.cuh"
 #include "mr_defer.cuh"
+#include "mr_tiled.cuh"
 #include "mr_microbench.cuh"
 
 using namespace mr;
@@ -175,6 +176,15 @@ struct mr_ctx {
     uint4 *d_dict = nullptr;
     uint4 *d_tiles = nullptr;
     int ndict = 0, ntx = 0, nty = 0, tile_bits = 16;
+    // Tile-ordered score accumulators of the dictionary path (mr_tiled.cuh; option MR_OPT_TILED_TALLY): ntx * nty * nz tiles of
+    // 64 / 32 / 16 doubles, moved into d_tally whenever the tally is looked at (flush_accumulators)
+    int tiled_tally_opt = 0;
+    double *d_tally_t = nullptr;
+    long long tally_t_cells = 0;
+    bool tiled_dirty = false;
+    // mr_tally_device_ptr has handed d_tally out: from then on (until the next mesh) every cast adds straight into d_tally, so that
+    // a view the caller keeps (an all-reduce buffer, a torch tensor) goes on following the tally -- no in-record / tile accumulators
+    bool tally_borrowed = false;
     // Block-constant compositions (MIXED, K <= 4, Cartesian): one LAYOUT_K4 record per aligned block of 2^cshift cells per axis,
     // built by mr_load_materials when every such block holds one record (option MR_OPT_COARSE_RECORDS); cshift = 0: none
     int coarse_opt = 1;
@@ -267,10 +277,35 @@ cudaError_t flush_fused(mr_ctx *c)
     return cudaGetLastError();
 }
 
+// Tile-ordered accumulators of the dictionary path: bring d_tally up to date (queued on the stream).
+cudaError_t flush_tiled(mr_ctx *c)
+{
+    if (!c->tiled_dirty || !c->d_tally_t || !c->d_tally) return cudaSuccess;
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    const unsigned grid = (unsigned)std::min<long long>((c->ncell + 255) / 256, (long long)sms * 16);
+    const int xs = c->tile_bits == 16 ? 2 : 3, ys = c->tile_bits == 4 ? 3 : 2;
+    flush_tiled_kernel<<<grid, 256, 0, c->stream>>>(c->d_tally_t, c->d_tally, c->nx, c->ny, c->nz, c->ntx, c->nty, xs, ys);
+    c->launches += 1;
+    c->tiled_dirty = false;
+    return cudaGetLastError();
+}
+
+// Everything the cast kernels accumulate outside d_tally (in-record sums, tile-ordered accumulators) -> d_tally.
+cudaError_t flush_accumulators(mr_ctx *c)
+{
+    const cudaError_t e = flush_fused(c);
+    return e != cudaSuccess ? e : flush_tiled(c);
+}
+
 void free_materials(mr_ctx *c)
 {
-    if (flush_fused(c) == cudaSuccess) cudaStreamSynchronize(c->stream);   // the sums live in the records about to go
+    if (flush_accumulators(c) == cudaSuccess) cudaStreamSynchronize(c->stream);   // the sums live in buffers about to go
     c->fused = false;
+    c->dev_free(c->d_tally_t);
+    c->d_tally_t = nullptr;
+    c->tally_t_cells = 0;
+    c->tiled_dirty = false;
     c->dev_free(c->d_recs);
     c->dev_free(c->d_ids);
     c->dev_free(c->d_dict);
@@ -390,21 +425,30 @@ int build_tiled_index(mr_ctx *c, int M, const double *density, int K, const int3
     (void)M;
     uint4 *d_dict = (uint4 *)c->dev_alloc(sizeof(uint4) * kDictMax);
     uint4 *d_tiles = (uint4 *)c->dev_alloc(tiles.size() * 4);
-    if (!d_dict || !d_tiles) {
+    // tile-ordered accumulators: one double per tile entry (positions are 31-bit in the kernel)
+    const long long acc_cells = ((long long)ntx * nty * nz) << (xs + ys);
+    double *d_acc = acc_cells < (1LL << 31) ? (double *)c->dev_alloc((size_t)acc_cells * 8) : nullptr;
+    if (!d_dict || !d_tiles || (!d_acc && acc_cells < (1LL << 31))) {
         c->dev_free(d_dict);
         c->dev_free(d_tiles);
+        c->dev_free(d_acc);
         return c->fail(MR_ERR_OOM, "device allocation failed (tiled mixture index)");
     }
     cudaError_t e = cudaMemcpyAsync(d_dict, entries.data(), entries.size() * 16, cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_tiles, tiles.data(), tiles.size() * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess && d_acc) e = cudaMemsetAsync(d_acc, 0, (size_t)acc_cells * 8, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) {
         c->dev_free(d_dict);
         c->dev_free(d_tiles);
+        c->dev_free(d_acc);
         return c->fail_cuda(e, "mr_load_materials (tiled index)");
     }
     c->d_dict = d_dict;
     c->d_tiles = d_tiles;
+    c->d_tally_t = d_acc;
+    c->tally_t_cells = d_acc ? acc_cells : 0;
+    c->tiled_dirty = false;
     c->ndict = (int)entries.size();
     c->ntx = ntx;
     c->nty = nty;
@@ -589,6 +633,45 @@ int launch_cast_or_coop(mr_ctx *c, const CastParams &P)
 {
     const bool coop = c->coop_opt == 1 || (c->coop_opt == 2 && c->resident_bytes() <= c->l2_bytes / 2);
     return coop ? launch_coop_t<Real, Rec>(c, P) : launch_cast_t<Real, Rec>(c, P);
+}
+
+// cast_tiled_kernel (mr_tiled.cuh): the dictionary path with tile-ordered accumulators
+template <int BITS, int MODE, bool COOP>
+int launch_tiled_m(mr_ctx *c, const CastParams &P, int block, size_t smem)
+{
+    const long long grid = (P.n + block - 1) / block;
+    if (grid > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
+    if (int rc = set_smem(c, cast_tiled_kernel<BITS, MODE, COOP>, smem)) return rc;
+    cast_tiled_kernel<BITS, MODE, COOP><<<(unsigned)grid, block, smem, c->work_stream()>>>(P);
+    c->launches += 1;
+    MR_CUDA(c, cudaGetLastError());
+    return MR_OK;
+}
+
+template <int BITS, bool COOP>
+int launch_tiled_c(mr_ctx *c, const CastParams &P)
+{
+    const int block = c->block_threads;
+    const size_t per_block = walker_smem_bytes(block) + (((size_t)(c->M + c->N) * block * sizeof(float) + 15) & ~(size_t)15) +
+                             (BITS == 4 ? (size_t)kPerEntryMax * block * sizeof(float) : 0) + (size_t)c->ndict * sizeof(uint4) +
+                             (COOP ? (size_t)(block / 32) * coop_warp_smem_bytes() : 0);
+    const int mode = edge_mode(c, per_block);
+    const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
+    if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "materials x block threads exceed shared memory; lower MR_OPT_BLOCK_THREADS");
+    switch (mode) {
+    case EDGES_ARITH: return launch_tiled_m<BITS, EDGES_ARITH, COOP>(c, P, block, smem);
+    case EDGES_SHARED: return launch_tiled_m<BITS, EDGES_SHARED, COOP>(c, P, block, smem);
+    default: return launch_tiled_m<BITS, EDGES_GLOBAL, COOP>(c, P, block, smem);
+    }
+}
+
+bool use_coop(const mr_ctx *c) { return c->coop_opt == 1 || (c->coop_opt == 2 && c->resident_bytes() <= c->l2_bytes / 2); }
+
+template <int BITS>
+int launch_tiled(mr_ctx *c, const CastParams &P)
+{
+    c->tiled_dirty = true;
+    return use_coop(c) ? launch_tiled_c<BITS, true>(c, P) : launch_tiled_c<BITS, false>(c, P);
 }
 
 int upload_xs_desc(mr_ctx *c)
@@ -988,7 +1071,7 @@ int record_path(const mr_ctx *c)
     case LAYOUT_K1: return MR_PATH_K1;
     case LAYOUT_K2: return c->pair_records ? MR_PATH_K2_PAIRS : MR_PATH_K2;
     case LAYOUT_K3: return c->pair_records ? MR_PATH_K3_PAIRS : MR_PATH_K3;
-    case LAYOUT_K4: return (c->fused && c->defer_opt != 1) ? MR_PATH_K4_FUSED : MR_PATH_K4;
+    case LAYOUT_K4: return (c->fused && c->defer_opt != 1 && !c->tally_borrowed) ? MR_PATH_K4_FUSED : MR_PATH_K4;
     case LAYOUT_D8: return MR_PATH_DENSE8;
     default: return MR_PATH_GENERIC;
     }
@@ -1036,8 +1119,12 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
         P.ndict = c->ndict;
         P.ntx = c->ntx;
         P.nty = c->nty;
-        rc = c->tile_bits == 4 ? launch_cast_or_coop<float, TiledRec<4>>(c, P)
-           : c->tile_bits == 8 ? launch_cast_or_coop<float, TiledRec<8>>(c, P) : launch_cast_or_coop<float, TiledRec<16>>(c, P);
+        if (c->tiled_tally_opt && c->d_tally_t && !c->tally_borrowed) {
+            P.tally_t = c->d_tally_t;
+            rc = c->tile_bits == 4 ? launch_tiled<4>(c, P) : c->tile_bits == 8 ? launch_tiled<8>(c, P) : launch_tiled<16>(c, P);
+        } else
+            rc = c->tile_bits == 4 ? launch_cast_or_coop<float, TiledRec<4>>(c, P)
+               : c->tile_bits == 8 ? launch_cast_or_coop<float, TiledRec<8>>(c, P) : launch_cast_or_coop<float, TiledRec<16>>(c, P);
         break;
     case MR_PATH_COARSE:
         P.crecs = c->d_crecs;
@@ -1270,6 +1357,7 @@ int load_mesh_common(mr_ctx *c, bool rz, int nx, int ny, int nz, const double *x
     c->d_tally = nullptr;
     c->d_prev = c->d_s2 = nullptr;
     c->nbatch = 0;
+    c->tally_borrowed = false;
     const int ne = nx + ny + nz + 3;
     std::vector<double> h(ne);
     std::memcpy(h.data(), xe, sizeof(double) * (nx + 1));
@@ -1679,7 +1767,7 @@ int mr_read_tally(mr_ctx *c, double *out)
     MR_ENTER(c);
     if (!out) return c->fail(MR_ERR_INVALID_ARG, "read_tally: out is NULL");
     if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
-    MR_CUDA(c, flush_fused(c));
+    MR_CUDA(c, flush_accumulators(c));
     MR_CUDA(c, cudaMemcpyAsync(out, c->d_tally, sizeof(double) * c->ncell, cudaMemcpyDeviceToHost, c->stream));
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
     return MR_OK;
@@ -1689,7 +1777,7 @@ int mr_clear_tally(mr_ctx *c)
 {
     MR_ENTER(c);
     if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
-    MR_CUDA(c, flush_fused(c));      // empties the in-record accumulators
+    MR_CUDA(c, flush_accumulators(c));      // empties the in-record accumulators
     MR_CUDA(c, cudaMemsetAsync(c->d_tally, 0, sizeof(double) * c->ncell, c->stream));
     MR_CUDA(c, cudaMemsetAsync(c->d_counters, 0, 4 * sizeof(unsigned long long), c->stream));
     if (c->d_prev) {   // the batch moments restart with the tally
@@ -1739,7 +1827,8 @@ int mr_tally_device_ptr(mr_ctx *c, double **out)
     MR_ENTER(c);
     if (!out) return c->fail(MR_ERR_INVALID_ARG, "tally_device_ptr: out is NULL");
     if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
-    MR_CUDA(c, flush_fused(c));
+    MR_CUDA(c, flush_accumulators(c));
+    c->tally_borrowed = true;
     *out = c->d_tally;
     return MR_OK;
 }
@@ -1960,7 +2049,7 @@ int mr_end_batch(mr_ctx *c)
         MR_CUDA(c, cudaMemsetAsync(c->d_prev, 0, sizeof(double) * c->ncell, c->stream));
         MR_CUDA(c, cudaMemsetAsync(c->d_s2, 0, sizeof(double) * c->ncell, c->stream));
     }
-    MR_CUDA(c, flush_fused(c));
+    MR_CUDA(c, flush_accumulators(c));
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
     const long long want = (c->ncell / 2 + 255) / 256 + 1;
@@ -2400,6 +2489,10 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "cooperative-flush option is 0 (off), 1 (on) or 2 (auto)");
         c->coop_opt = (int)value;
         return MR_OK;
+    case MR_OPT_TILED_TALLY:
+        if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "tiled-tally option is 0 or 1");
+        c->tiled_tally_opt = (int)value;
+        return MR_OK;
     case MR_OPT_COARSE_RECORDS:
         if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "coarse-records option is 0 or 1");
         c->coarse_opt = (int)value;
@@ -2419,7 +2512,7 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
     case MR_OPT_DEFERRED_TALLY:
         if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "deferred-tally option is 0 (off), 1 (on) or 2 (auto)");
         if (value == 1 && c->fused && c->fused_dirty) {
-            MR_CUDA(c, flush_fused(c));
+            MR_CUDA(c, flush_accumulators(c));
         }
         c->defer_opt = (int)value;
         return MR_OK;
@@ -2444,6 +2537,7 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     case MR_OPT_AGGREGATE_FIRST: *value = c->agg_first; return MR_OK;
     case MR_OPT_COARSE_RECORDS: *value = c->coarse_opt; return MR_OK;
     case MR_OPT_COOP_FLUSH: *value = c->coop_opt; return MR_OK;
+    case MR_OPT_TILED_TALLY: *value = c->tiled_tally_opt; return MR_OK;
     case MR_INFO_RECORD_PATH: *value = record_path(c); return MR_OK;
     case MR_INFO_DISTINCT_RECORDS: *value = c->ndict; return MR_OK;
     case MR_INFO_COARSE_SHIFT: *value = c->cshift; return MR_OK;

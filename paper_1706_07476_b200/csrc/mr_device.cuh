@@ -72,6 +72,7 @@ struct CastParams {
     long long n;
     int agg_first;         // warp-aggregate the tally atomics of the first agg_first segments of every ray (0: never)
     double *tally;
+    double *tally_t;       // dictionary path with tile-ordered accumulators (mr_tiled.cuh): acc[tile * cells_per_tile + entry]
     unsigned long long *counters;  // [0] accepted [1] rejected [2] segments
 };
 
@@ -734,6 +735,17 @@ template <bool FULL>
 __device__ __forceinline__ void score_terms(double S, double len, double &g, double &ex)
 {
     const double x = S * len;
+    if (!FULL && x <= 0.34657359027997264) {
+        // Mixed mode, thin cell (k = 0): its own arm, so that the warps whose 32 lanes are all here (85 % of the
+        // warp-steps on the PWR-like mesh) do not issue the predicated-off range reduction of the general arm below
+        const double r = -x;
+        double q = c_expq[5];
+#pragma unroll
+        for (int i = 6; i < 12; ++i) q = fma(q, r, c_expq[i]);
+        ex = 1.0 + fma(r * r, q, r);
+        g = fma(len * r, q, len);
+        return;
+    }
     double r = -x;
     int k = 0;
     if (x > 0.34657359027997264) {                                   // ln2 / 2

@@ -414,7 +414,10 @@ def test_fused_in_record_tally_for_k4(fused):
         st = m.get_stats()
         m.clear_tally()
         assert not m.read_tally().any()
-        m.cast_rays(rays[:100])
+        view = m.tally_tensor()
+        m.cast_rays(rays[:10_000])                              # a cast AFTER the pointer was borrowed lands in the view
+        m.sync()
+        assert_tally(view.cpu().numpy(), _oracle(prob).cast(rays[:10_000], threads=_threads()).tally, 0)
         assert m.read_tally().any()
     assert nb == 2 and np.array_equal(s1, got)
     assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
@@ -534,6 +537,58 @@ def test_cooperative_transposed_tally_adds():
                 st = m.get_stats()
                 assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
                 assert_tally(m.read_tally(), ref.tally, 0)
+
+
+def test_tile_ordered_accumulators_of_the_dictionary_path():
+    """MR_OPT_TILED_TALLY: cast_tiled_kernel walks in tile coordinates and adds into tile-ordered accumulators that are moved
+    into the linear tally whenever it is looked at.  Same counters, tallies within tolerance of the oracle for 4-, 8- and
+    16-bit index tiles, with and without the transposed adds, on meshes whose sides are not multiples of the tile, with
+    non-uniform planes (plane table in shared memory), rejected rays and a ragged last warp; read / end_batch / clear see
+    everything; once the device pointer has been borrowed the casts add straight into it (the view follows the tally)."""
+    from paper_1706_07476_b200 import MR_OPT_COOP_FLUSH, MR_OPT_TILED_TALLY, MonteRay
+
+    cases = []
+    p3 = make_problem(3, nx=68, ny=68, nz=41, n_e=2000)                      # 12 distinct records: 4-bit tiles of 8 x 8, arithmetic mesh
+    cases.append((p3, make_rays(p3, 50_001), "tiled4"))
+    p2 = make_problem(2, nx=61, ny=59, nz=30, n_e=2000)                      # ragged tile edges
+    cases.append((p2, make_rays(p2, 40_003), "tiled4"))
+    p8 = tiny_problem(641, nx=13, ny=11, nz=6, M=4, K=3, n_e=33)             # repeating pattern of 100 records: 8-bit tiles of 8 x 4
+    p8.cell_mat[:] = p8.cell_mat[np.arange(p8.ncell) % 100]
+    p8.cell_frac[:] = p8.cell_frac[np.arange(p8.ncell) % 100]
+    cases.append((p8, tiny_rays(p8, 641, 20_001, axis_aligned_share=0.1), "tiled8"))
+    p16 = tiny_problem(642, nx=9, ny=8, nz=7, M=4, K=2, n_e=33)              # some 500 distinct records: 16-bit tiles of 4 x 4
+    cases.append((p16, tiny_rays(p16, 642, 20_001, axis_aligned_share=0.1), "tiled16"))
+    for prob, rays, path in cases:
+        rays[::501, 6] = -1.0
+        ref = _oracle(prob).cast(rays, threads=_threads())
+        with MonteRay(0, 0) as m:
+            m.set_option(MR_OPT_TILED_TALLY, 1)
+            m.load_problem(prob)
+            assert m.record_path() == path
+            for coop in (1, 0):
+                m.set_option(MR_OPT_COOP_FLUSH, coop)
+                m.clear_tally()
+                m.cast_rays(rays)
+                st = m.get_stats()
+                assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+                assert_tally(m.read_tally(), ref.tally, 0)
+            m.clear_tally()
+            assert not m.read_tally().any()
+            half = len(rays) // 2
+            m.cast_rays(rays[:half])
+            m.end_batch()
+            m.cast_rays(rays[half:])
+            m.end_batch()
+            s1, s2, nb = m.read_moments()
+            assert nb == 2
+            assert_tally(s1, ref.tally, 0)
+            view = m.tally_tensor()                                          # borrowed: later casts add straight into it
+            before = view.cpu().numpy().copy()
+            assert_tally(before, ref.tally, 0)
+            m.cast_rays(rays)
+            m.sync()
+            assert_tally(view.cpu().numpy(), 2.0 * ref.tally, 0)
+            assert_tally(m.read_tally(), 2.0 * ref.tally, 0)
 
 
 @pytest.mark.parametrize("coarse", [1, 0])
