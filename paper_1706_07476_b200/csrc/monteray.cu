@@ -836,7 +836,7 @@ int order_rays(mr_ctx *c, long long n, const void *d_rays, const uint32_t **perm
 template <typename Real, typename Rec, bool TRACE>
 int launch_rz_t(mr_ctx *c, const RzParams &Q, int block)
 {
-    const size_t smem = edges_smem_bytes(c) + (TRACE ? 0 : (((size_t)(c->M + c->N) * block * sizeof(Real) + 15) & ~(size_t)15) +
+    const size_t smem = edges_smem_bytes(c) + rz_re2_bytes(c->nx) + (TRACE ? 0 : (((size_t)(c->M + c->N) * block * sizeof(Real) + 15) & ~(size_t)15) +
                                                            (size_t)(block / 32) * coop_warp_smem_bytes());
     if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "rz mesh: planes and materials exceed shared memory");
     if (int rc = set_smem(c, rz_kernel<Real, Rec, TRACE>, smem)) return rc;

@@ -1149,6 +1149,23 @@ __device__ __forceinline__ double rz_t_radial(double b, double a, double inv_a, 
 // per-ray set-up rare.
 constexpr int kRefillLanes = 8;
 
+// squares of the radii, kept beside the radii in shared memory (r_p * r_p rounded once: the value every D_p is formed from)
+__host__ __device__ constexpr size_t rz_re2_bytes(int nr) { return sizeof(double) * (size_t)((nr + 2) & ~1); }
+
+__device__ __forceinline__ double lds_f64(unsigned addr)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+
+// D_p = b*b - a*(rho0^2 - r_p^2), every operation rounded to nearest (Z4); r2 = r_p * r_p
+__device__ __forceinline__ double rz_disc(double bb, double a, double rho2, double r2)
+{
+    return __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, r2)));
+}
+
+//   dynamic shared memory: [edges] [r_p^2: nr + 1 doubles] [sigma: (M+N) x blockDim Real] [cast: per warp 32 x 9 staged pairs]
 template <typename Real, typename Rec, bool TRACE>
 __global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzParams Q)
 {
@@ -1157,14 +1174,21 @@ __global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzPa
     const int stride = blockDim.x;
     const int nr = P.mesh.nx, nz = P.mesh.nz;
     double *s_edges = reinterpret_cast<double *>(smem_raw);
-    Real *sig = reinterpret_cast<Real *>(smem_raw + edges_smem_bytes_for(P.mesh.nedges)) + threadIdx.x;
+    double *s_re2 = reinterpret_cast<double *>(smem_raw + edges_smem_bytes_for(P.mesh.nedges));
+    unsigned char *sp = smem_raw + edges_smem_bytes_for(P.mesh.nedges) + rz_re2_bytes(nr);
+    Real *sig = reinterpret_cast<Real *>(sp) + threadIdx.x;
     // cast launches only: per warp 32 x 9 staged (score, cell) pairs behind the sigma columns
-    unsigned char *stage = smem_raw + edges_smem_bytes_for(P.mesh.nedges) + ((sizeof(Real) * (size_t)(P.M + P.N) * stride + 15) & ~(size_t)15);
+    unsigned char *stage = sp + ((sizeof(Real) * (size_t)(P.M + P.N) * stride + 15) & ~(size_t)15);
     double *c_score = reinterpret_cast<double *>(stage + (threadIdx.x >> 5) * coop_warp_smem_bytes());
     unsigned *c_cell = reinterpret_cast<unsigned *>(c_score + 32 * (kCoopWindow + 1));
-    for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
+    for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) {
+        const double v = __ldg(P.mesh.edges + i);
+        s_edges[i] = v;
+        if (i <= nr) s_re2[i] = __dmul_rn(v, v);
+    }
     __syncthreads();
-    const double *re = s_edges, *ze = s_edges + nr + 3;        // Cartesian layout with ny = 1: x | y (2 planes) | z
+    const double *re2 = s_re2, *ze = s_edges + nr + 3;        // Cartesian layout with ny = 1: x | y (2 planes) | z
+    const unsigned re2_addr = (unsigned)__cvta_generic_to_shared(s_re2), ze_addr = (unsigned)__cvta_generic_to_shared(ze);
     const bool sph = Q.spherical != 0;
     const unsigned full = 0xffffffffu;
     const unsigned lane = threadIdx.x & 31;
@@ -1173,8 +1197,9 @@ __global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzPa
     // per-lane ray state
     long long r = -1;
     bool active = false, inward = false;
-    double oz = 0.0, rho2 = 0.0, a = 0.0, b = 0.0, inv_a = 0.0, inv_z = 0.0, t_r = inf, t_z = inf, t_cur = 0.0, wa = 0.0;
+    double oz = 0.0, rho2 = 0.0, a = 0.0, b = 0.0, bb = 0.0, inv_a = 0.0, inv_z = 0.0, t_r = inf, t_z = inf, t_cur = 0.0, wa = 0.0;
     int ir = 0, iz = 0, pz = 0, stepz = 0;
+    int i_turn = 1;          // innermost cylinder the ray crosses: D_p > 0 exactly for p >= i_turn (D_p is non-decreasing in p)
     unsigned nseg = 0;
     unsigned long long h = 0;
     Rec rec;
@@ -1214,8 +1239,7 @@ __global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzPa
                     const bool radial = (a != 0.0) && isfinite(inv_a) && isfinite(a);
                     inv_z = (dz != 0.0) ? __drcp_rn(dz) : 0.0;
                     const bool axial = !sph && (dz != 0.0) && isfinite(inv_z);
-                    const bool accepted = fin && (radial || axial) && (rho2 < __dmul_rn(re[nr], re[nr])) &&
-                                          (sph || (oz >= ze[0] && oz < ze[nz]));
+                    const bool accepted = fin && (radial || axial) && (rho2 < re2[nr]) && (sph || (oz >= ze[0] && oz < ze[nz]));
                     nseg = 0;
                     h = 0;
                     if (accepted) {
@@ -1224,22 +1248,34 @@ __global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzPa
                         int lo = 0, hi = nr + 1;
                         while (lo < hi) {
                             const int mid = (lo + hi) >> 1;
-                            if (__dmul_rn(re[mid], re[mid]) <= rho2) lo = mid + 1; else hi = mid;
+                            if (re2[mid] <= rho2) lo = mid + 1; else hi = mid;
                         }
                         ir = lo - 1;
                         iz = sph ? 0 : upper_bound_edges(ze, nz + 1, oz) - 1;
                         // Z4
                         b = __dadd_rn(__dmul_rn(ox, dx), __dmul_rn(oy, dy));
                         if (sph) b = __dadd_rn(b, __dmul_rn(oz, dz));
+                        bb = __dmul_rn(b, b);
                         inward = false;
+                        i_turn = ir + 1;
                         t_r = inf; t_z = inf; t_cur = 0.0; pz = 0; stepz = 0;
                         if (radial) {
                             if (b < 0.0 && ir >= 1) {
-                                const double cc = __dsub_rn(rho2, __dmul_rn(re[ir], re[ir]));
-                                const double D = __dsub_rn(__dmul_rn(b, b), __dmul_rn(a, cc));
-                                if (D > 0.0) { inward = true; t_r = fmax(0.0, __dmul_rn(__dsub_rn(-b, __dsqrt_rn(D)), inv_a)); }
+                                // The walk asks "D_p > 0 ?" of every inner cylinder it comes to.  D_p is a non-decreasing function of p
+                                // (r_p^2 is, and every operation of rz_disc is monotone under round-to-nearest), so the answers are
+                                // known from ONE index, found here by bisection with the walk's own expression: the decisions are
+                                // those of Z4 bit for bit, and a step evaluates the discriminant of one cylinder only.
+                                int l = 1, u = ir + 1;
+                                while (l < u) {
+                                    const int mid = (l + u) >> 1;
+                                    if (rz_disc(bb, a, rho2, re2[mid]) > 0.0) u = mid; else l = mid + 1;
+                                }
+                                i_turn = l;
+                                inward = ir >= i_turn;
                             }
-                            if (!inward) t_r = rz_t_radial(b, a, inv_a, rho2, re[ir + 1], true);
+                            const double D = rz_disc(bb, a, rho2, re2[inward ? ir : ir + 1]);
+                            const double sq = __dsqrt_rn(D);
+                            t_r = fmax(0.0, __dmul_rn(inward ? __dsub_rn(-b, sq) : __dadd_rn(-b, sq), inv_a));
                         }
                         if (axial) {
                             stepz = dz > 0.0 ? 1 : -1;
@@ -1273,6 +1309,8 @@ __global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzPa
         // consecutive cells of a ray are mostly radial neighbours, i.e. neighbours in the tally: 4 of them share a 32-byte
         // sector, and the L2 request rate (1 atomic + 1 record load per segment) is what bounds this kernel.
         int k = 0;
+        double *st_score = c_score + lane * (kCoopWindow + 1);
+        unsigned *st_cell = c_cell + lane * (kCoopWindow + 1);
 #pragma unroll 1
         for (int j = 0; j < (TRACE ? 1 : kCoopWindow); ++j)
         if (active) {
@@ -1283,6 +1321,7 @@ __global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzPa
             const int cell = ir + nr * iz;
             const int iz_n = ax ? iz + stepz : iz;
             const int ir_n = ax ? ir : (inward ? ir - 1 : ir + 1);
+            const bool out = iz_n < 0 || iz_n >= nz || ir_n >= nr;      // the ray leaves the mesh with this segment
             if (TRACE) {
                 if ((long long)nseg < Q.cap) {
                     if (Q.cells) Q.cells[r * Q.cap + nseg] = cell;
@@ -1298,24 +1337,21 @@ __global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzPa
                 // the record of `cell` was requested one step ago (or at the refill); the next cell's is requested now,
                 // before this segment is scored, so that its L2 latency hides behind the score and the next crossing
                 const typename Rec::Value cur = rec.value();
-                if (!(iz_n < 0 || iz_n >= nz || ir_n >= nr)) rec.load(P.recs, P.ids, P.K, ir_n + nr * iz_n);
+                if (!out) rec.load(P.recs, P.ids, P.K, ir_n + nr * iz_n);
                 const double S = (double)Rec::sigma(cur, sig, stride, P.K);
                 double g, ex;
                 score_terms<sizeof(Real) == 8>(S, len, g, ex);
                 if (len > 0.0) {
-                    c_cell[lane * (kCoopWindow + 1) + k] = (unsigned)cell;
-                    c_score[lane * (kCoopWindow + 1) + k] = wa * g;
+                    *st_cell++ = (unsigned)cell;
+                    *st_score++ = wa * g;
                     ++k;
                 }
                 wa *= ex;
             }
             ++nseg;
             t_cur = tn;
-            // One instruction stream for the three kinds of step (axial, inward, outward): the next crossing of BOTH
-            // families is evaluated and the one that applies is selected, never branched on.  The values that are kept
-            // come from exactly the operations of Z4.
-            if (iz_n < 0 || iz_n >= nz || ir_n >= nr) {
-                active = false;                             // the ray has left the mesh
+            if (out) {
+                active = false;
                 n_seg += nseg;
                 if (TRACE) {
                     if (Q.nseg) Q.nseg[r] = nseg;
@@ -1326,23 +1362,17 @@ __global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzPa
                 ir = ir_n;
                 if (ax) {                                   // predicated: lanes on a radial step read nothing here
                     pz += stepz;
-                    t_z = __dmul_rn(__dsub_rn(ze[pz], oz), inv_z);
+                    t_z = __dmul_rn(__dsub_rn(lds_f64(ze_addr + 8u * (unsigned)pz), oz), inv_z);
                 }
-                // one radius per step (the kernel is bound by shared-memory wavefronts: lanes read different shells):
-                // the inner cylinder while the ray may still go inward, else the outer one; only at the turning point
-                // (inner cylinder missed, once per ray) is the outer radius read as well
-                const bool may_in = !ax && inward && ir >= 1;               // inward implies b < 0
-                const double rp = re[may_in ? ir : ir + 1];
-                const double bb = __dmul_rn(b, b);
-                double D = __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, __dmul_rn(rp, rp))));
-                bool go_in = may_in && D > 0.0;
-                if (may_in && !go_in) {
-                    const double ro = re[ir + 1];
-                    D = __dsub_rn(bb, __dmul_rn(a, __dsub_rn(rho2, __dmul_rn(ro, ro))));
-                }
+                // One instruction stream for the three kinds of step (axial, inward, outward): the next radial crossing is
+                // evaluated every time and kept on a radial step.  It is the inner cylinder of the new shell while the ray still
+                // goes inward (ir >= i_turn: D_ir > 0, see the refill), else the outer one: one radius^2 and one discriminant.
+                const bool go_in = !ax && inward && ir >= i_turn;
+                const double D = rz_disc(bb, a, rho2, lds_f64(re2_addr + 8u * (unsigned)(go_in ? ir : ir + 1)));
                 const double sq = __dsqrt_rn(D);
                 const double num = go_in ? __dsub_rn(-b, sq) : __dadd_rn(-b, sq);
-                const double tr_new = fmax(0.0, __dmul_rn(num, inv_a));
+                const double tq = __dmul_rn(num, inv_a);
+                const double tr_new = tq > 0.0 ? tq : 0.0;  // = fmax(0, tq) for every tq (+0 for -0 and for NaN), without the NaN fix-up code
                 t_r = ax ? t_r : tr_new;
                 inward = ax ? inward : go_in;
             }
