@@ -90,6 +90,18 @@ __device__ __forceinline__ void stg_stream_d4(void *p, double a, double b, doubl
 {
     asm volatile("st.global.L1::no_allocate.L2::evict_first.v4.b64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
 }
+__device__ __forceinline__ uint32_t ldg_stream_u32(const void *p)
+{
+    uint32_t v;
+    asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ double ldg_stream_f64(const void *p)
+{
+    double v;
+    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ void ldg_stream_u8(const void *p, uint4 &a, uint4 &b)
 {
     asm volatile("ld.global.nc.L1::no_allocate.L2::evict_first.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
@@ -359,23 +371,12 @@ __global__ void __launch_bounds__(256) defer_scatter_kernel(const DeferParams D,
         const unsigned cnt = (unsigned)min((unsigned long long)kDeferChunk, D.cursor[b] - k * kDeferChunk);   // a multiple of kDeferRange
         const uint32_t *cells = D.cells + (size_t)id * kDeferChunk;
         const double *scores = D.scores + (size_t)id * kDeferChunk;
-        for (unsigned i = threadIdx.x * 8; i < cnt; i += blockDim.x * 8) {
-            uint4 c0, c1;
-            ldg_stream_u8(cells + i, c0, c1);
-            if (c0.x == kDeferNoCell) continue;                    // a write-out fills its 8-entry slot from the front
-            double s0, s1, s2, s3;
-            ldg_stream_d4(scores + i, s0, s1, s2, s3);
-            red_add_f64(tally + c0.x, s0);
-            if (c0.y != kDeferNoCell) red_add_f64(tally + c0.y, s1);
-            if (c0.z != kDeferNoCell) red_add_f64(tally + c0.z, s2);
-            if (c0.w != kDeferNoCell) red_add_f64(tally + c0.w, s3);
-            if (c1.x != kDeferNoCell) {
-                ldg_stream_d4(scores + i + 4, s0, s1, s2, s3);
-                red_add_f64(tally + c1.x, s0);
-                if (c1.y != kDeferNoCell) red_add_f64(tally + c1.y, s1);
-                if (c1.z != kDeferNoCell) red_add_f64(tally + c1.z, s2);
-                if (c1.w != kDeferNoCell) red_add_f64(tally + c1.w, s3);
-            }
+        // One entry per lane: a write-out slot holds 8 CONSECUTIVE cells of one ray, so 8 neighbouring lanes of an add
+        // instruction carry neighbouring cells (x steps share a 32-byte sector of the tally): fewer L2 requests than
+        // entries, where a lane adding its own slot entry by entry would make every add a request of its own.
+        for (unsigned i = threadIdx.x; i < cnt; i += blockDim.x) {
+            const uint32_t cell = ldg_stream_u32(cells + i);
+            if (cell != kDeferNoCell) red_add_f64(tally + cell, ldg_stream_f64(scores + i));
         }
     }
 }

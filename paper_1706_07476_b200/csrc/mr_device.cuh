@@ -731,13 +731,17 @@ __constant__ double c_expq[12] = {
     1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 39916800.0, 1.0 / 3628800.0, 1.0 / 362880.0, 1.0 / 40320.0,
     1.0 / 5040.0, 1.0 / 720.0, 1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0, 0.5};
 
-template <bool FULL>
+template <bool FULL, bool WARP_VOTE = true>
 __device__ __forceinline__ void score_terms(double S, double len, double &g, double &ex)
 {
     const double x = S * len;
-    if (!FULL && x <= 0.34657359027997264) {
-        // Mixed mode, thin cell (k = 0): its own arm, so that the warps whose 32 lanes are all here (85 % of the
-        // warp-steps on the PWR-like mesh) do not issue the predicated-off range reduction of the general arm below
+    const bool thin = x <= 0.34657359027997264;
+    // WARP_VOTE false (the R-Z kernel, measured 6.3 against 6.6 ms): every lane picks its own arm
+    if (!FULL && (WARP_VOTE ? __all_sync(__activemask(), thin) : thin)) {
+        // Mixed mode, EVERY lane of the warp in a thin cell (k = 0; 85 % of the warp-steps on the PWR-like mesh): the same
+        // expressions as the k = 0 case of the general path below (bit-identical results), without its predicated-off
+        // range reduction.  The vote only picks the cheaper instruction stream: a warp with one thick cell takes the
+        // general path for all its lanes instead of both arms one after the other.
         const double r = -x;
         double q = c_expq[5];
 #pragma unroll
@@ -1340,7 +1344,7 @@ __global__ void __launch_bounds__(256, 3) rz_kernel(const __grid_constant__ RzPa
                 if (!out) rec.load(P.recs, P.ids, P.K, ir_n + nr * iz_n);
                 const double S = (double)Rec::sigma(cur, sig, stride, P.K);
                 double g, ex;
-                score_terms<sizeof(Real) == 8>(S, len, g, ex);
+                score_terms<sizeof(Real) == 8, false>(S, len, g, ex);
                 if (len > 0.0) {
                     *st_cell++ = (unsigned)cell;
                     *st_score++ = wa * g;
