@@ -1937,9 +1937,41 @@ int launch_ne_t(mr_ctx *c, const NextEventParams &P, int ndet_launch)
     }
 }
 
+// next_event_tiled_kernel (mr_tiled.cuh): dictionary path with at most 16 distinct records
+template <int MODE, bool TRACE>
+int launch_ne_tiled_m(mr_ctx *c, const NextEventParams &P, const NextEventTiles &T, int ndet_launch, int block, size_t smem)
+{
+    const long long gx = (P.n + block - 1) / block;
+    if (gx > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
+    if (int rc = set_smem(c, next_event_tiled_kernel<MODE, TRACE>, smem)) return rc;
+    next_event_tiled_kernel<MODE, TRACE><<<dim3((unsigned)gx, (unsigned)ndet_launch), block, smem, c->work_stream()>>>(P, T);
+    c->launches += 1;
+    MR_CUDA(c, cudaGetLastError());
+    return MR_OK;
+}
+
+template <bool TRACE>
+int launch_ne_tiled(mr_ctx *c, const NextEventParams &P, int ndet_launch)
+{
+    const NextEventTiles T{c->d_dict, c->d_tiles, c->ndict, c->ntx, c->nty};
+    const int block = c->block_threads;
+    const size_t per_block = walker_smem_bytes(block) + (((size_t)(c->M + c->N) * block * sizeof(float) + 15) & ~(size_t)15) +
+                             (size_t)kPerEntryMax * block * sizeof(float) + (size_t)c->ndict * sizeof(uint4);
+    const int mode = edge_mode(c, per_block);
+    const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
+    if (smem > 227 * 1024) return c->fail(MR_ERR_UNSUPPORTED, "materials x block threads exceed shared memory; lower MR_OPT_BLOCK_THREADS");
+    switch (mode) {
+    case EDGES_ARITH: return launch_ne_tiled_m<EDGES_ARITH, TRACE>(c, P, T, ndet_launch, block, smem);
+    case EDGES_SHARED: return launch_ne_tiled_m<EDGES_SHARED, TRACE>(c, P, T, ndet_launch, block, smem);
+    default: return launch_ne_tiled_m<EDGES_GLOBAL, TRACE>(c, P, T, ndet_launch, block, smem);
+    }
+}
+
 template <bool TRACE>
 int launch_next_event(mr_ctx *c, const NextEventParams &P, int ndet_launch)
 {
+    // (K = 1 meshes keep their 8-byte records: measured on config 2, 2.46 ms against 2.93 ms with the index tiles)
+    if (record_path(c) == MR_PATH_TILED4 && c->layout != LAYOUT_K1) return launch_ne_tiled<TRACE>(c, P, ndet_launch);
     if (c->precision == MR_PRECISION_DOUBLE)
         return c->layout == LAYOUT_DK3 ? launch_ne_t<double, CellRec<LAYOUT_DK3>, TRACE>(c, P, ndet_launch)
                                        : launch_ne_t<double, CellRecGeneric<double>, TRACE>(c, P, ndet_launch);

@@ -243,6 +243,170 @@ __global__ void __launch_bounds__(256) cast_tiled_kernel(const __grid_constant__
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Next-event cast (NEXT-3, steps N1-N6 of DESIGN.md section 10.3) on the dictionary path with at most 16 distinct records:
+// next_event_kernel with the walk in tile coordinates -- tile id and entry word as in cast_tiled_kernel, Sigma_t of every
+// dictionary entry evaluated once per (event, detector) pair -- so that a step costs one 4-byte shared load and, every
+// fifth step or so, one 32-byte index tile, where the record-pair path costs 0.65 uncoalesced record loads and K sigma
+// reads per step (that kernel sits on the LSU pipe, 82 %, and on instruction issue, 80 %).  Crossing parameters, their
+// order, the end at t = 1 and tau are those of next_event_kernel operation by operation; the linear cell index (needed for
+// the FNV hash of the test entry only) is rebuilt from (tile, entry).
+//   dynamic shared memory: [edges (EDGES_SHARED only)] [walker: 3 x blockDim x 16 B] [sigma: (M+N) x blockDim floats]
+//                          [per-entry Sigma_t: 16 x blockDim floats] [dictionary: ndict x 16 B]
+// ------------------------------------------------------------------------------------------------
+struct NextEventTiles {
+    const uint4 *dict;
+    const uint4 *tiles;
+    int ndict, ntx, nty;
+};
+
+template <int EDGE_MODE, bool TRACE>
+__global__ void __launch_bounds__(256) next_event_tiled_kernel(const __grid_constant__ NextEventParams P, const __grid_constant__ NextEventTiles T)
+{
+    using G = TileGeom<4>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double s_part[8];
+    const int stride = blockDim.x;
+    unsigned char *sp = smem_raw;
+    double *s_edges = reinterpret_cast<double *>(sp);
+    if (EDGE_MODE == EDGES_SHARED) sp += edges_smem_bytes_for(P.mesh.nedges);
+    AxisF *axf = reinterpret_cast<AxisF *>(sp) + threadIdx.x;
+    sp += sizeof(AxisF) * 3 * stride;
+    float *sig = reinterpret_cast<float *>(sp) + threadIdx.x;
+    sp += (sizeof(float) * (size_t)(P.M + P.N) * stride + 15) & ~(size_t)15;
+    float *sig_e = reinterpret_cast<float *>(sp) + threadIdx.x;
+    sp += sizeof(float) * (size_t)kPerEntryMax * stride;
+    uint4 *s_dict = reinterpret_cast<uint4 *>(sp);
+    const double *e = (EDGE_MODE == EDGES_SHARED) ? s_edges : P.mesh.edges;
+    if (EDGE_MODE == EDGES_SHARED) {
+        for (int i = threadIdx.x; i < P.mesh.nedges; i += blockDim.x) s_edges[i] = __ldg(P.mesh.edges + i);
+    }
+    for (int i = threadIdx.x; i < T.ndict; i += blockDim.x) s_dict[i] = __ldg(T.dict + i);
+    __syncthreads();
+    const unsigned axf_addr = smem_addr(axf), axf_step = (unsigned)stride * (unsigned)sizeof(AxisF);
+    const unsigned sige_addr = smem_addr(sig_e), sig_step = (unsigned)stride * 4u;
+    const int det = P.det_first + blockIdx.y;
+    const double D[3] = {__ldg(P.det + 3 * det), __ldg(P.det + 3 * det + 1), __ldg(P.det + 3 * det + 2)};
+
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = i < P.n;
+    bool accepted = false;
+    unsigned nseg = 0;
+    unsigned long long h = 0;
+    double tau = 0.0, score = 0.0;
+    if (live) {
+        const long long r = P.perm ? (long long)__ldg(P.perm + (size_t)blockIdx.y * P.n + i) : i;
+        const Ray<float> R = load_ray<float>(P.rays, r);
+        // N1: only x, y, z, E, W are looked at (the direction fields of the record are ignored)
+        const bool fin = isfinite(R.o[0]) && isfinite(R.o[1]) && isfinite(R.o[2]) && isfinite((double)R.E) && isfinite(R.W);
+        const double d[3] = {__dsub_rn(D[0], R.o[0]), __dsub_rn(D[1], R.o[1]), __dsub_rn(D[2], R.o[2])};
+        const double R2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+        Walker w;
+        accepted = fin && (R.E > 0.f) && isfinite(R2) && (R2 > 0.0) && walker_init<EDGE_MODE>(w, axf, stride, P.mesh, e, R.o, d);
+        if (accepted) {
+            const double Rd = sqrt(R2);
+            sigma_all<float>(P.xs, P.M, P.N, P.mix_off, P.mix_nuc, P.mix_w, R.E, sig, stride);   // N2
+            for (int q = 0; q < T.ndict; ++q) sig_e[q * stride] = TiledRec<4>::sigma_rec(s_dict[q], sig, stride, P.K);
+            asm volatile("" ::: "memory");                          // the column is read through asm loads below: keep the stores above them
+            if (TRACE) h = 0xcbf29ce484222325ULL;
+            double t0 = w.t0, t1 = w.t1, t2 = w.t2, tcur = 0.0;
+            int pl0 = w.pl0, pl1 = w.pl1, pl2 = w.pl2;
+            const int s0 = (w.dc0 > 0) - (w.dc0 < 0), s1 = (w.dc1 > 0) - (w.dc1 < 0), s2 = (w.dc2 > 0) - (w.dc2 < 0);
+            const int ix = walker_cell_index(w.pl0, w.dc0), iy = walker_cell_index(w.pl1, w.dc1), iz = walker_cell_index(w.pl2, w.dc2);
+            const int ntx = T.ntx, ntxy = T.ntx * T.nty;
+            int tag = (ix >> G::kXs) + ntx * (iy >> G::kYs) + ntxy * iz;
+            unsigned E = (((unsigned)ix | (unsigned)(iy << 8)) & G::kWrap) | G::kGuard;
+            uint4 ta, tb;
+            ldg_256(T.tiles + 2 * (size_t)tag, ta, tb);
+            for (;;) {                                               // N5
+                const bool ysel = t1 < t0;                           // ties keep x
+                const double tm = ysel ? t1 : t0;
+                const bool zsel = t2 < tm;                           // ties keep x / y
+                const double tn = zsel ? t2 : tm;
+                // the cell the walker stands in: entry of the resident tile -> Sigma_t
+                const unsigned en = (((E >> 8) << G::kXs) | (E & ((1u << G::kXs) - 1u))) & ((1u << G::kCellsLog) - 1u);
+                const unsigned bit = en * 4u;
+                const unsigned rr = bit >> 5;
+                const uint32_t lo4 = (rr & 2) ? ((rr & 1) ? ta.w : ta.z) : ((rr & 1) ? ta.y : ta.x);
+                const uint32_t hi4 = (rr & 2) ? ((rr & 1) ? tb.w : tb.z) : ((rr & 1) ? tb.y : tb.x);
+                const unsigned idx = (((rr & 4) ? hi4 : lo4) >> (bit & 31)) & 15u;
+                const float Sf = lds_f32(sige_addr + idx * sig_step);
+                if (TRACE) {
+                    // linear cell index from (tile, entry): tile = tx + ntx * (ty + nty * iz)
+                    const int tz = tag / ntxy, trem = tag - tz * ntxy, ty = trem / ntx, tx = trem - ty * ntx;
+                    const unsigned cu = (unsigned)(((tx << G::kXs) | (int)(en & ((1u << G::kXs) - 1u))) +
+                                                   P.mesh.nx * (((ty << G::kYs) | (int)(en >> G::kXs)) + P.mesh.ny * tz));
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        h ^= (unsigned long long)((cu >> (8 * b)) & 0xffu);
+                        h *= 0x100000001b3ULL;
+                    }
+                }
+                ++nseg;
+                if (tn >= 1.0) {                                     // the pending crossing lies beyond the detector: the walk ends AT it
+                    tau = fma((double)Sf, __dsub_rn(1.0, tcur) * Rd, tau);
+                    break;
+                }
+                const int a = zsel ? 2 : (ysel ? 1 : 0);
+                const int pl = zsel ? pl2 : (ysel ? pl1 : pl0);
+                const int s = zsel ? s2 : (ysel ? s1 : s0);
+                double ao, aiv;
+                lds_f64x2(axf_addr + (unsigned)a * axf_step, ao, aiv);
+                const double len = __dsub_rn(tn, tcur);
+                tcur = tn;
+                tau = fma((double)Sf, len * Rd, tau);
+                const int p = pl & 0xffff;
+                if (p == (int)((unsigned)pl >> 16)) break;           // left the mesh (outside is void)
+                const int pq = p + s;
+                const int base = (EDGE_MODE == EDGES_ARITH) ? 0 : (zsel ? P.mesh.nx + P.mesh.ny + 2 : (ysel ? P.mesh.nx + 1 : 0));
+                const double tnew = __dmul_rn(__dsub_rn(plane_pos<EDGE_MODE>(P.mesh, e, a, base, pq), ao), aiv);
+                const int pln = pl + s;
+                t0 = (zsel || ysel) ? t0 : tnew;
+                t1 = (!zsel && ysel) ? tnew : t1;
+                t2 = zsel ? tnew : t2;
+                pl0 = (zsel || ysel) ? pl0 : pln;
+                pl1 = (!zsel && ysel) ? pln : pl1;
+                pl2 = zsel ? pln : pl2;
+                E += (unsigned)s << (8 * a);
+                if (zsel || (~E & G::kGuard) != 0u) {
+                    tag += s * (zsel ? ntxy : (ysel ? ntx : 1));
+                    E = (E & G::kWrap) | G::kGuard;
+                    ldg_256(T.tiles + 2 * (size_t)tag, ta, tb);
+                }
+            }
+            score = R.W * exp_neg(tau) / R2;                         // N6
+        }
+        if (TRACE) {
+            const long long r = i;                                   // trace launches are never reordered
+            if (P.nseg) P.nseg[r] = nseg;
+            if (P.hash) P.hash[r] = h;
+            if (P.tau) P.tau[r] = tau;
+            if (P.score) P.score[r] = score;
+        }
+    }
+    // CTA totals: one fp64 atomic per CTA into the detector's sum, three counter atomics per warp
+    const unsigned full = 0xffffffffu;
+    double v = score;
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(full, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) s_part[warp] = v;
+    const unsigned acc = __popc(__ballot_sync(full, accepted));
+    const unsigned rej = __popc(__ballot_sync(full, live && !accepted));
+    unsigned long long segs = nseg;
+    for (int o = 16; o > 0; o >>= 1) segs += __shfl_xor_sync(full, segs, o);
+    if (lane == 0 && P.counters) {
+        if (acc) atomicAdd(P.counters + 0, (unsigned long long)acc);
+        if (rej) atomicAdd(P.counters + 1, (unsigned long long)rej);
+        if (segs) atomicAdd(P.counters + 2, segs);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && P.det_sum) {
+        double t = 0.0;
+        for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += s_part[i];
+        if (t != 0.0) red_add_f64(P.det_sum + det, t);
+    }
+}
+
 // Moves the tile-ordered accumulators into the linear tally (tally[c] += acc[pos(c)]; acc = 0).  One thread per cell of
 // the linear order; xs / ys = log2 of the tile extents.
 __global__ void __launch_bounds__(256) flush_tiled_kernel(double *__restrict__ acc, double *__restrict__ tally, int nx, int ny, int nz,

@@ -77,6 +77,24 @@ def test_next_event_tiny_problems(seed, K, M, uniform, precision):
     assert refs[4].rays_rejected >= 1
 
 
+@pytest.mark.parametrize("seed,K,uniform,dims", [(211, 2, False, (13, 11, 5)), (212, 3, True, (17, 9, 4)), (213, 3, False, (8, 8, 3))])
+def test_next_event_on_the_dictionary_path_with_few_records(seed, K, uniform, dims):
+    """Meshes with at most 16 distinct cell records and K >= 2 take next_event_tiled_kernel (walk in tile coordinates, per-entry
+    Sigma_t): same cell sequences (hash of the LINEAR cell indices, rebuilt from tile and entry), tau, scores and sums as the
+    oracle; plane table in shared memory (non-uniform) and arithmetic planes (uniform), sides that are not multiples of the
+    8 x 8 tile, detectors inside, on a lattice point, outside the mesh and at an event's origin."""
+    prob = tiny_problem(seed, nx=dims[0], ny=dims[1], nz=dims[2], M=4, K=K, n_e=33, uniform=uniform)
+    prob.cell_mat[:] = prob.cell_mat[np.arange(prob.ncell) % 11]         # a repeating pattern of 11 records
+    prob.cell_frac[:] = prob.cell_frac[np.arange(prob.ncell) % 11]
+    rays = tiny_rays(prob, seed, 3001, axis_aligned_share=0.1)
+    dets = [[0.31, 0.17, 0.77], [float(prob.xe[3]), float(prob.ye[2]), float(prob.ze[1])], [9.0, -7.0, 3.0],
+            rays[5, :3].astype(np.float64)]
+    with _mr(prob, 0) as m:
+        assert m.record_path() == "tiled4"
+    refs = check_next_event(prob, rays, dets, 0)
+    assert refs[3].rays_rejected >= 1
+
+
 def test_next_event_rejection_rules():
     prob = tiny_problem(261, uniform=True)
     ok = [0.0, 0.0, 0.0, np.nan, np.inf, 0.0, 1.0, 1.0]          # direction fields ignored, even non-finite
