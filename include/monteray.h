@@ -293,6 +293,16 @@ MR_API int mr_ring_close(mr_ctx *ctx);
 
 MR_API int mr_ring_get_stats(mr_ctx *ctx, mr_ring_stats *out);
 
+/* Measurement aid for Fig. 4's overlap (the CPU goes on filling the next buffer while the GPU works on
+ * the last one): `producers` (1..256) host threads created INSIDE the library push the n rays of the HOST array `rays`
+ * through mr_ring_push in pieces of rays_per_push rays (thread k owns the k-th contiguous share), then mr_ring_flush is
+ * called; *wall_ms (may be NULL) = wall-clock time from the first push to the return of the flush (the GPU work it queued
+ * may still be running: mr_read_tally waits for it).  dry_run != 0: the threads copy the same pieces into private
+ * scratch buffers instead -- no ring, no GPU: what the producers alone cost.  Requires an open ring unless dry_run.
+ * Errors: INVALID_ARG, STATE (ring not open), and those of mr_ring_push / mr_ring_flush. */
+MR_API int mr_ring_bench_producers(mr_ctx *ctx, int64_t n, const void *rays, int producers, int64_t rays_per_push, int dry_run,
+                                   double *wall_ms);
+
 /* ---- test / diagnostic entry point ------------------------------------------------------- */
 
 /* The same walk as mr_cast_rays with no tally update.  Per ray r (host outputs, any may be

@@ -44,7 +44,7 @@ EXPORTS = [
     "mr_load_materials", "mr_load_xs", "mr_cast_rays", "mr_read_tally", "mr_clear_tally", "mr_sync",
     "mr_get_stats", "mr_tally_device_ptr", "mr_trace_rays", "mr_set_option", "mr_get_option",
     "mr_end_batch", "mr_read_moments", "mr_read_mean_sigma", "mr_load_nuclide_xs", "mr_define_material", "mr_load_mesh_rz", "mr_load_mesh_sphere",
-    "mr_ring_open", "mr_ring_push", "mr_ring_flush", "mr_ring_close", "mr_ring_get_stats",
+    "mr_ring_open", "mr_ring_push", "mr_ring_flush", "mr_ring_close", "mr_ring_get_stats", "mr_ring_bench_producers",
     "mr_load_detectors", "mr_cast_next_event", "mr_read_detectors", "mr_clear_detectors", "mr_trace_next_event",
     "mr_microbench_red",
 ]
@@ -112,6 +112,7 @@ def load_library() -> C.CDLL:
         "mr_ring_flush": [vp],
         "mr_ring_close": [vp],
         "mr_ring_get_stats": [vp, C.POINTER(mr_ring_stats)],
+        "mr_ring_bench_producers": [vp, i64, vp, i32, i64, i32, C.POINTER(C.c_double)],
         "mr_load_nuclide_xs": [vp, i32, i64, vp, vp],
         "mr_define_material": [vp, i32, i32, vp, vp],
         "mr_end_batch": [vp],
@@ -409,6 +410,14 @@ class MonteRay:
         self._check(self.lib.mr_ring_get_stats(self._h, C.byref(s)))
         return {"rays_pushed": int(s.rays_pushed), "slots_shipped": int(s.slots_shipped),
                 "producer_wait_ms": float(s.producer_wait_ms)}
+
+    def ring_bench_producers(self, rays, producers: int, rays_per_push: int, dry_run: bool = False) -> float:
+        """mr_ring_bench_producers: library-side producer threads push the host batch through the ring; wall ms."""
+        rays = np.ascontiguousarray(rays, dtype=self.ray_dtype)
+        ms = C.c_double(0.0)
+        self._check(self.lib.mr_ring_bench_producers(self._h, rays.size // 8, rays.ctypes.data_as(C.c_void_p), int(producers),
+                                                     int(rays_per_push), 1 if dry_run else 0, C.byref(ms)))
+        return float(ms.value)
 
     # ---- per-batch moments (NEXT-2)
     def end_batch(self):

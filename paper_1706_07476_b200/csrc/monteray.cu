@@ -12,6 +12,7 @@
 #include <chrono>
 #include <cmath>
 #include <condition_variable>
+#include <memory>
 #include <mutex>
 #include <cstdio>
 #include <cstring>
@@ -255,6 +256,10 @@ struct mr_ctx {
         cudaError_t e_ = (call);                                        \
         if (e_ != cudaSuccess) return (ctx)->fail_cuda(e_, #call);      \
     } while (0)
+
+// The set-up calls free or replace buffers the producer ring's ship path (other threads) dereferences: refused while a ring is open.
+#define MR_NO_RING(ctx, what) \
+    if ((ctx)->ring) return (ctx)->fail(MR_ERR_STATE, std::string(what) + ": close the producer ring first (mr_ring_close)")
 
 #define MR_ENTER(ctx)                                                                      \
     if (!(ctx)) return MR_ERR_INVALID_ARG;                                                 \
@@ -1272,6 +1277,7 @@ int mr_destroy(mr_ctx *c)
     DeviceGuard guard(c->device);
     cudaStreamSynchronize(c->stream);
     if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
+    if (c->stream2) cudaStreamSynchronize(c->stream2);     // before anything its kernels may still read is freed
     if (c->ring) {
         for (RingSlot *s : c->ring->slots) {
             if (s->ev_copied) { cudaEventSynchronize(s->ev_copied); cudaEventDestroy(s->ev_copied); }
@@ -1327,8 +1333,10 @@ int mr_destroy(mr_ctx *c)
 int mr_set_stream(mr_ctx *c, void *cuda_stream)
 {
     MR_ENTER(c);
+    if (c->ring) return c->fail(MR_ERR_STATE, "set_stream: close the producer ring first (its pushes queue work on the stream)");
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
     MR_CUDA(c, cudaStreamSynchronize(c->copy_stream));
+    if (c->stream2) MR_CUDA(c, cudaStreamSynchronize(c->stream2));
     c->stream = (cudaStream_t)cuda_stream;
     return MR_OK;
 }
@@ -1401,12 +1409,14 @@ extern "C" {
 int mr_load_mesh(mr_ctx *c, int nx, int ny, int nz, const double *xe, const double *ye, const double *ze)
 {
     MR_ENTER(c);
+    MR_NO_RING(c, "mr_load_mesh");
     return load_mesh_common(c, false, nx, ny, nz, xe, ye, ze);
 }
 
 int mr_load_mesh_rz(mr_ctx *c, int nr, int nz, const double *re, const double *ze)
 {
     MR_ENTER(c);
+    MR_NO_RING(c, "mr_load_mesh_rz");
     if (nr < 1 || !re) return c->fail(MR_ERR_INVALID_ARG, "rz mesh: bad size or NULL radius array");
     if (re[0] != 0.0) return c->fail(MR_ERR_INVALID_ARG, "rz mesh: the first radius must be 0");
     const double ye[2] = {0.0, 1.0};
@@ -1416,6 +1426,7 @@ int mr_load_mesh_rz(mr_ctx *c, int nr, int nz, const double *re, const double *z
 int mr_load_mesh_sphere(mr_ctx *c, int nr, const double *re)
 {
     MR_ENTER(c);
+    MR_NO_RING(c, "mr_load_mesh_sphere");
     if (nr < 1 || !re) return c->fail(MR_ERR_INVALID_ARG, "spherical mesh: bad size or NULL radius array");
     if (re[0] != 0.0) return c->fail(MR_ERR_INVALID_ARG, "spherical mesh: the first radius must be 0");
     const double one[2] = {0.0, 1.0};
@@ -1427,6 +1438,7 @@ int mr_load_mesh_sphere(mr_ctx *c, int nr, const double *re)
 int mr_load_materials(mr_ctx *c, int M, const double *density, int K, const int32_t *cell_mat, const double *cell_frac)
 {
     MR_ENTER(c);
+    MR_NO_RING(c, "mr_load_materials");
     if (!c->d_tally) return c->fail(MR_ERR_STATE, "load the mesh before the materials");
     if (M < 1 || K < 1 || !density || !cell_mat || !cell_frac) return c->fail(MR_ERR_INVALID_ARG, "materials: bad size or NULL array");
     if (M > MR_MAX_MATERIALS) return c->fail(MR_ERR_UNSUPPORTED, "materials: M > MR_MAX_MATERIALS");
@@ -1621,6 +1633,7 @@ extern "C" {
 int mr_load_xs(mr_ctx *c, int material, int64_t n, const double *energy, const double *sigma_t)
 {
     MR_ENTER(c);
+    MR_NO_RING(c, "mr_load_xs");
     if (!c->d_recs) return c->fail(MR_ERR_STATE, "load the materials before the tables");
     if (material < 0 || material >= c->M || n < 1 || n > 0x7fffffff || !energy || !sigma_t)
         return c->fail(MR_ERR_INVALID_ARG, "xs: bad material index, size or NULL array");
@@ -1632,6 +1645,7 @@ int mr_load_xs(mr_ctx *c, int material, int64_t n, const double *energy, const d
 int mr_load_nuclide_xs(mr_ctx *c, int nuclide, int64_t n, const double *energy, const double *sigma)
 {
     MR_ENTER(c);
+    MR_NO_RING(c, "mr_load_nuclide_xs");
     if (nuclide < 0 || nuclide >= MR_MAX_NUCLIDES || n < 1 || n > 0x7fffffff || !energy || !sigma)
         return c->fail(MR_ERR_INVALID_ARG, "nuclide xs: bad nuclide index, size or NULL array");
     return load_table(c, &c->nuc_grid_of[nuclide], &c->nuc_S[nuclide], &c->nuc_n[nuclide], n, energy, sigma);
@@ -1640,6 +1654,7 @@ int mr_load_nuclide_xs(mr_ctx *c, int nuclide, int64_t n, const double *energy, 
 int mr_define_material(mr_ctx *c, int material, int nnuc, const int32_t *nuclides, const double *weights)
 {
     MR_ENTER(c);
+    MR_NO_RING(c, "mr_define_material");
     if (!c->d_recs) return c->fail(MR_ERR_STATE, "load the materials before defining their composition");
     if (material < 0 || material >= c->M || nnuc < 1 || nnuc > MR_MAX_MIX || !nuclides || !weights)
         return c->fail(MR_ERR_INVALID_ARG, "define_material: bad material index, nuclide count or NULL array");
@@ -1710,10 +1725,26 @@ int run_batch(mr_ctx *c, int64_t n, const void *rays, int where, Work work)
     // 0.2 ms (a CTA lives as long as its longest ray), and with one stream those ramps add up chunk after chunk.
     // (Not on R-Z meshes: their persistent kernel has one work counter.)
     const bool two_lanes = !c->mesh_rz && n > chunk;
-    struct LaneReset { mr_ctx *c; ~LaneReset() { c->lane = 0; } } lane_reset{c};
+    // on EVERY exit path (errors included) lane 1 is joined back into the context's stream: work the caller queues there
+    // afterwards, and the frees of mr_destroy, come after everything this call launched
+    struct LaneReset {
+        mr_ctx *c;
+        bool forked = false;
+        void join()
+        {
+            c->lane = 0;
+            if (forked) {
+                forked = false;
+                if (cudaEventRecord(c->ev_lane, c->stream2) == cudaSuccess) cudaStreamWaitEvent(c->stream, c->ev_lane, 0);
+                else cudaGetLastError();
+            }
+        }
+        ~LaneReset() { join(); }
+    } lane_reset{c};
     if (two_lanes) {
         MR_CUDA(c, cudaEventRecord(c->ev_lane, c->stream));
         MR_CUDA(c, cudaStreamWaitEvent(c->stream2, c->ev_lane, 0));
+        lane_reset.forked = true;
     }
     int k = 0;
     for (int64_t first = 0, count = 0; first < n; first += count, chunk = std::min<int64_t>(2 * chunk, (int64_t)big), ++k) {
@@ -1735,11 +1766,7 @@ int run_batch(mr_ctx *c, int64_t n, const void *rays, int where, Work work)
         MR_CUDA(c, cudaEventRecord(c->ev_done[s], c->work_stream()));
         last_slot = s;
     }
-    c->lane = 0;
-    if (two_lanes) {   // the context's stream continues after both lanes
-        MR_CUDA(c, cudaEventRecord(c->ev_lane, c->stream2));
-        MR_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_lane, 0));
-    }
+    lane_reset.join();   // the context's stream continues after both lanes
     MR_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
     c->have_timing = true;
     // the caller's buffer is consumed when the call returns: wait for the last DMA out of it
@@ -2446,6 +2473,52 @@ int mr_ring_flush(mr_ctx *c)
         return r->error;
     }
     return MR_OK;
+}
+
+// Measurement aid for the producer ring: `producers` threads INSIDE the library push the host batch through mr_ring_push
+// in pieces of `rays_per_push` rays (thread k owns the k-th contiguous share), then the ring is flushed.  A producer written in
+// Python measures the interpreter, not the ring.  dry_run != 0: the threads copy the same pieces into private scratch buffers
+// instead (what the producers cost with no ring and no GPU behind them).
+int mr_ring_bench_producers(mr_ctx *c, int64_t n, const void *rays, int producers, int64_t rays_per_push, int dry_run, double *wall_ms)
+{
+    if (!c || n < 0 || (n > 0 && !rays) || producers < 1 || producers > 256 || rays_per_push < 1) return MR_ERR_INVALID_ARG;
+    if (!dry_run && !c->ring) return MR_ERR_STATE;
+    const size_t rb = c->ray_bytes();
+    std::atomic<int> rc{MR_OK};
+    // dry run: every thread's whole share goes to a private buffer of its own size (destination lines not in cache, as in the
+    // ring), allocated and touched before the clock starts
+    std::vector<std::unique_ptr<char[]>> scratches((size_t)producers);
+    if (dry_run)
+        for (int k = 0; k < producers; ++k) {
+            const size_t bytes = (size_t)std::max<int64_t>(n * (k + 1) / producers - n * k / producers, 1) * rb;
+            scratches[(size_t)k].reset(new char[bytes]);
+            std::memset(scratches[(size_t)k].get(), 0, bytes);
+        }
+    const auto t0 = std::chrono::steady_clock::now();
+    std::vector<std::thread> pool;
+    for (int k = 0; k < producers; ++k) {
+        const int64_t lo = n * k / producers, hi = n * (k + 1) / producers;
+        char *const scratch_k = scratches[(size_t)k].get();
+        pool.emplace_back([=, &rc]() {
+            struct { char *p; char *get() const { return p; } } scratch{scratch_k};
+            for (int64_t i = lo; i < hi; i += rays_per_push) {
+                const int64_t m = std::min<int64_t>(rays_per_push, hi - i);
+                const char *src = (const char *)rays + (size_t)i * rb;
+                if (dry_run) {
+                    std::memcpy(scratch.get() + (size_t)(i - lo) * rb, src, (size_t)m * rb);
+                    asm volatile("" ::"r"(scratch.get()) : "memory");
+                } else {
+                    const int r = mr_ring_push(c, m, src);
+                    if (r != MR_OK) { rc.store(r); return; }
+                }
+            }
+        });
+    }
+    for (std::thread &t : pool) t.join();
+    int ret = rc.load();
+    if (!dry_run && ret == MR_OK) ret = mr_ring_flush(c);
+    if (wall_ms) *wall_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    return ret;
 }
 
 int mr_ring_close(mr_ctx *c)

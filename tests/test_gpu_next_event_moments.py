@@ -267,6 +267,33 @@ def test_producer_ring_many_threads_equals_one_call(precision, producers, slots,
     assert np.all(d <= bound)
 
 
+def test_ring_library_side_producers():
+    """mr_ring_bench_producers (the bench's producers: C threads inside the library): the union of what 1, 3 and 7 producer
+    threads push in ragged pieces equals one mr_cast_rays call (counters exact, tally within tolerance of the oracle); the
+    dry run touches nothing; without an open ring it is a call-order error."""
+    from paper_1706_07476_b200 import MonteRayError
+
+    prob = make_problem(1)
+    rays = make_rays(prob, 30_011)
+    ref = _oracle(prob).cast(rays)
+    with _mr(prob, 0) as m:
+        with pytest.raises(MonteRayError):
+            m.ring_bench_producers(rays, 2, 100)
+        assert m.ring_bench_producers(rays, 2, 100, dry_run=True) >= 0.0
+        assert not m.read_tally().any()
+        for producers, piece in ((1, 4096), (3, 777), (7, 50)):
+            m.clear_tally()
+            m.ring_open(3, 4096)
+            assert m.ring_bench_producers(rays, producers, piece) > 0.0
+            tally = m.read_tally()
+            st = m.get_stats()
+            assert m.ring_stats()["rays_pushed"] == len(rays)
+            m.ring_close()
+            assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+            d = np.abs(tally - ref.tally)
+            assert np.all(d <= 1e-4 * np.abs(ref.tally) + 1e-7 * ref.tally.max())
+
+
 def test_ring_call_order_errors():
     from paper_1706_07476_b200 import MonteRay, MonteRayError
 
@@ -282,8 +309,17 @@ def test_ring_call_order_errors():
         m.ring_open(2, 4096)
         with pytest.raises(MonteRayError):
             m.ring_open(2, 4096)                 # already open
+        # set-up calls would free buffers the ring's ship path uses: refused while the ring is open
+        with pytest.raises(MonteRayError):
+            m.load_mesh(prob.xe, prob.ye, prob.ze)
+        with pytest.raises(MonteRayError):
+            m.load_materials(prob.density, prob.cell_mat, prob.cell_frac)
+        with pytest.raises(MonteRayError):
+            m.load_xs(0, *prob.xs[0])
+        m.ring_push(make_rays(prob, 10))         # the ring still works
         m.ring_close()
         m.ring_close()                           # idempotent
+        m.load_xs(0, *prob.xs[0])                # and set-up works again
 
 
 # ------------------------------------------------------------------------------------- multi-nuclide materials (NEXT-4)
