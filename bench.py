@@ -60,6 +60,9 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+TRAFFIC_SOURCES = {}
+
+
 def committed_profile(workload: str, kernel: str):
     """(dram bytes per launch, limiter dict) of `kernel` on `workload` from the committed ncu captures
     (profiles/traffic.txt: `workload kernel dram_bytes commit`; profiles/limiters.json), or (None, None)."""
@@ -69,6 +72,7 @@ def committed_profile(workload: str, kernel: str):
             w = line.split()
             if len(w) >= 3 and not line.startswith("#") and w[0] == workload and w[1] == kernel:
                 traffic = float(w[2])
+                TRAFFIC_SOURCES[f"{workload}:{kernel}"] = " ".join(w[3:])   # commit and capture the figure comes from
     except OSError:
         pass
     try:
@@ -339,7 +343,13 @@ def main():
         if args.double:
             alg = seg_launch * (16 + 9 * prob.K) + n_rays * (64 + 32 * prob.M)
         achieved = alg / (kernel_ms * 1e-3) / 1e9
-        traffic, limiter = committed_profile(workload + ("_double" if args.double else ""), kernel_name)
+        wl_key = workload + ("_double" if args.double else "")
+        if "+" in kernel_name:      # the deferred tally is two kernels per cast: traffic is their sum, the limiter phase A's
+            parts = [committed_profile(wl_key, k) for k in kernel_name.split("+")]
+            traffic = sum(t for t, _ in parts) if all(t is not None for t, _ in parts) else None
+            limiter = {k: l for k, (_, l) in zip(kernel_name.split("+"), parts)} if any(l for _, l in parts) else None
+        else:
+            traffic, limiter = committed_profile(wl_key, kernel_name)
         return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "achieved_is": "algorithmic bytes (SURVEY.md 8(d)) / cast-kernel time; not DRAM traffic",
                 "peak_source": peak_src, "kernel": kernel_name, "kernel_ms": kernel_ms,
@@ -431,6 +441,8 @@ def main():
                 "ms_per_step": ms, "events": n_ne, "detectors": args.ne_detectors, "segments_per_step": int(ne_seg),
                 "roofline": {"bound": "hbm", "achieved": ne_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                              "frac": ne_bytes / (ms * 1e-3) / 1e9 / peak,
+                             "traffic": committed_profile(workload, "next_event_kernel")[0] if (n_ne, args.ne_detectors) == (2_000_000, 4) else None,
+                             "limiter": committed_profile(workload, "next_event_kernel")[1],
                              "algorithmic_bytes": "5K (4K dense) per segment + (32 + 16 M) per (event, detector) pair"}}
             for _ in range(3):
                 m.end_batch()
@@ -511,7 +523,9 @@ def main():
                 "value": rz_seg / (ms * 1e-3), "unit": UNIT, "rays_per_sec": rz_rays.shape[0] / (ms * 1e-3), "ms_per_step": ms,
                 "workload": rzp.name, "rays": int(rz_rays.shape[0]), "segments_per_step": int(rz_seg),
                 "roofline": {"bound": "hbm", "achieved": rz_bytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                             "frac": rz_bytes / (ms * 1e-3) / 1e9 / peak}}
+                             "frac": rz_bytes / (ms * 1e-3) / 1e9 / peak,
+                             "traffic": committed_profile(rzp.name, "rz_kernel")[0],
+                             "limiter": committed_profile(rzp.name, "rz_kernel")[1]}}
         except Exception as e:  # noqa: BLE001 -- report, do not lose the JSON line
             next_rows["error"] = repr(e)
     total_launches = m.get_stats().kernel_launches
@@ -558,6 +572,9 @@ def main():
                        if args.config == 3 else "no flush"},
             "rays_per_sec": rays_all * args.steps / (ms_total * 1e-3),
             "roofline": roofline, "roofline_plain_records": roofline_plain, "cpu_baseline": cpu, "e2e": e2e, "next_rows": next_rows,
+            "traffic_is": "dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures "
+                          "(profiles/traffic.txt), not measured by this run",
+            "traffic_sources": TRAFFIC_SOURCES,
             "allreduce_ms": allreduce_ms,
             "gpu_launches": int(launches), "gpu_launches_total": int(total_launches),
             "clocks": sampler.report() if sampler else None,
