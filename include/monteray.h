@@ -362,6 +362,12 @@ enum {
                                  MR_OPT_COOP_FLUSH the transposed adds then share 128-byte lines (L2 requests per segment 1.0 -> 0.45).
                                  0 (default): the kernel adds straight into the linear tally -- measured faster on every config
                                  (the kernel is bound by instruction issue once the requests are gone) */
+    MR_OPT_PERSISTENT_LANES = 17, /* the cast kernel with persistent lanes (dictionary / K = 1 / K = 3 pairs / dense-8 record paths, MIXED): the
+                                 grid is as many CTAs as are resident at once and a lane whose ray has left the mesh takes the next ray
+                                 (in the order of the MR_OPT_SORT_RAYS pre-pass) from a counter -- no tail of half-empty CTAs, no ramp per
+                                 launch.  0 (default) = never, 1 = always, 2 = auto (currently never).  Measured slower than one ray per thread on
+                                 every config: after the ordering pre-pass 29-31 of 32 lanes are busy anyway, and
+                                 the refill test, the per-lane "active" predicate and the divergent set-up cost more than the tail */
     MR_OPT_AGGREGATE_FIRST = 9 /* n >= 0: the tally atomics of the first n segments of every ray are warp-aggregated (lanes that score
                                  into the same cell are found with match.any and one of them adds the sum): for batches born in a
                                  region of a few cells, where same-address atomics serialise in L2.  Default 2; 0 = off */

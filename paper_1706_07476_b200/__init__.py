@@ -23,6 +23,7 @@ from .binding import (  # noqa: F401
     MR_OPT_FUSED_TALLY,
     MR_OPT_ORDER_MODE,
     MR_OPT_PAIR_RECORDS,
+    MR_OPT_PERSISTENT_LANES,
     MR_OPT_RZ_BLOCK_THREADS,
     MR_OPT_TILED_TALLY,
     MR_OPT_SORT_RAYS,
