@@ -352,7 +352,10 @@ enum {
                                  cells of a ray often share a 32-byte tally sector; cells of unrelated rays never do).  MIXED mode,
                                  dictionary / K = 1 / K = 3 pairs / dense-8 record paths; elsewhere ignored.  0: one atomic per
                                  segment straight from the walking lane.  2 (default) = auto: on when tally + cell records fit in
-                                 half the L2 (it wins there: contended, resident tallies), off when they stream through it */
+                                 half the L2 (it wins there: contended, resident tallies) and on the K = 3 record-pair path at any
+                                 size, off elsewhere.  3 = the same idea with pairs instead of windows of 8: every lane walks two steps
+                                 and swaps one (cell, score) pair with its neighbour lane by shuffles (no shared memory; measured
+                                 no better than 1 anywhere) */
     MR_OPT_RZ_BLOCK_THREADS = 15, /* threads per CTA of the R-Z / spherical cast kernel (multiple of 32, <= 256; default 256: every CTA stages
                                  the mesh's radii and planes in shared memory) */
     MR_OPT_TILED_TALLY = 16,  /* 1: on the dictionary path (MR_OPT_TILED_INDEX) the cast kernel keeps the walk in tile coordinates

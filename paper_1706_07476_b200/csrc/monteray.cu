@@ -612,6 +612,13 @@ int launch_coop_m(mr_ctx *c, const CastParams &P, int block, size_t smem)
 {
     const long long grid = (P.n + block - 1) / block;
     if (grid > 0x7fffffffLL) return c->fail(MR_ERR_UNSUPPORTED, "batch too large for one launch");
+    if (c->coop_opt == 3) {     // pair exchange by shuffles instead of the 8-step staging
+        if (int rc = set_smem(c, cast_coop_kernel<Real, Rec, MODE, true>, smem)) return rc;
+        cast_coop_kernel<Real, Rec, MODE, true><<<(unsigned)grid, block, smem, c->work_stream()>>>(P);
+        c->launches += 1;
+        MR_CUDA(c, cudaGetLastError());
+        return MR_OK;
+    }
     if (int rc = set_smem(c, cast_coop_kernel<Real, Rec, MODE>, smem)) return rc;
     cast_coop_kernel<Real, Rec, MODE><<<(unsigned)grid, block, smem, c->work_stream()>>>(P);
     c->launches += 1;
@@ -672,9 +679,12 @@ int launch_persist_t(mr_ctx *c, const CastParams &P)
 }
 
 template <typename Real, typename Rec>
-int launch_cast_or_coop(mr_ctx *c, const CastParams &P)
+int launch_cast_or_coop(mr_ctx *c, const CastParams &P, bool coop_auto_always = false)
 {
-    const bool coop = c->coop_opt == 1 || (c->coop_opt == 2 && c->resident_bytes() <= c->l2_bytes / 2);
+    // auto: contended, L2-resident tallies -- and the 16-byte record-pair path at any size, where a segment costs an L2 request
+    // for its record as well as for its add (config 3 with the dictionary off: 8.42 -> 7.80 ms)
+    const bool coop = c->coop_opt == 1 || c->coop_opt == 3 ||
+                      (c->coop_opt == 2 && (coop_auto_always || c->resident_bytes() <= c->l2_bytes / 2));
     const bool persist = c->persist_opt == 1 || (c->persist_opt == 2 && P.n <= c->persist_auto_max);
     if (persist) return coop ? launch_persist_t<Real, Rec, true>(c, P) : launch_persist_t<Real, Rec, false>(c, P);
     return coop ? launch_coop_t<Real, Rec>(c, P) : launch_cast_t<Real, Rec>(c, P);
@@ -1182,7 +1192,7 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     case MR_PATH_K2: rc = launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
     case MR_PATH_K3: rc = launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P); break;
     case MR_PATH_K2_PAIRS: rc = launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P); break;
-    case MR_PATH_K3_PAIRS: rc = launch_cast_or_coop<float, CellRec<LAYOUT_K3P>>(c, P); break;
+    case MR_PATH_K3_PAIRS: rc = launch_cast_or_coop<float, CellRec<LAYOUT_K3P>>(c, P, true); break;
     case MR_PATH_K4_FUSED: rc = launch_cast_t<float, CellRec<LAYOUT_K4F>>(c, P); c->fused_dirty = true; break;
     case MR_PATH_K4:
         rc = use_deferred(c, MR_PATH_K4) ? cast_deferred<CellRec<LAYOUT_K4>>(c, P) : launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P);
@@ -2631,7 +2641,7 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         c->copy_threads = (int)value;
         return MR_OK;
     case MR_OPT_COOP_FLUSH:
-        if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "cooperative-flush option is 0 (off), 1 (on) or 2 (auto)");
+        if (value < 0 || value > 3) return c->fail(MR_ERR_INVALID_ARG, "cooperative-flush option is 0 (off), 1 (on), 2 (auto) or 3 (pairs by shuffle)");
         c->coop_opt = (int)value;
         return MR_OK;
     case MR_OPT_PERSISTENT_LANES:

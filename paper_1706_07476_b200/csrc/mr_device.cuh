@@ -924,7 +924,11 @@ __global__ void __launch_bounds__(256) cast_kernel(const __grid_constant__ CastP
 constexpr int kCoopWindow = 8;
 __host__ __device__ constexpr size_t coop_warp_smem_bytes() { return (size_t)32 * (kCoopWindow + 1) * 12; }
 
-template <typename Real, typename Rec, int EDGE_MODE>
+// PAIR: instead of the 8-step shared-memory staging, every lane walks TWO steps and exchanges one (cell, score) pair with its
+// neighbour lane by shuffles, so that lanes 2i and 2i+1 of an add instruction carry two consecutive segments of one ray
+// (the same 128-byte tally line for 15 of 16 x-steps): fewer L2 requests than segments at 3 shuffles and a few selects per
+// two segments, no shared memory.
+template <typename Real, typename Rec, int EDGE_MODE, bool PAIR = false>
 __global__ void __launch_bounds__(256) cast_coop_kernel(const __grid_constant__ CastParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -1020,6 +1024,29 @@ __global__ void __launch_bounds__(256) cast_coop_kernel(const __grid_constant__ 
             if (add) red_add_f64(P.tally + cell, v);
         }
     }
+    if (PAIR) {
+        const bool even = !(lane & 1);
+        while (__any_sync(full, !left)) {
+            int cA = -1, cB = -1;                      // -1: nothing to add (zero-length segment, finished ray)
+            double vA = 0.0, vB = 0.0;
+            if (!left) {
+                int cell;
+                if (segment(cell, vA)) cA = cell;
+            }
+            if (!left) {
+                int cell;
+                if (segment(cell, vB)) cB = cell;
+            }
+            const int gc = even ? cB : cA;
+            const double gv = even ? vB : vA;
+            const int rc = __shfl_xor_sync(full, gc, 1);
+            const double rv = __shfl_xor_sync(full, gv, 1);
+            const int c1 = even ? cA : rc, c2 = even ? rc : cB;       // instruction 1: ray 2i's A and B; instruction 2: ray 2i+1's
+            const double v1 = even ? vA : rv, v2 = even ? rv : vB;
+            if (c1 >= 0) red_add_f64(P.tally + c1, v1);
+            if (c2 >= 0) red_add_f64(P.tally + c2, v2);
+        }
+    } else
     // windows of kCoopWindow steps, then the transposed adds
     while (__any_sync(full, !left)) {
         int k = 0;

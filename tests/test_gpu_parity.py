@@ -530,7 +530,7 @@ def test_cooperative_transposed_tally_adds():
             m.set_option(MR_OPT_TILED_INDEX, tiled)
             m.load_problem(prob)
             assert m.record_path() == path
-            for coop, persist in ((1, 0), (0, 0), (1, 1), (0, 1)):      # persist: cast_persist_kernel (MR_OPT_PERSISTENT_LANES)
+            for coop, persist in ((1, 0), (0, 0), (3, 0), (1, 1), (0, 1)):   # 3: pairs by shuffle; persist: cast_persist_kernel
                 m.set_option(MR_OPT_COOP_FLUSH, coop)
                 m.set_option(MR_OPT_PERSISTENT_LANES, persist)
                 m.clear_tally()
