@@ -349,11 +349,12 @@ enum {
                                  until they cover the mesh); 0 (default) = the largest s with 8 * 2^s bytes <= L2/8 */
     MR_OPT_COOP_FLUSH = 14,   /* 1: the cast kernel stages every lane's (cell, score) pairs for 8 steps in shared memory and the warp then
                                  adds them TRANSPOSED, one instruction carrying 8 consecutive segments of each of 4 rays (consecutive
-                                 cells of a ray often share a 32-byte tally sector; cells of unrelated rays never do).  MIXED mode,
-                                 dictionary / K = 1 / K = 3 pairs / dense-8 record paths; elsewhere ignored.  0: one atomic per
+                                 cells of a ray often share a 32-byte tally sector; cells of unrelated rays never do).  MIXED mode:
+                                 dictionary / K = 1 / K = 3 pairs / dense-8 record paths; DOUBLE mode: the K <= 3 record path;
+                                 elsewhere ignored.  0: one atomic per
                                  segment straight from the walking lane.  2 (default) = auto: on when tally + cell records fit in
-                                 half the L2 (it wins there: contended, resident tallies) and on the K = 3 record-pair path at any
-                                 size, off elsewhere.  3 = the same idea with pairs instead of windows of 8: every lane walks two steps
+                                 half the L2 (it wins there: contended, resident tallies) and on the K = 3 record-pair path and the
+                                 DOUBLE-mode K <= 3 path at any size, off elsewhere.  3 = the same idea with pairs instead of windows of 8: every lane walks two steps
                                  and swaps one (cell, score) pair with its neighbour lane by shuffles (no shared memory; measured
                                  no better than 1 anywhere) */
     MR_OPT_RZ_BLOCK_THREADS = 15, /* threads per CTA of the R-Z / spherical cast kernel (multiple of 32, <= 256; default 256: every CTA stages

@@ -1166,7 +1166,7 @@ int cast_device(mr_ctx *c, long long n, const void *d_rays)
     int rc;
     switch (record_path(c)) {
     case MR_PATH_RZ: rc = launch_rz_cast(c, P); break;
-    case MR_PATH_DOUBLE_K3: rc = launch_cast_t<double, CellRec<LAYOUT_DK3>>(c, P); break;
+    case MR_PATH_DOUBLE_K3: rc = launch_cast_or_coop<double, CellRec<LAYOUT_DK3>>(c, P, true); break;
     case MR_PATH_DOUBLE_GENERIC: rc = launch_cast_t<double, CellRecGeneric<double>>(c, P); break;
     case MR_PATH_TILED4: case MR_PATH_TILED8: case MR_PATH_TILED16:
         P.dict = c->d_dict;
