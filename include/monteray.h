@@ -188,10 +188,19 @@ MR_API int mr_cast_rays(mr_ctx *ctx, int64_t n, const void *rays, int where);
  * snapshot: all work queued before the call is included.  Errors: INVALID_ARG, STATE, CUDA. */
 MR_API int mr_read_tally(mr_ctx *ctx, double *out);
 
+/* The same snapshot without waiting for it: a device-side copy of the tally is taken in stream order (it holds exactly the
+ * work queued before this call) and copied to `out` on a stream of its own, so that the transfer overlaps the casts
+ * queued AFTER the call -- a host loop that casts batch after batch and wants every batch's running tally on the host
+ * pays for the read-back once, at the end, instead of once per batch (the paper's own flow reads the tally only at the
+ * end).  `out` (ncell doubles; page-locked memory if the copy is to be asynchronous) is valid after the next
+ * mr_sync or mr_read_tally; a second mr_read_tally_async waits, on the device, for the first to have left the snapshot
+ * buffer.  Allocates ncell doubles of device memory on first use.  Errors: INVALID_ARG, STATE, OOM, CUDA. */
+MR_API int mr_read_tally_async(mr_ctx *ctx, double *out);
+
 /* Zeroes the tally and the ray/segment counters (queued on the stream). */
 MR_API int mr_clear_tally(mr_ctx *ctx);
 
-/* Blocks until all queued work of the context has finished. */
+/* Blocks until all queued work of the context has finished, pending mr_read_tally_async transfers included. */
 MR_API int mr_sync(mr_ctx *ctx);
 
 /* Synchronises and fills *out. */

@@ -42,7 +42,7 @@ _STATUS = {1: "MR_ERR_INVALID_ARG", 2: "MR_ERR_STATE", 3: "MR_ERR_CUDA", 4: "MR_
 
 EXPORTS = [
     "mr_create", "mr_create_ex", "mr_destroy", "mr_set_stream", "mr_last_error", "mr_load_mesh",
-    "mr_load_materials", "mr_load_xs", "mr_cast_rays", "mr_read_tally", "mr_clear_tally", "mr_sync",
+    "mr_load_materials", "mr_load_xs", "mr_cast_rays", "mr_read_tally", "mr_read_tally_async", "mr_clear_tally", "mr_sync",
     "mr_get_stats", "mr_tally_device_ptr", "mr_trace_rays", "mr_set_option", "mr_get_option",
     "mr_end_batch", "mr_read_moments", "mr_read_mean_sigma", "mr_load_nuclide_xs", "mr_define_material", "mr_load_mesh_rz", "mr_load_mesh_sphere",
     "mr_ring_open", "mr_ring_push", "mr_ring_flush", "mr_ring_close", "mr_ring_get_stats", "mr_ring_bench_producers",
@@ -101,6 +101,7 @@ def load_library() -> C.CDLL:
         "mr_load_xs": [vp, i32, i64, vp, vp],
         "mr_cast_rays": [vp, i64, vp, i32],
         "mr_read_tally": [vp, vp],
+        "mr_read_tally_async": [vp, vp],
         "mr_clear_tally": [vp],
         "mr_sync": [vp],
         "mr_get_stats": [vp, C.POINTER(mr_stats)],
@@ -346,6 +347,10 @@ class MonteRay:
     def read_tally_into(self, host_ptr: int):
         """mr_read_tally into caller-owned host memory (e.g. a pinned torch tensor's data_ptr())."""
         self._check(self.lib.mr_read_tally(self._h, C.c_void_p(host_ptr)))
+
+    def read_tally_async_into(self, host_ptr: int):
+        """mr_read_tally_async into caller-owned (page-locked) host memory; valid after sync()."""
+        self._check(self.lib.mr_read_tally_async(self._h, C.c_void_p(host_ptr)))
 
     def clear_tally(self):
         self._check(self.lib.mr_clear_tally(self._h))

@@ -84,6 +84,11 @@ struct mr_ctx {
     int precision = MR_PRECISION_MIXED;
     cudaStream_t stream = nullptr;
     cudaStream_t copy_stream = nullptr;
+    // mr_read_tally_async: device snapshot of the tally, its own D2H stream and events
+    cudaStream_t read_stream = nullptr;
+    double *d_snap = nullptr;
+    cudaEvent_t ev_snap = nullptr, ev_read = nullptr;
+    bool read_pending = false;
     mr_allocator alloc{nullptr, nullptr, nullptr};
     std::string err;
     bool sticky_cuda = false;
@@ -1328,6 +1333,13 @@ int mr_destroy(mr_ctx *c)
     cudaStreamSynchronize(c->stream);
     if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
     if (c->stream2) cudaStreamSynchronize(c->stream2);     // before anything its kernels may still read is freed
+    if (c->read_stream) {
+        cudaStreamSynchronize(c->read_stream);
+        cudaStreamDestroy(c->read_stream);
+        if (c->ev_snap) cudaEventDestroy(c->ev_snap);
+        if (c->ev_read) cudaEventDestroy(c->ev_read);
+    }
+    c->dev_free(c->d_snap);
     if (c->ring) {
         for (RingSlot *s : c->ring->slots) {
             if (s->ev_copied) { cudaEventSynchronize(s->ev_copied); cudaEventDestroy(s->ev_copied); }
@@ -1387,6 +1399,8 @@ int mr_set_stream(mr_ctx *c, void *cuda_stream)
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
     MR_CUDA(c, cudaStreamSynchronize(c->copy_stream));
     if (c->stream2) MR_CUDA(c, cudaStreamSynchronize(c->stream2));
+    if (c->read_stream) MR_CUDA(c, cudaStreamSynchronize(c->read_stream));
+    c->read_pending = false;
     c->stream = (cudaStream_t)cuda_stream;
     return MR_OK;
 }
@@ -1411,6 +1425,10 @@ int load_mesh_common(mr_ctx *c, bool rz, int nx, int ny, int nz, const double *x
     c->dev_free(c->d_tally);
     c->dev_free(c->d_prev);
     c->dev_free(c->d_s2);
+    if (c->read_stream) cudaStreamSynchronize(c->read_stream);
+    c->read_pending = false;
+    c->dev_free(c->d_snap);
+    c->d_snap = nullptr;
     c->d_edges = nullptr;
     c->d_tally = nullptr;
     c->d_prev = c->d_s2 = nullptr;
@@ -1847,6 +1865,10 @@ int mr_read_tally(mr_ctx *c, double *out)
     MR_CUDA(c, flush_accumulators(c));
     MR_CUDA(c, cudaMemcpyAsync(out, c->d_tally, sizeof(double) * c->ncell, cudaMemcpyDeviceToHost, c->stream));
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->read_stream && c->read_pending) {       // earlier mr_read_tally_async transfers are complete too
+        MR_CUDA(c, cudaStreamSynchronize(c->read_stream));
+        c->read_pending = false;
+    }
     return MR_OK;
 }
 
@@ -1869,6 +1891,37 @@ int mr_sync(mr_ctx *c)
 {
     MR_ENTER(c);
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->read_stream && c->read_pending) {
+        MR_CUDA(c, cudaStreamSynchronize(c->read_stream));
+        c->read_pending = false;
+    }
+    return MR_OK;
+}
+
+int mr_read_tally_async(mr_ctx *c, double *out)
+{
+    MR_ENTER(c);
+    if (!out) return c->fail(MR_ERR_INVALID_ARG, "read_tally_async: out is NULL");
+    if (!c->d_tally) return c->fail(MR_ERR_STATE, "no mesh loaded");
+    if (!c->read_stream) {
+        MR_CUDA(c, cudaStreamCreateWithFlags(&c->read_stream, cudaStreamNonBlocking));
+        MR_CUDA(c, cudaEventCreateWithFlags(&c->ev_snap, cudaEventDisableTiming));
+        MR_CUDA(c, cudaEventCreateWithFlags(&c->ev_read, cudaEventDisableTiming));
+    }
+    if (!c->d_snap) {
+        c->d_snap = (double *)c->dev_alloc(sizeof(double) * c->ncell);
+        if (!c->d_snap) return c->fail(MR_ERR_OOM, "device allocation failed (tally snapshot)");
+    }
+    MR_CUDA(c, flush_accumulators(c));
+    // the snapshot is taken in stream order (after everything queued so far, before anything queued later); the previous
+    // read, if any, must have left the snapshot buffer
+    if (c->read_pending) MR_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_read, 0));
+    MR_CUDA(c, cudaMemcpyAsync(c->d_snap, c->d_tally, sizeof(double) * c->ncell, cudaMemcpyDeviceToDevice, c->stream));
+    MR_CUDA(c, cudaEventRecord(c->ev_snap, c->stream));
+    MR_CUDA(c, cudaStreamWaitEvent(c->read_stream, c->ev_snap, 0));
+    MR_CUDA(c, cudaMemcpyAsync(out, c->d_snap, sizeof(double) * c->ncell, cudaMemcpyDeviceToHost, c->read_stream));
+    MR_CUDA(c, cudaEventRecord(c->ev_read, c->read_stream));
+    c->read_pending = true;
     return MR_OK;
 }
 

@@ -540,6 +540,54 @@ def test_cooperative_transposed_tally_adds():
                 assert_tally(m.read_tally(), ref.tally, 0)
 
 
+def test_read_tally_async_snapshots_in_stream_order():
+    """mr_read_tally_async: a device snapshot taken in stream order and copied out on its own stream.  Batch after batch is
+    cast from host memory with an asynchronous read after each (two alternating page-locked buffers, as bench.py's e2e loop
+    does); after mr_sync each buffer holds the running tally as of ITS batch -- not a later one -- and equals what the
+    blocking mr_read_tally returned at the same point of a second, blocking pass.  Also on a mesh whose scores live in
+    in-record accumulators (fused K = 4), and after a mesh reload (the snapshot buffer follows the mesh)."""
+    import torch
+
+    from paper_1706_07476_b200 import MR_OPT_FUSED_TALLY, MonteRay
+
+    for cfg, kw, fused in ((3, dict(nx=68, ny=68, nz=40, n_e=2000), 0), (4, dict(n=48, n_e=3000), 1)):
+        prob = make_problem(cfg, **kw)
+        rays = make_rays(prob, 60_000)
+        parts = [rays[:25_000], rays[25_000:40_000], rays[40_000:]]
+        with MonteRay(0, 0) as m:
+            m.set_option(MR_OPT_FUSED_TALLY, fused)
+            m.load_problem(prob)
+            blocking = []
+            for part in parts:
+                m.cast_rays(part)
+                blocking.append(m.read_tally())
+            m.clear_tally()
+            bufs = [torch.zeros(prob.ncell, dtype=torch.float64).pin_memory() for _ in range(3)]
+            for part, buf in zip(parts, bufs):
+                m.cast_rays(part)
+                m.read_tally_async_into(buf.data_ptr())
+            m.sync()
+            ref = _oracle(prob).cast(rays, threads=_threads())
+            for k, (buf, want) in enumerate(zip(bufs, blocking)):
+                got = buf.numpy()
+                np.testing.assert_allclose(got, want, rtol=1e-9, atol=1e-9 * want.max(), err_msg=f"snapshot {k}")
+                assert k == 2 or not np.array_equal(got, bufs[2].numpy())       # an earlier snapshot is not the final tally
+            assert_tally(bufs[2].numpy(), ref.tally, 0)
+            assert_tally(m.read_tally(), ref.tally, 0)
+            # the same buffer twice in a row: the second read waits for the first to leave the snapshot
+            m.read_tally_async_into(bufs[0].data_ptr())
+            m.read_tally_async_into(bufs[1].data_ptr())
+            assert_tally(m.read_tally(), ref.tally, 0)                           # a blocking read completes the pending ones too
+            assert np.array_equal(bufs[0].numpy(), bufs[1].numpy())
+            small = make_problem(1)
+            m.load_problem(small)                                                # new mesh: new snapshot buffer
+            m.cast_rays(make_rays(small, 5000))
+            out = torch.zeros(small.ncell, dtype=torch.float64).pin_memory()
+            m.read_tally_async_into(out.data_ptr())
+            m.sync()
+            assert np.array_equal(out.numpy(), m.read_tally())
+
+
 def test_tile_ordered_accumulators_of_the_dictionary_path():
     """MR_OPT_TILED_TALLY: cast_tiled_kernel walks in tile coordinates and adds into tile-ordered accumulators that are moved
     into the linear tally whenever it is looked at.  Same counters, tallies within tolerance of the oracle for 4-, 8- and
