@@ -375,6 +375,12 @@ enum {
                                  MR_OPT_COOP_FLUSH the transposed adds then share 128-byte lines (L2 requests per segment 1.0 -> 0.45).
                                  0 (default): the kernel adds straight into the linear tally -- measured faster on every config
                                  (the kernel is bound by instruction issue once the requests are gone) */
+    MR_OPT_WHOLE_BATCH = 18,  /* page-locked HOST batches of mr_cast_rays: 0 = always the chunked pipeline of MR_OPT_STAGE_RAYS (the first kernel
+                                 starts after a short copy: lowest latency of a call on an idle GPU); 1 = always one DMA of the whole batch
+                                 into one of two device buffers and ONE cast behind it; 2 (default) = auto: whole-batch when the context's
+                                 stream is still busy with earlier work when the call is made (a caller casting batch after batch without
+                                 waiting: the copy then hides behind the previous cast, and one launch is 20 % cheaper than its chunks),
+                                 chunked otherwise.  Batches above 2 GB are always chunked */
     MR_OPT_PERSISTENT_LANES = 17, /* the cast kernel with persistent lanes (dictionary / K = 1 / K = 3 pairs / dense-8 record paths, MIXED): the
                                  grid is as many CTAs as are resident at once and a lane whose ray has left the mesh takes the next ray
                                  (in the order of the MR_OPT_SORT_RAYS pre-pass) from a counter -- no tail of half-empty CTAs, no ramp per

@@ -26,6 +26,7 @@ from .binding import (  # noqa: F401
     MR_OPT_PERSISTENT_LANES,
     MR_OPT_RZ_BLOCK_THREADS,
     MR_OPT_TILED_TALLY,
+    MR_OPT_WHOLE_BATCH,
     MR_OPT_SORT_RAYS,
     MR_OPT_STAGE_RAYS,
     MR_OPT_TILED_INDEX,

@@ -33,6 +33,7 @@ MR_OPT_COOP_FLUSH = 14
 MR_OPT_RZ_BLOCK_THREADS = 15
 MR_OPT_TILED_TALLY = 16
 MR_OPT_PERSISTENT_LANES = 17
+MR_OPT_WHOLE_BATCH = 18
 MR_INFO_RECORD_PATH, MR_INFO_DISTINCT_RECORDS, MR_INFO_COARSE_SHIFT = 100, 101, 102
 MR_INFO_DEFERRED, MR_INFO_DEFER_DIRECT_PAIRS = 103, 104
 MR_PATH_NAMES = {0: "none", 1: "k1", 2: "k2", 3: "k3", 4: "k4", 5: "k2_pairs", 6: "k3_pairs", 7: "k4_fused", 8: "dense8",

@@ -152,6 +152,12 @@ struct mr_ctx {
     int next_slot = 0;
     int copy_threads = 4;            // option MR_OPT_COPY_THREADS
 
+    // Whole-batch staging for back-to-back host batches (run_batch): two device buffers that each hold a complete batch
+    void *d_whole[2] = {nullptr, nullptr};
+    size_t whole_cap_bytes = 0;
+    cudaEvent_t ev_whole_copied = nullptr, ev_whole_done[2] = {nullptr, nullptr};
+    int whole_next = 0;
+    int whole_opt = 2;               // option MR_OPT_WHOLE_BATCH: 0 never, 1 always (pinned source), 2 auto = when the stream is still busy
     cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;
     bool have_timing = false;
     std::vector<cudaEvent_t> kev;  // (start, stop) pairs around each cast-kernel launch of the last call
@@ -1352,6 +1358,11 @@ int mr_destroy(mr_ctx *c)
         c->ring = nullptr;
     }
     free_stage(c);
+    for (int b = 0; b < 2; ++b) {
+        c->dev_free(c->d_whole[b]);
+        if (c->ev_whole_done[b]) cudaEventDestroy(c->ev_whole_done[b]);
+    }
+    if (c->ev_whole_copied) cudaEventDestroy(c->ev_whole_copied);
     free_tables(c);
     for (int q = 0; q < MR_MAX_NUCLIDES; ++q) {
         unref_grid(c, c->nuc_grid_of[q]);
@@ -1780,6 +1791,50 @@ int run_batch(mr_ctx *c, int64_t n, const void *rays, int where, Work work)
                 pinned_src = false;
             }
         }
+    }
+    // Back-to-back host batches: when the context's stream is still busy with earlier work (a caller that casts batch after
+    // batch without waiting), the chunked pipeline below buys nothing -- its point is to start the first kernel early on an
+    // IDLE GPU -- and costs 20 % in kernel time (chunks of 2^18..2^21 rays are cast less efficiently than the batch in one
+    // launch).  Then the whole batch is DMA'd into one of two device buffers while the earlier work runs, and cast in one
+    // launch behind it: in steady state the copy of batch i+1 hides behind the cast of batch i.
+    constexpr size_t kWholeMaxBytes = (size_t)2 << 30;
+    bool stream_busy = false;
+    if (c->whole_opt == 2) {
+        stream_busy = cudaStreamQuery(c->stream) == cudaErrorNotReady;
+        cudaGetLastError();
+    }
+    if (pinned_src && (c->whole_opt == 1 || stream_busy) && (size_t)n * rb <= kWholeMaxBytes && (size_t)n > per) {
+        const size_t bytes = (size_t)n * rb;
+        if (!c->ev_whole_copied) {
+            MR_CUDA(c, cudaEventCreateWithFlags(&c->ev_whole_copied, cudaEventDisableTiming));
+            for (int b = 0; b < 2; ++b) MR_CUDA(c, cudaEventCreateWithFlags(&c->ev_whole_done[b], cudaEventDisableTiming));
+        }
+        if (bytes > c->whole_cap_bytes) {
+            MR_CUDA(c, cudaStreamSynchronize(c->stream));
+            MR_CUDA(c, cudaStreamSynchronize(c->copy_stream));
+            for (int b = 0; b < 2; ++b) {
+                c->dev_free(c->d_whole[b]);
+                c->d_whole[b] = c->dev_alloc(bytes);
+            }
+            c->whole_cap_bytes = (c->d_whole[0] && c->d_whole[1]) ? bytes : 0;
+            if (!c->whole_cap_bytes) {
+                for (int b = 0; b < 2; ++b) { c->dev_free(c->d_whole[b]); c->d_whole[b] = nullptr; }
+                return c->fail(MR_ERR_OOM, "device allocation failed (whole-batch staging)");
+            }
+        }
+        const int b = c->whole_next;
+        c->whole_next ^= 1;
+        MR_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
+        MR_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_whole_done[b], 0));   // the cast that last read this buffer is done
+        MR_CUDA(c, cudaMemcpyAsync(c->d_whole[b], rays, bytes, cudaMemcpyHostToDevice, c->copy_stream));
+        MR_CUDA(c, cudaEventRecord(c->ev_whole_copied, c->copy_stream));
+        MR_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_whole_copied, 0));
+        if (int rc = work((long long)n, (const void *)c->d_whole[b])) return rc;
+        MR_CUDA(c, cudaEventRecord(c->ev_whole_done[b], c->stream));
+        MR_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
+        c->have_timing = true;
+        MR_CUDA(c, cudaEventSynchronize(c->ev_whole_copied));      // the caller's buffer is consumed when the call returns
+        return MR_OK;
     }
     // Chunk sizes grow: per/4, per/2, per, 2 per, 2 per, ...  The first copy is short, so the first kernel starts
     // early, and the later chunks are large, where the ordering pre-pass keeps the cast kernel's working set in L2
@@ -2697,6 +2752,10 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         if (value < 0 || value > 3) return c->fail(MR_ERR_INVALID_ARG, "cooperative-flush option is 0 (off), 1 (on), 2 (auto) or 3 (pairs by shuffle)");
         c->coop_opt = (int)value;
         return MR_OK;
+    case MR_OPT_WHOLE_BATCH:
+        if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "whole-batch option is 0 (never), 1 (always) or 2 (auto)");
+        c->whole_opt = (int)value;
+        return MR_OK;
     case MR_OPT_PERSISTENT_LANES:
         if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "persistent-lanes option is 0 (off), 1 (on) or 2 (auto)");
         c->persist_opt = (int)value;
@@ -2751,6 +2810,7 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     case MR_OPT_COOP_FLUSH: *value = c->coop_opt; return MR_OK;
     case MR_OPT_TILED_TALLY: *value = c->tiled_tally_opt; return MR_OK;
     case MR_OPT_PERSISTENT_LANES: *value = c->persist_opt; return MR_OK;
+    case MR_OPT_WHOLE_BATCH: *value = c->whole_opt; return MR_OK;
     case MR_INFO_RECORD_PATH: *value = record_path(c); return MR_OK;
     case MR_INFO_DISTINCT_RECORDS: *value = c->ndict; return MR_OK;
     case MR_INFO_COARSE_SHIFT: *value = c->cshift; return MR_OK;

@@ -242,6 +242,35 @@ def test_host_device_and_chunked_staging_agree():
     np.testing.assert_allclose(t_host, t_dev, rtol=1e-12, atol=1e-14)
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+def test_whole_batch_staging_of_back_to_back_host_batches(precision):
+    """MR_OPT_WHOLE_BATCH: a page-locked host batch is DMA'd in one piece into one of two device buffers and cast in one launch
+    (auto: when the stream is still busy with the previous batch).  Batches of different sizes back to back without waiting,
+    the caller's buffer overwritten right after each call returns (it is consumed by then), forced on, forced off and auto:
+    same counters, tally within tolerance of the oracle over the union."""
+    import torch
+
+    from paper_1706_07476_b200 import MR_OPT_STAGE_RAYS, MR_OPT_WHOLE_BATCH
+
+    prob = make_problem(3, nx=68, ny=68, nz=40, n_e=2000)
+    rays = make_rays(prob, 90_000)
+    cuts = [0, 30_000, 30_500, 70_001, 90_000]
+    ref = _oracle(prob).cast(rays, threads=_threads())
+    with _mr(prob, precision) as m:
+        m.set_option(MR_OPT_STAGE_RAYS, 2048)               # batches larger than a chunk: eligible for the whole-batch path
+        host = torch.empty((40_000, 8), dtype=torch.float64 if precision else torch.float32).pin_memory()
+        for mode in (1, 2, 0):
+            m.set_option(MR_OPT_WHOLE_BATCH, mode)
+            m.clear_tally()
+            for a, b in zip(cuts[:-1], cuts[1:]):
+                host[: b - a] = torch.from_numpy(rays[a:b].astype(m.ray_dtype))
+                m.cast_rays(host[: b - a])                   # returns once the buffer has been copied out of
+                host.fill_(float("nan"))                     # scribbling over it must not matter
+            st = m.get_stats()
+            assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+            assert_tally(m.read_tally(), ref.tally, precision)
+
+
 def test_block_size_option_and_torch_stream():
     import torch
 
