@@ -228,7 +228,7 @@ __device__ __forceinline__ void defer_drain(const DeferParams &D, const WarpBins
 //   dynamic shared memory: [edges (EDGES_SHARED only)] [walker: 3 x blockDim x 16 B] [sigma: (M+N) x blockDim floats]
 //                          [per warp: defer_warp_smem_bytes(nbin)]
 // ------------------------------------------------------------------------------------------------
-constexpr int kDeferRefillLanes = 8;
+constexpr int kDeferRefillLanes = 4;
 
 template <typename Rec, int EDGE_MODE>
 __global__ void __launch_bounds__(128) cast_defer_kernel(const __grid_constant__ CastParams P, const __grid_constant__ DeferParams D)
