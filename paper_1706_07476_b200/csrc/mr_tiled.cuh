@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(256) cast_tiled_kernel(const __grid_constant__
             s0 = (w.dc0 > 0) - (w.dc0 < 0); s1 = (w.dc1 > 0) - (w.dc1 < 0); s2 = (w.dc2 > 0) - (w.dc2 < 0);
             const int ix = walker_cell_index(w.pl0, w.dc0), iy = walker_cell_index(w.pl1, w.dc1), iz = walker_cell_index(w.pl2, w.dc2);
             tag = (ix >> G::kXs) + ntx * (iy >> G::kYs) + ntxy * iz;
-            E = (((unsigned)ix | (unsigned)(iy << 8)) & G::kWrap) | G::kGuard;
+            E = (((unsigned)ix & ((1u << G::kXs) - 1u)) | (((unsigned)iy & ((1u << G::kYs) - 1u)) << 8)) | G::kGuard;
             ldg_256(P.tiles + 2 * (size_t)tag, ta, tb);
         }
     }
@@ -315,7 +315,7 @@ __global__ void __launch_bounds__(256) next_event_tiled_kernel(const __grid_cons
             const int ix = walker_cell_index(w.pl0, w.dc0), iy = walker_cell_index(w.pl1, w.dc1), iz = walker_cell_index(w.pl2, w.dc2);
             const int ntx = T.ntx, ntxy = T.ntx * T.nty;
             int tag = (ix >> G::kXs) + ntx * (iy >> G::kYs) + ntxy * iz;
-            unsigned E = (((unsigned)ix | (unsigned)(iy << 8)) & G::kWrap) | G::kGuard;
+            unsigned E = (((unsigned)ix & ((1u << G::kXs) - 1u)) | (((unsigned)iy & ((1u << G::kYs) - 1u)) << 8)) | G::kGuard;
             uint4 ta, tb;
             ldg_256(T.tiles + 2 * (size_t)tag, ta, tb);
             for (;;) {                                               // N5

@@ -77,7 +77,8 @@ def test_next_event_tiny_problems(seed, K, M, uniform, precision):
     assert refs[4].rays_rejected >= 1
 
 
-@pytest.mark.parametrize("seed,K,uniform,dims", [(211, 2, False, (13, 11, 5)), (212, 3, True, (17, 9, 4)), (213, 3, False, (8, 8, 3))])
+@pytest.mark.parametrize("seed,K,uniform,dims", [(211, 2, False, (13, 11, 5)), (212, 3, True, (17, 9, 4)), (213, 3, False, (8, 8, 3)),
+                                                 (214, 2, True, (300, 9, 2)), (215, 3, False, (9, 300, 2))])   # more than 256 cells along x / y
 def test_next_event_on_the_dictionary_path_with_few_records(seed, K, uniform, dims):
     """Meshes with at most 16 distinct cell records and K >= 2 take next_event_tiled_kernel (walk in tile coordinates, per-entry
     Sigma_t): same cell sequences (hash of the LINEAR cell indices, rebuilt from tile and entry), tau, scores and sums as the

@@ -636,6 +636,11 @@ def test_tile_ordered_accumulators_of_the_dictionary_path():
     cases.append((p8, tiny_rays(p8, 641, 20_001, axis_aligned_share=0.1), "tiled8"))
     p16 = tiny_problem(642, nx=9, ny=8, nz=7, M=4, K=2, n_e=33)              # some 500 distinct records: 16-bit tiles of 4 x 4
     cases.append((p16, tiny_rays(p16, 642, 20_001, axis_aligned_share=0.1), "tiled16"))
+    for seed, dims in ((643, (300, 9, 2)), (644, (9, 300, 2))):              # more than 256 cells along an axis (entry-word fields are 8 bits apart)
+        pw = tiny_problem(seed, nx=dims[0], ny=dims[1], nz=dims[2], M=4, K=2, n_e=33)
+        pw.cell_mat[:] = pw.cell_mat[np.arange(pw.ncell) % 11]
+        pw.cell_frac[:] = pw.cell_frac[np.arange(pw.ncell) % 11]
+        cases.append((pw, tiny_rays(pw, seed, 20_001, axis_aligned_share=0.1), "tiled4"))
     for prob, rays, path in cases:
         rays[::501, 6] = -1.0
         ref = _oracle(prob).cast(rays, threads=_threads())
