@@ -83,3 +83,52 @@ def test_random_shapes_every_cast_variant(seed):
                     want = np.array([rn.det_sum for rn in ne])
                     assert np.all(np.abs(sums - want) <= (1e-4 if precision == 0 else 1e-10) * np.abs(want) + 1e-300), what
     assert len(paths) >= 4, paths      # the draw reached several record paths
+
+
+@pytest.mark.parametrize("seed", [21, 22])
+def test_random_rz_and_spherical_shapes(seed):
+    """R-Z and spherical meshes of random proportions (1 ... 300 shells, 1 ... 40 slabs, uniform and non-uniform radii), every
+    record layout, both modes: cells AND lengths of every ray bit-exact (the kernel finds the turning shell by bisection and
+    evaluates one discriminant per step -- every decision must still be the oracle's), counters, tallies, and the next-event
+    cell sequences and sums for a detector inside and one outside."""
+    from tests.test_gpu_rz import _check, _check_next_event_rz
+    from tests.tiny import tiny_rz_problem, tiny_rz_rays, tiny_sphere_problem, tiny_sphere_rays
+
+    g = np.random.default_rng(seed)
+    for it in range(8):
+        nr = int(g.choice([1, 2, 3, 17, 64, 129, 300]))
+        nz = int(g.choice([1, 2, 5, 40]))
+        K = int(g.choice([1, 2, 3, 4, 8]))
+        M = 8 if K == 8 else int(g.integers(max(2, K), 6))
+        uniform = bool(g.integers(0, 2))
+        if g.integers(0, 3) == 0:
+            prob = tiny_sphere_problem(100 * seed + it, nr=nr, M=M, K=K, n_e=33, uniform=uniform)
+            rays = tiny_sphere_rays(prob, 100 * seed + it, 6001, through_centre_share=0.05)
+            sphere = True
+        else:
+            prob = tiny_rz_problem(100 * seed + it, nr=nr, nz=nz, M=M, K=K, n_e=33, uniform=uniform)
+            rays = tiny_rz_rays(prob, 100 * seed + it, 6001, axis_parallel_share=0.05, through_axis_share=0.05)
+            sphere = False
+        R = float(prob.re[-1])
+        dets = [[0.3 * R, 0.1 * R, 0.2], [2.0 * R, 0.5 * R, -3.0]]
+        for precision in (0, 1):
+            if sphere:
+                from oracle.vrc_oracle import Oracle
+                from paper_1706_07476_b200 import MonteRay
+
+                cap = 2 * nr + 1
+                ref = Oracle(prob).cast_sphere(rays, prob.re, cap=cap)
+                with MonteRay(0, precision) as m:
+                    m.load_problem(prob)
+                    r = rays.astype(m.ray_dtype)
+                    m.cast_rays(r)
+                    got = m.read_tally()
+                    st = m.get_stats()
+                    nseg, hsh, cells, lens = m.trace_rays(r, cap=cap)
+                assert np.array_equal(nseg, ref.nseg) and np.array_equal(hsh, ref.hash)
+                assert np.array_equal(cells, ref.cells) and np.array_equal(lens, ref.lens)
+                assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+                assert np.all(np.abs(got - ref.tally) <= _tol(ref.tally, precision))
+            else:
+                _check(prob, rays, precision, cap=2 * nr + nz + 2)
+            _check_next_event_rz(prob, rays[:1500], dets, precision, sphere)
