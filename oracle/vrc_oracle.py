@@ -355,3 +355,32 @@ def mean_and_sigma(s1, s2, B: int):
 def figure_of_merit(sigma, T: float):
     """PAPER.md:93 Eq. (5): FOM = 1 / (sigma^2 T)."""
     return 1.0 / (sigma * sigma * T)
+
+
+def fom_ratio(sigma_a, T_a: float, sigma_b, T_b: float):
+    """PAPER.md:97 Eq. (6): eta = FOM_a / FOM_b = (sigma_b^2 / sigma_a^2) * (T_b / T_a)."""
+    return (sigma_b * sigma_b) / (sigma_a * sigma_a) * (T_b / T_a)
+
+
+def relative_difference(phi_ref, phi):
+    """PAPER.md:118 Eq. (7): Delta_phi(i) = |phi_ref(i) - phi(i)| / phi_ref(i), the paper's measure of single-precision ray casting
+    on the GPU against double precision on the CPU (phi_ref); cells with phi_ref = 0 give 0 where phi = 0 too, else +inf."""
+    a, b = np.asarray(phi_ref, dtype=np.float64), np.asarray(phi, dtype=np.float64)
+    d = np.abs(a - b)
+    out = np.zeros_like(d)
+    nz = a != 0.0
+    out[nz] = d[nz] / np.abs(a[nz])
+    out[~nz & (d > 0.0)] = np.inf
+    return out
+
+
+def fractional_difference(phi_ref, phi, sigma):
+    """PAPER.md:122 Eq. (8): eps_phi(i) = |phi_ref(i) - phi(i)| / sigma(i), "the ratio of the absolute difference to the standard
+    deviation of the fluence": whether a difference is statistically significant.  sigma = 0 gives 0 for equal values, else +inf."""
+    a, b, s = (np.asarray(v, dtype=np.float64) for v in (phi_ref, phi, sigma))
+    d = np.abs(a - b)
+    out = np.zeros_like(d)
+    nz = s > 0.0
+    out[nz] = d[nz] / s[nz]
+    out[~nz & (d > 0.0)] = np.inf
+    return out

@@ -8,7 +8,8 @@ with Sigma_t = 0 outside the mesh.  The paper prints no worked example for it.
 import numpy as np
 import pytest
 
-from oracle.vrc_oracle import Oracle, batch_moments, figure_of_merit, fnv1a_cells, mean_and_sigma
+from oracle.vrc_oracle import (Oracle, batch_moments, figure_of_merit, fnv1a_cells, fom_ratio, fractional_difference, mean_and_sigma,
+                               relative_difference)
 from tests.test_oracle_pins import np_sigma_cell
 from tests.tiny import tiny_problem, tiny_rays
 
@@ -180,3 +181,16 @@ def test_batch_moments_against_numpy_statistics():
     _, sig0 = mean_and_sigma(s1, s2, 4)
     assert np.all(sig0 <= 1e-7 * x[0]) and np.all(np.isfinite(sig0))
     assert figure_of_merit(0.5, 4.0) == 1.0
+
+
+def test_paper_comparison_metrics_eq6_eq7_eq8():
+    """Eqs. (6)-(8) on hand-computed values, and the number the paper prints for Eq. (6): with equal
+    variances the criticality-accident run's eta would be the time ratio alone."""
+    assert fom_ratio(0.5, 2.0, 1.0, 3.0) == (1.0 / 0.25) * (3.0 / 2.0)
+    assert fom_ratio(0.1, 600.0, 0.1, 5893.0) == pytest.approx(5893.0 / 600.0)          # PAPER.md:158, variance ratio 1
+    ref = np.array([2.0, 4.0, 0.0, 0.0, -8.0])
+    got = np.array([2.5, 3.0, 0.0, 1.0, -6.0])
+    assert np.array_equal(relative_difference(ref, got), np.array([0.25, 0.25, 0.0, np.inf, 0.25]))
+    sig = np.array([0.25, 2.0, 0.0, 0.0, 4.0])
+    assert np.array_equal(fractional_difference(ref, got, sig), np.array([2.0, 0.5, 0.0, np.inf, 0.5]))
+    assert np.array_equal(relative_difference(ref, ref), np.zeros(5))
