@@ -70,6 +70,7 @@ enum { MR_WHERE_HOST = 0, MR_WHERE_DEVICE = 1 };
 #define MR_MAX_SLOTS 16
 #define MR_MAX_NUCLIDES 64
 #define MR_MAX_MIX 16
+#define MR_STATIC_MAX_RAYS 262144 /* most rays one mr_cast_rays_static call takes (2^18) */
 
 /* Optional device-memory allocator supplied by the caller (the Python binding passes one that
  * hands out torch caching-allocator blocks).  alloc returns a device pointer aligned to 256 B
@@ -182,6 +183,43 @@ MR_API int mr_define_material(mr_ctx *ctx, int material, int nnuc, const int32_t
  * if it is page-locked, DMA'd out of) and the work is queued.  n = 0 is a no-op.
  * Requires mesh, materials and all M tables.  Errors: INVALID_ARG, STATE, OOM, CUDA. */
 MR_API int mr_cast_rays(mr_ctx *ctx, int64_t n, const void *rays, int where);
+
+/* mr_cast_rays for a caller that must not allocate device memory while it runs.
+ *
+ * Who that is: a transport code that hands the whole GPU to its own memory pool at start-up, so that nothing is left for
+ * a library to allocate from; a host loop that cannot afford the device-wide wait a cudaMalloc / cudaFree implies (it
+ * breaks the CPU/GPU overlap of PAPER.md:79-83); a job with a fixed memory budget per process.  mr_cast_rays does
+ * allocate on their hot path: its ray-ordering pre-pass keeps a key and a sorted position per ray plus a histogram in
+ * scratch memory that is allocated on the first batch and re-allocated whenever a batch is larger than any before.
+ *
+ * This call does the same work -- same ordering keys, same cast kernels, same tally, same counters -- but its pre-pass
+ * works in a fixed array inside the library image, so it calls no cudaMalloc, no cudaFree, not the context's
+ * mr_allocator, and no library routine that allocates.  The price is a limit and a reservation: at most
+ * MR_STATIC_MAX_RAYS (262 144) rays per call -- more is refused with MR_ERR_INVALID_ARG and a message, split the batch --
+ * and 2.1 MB of device memory on EVERY GPU the process uses, held from the moment the library is loaded until the process
+ * exits, whether or not this call is ever made.
+ *
+ * `d_rays`: n ray records in DEVICE memory (layout as mr_cast_rays, 16-byte aligned); the caller owns them and must
+ * keep them alive and unchanged until the queued work has run.  The tally is the context's, as for mr_cast_rays;
+ * the two calls can be mixed freely on one context.  Asynchronous; n = 0 is a no-op.
+ *
+ * Before the first call: all allocation belongs to set-up.  Load mesh, materials and tables, then make ONE ordinary
+ * mr_cast_rays call (a single ray is enough): it creates the small table-descriptor buffers.  Until that has happened
+ * this call returns MR_ERR_STATE.  Tables re-loaded later are picked up without allocating.
+ * First call on each device: looks up the device address of the fixed array (once per device, with the context's device
+ * current).  Make that first call outside any stream capture.
+ *
+ * Sharing: there is one array per GPU, not per context or stream, and every call leaves its keys and positions in it (the
+ * part that has to start at zero, the histogram, is cleared by each call on the context's stream).  Calls whose GPU work
+ * can run at the same time -- two contexts on one GPU, or one context switched to another stream by mr_set_stream while
+ * an earlier call is still in flight -- race on it and scramble each other's ray order.  Serialise them: one context
+ * per GPU on one stream, or an event / mr_sync between calls from different contexts.
+ *
+ * Not available for R-Z / spherical meshes, nor when the deferred two-phase tally is active (MR_INFO_DEFERRED = 1; its pair
+ * pool is sized per batch -- set MR_OPT_DEFERRED_TALLY to 0): MR_ERR_UNSUPPORTED.  Not while a producer ring is open:
+ * MR_ERR_STATE.  mr_stats.last_kernel_ms reads 0 after this call (the per-kernel event list is not grown here);
+ * last_cast_ms covers pre-pass + cast.  Errors: INVALID_ARG, STATE, UNSUPPORTED, CUDA. */
+MR_API int mr_cast_rays_static(mr_ctx *ctx, int64_t n, const void *d_rays);
 
 /* Synchronises and copies the ncell raw fp64 sums to the host array `out` ("the
  * tally remained on the GPU until the termination of the simulation").  A consistent

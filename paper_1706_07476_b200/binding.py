@@ -20,6 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libmonteray.so")
 MR_OK, MR_ERR_INVALID_ARG, MR_ERR_STATE, MR_ERR_CUDA, MR_ERR_OOM, MR_ERR_UNSUPPORTED = range(6)
 MR_PRECISION_MIXED, MR_PRECISION_DOUBLE = 0, 1
 MR_WHERE_HOST, MR_WHERE_DEVICE = 0, 1
+MR_STATIC_MAX_RAYS = 1 << 18
 MR_OPT_BLOCK_THREADS, MR_OPT_SORT_RAYS, MR_OPT_STAGE_RAYS, MR_OPT_COPY_THREADS, MR_OPT_PAIR_RECORDS = 1, 2, 3, 4, 5
 MR_OPT_ORDER_MODE = 6
 MR_OPT_FUSED_TALLY = 7
@@ -43,7 +44,7 @@ _STATUS = {1: "MR_ERR_INVALID_ARG", 2: "MR_ERR_STATE", 3: "MR_ERR_CUDA", 4: "MR_
 
 EXPORTS = [
     "mr_create", "mr_create_ex", "mr_destroy", "mr_set_stream", "mr_last_error", "mr_load_mesh",
-    "mr_load_materials", "mr_load_xs", "mr_cast_rays", "mr_read_tally", "mr_read_tally_async", "mr_clear_tally", "mr_sync",
+    "mr_load_materials", "mr_load_xs", "mr_cast_rays", "mr_cast_rays_static", "mr_read_tally", "mr_read_tally_async", "mr_clear_tally", "mr_sync",
     "mr_get_stats", "mr_tally_device_ptr", "mr_trace_rays", "mr_set_option", "mr_get_option",
     "mr_end_batch", "mr_read_moments", "mr_read_mean_sigma", "mr_load_nuclide_xs", "mr_define_material", "mr_load_mesh_rz", "mr_load_mesh_sphere",
     "mr_ring_open", "mr_ring_push", "mr_ring_flush", "mr_ring_close", "mr_ring_get_stats", "mr_ring_bench_producers",
@@ -101,6 +102,7 @@ def load_library() -> C.CDLL:
         "mr_load_materials": [vp, i32, vp, i32, vp, vp],
         "mr_load_xs": [vp, i32, i64, vp, vp],
         "mr_cast_rays": [vp, i64, vp, i32],
+        "mr_cast_rays_static": [vp, i64, vp],
         "mr_read_tally": [vp, vp],
         "mr_read_tally_async": [vp, vp],
         "mr_clear_tally": [vp],
@@ -336,6 +338,16 @@ class MonteRay:
     def cast_rays(self, rays):
         ptr, n, where, keep = self._ray_arg(rays)
         self._check(self.lib.mr_cast_rays(self._h, n, C.c_void_p(ptr), where))
+        return n
+
+    def cast_rays_static(self, rays):
+        """mr_cast_rays_static: casts a torch CUDA tensor of at most MR_STATIC_MAX_RAYS rays without allocating device
+        memory (the ordering scratch is a fixed array in the library).  For hosts that own all device memory
+        themselves or cannot stall on cudaMalloc inside their loop; see include/monteray.h for the rules."""
+        ptr, n, where, keep = self._ray_arg(rays)
+        if where != MR_WHERE_DEVICE:
+            raise MonteRayError(MR_ERR_INVALID_ARG, "cast_rays_static takes device-resident rays (a torch CUDA tensor)")
+        self._check(self.lib.mr_cast_rays_static(self._h, n, C.c_void_p(ptr)))
         return n
 
     def read_tally(self, out: Optional[np.ndarray] = None) -> np.ndarray:

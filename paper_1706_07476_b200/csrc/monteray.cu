@@ -2893,3 +2893,166 @@ extern "C" int mr_microbench_red(int device, int64_t ncell, int group, int gathe
     if (mean_ms) *mean_ms = sum / reps;
     return done(MR_OK);
 }
+
+// ---- mr_cast_rays_static: the cast for callers that cannot allocate device memory ------------------------------
+//
+// mr_cast_rays orders a batch before it casts it (mr_sort.cuh), and the ordering pre-pass needs scratch in global
+// memory -- a key and a sorted position per ray, a histogram of the keys -- which order_rays() allocates, and grows,
+// on demand.  Some hosts cannot allow that inside their transport loop:
+//   * a Monte Carlo code that claims the whole device for its own pool at start-up leaves nothing to allocate from;
+//   * cudaMalloc / cudaFree wait for the device to go idle, which stalls the CPU/GPU overlap the method lives on
+//      and can deadlock a thread that holds a lock another stream's callback wants;
+//   * code under a fixed memory budget (several ranks sharing one GPU) must know its footprint before the run.
+// For them the same pre-pass runs here out of ONE fixed array that is part of the library image.  The array is device
+// memory of every GPU that loads libmonteray.so, from load to process exit, whether or not this entry point is used.
+//
+// Shared state: every context and every stream of a device use the same array, and a call leaves its keys and
+// positions in it.  Only the histogram has to start at zero; it is cleared on the stream at the start of every call.
+// Two calls whose GPU work overlaps in time (two contexts, or one context moved to another stream while the earlier
+// call is still running) race on the array and corrupt each other's ray order.
+constexpr int kStaticMaxKeys = 256 * 128 + 1;                     // order_rays(): <= 256 z-slabs x 128 length buckets + "rejected"
+constexpr size_t kStaticHistWords = ((size_t)kStaticMaxKeys + 1 + 63) & ~(size_t)63;
+constexpr size_t kStaticWords = 2 * (size_t)MR_STATIC_MAX_RAYS + kStaticHistWords;   // keys | positions | histogram
+
+static __device__ __align__(256) uint32_t g_static_scratch[kStaticWords];           // 2.1 MB per GPU
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+uint32_t *g_static_addr[kStaticMaxDevices] = {};
+
+// Device address of g_static_scratch on the CURRENT device (the caller has made the context's device current).  In host
+// code the name g_static_scratch is only a handle for the runtime, not a pointer a kernel could use: the address has
+// to be asked for, once per device.
+int static_scratch(mr_ctx *c, uint32_t **out)
+{
+    if (c->device < 0 || c->device >= kStaticMaxDevices) return c->fail(MR_ERR_UNSUPPORTED, "cast_rays_static: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_addr[c->device]) {
+        void *p = nullptr;
+        MR_CUDA(c, cudaGetSymbolAddress(&p, g_static_scratch));
+        g_static_addr[c->device] = static_cast<uint32_t *>(p);
+    }
+    *out = g_static_addr[c->device];
+    return MR_OK;
+}
+
+}  // namespace
+
+extern "C" int mr_cast_rays_static(mr_ctx *c, int64_t n, const void *d_rays)
+{
+    MR_ENTER(c);
+    if (n < 0 || (n > 0 && !d_rays)) return c->fail(MR_ERR_INVALID_ARG, "cast_rays_static: bad count or NULL buffer");
+    if (n > MR_STATIC_MAX_RAYS)
+        return c->fail(MR_ERR_INVALID_ARG, "cast_rays_static: " + std::to_string((long long)n) + " rays in one call, the fixed scratch holds " +
+                                               std::to_string((long long)MR_STATIC_MAX_RAYS) + " (MR_STATIC_MAX_RAYS): split the batch");
+    if ((uintptr_t)d_rays & 15) return c->fail(MR_ERR_INVALID_ARG, "cast_rays_static: device ray buffer must be 16-byte aligned");
+    MR_NO_RING(c, "cast_rays_static");
+    if (int rc = ready_to_cast(c)) return rc;
+    const int path = record_path(c);
+    if (path == MR_PATH_RZ) return c->fail(MR_ERR_UNSUPPORTED, "cast_rays_static: Cartesian meshes only");
+    if (use_deferred(c, path))
+        return c->fail(MR_ERR_UNSUPPORTED, "cast_rays_static: the deferred tally keeps a pool that is sized per batch; set MR_OPT_DEFERRED_TALLY to 0");
+    if (c->xs_dirty) {
+        // the table descriptors are re-sent after every table load; their device buffers are made by the first ordinary cast
+        bool mixtures = false;
+        for (int m = 0; m < c->M && m < (int)c->mix.size(); ++m) mixtures = mixtures || !c->mix[m].empty();
+        if (!c->d_xs || (mixtures && !c->d_mix_off))
+            return c->fail(MR_ERR_STATE, "cast_rays_static: set-up is not finished -- make one mr_cast_rays call (one ray is enough) after loading the tables");
+        if (int rc = upload_xs_desc(c)) return rc;
+    }
+    if (n == 0) return MR_OK;
+    uint32_t *scratch = nullptr;
+    if (int rc = static_scratch(c, &scratch)) return rc;
+
+    cudaStream_t ws = c->work_stream();
+    c->kev_used = 0;            // no per-kernel events here (mr_stats.last_kernel_ms stays 0): growing that list allocates
+    MR_CUDA(c, cudaEventRecord(c->ev_t0, ws));
+
+    CastParams P{};
+    P.mesh = mesh_dev(c);
+    P.recs = c->d_recs;
+    P.ids = c->d_ids;
+    P.K = c->K;
+    P.M = c->M;
+    P.xs = c->d_xs;
+    P.N = c->N;
+    P.mix_off = c->d_mix_off;
+    P.mix_nuc = c->d_mix_nuc;
+    P.mix_w = c->d_mix_w;
+    P.rays = d_rays;
+    P.perm = nullptr;
+    P.n = n;
+    P.agg_first = c->agg_first;
+    P.tally = c->d_tally;
+    P.counters = c->d_counters;
+
+    // the ordering pre-pass, as order_rays() decides it, in its global-atomic form (classify, scan, scatter): that form
+    // needs no per-CTA histograms, so the scratch stays small
+    if (c->sort_rays && n >= kSortMinRays && edges_smem_bytes(c) <= kEdgesSmemMax) {
+        const int nlen = 128;
+        const int zdiv = (c->nz + 255) / 256;
+        const int nslab = (c->nz + zdiv - 1) / zdiv;
+        const int maxlen = c->nx + c->ny + c->nz;
+        int lshift = 0;
+        while ((maxlen >> lshift) >= nlen) ++lshift;
+        const int nkeys = nslab * nlen + 1;
+        if (nkeys > kStaticMaxKeys) return c->fail(MR_ERR_UNSUPPORTED, "cast_rays_static: more ordering keys than the fixed scratch holds");
+        uint32_t *d_keys = scratch, *d_perm = scratch + MR_STATIC_MAX_RAYS, *d_hist = scratch + 2 * (size_t)MR_STATIC_MAX_RAYS;
+        SortParams S{mesh_dev(c), d_rays, (long long)n, c->precision == MR_PRECISION_DOUBLE ? 1 : 0,
+                     zdiv, lshift, nlen, nkeys, d_keys, d_hist, d_perm, nullptr, 0,
+                     c->order_mode == 2 || (c->order_mode == 0 && c->resident_bytes() <= c->l2_bytes / 2) ? 1 : 0, nslab,
+                     c->mesh_arith ? 1 : 0, 0, nullptr};
+        const size_t smem = edges_smem_bytes(c);
+        MR_CUDA(c, cudaMemsetAsync(d_hist, 0, ((size_t)nkeys + 1) * 4, ws));     // the last call's prefix sums are still there
+        const unsigned grid = (unsigned)((n + 255) / 256);
+        if (int rc = set_smem(c, classify_kernel, smem)) return rc;
+        classify_kernel<<<grid, 256, smem, ws>>>(S);
+        scan_kernel<<<1, 1024, 0, ws>>>(d_hist, nkeys);
+        scatter_kernel<<<grid, 256, 0, ws>>>(S);
+        c->launches += 3;
+        MR_CUDA(c, cudaGetLastError());
+        P.perm = d_perm;
+    }
+
+    // the record paths of cast_device(), minus the two refused above
+    int rc;
+    switch (path) {
+    case MR_PATH_DOUBLE_K3: rc = launch_cast_or_coop<double, CellRec<LAYOUT_DK3>>(c, P, true); break;
+    case MR_PATH_DOUBLE_GENERIC: rc = launch_cast_t<double, CellRecGeneric<double>>(c, P); break;
+    case MR_PATH_TILED4: case MR_PATH_TILED8: case MR_PATH_TILED16:
+        P.dict = c->d_dict;
+        P.tiles = c->d_tiles;
+        P.ndict = c->ndict;
+        P.ntx = c->ntx;
+        P.nty = c->nty;
+        if (c->tiled_tally_opt && c->d_tally_t && !c->tally_borrowed) {
+            P.tally_t = c->d_tally_t;
+            rc = c->tile_bits == 4 ? launch_tiled<4>(c, P) : c->tile_bits == 8 ? launch_tiled<8>(c, P) : launch_tiled<16>(c, P);
+        } else
+            rc = c->tile_bits == 4 ? launch_cast_or_coop<float, TiledRec<4>>(c, P)
+               : c->tile_bits == 8 ? launch_cast_or_coop<float, TiledRec<8>>(c, P) : launch_cast_or_coop<float, TiledRec<16>>(c, P);
+        break;
+    case MR_PATH_COARSE:
+        P.crecs = c->d_crecs;
+        P.cshift = c->cshift;
+        P.cnx = c->cnx;
+        P.cny = c->cny;
+        rc = launch_cast_t<float, CellRec<LAYOUT_C4>>(c, P);
+        break;
+    case MR_PATH_K1: rc = launch_cast_or_coop<float, CellRec<LAYOUT_K1>>(c, P); break;
+    case MR_PATH_K2: rc = launch_cast_t<float, CellRec<LAYOUT_K2>>(c, P); break;
+    case MR_PATH_K3: rc = launch_cast_t<float, CellRec<LAYOUT_K3>>(c, P); break;
+    case MR_PATH_K2_PAIRS: rc = launch_cast_t<float, CellRec<LAYOUT_K2P>>(c, P); break;
+    case MR_PATH_K3_PAIRS: rc = launch_cast_or_coop<float, CellRec<LAYOUT_K3P>>(c, P, true); break;
+    case MR_PATH_K4_FUSED: rc = launch_cast_t<float, CellRec<LAYOUT_K4F>>(c, P); c->fused_dirty = true; break;
+    case MR_PATH_K4: rc = launch_cast_t<float, CellRec<LAYOUT_K4>>(c, P); break;
+    case MR_PATH_DENSE8: rc = launch_cast_or_coop<float, CellRec<LAYOUT_D8>>(c, P); break;
+    default: rc = launch_cast_t<float, CellRecGeneric<float>>(c, P);
+    }
+    if (rc) return rc;
+    MR_CUDA(c, cudaEventRecord(c->ev_t1, ws));
+    c->have_timing = true;
+    return MR_OK;
+}
