@@ -1014,6 +1014,7 @@ int ensure_defer_pool(mr_ctx *c, long long entries)
     chunks = std::max<long long>(1, std::min(max_chunks_total, chunks));
     if (c->defer_pool_fixed == 0 ? chunks <= c->defer_pool_chunks : (chunks == c->defer_pool_chunks && c->d_defer_table)) return MR_OK;
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->stream2) MR_CUDA(c, cudaStreamSynchronize(c->stream2));
     free_defer(c);
     if (!c->h_defer_ctl) {
         MR_CUDA(c, cudaMallocHost((void **)&c->h_defer_ctl, 4 * sizeof(unsigned long long)));
@@ -1431,7 +1432,13 @@ int load_mesh_common(mr_ctx *c, bool rz, int nx, int ny, int nz, const double *x
     if (!finite_increasing(xe, nx + 1) || !finite_increasing(ye, ny + 1) || !finite_increasing(ze, nz + 1))
         return c->fail(MR_ERR_INVALID_ARG, "mesh: plane positions must be finite and strictly increasing");
     MR_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->stream2) MR_CUDA(c, cudaStreamSynchronize(c->stream2));
     free_materials(c);
+    // the deferred tally's chunk table is laid out for the regions of ONE mesh (nbin rows), and its pool estimate is that
+    // mesh's segments per ray: a new mesh starts from nothing
+    free_defer(c);
+    c->defer_entries_per_ray = 0.0;
+    c->defer_direct_seen = 0;
     c->dev_free(c->d_edges);
     c->dev_free(c->d_tally);
     c->dev_free(c->d_prev);
@@ -1760,8 +1767,10 @@ int mr_define_material(mr_ctx *c, int material, int nnuc, const int32_t *nuclide
 namespace {
 
 // Runs `work(count, device rays)` over a batch: a device batch in one piece, a host batch in staged chunks.
+// one_lane: the work keeps per-context device state that two chunks in flight would share (the deferred tally's control
+// words, chunk table and pool): its chunks stay on the context's stream, one after the other.
 template <typename Work>
-int run_batch(mr_ctx *c, int64_t n, const void *rays, int where, Work work)
+int run_batch(mr_ctx *c, int64_t n, const void *rays, int where, Work work, bool one_lane = false)
 {
     c->kev_used = 0;
     if (where == MR_WHERE_DEVICE) {
@@ -1846,8 +1855,8 @@ int run_batch(mr_ctx *c, int64_t n, const void *rays, int where, Work work)
     int last_slot = -1;
     // Consecutive chunks alternate between the two compute lanes: every cast kernel ramps up and down for about
     // 0.2 ms (a CTA lives as long as its longest ray), and with one stream those ramps add up chunk after chunk.
-    // (Not on R-Z meshes: their persistent kernel has one work counter.)
-    const bool two_lanes = !c->mesh_rz && n > chunk;
+    // (Not on R-Z meshes: their persistent kernel has one work counter.  Not with the deferred tally: see one_lane.)
+    const bool two_lanes = !c->mesh_rz && !one_lane && n > chunk;
     // on EVERY exit path (errors included) lane 1 is joined back into the context's stream: work the caller queues there
     // afterwards, and the frees of mr_destroy, come after everything this call launched
     struct LaneReset {
@@ -1909,7 +1918,8 @@ int mr_cast_rays(mr_ctx *c, int64_t n, const void *rays, int where)
     if (int rc = ready_to_cast(c)) return rc;
     if (n == 0) return MR_OK;
     if (int rc = upload_xs_desc(c)) return rc;
-    return run_batch(c, n, rays, where, [c](long long count, const void *d_rays) { return cast_device(c, count, d_rays); });
+    return run_batch(c, n, rays, where, [c](long long count, const void *d_rays) { return cast_device(c, count, d_rays); },
+                     use_deferred(c, record_path(c)));
 }
 
 int mr_read_tally(mr_ctx *c, double *out)
