@@ -2649,10 +2649,13 @@ int mr_ring_flush(mr_ctx *c)
 // instead (what the producers cost with no ring and no GPU behind them).
 int mr_ring_bench_producers(mr_ctx *c, int64_t n, const void *rays, int producers, int64_t rays_per_push, int dry_run, double *wall_ms)
 {
-    if (!c || n < 0 || (n > 0 && !rays) || producers < 1 || producers > 256 || rays_per_push < 1) return MR_ERR_INVALID_ARG;
-    if (!dry_run && !c->ring) return MR_ERR_STATE;
+    MR_ENTER(c);
+    if (n < 0 || (n > 0 && !rays) || producers < 1 || producers > 256 || rays_per_push < 1)
+        return c->fail(MR_ERR_INVALID_ARG, "ring_bench_producers: bad count, NULL buffer, or producers / rays_per_push out of range");
+    if (!dry_run && !c->ring) return c->fail(MR_ERR_STATE, "ring_bench_producers: no producer ring is open");
     const size_t rb = c->ray_bytes();
     std::atomic<int> rc{MR_OK};
+    std::atomic<bool> stop{false};      // one producer's failed push ends the others' loops too
     // dry run: every thread's whole share goes to a private buffer of its own size (destination lines not in cache, as in the
     // ring), allocated and touched before the clock starts
     std::vector<std::unique_ptr<char[]>> scratches((size_t)producers);
@@ -2667,9 +2670,9 @@ int mr_ring_bench_producers(mr_ctx *c, int64_t n, const void *rays, int producer
     for (int k = 0; k < producers; ++k) {
         const int64_t lo = n * k / producers, hi = n * (k + 1) / producers;
         char *const scratch_k = scratches[(size_t)k].get();
-        pool.emplace_back([=, &rc]() {
+        pool.emplace_back([=, &rc, &stop]() {
             struct { char *p; char *get() const { return p; } } scratch{scratch_k};
-            for (int64_t i = lo; i < hi; i += rays_per_push) {
+            for (int64_t i = lo; i < hi && !stop.load(std::memory_order_relaxed); i += rays_per_push) {
                 const int64_t m = std::min<int64_t>(rays_per_push, hi - i);
                 const char *src = (const char *)rays + (size_t)i * rb;
                 if (dry_run) {
@@ -2677,14 +2680,17 @@ int mr_ring_bench_producers(mr_ctx *c, int64_t n, const void *rays, int producer
                     asm volatile("" ::"r"(scratch.get()) : "memory");
                 } else {
                     const int r = mr_ring_push(c, m, src);
-                    if (r != MR_OK) { rc.store(r); return; }
+                    if (r != MR_OK) { rc.store(r); stop.store(true); return; }
                 }
             }
         });
     }
     for (std::thread &t : pool) t.join();
     int ret = rc.load();
-    if (!dry_run && ret == MR_OK) ret = mr_ring_flush(c);
+    if (!dry_run) {     // also after a failed push: what the other producers had put into open slots is shipped, no slot stays half filled
+        const int flushed = mr_ring_flush(c);
+        if (ret == MR_OK) ret = flushed;
+    }
     if (wall_ms) *wall_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
     return ret;
 }
