@@ -208,6 +208,45 @@ def run_reference(args, prob_kw):
     return 0
 
 
+def other_config_rows(steps: int, timeout_s: int = 900):
+    """BASELINE.json's other configurations and the all-double mode, beside the headline: north_star's acceptance is
+    stated "on all five configs".  Each row is a short default-arm run of THIS script in a process of its own (so a
+    failure or a time-out there can never cost the headline line), with the CPU-oracle leg, the SURVEY 8(f) rows and this
+    very step switched off.  Config 1 (7e4 segments, launch-bound: SURVEY.md 8(d) "not meaningful") is a parity case only."""
+    import subprocess
+
+    rows = {}
+    for key, extra in (("config2", ["--config", "2"]), ("config5", ["--config", "5"]), ("config4", ["--config", "4"]),
+                       ("config3_double", ["--config", "3", "--double"])):
+        cmd = [sys.executable, os.path.abspath(__file__), "--gpus", "1", "--steps", str(steps), "--warmup", "3",
+               "--no-cpu-baseline", "--no-next", "--no-other"] + extra
+        t0 = time.perf_counter()
+        try:
+            env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+            r = subprocess.run(cmd, capture_output=True, text=True, timeout=timeout_s, env=env)
+            line = next((ln for ln in reversed(r.stdout.splitlines()) if ln.startswith("{")), None)
+            if r.returncode != 0 or line is None:
+                rows[key] = {"error": f"rc={r.returncode}: {(r.stderr or r.stdout)[-400:]}"}
+                continue
+            j = json.loads(line)
+            rf, e2e = j.get("roofline") or {}, j.get("e2e") or {}
+            rows[key] = {
+                "workload": j["config"]["workload"], "precision": j["config"]["precision"], "value": j["value"], "unit": j["unit"],
+                "rays_per_sec": j["rays_per_sec"], "ms_per_step": j["ms_per_step"], "steps": j["steps"],
+                "rays_per_step": j["config"]["rays_per_step_per_gpu"], "segments_per_step": j["config"]["segments_per_step_per_gpu"],
+                "distinct_batches_cycled": j["config"]["distinct_batches_cycled"],
+                "cell_record_path": j["config"]["cell_record_path"], "deferred_tally": j["config"]["deferred_tally"],
+                "roofline": {k: rf.get(k) for k in ("frac", "kernel", "kernel_ms", "whole_step_frac", "achieved", "peak", "unit",
+                                                    "algorithmic_bytes_per_launch", "frac_of_red_ceiling")},
+                "e2e": {k: e2e.get(k) for k in ("value", "ms_per_step", "h2d_bytes_per_step", "d2h_bytes_per_step")},
+                "gpu_launches": j.get("gpu_launches"), "clocks": j.get("clocks"),
+                "wall_s": round(time.perf_counter() - t0, 1), "command": " ".join(["python", "bench.py"] + cmd[2:]),
+            }
+        except Exception as e:  # noqa: BLE001 -- a context row must not lose the headline line
+            rows[key] = {"error": repr(e), "wall_s": round(time.perf_counter() - t0, 1)}
+    return rows
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -224,6 +263,9 @@ def main():
                     "not the headline; the roofline then uses B_seg = 16 + 9K, B_ray = 64 + 32M (SURVEY.md 8(d)); implies --no-next")
     ap.add_argument("--no-next", action="store_true", help="skip the SURVEY 8(f) rows (next-event cast, batch-moment fold)")
     ap.add_argument("--microbench", default="", choices=["", "red"], help="run a micro-benchmark alone and exit")
+    ap.add_argument("--no-other", action="store_true", help="skip the other_configs rows (configs 2, 5, 4 and config 3 all-double, each a short "
+                                                            "run of this script in a process of its own)")
+    ap.add_argument("--other-steps", type=int, default=5, help="timed steps of each other_configs row")
     ap.add_argument("--no-plain", action="store_true", help="skip the second roofline with the dictionary / tiled-index path off")
     ap.add_argument("--batches", type=int, default=0, help="distinct ray batches cycled through (default: 1; config 4: 8 of its 100)")
     ap.add_argument("--ne-rays", type=int, default=2_000_000, help="events per next-event step")
@@ -386,6 +428,11 @@ def main():
                                  f"{m.get_option(MR_INFO_DISTINCT_RECORDS)} distinct cell records); a mesh with more than 1024 "
                                  "distinct records gets this path")
         m.set_option(MR_OPT_TILED_INDEX, 1)
+
+    # the two qualifiers of the headline fraction, inside `roofline` where the driver's parser keeps them
+    roofline["frac_of_red_ceiling"] = (roofline.get("atomic_ceiling") or {}).get("frac_of_red_ceiling")
+    roofline["plain_records_frac"] = roofline_plain["frac"] if roofline_plain else None
+    roofline["plain_records_kernel_ms"] = roofline_plain["kernel_ms"] if roofline_plain else None
 
     # ---------------------------------------------------------------- end to end through the C ABI, host buffers
     e2e = None
@@ -589,11 +636,16 @@ def main():
                "sample": f"first {n_s} rays of the batch ({segs} segments), {dt:.1f} s wall on {used} threads",
                "single_thread": {"value": rate1, "unit": UNIT, "sample": f"first {n_1} rays ({segs1} segments), {dt1:.1f} s wall"}}
 
+    other = None
+    if rank == 0 and world == 1 and not args.no_other and args.config == 3 and not args.double and not args.rays:
+        torch.cuda.synchronize()
+        other = other_config_rows(args.other_steps)
+
     if rank == 0:
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
+            "dtype": "f64 (everything)" if args.double else "mixed: fp32 tables/rays/coefficients, fp64 walk/score/tally", "data": "synthetic",
             "config": {"workload": CONFIG_NAMES[args.config], "mesh": [prob.nx, prob.ny, prob.nz], "K": prob.K, "M": prob.M,
                        "rays_per_step_per_gpu": n_rays, "segments_per_step_per_gpu": int(seg_step),
                        "precision": "double (everything fp64)" if args.double else "mixed (fp32 tables/rays/coefficients, fp64 walk/score/tally)",
@@ -605,6 +657,7 @@ def main():
                        if args.config == 3 else "no flush"},
             "rays_per_sec": rays_all * args.steps / (ms_total * 1e-3),
             "roofline": roofline, "roofline_plain_records": roofline_plain, "cpu_baseline": cpu, "e2e": e2e, "next_rows": next_rows,
+            "other_configs": other,
             "traffic_is": "dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures "
                           "(profiles/traffic.txt), not measured by this run",
             "traffic_sources": TRAFFIC_SOURCES,

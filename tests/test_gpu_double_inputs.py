@@ -263,3 +263,35 @@ def test_full_size_all_double_in_bench_configuration(cfg):
     assert np.array_equal(nseg, ref.nseg), "segment counts differ"
     assert np.array_equal(hsh, ref.hash), "cell-sequence hashes differ"
     assert_tally_double(got, ref.tally)
+
+
+@pytest.mark.slow
+def test_config4_all_double_batches_49_and_99_on_the_full_mesh():
+    """Config 4 in ALL-DOUBLE mode beyond its first batch (test_full_size_all_double_in_bench_configuration[4] casts
+    batch 0): two more of its 100 seeded batches, from the middle and the end of the run, on one context -- traces of
+    every ray, counters, and each batch's tally increment against the oracle at 1e-10."""
+    import torch
+
+    from paper_1706_07476_b200 import MonteRay
+
+    prob = make_problem(4, double_inputs=True)
+    orc = _oracle(prob)
+    with MonteRay(0, DOUBLE) as m:
+        m.load_problem(prob)
+        seg = 0
+        for batch in (49, 99):
+            rays = make_rays(prob, 1_000_000, batch=batch, dtype=np.float64)
+            assert not_fp32(rays[:, 0], rays[:, 3], rays[:, 6], rays[:, 7])
+            ref = orc.cast(rays, per_ray=True, threads=_threads())
+            d_rays = torch.from_numpy(rays).cuda()
+            before = m.read_tally()
+            m.cast_rays(d_rays)
+            got = m.read_tally()
+            nseg, hsh, _, _ = m.trace_rays(d_rays)
+            assert np.array_equal(nseg, ref.nseg) and np.array_equal(hsh, ref.hash), f"batch {batch}: traces differ"
+            # the increment is a difference of running sums: the bar is taken on the running sum's scale
+            d = np.abs((got - before) - ref.tally)
+            assert np.all(d <= 1e-10 * np.abs(ref.tally) + 2e-15 * np.abs(got) + 1e-290), f"batch {batch}"
+            seg += ref.segments
+        st = m.get_stats()
+        assert (st.rays_accepted, st.rays_rejected, st.segments) == (2_000_000, 0, seg)

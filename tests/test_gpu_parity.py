@@ -179,12 +179,16 @@ def test_full_size_configs_in_bench_configuration(cfg):
     assert_tally(got, ref.tally, 0)
 
 
+CONFIG4_BATCHES = (0, 1, 9, 19, 29, 39, 49, 59, 69, 79, 89, 99)
+
+
 @pytest.mark.slow
-def test_config4_batches_0_1_99_on_the_full_mesh():
+def test_config4_twelve_spaced_batches_on_the_full_mesh():
     """BASELINE.json config 4 is 10^8 rays in 100 batches of 10^6 on the 512^3 mesh.  The oracle needs about
-    3.4e8 segments per batch on the host cores, so parity covers 3 OF THE 100 BATCHES -- the first two and the
-    last (every batch has its own seeded stream, SeedSequence([.., 4, 9, batch])) -- each against its own oracle
-    tally, then the three together (the resident tally is the running sum over batches)."""
+    3.4e8 segments per batch (a few seconds on the host cores), so parity covers 12 OF THE 100 BATCHES, spaced over the
+    whole run -- every batch has its own seeded stream, SeedSequence([.., 4, 9, batch]) -- each against its own oracle
+    tally (every ray's segment count and cell-sequence hash, every cell of the batch's tally increment), then the
+    twelve together (the resident tally is the running sum over batches)."""
     import torch
 
     prob = make_problem(4)
@@ -192,7 +196,7 @@ def test_config4_batches_0_1_99_on_the_full_mesh():
     total = np.zeros(prob.ncell)
     with _mr(prob, 0) as m:
         seg = 0
-        for batch in (0, 1, 99):
+        for batch in CONFIG4_BATCHES:
             rays = make_rays(prob, 1_000_000, batch=batch)
             ref = orc.cast(rays, per_ray=True, threads=_threads())
             d_rays = torch.from_numpy(rays).cuda()
@@ -205,7 +209,7 @@ def test_config4_batches_0_1_99_on_the_full_mesh():
             total += ref.tally
             seg += ref.segments
         st = m.get_stats()
-        assert (st.rays_accepted, st.rays_rejected, st.segments) == (3_000_000, 0, seg)
+        assert (st.rays_accepted, st.rays_rejected, st.segments) == (len(CONFIG4_BATCHES) * 1_000_000, 0, seg)
         assert_tally(m.read_tally(), total, 0)
 
 
