@@ -553,6 +553,7 @@ def main():
             ring_step(0)
             m.sync()
             w0 = m.ring_stats()["producer_wait_ms"]
+            casts0, slots0 = m.ring_stats()["casts"], m.ring_stats()["slots_shipped"]
             barrier()
             reps = max(2, min(args.steps, 5))
             t0 = time.perf_counter()
@@ -570,6 +571,9 @@ def main():
                 "value": seg_step / dt, "unit": UNIT, "ms_per_step": ring_ms, "producers": P, "rays_per_push": piece,
                 "producer_kind": "C threads inside the library (mr_ring_bench_producers)",
                 "slots": args.ring_slots, "rays_per_slot": slot_rays,
+                # MR_OPT_RING_MERGE (auto): buffers shipped while an earlier cast still runs are cast together, in one launch
+                "buffers_shipped_per_step": (rs["slots_shipped"] - slots0) / reps, "casts_per_step": (rs["casts"] - casts0) / reps,
+                "rays_per_cast": n_rays * reps / max(1, rs["casts"] - casts0),
                 "push_and_flush_ms_per_step": statistics.mean(push_ms),
                 "producer_wait_ms_per_step": (rs["producer_wait_ms"] - w0) / reps,
                 "producers_alone_ms_per_step": producer_ms,
@@ -578,7 +582,7 @@ def main():
                 # 1 = the shorter of (producers, device) is hidden completely behind the longer one; 0 = they run back to back
                 "overlap": 1.0 - (ring_ms - hi_ms) / lo_ms if lo_ms > 0 else None,
                 "overlap_is": "1 - (ring step - max(producers alone, device only)) / min(producers alone, device only); the ring step "
-                              "also reads the tally back (D2H of ncell doubles) and casts slot by slot, which neither reference time contains",
+                              "also reads the tally back (D2H of ncell doubles) and casts in several launches (casts_per_step), which neither reference time contains",
                 "h2d_bytes_per_step": int(rays.nbytes), "d2h_bytes_per_step": int(prob.ncell * 8)}
             # NEXT-4: the same estimator on an R-Z (cylindrical) pin-cell mesh, its own context
             from workloads import make_rz_problem, make_rz_rays

@@ -177,8 +177,10 @@ MR_API int mr_define_material(mr_ctx *ctx, int material, int nnuc, const int32_t
  *     x = Sigma_i * l_i;   score = W * exp(-tau) * (x > 0 ? (1 - exp(-x)) / Sigma_i : l_i);
  *     tally[i] += score;   tau += x
  * until the ray leaves the mesh (no cut-off, no reflection: readings Q7, F5).  A ray is
- * REJECTED (counted, no contribution) if any field is not finite, E <= 0, the direction is
- * the zero vector, or the origin is outside the half-open box [lo, hi) on any axis.
+ * REJECTED (counted, no contribution) if any field is not finite, E <= 0, no axis has a
+ * finite 1/d_a (the zero vector, or components so small that every reciprocal overflows: an
+ * axis whose 1/d_a is not finite never steps, reading Q10, and a ray that steps on no axis
+ * never leaves the mesh), or the origin is outside the half-open box [lo, hi) on any axis.
  * Asynchronous: returns once the batch is staged (a host buffer has been copied out of, or,
  * if it is page-locked, DMA'd out of) and the work is queued.  n = 0 is a no-op.
  * Requires mesh, materials and all M tables.  Errors: INVALID_ARG, STATE, OOM, CUDA. */
@@ -313,14 +315,18 @@ typedef struct {
     int64_t rays_pushed;      /* rays accepted by mr_ring_push since mr_ring_open */
     int64_t slots_shipped;    /* buffers handed to the GPU (full ones and flushed partial ones) */
     double producer_wait_ms;  /* total time producers spent blocked because every slot was in flight */
-    double reserved[3];
+    int64_t casts;            /* cast launches (each with its ordering pre-pass) the shipped buffers were merged into */
+    double reserved[2];
 } mr_ring_stats;
 
 /* Opens a ring of `slots` (2..16) page-locked host buffers of `rays_per_slot` rays each (>= 1024), with as many
  * device buffers behind them.  Producers append rays with mr_ring_push; a buffer that becomes full is shipped:
  * H2D copy on the copy stream, then the ordering pre-pass and the cast kernel on the context's stream, without
  * blocking the producer -- which goes on filling the next buffer while the GPU works (Fig. 4).  A producer
- * blocks only when every buffer is still being copied out.  Requires mesh, materials and all tables.
+ * blocks only when every buffer is still being copied out.  While an earlier cast of the ring is still running, a
+ * shipped buffer is copied at once but its cast is held back and merged with the buffers that follow it into ONE
+ * launch (MR_OPT_RING_MERGE; the device buffers are consecutive pieces of one allocation): the GPU is busy anyway,
+ * and one cast of k buffers is cheaper than k casts.  mr_ring_flush queues whatever is held back.  Requires mesh, materials and all tables.
  * Errors: INVALID_ARG, STATE (ring already open, set-up incomplete), OOM, CUDA. */
 MR_API int mr_ring_open(mr_ctx *ctx, int slots, int64_t rays_per_slot);
 
@@ -419,6 +425,10 @@ enum {
                                  stream is still busy with earlier work when the call is made (a caller casting batch after batch without
                                  waiting: the copy then hides behind the previous cast, and one launch is 20 % cheaper than its chunks),
                                  chunked otherwise.  Batches above 2 GB are always chunked */
+    MR_OPT_RING_MERGE = 19,   /* producer ring: 0 = every shipped buffer gets its own ordering pre-pass and cast; 1 (default) = auto: a buffer
+                                 shipped while an earlier cast of the ring is still running waits, and consecutive waiting buffers are cast
+                                 in one launch by the next ship that finds the GPU free, by a ship that wraps around the ring, or by
+                                 mr_ring_flush; 2 = always wait (one cast per ring revolution or flush).  Set before mr_ring_open */
     MR_OPT_PERSISTENT_LANES = 17, /* the cast kernel with persistent lanes (dictionary / K = 1 / K = 3 pairs / dense-8 record paths, MIXED): the
                                  grid is as many CTAs as are resident at once and a lane whose ray has left the mesh takes the next ray
                                  (in the order of the MR_OPT_SORT_RAYS pre-pass) from a counter -- no tail of half-empty CTAs, no ramp per

@@ -35,6 +35,7 @@ MR_OPT_RZ_BLOCK_THREADS = 15
 MR_OPT_TILED_TALLY = 16
 MR_OPT_PERSISTENT_LANES = 17
 MR_OPT_WHOLE_BATCH = 18
+MR_OPT_RING_MERGE = 19
 MR_INFO_RECORD_PATH, MR_INFO_DISTINCT_RECORDS, MR_INFO_COARSE_SHIFT = 100, 101, 102
 MR_INFO_DEFERRED, MR_INFO_DEFER_DIRECT_PAIRS = 103, 104
 MR_PATH_NAMES = {0: "none", 1: "k1", 2: "k2", 3: "k3", 4: "k4", 5: "k2_pairs", 6: "k3_pairs", 7: "k4_fused", 8: "dense8",
@@ -67,7 +68,7 @@ class mr_stats(C.Structure):
 
 class mr_ring_stats(C.Structure):
     _fields_ = [("rays_pushed", C.c_int64), ("slots_shipped", C.c_int64), ("producer_wait_ms", C.c_double),
-                ("reserved", C.c_double * 3)]
+                ("casts", C.c_int64), ("reserved", C.c_double * 2)]
 
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_void_p, C.c_size_t, C.c_int)
@@ -428,7 +429,7 @@ class MonteRay:
         s = mr_ring_stats()
         self._check(self.lib.mr_ring_get_stats(self._h, C.byref(s)))
         return {"rays_pushed": int(s.rays_pushed), "slots_shipped": int(s.slots_shipped),
-                "producer_wait_ms": float(s.producer_wait_ms)}
+                "producer_wait_ms": float(s.producer_wait_ms), "casts": int(s.casts)}
 
     def ring_bench_producers(self, rays, producers: int, rays_per_push: int, dry_run: bool = False) -> float:
         """mr_ring_bench_producers: library-side producer threads push the host batch through the ring; wall ms."""

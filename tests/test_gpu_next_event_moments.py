@@ -268,6 +268,87 @@ def test_producer_ring_many_threads_equals_one_call(precision, producers, slots,
     assert np.all(d <= bound)
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+def test_producer_ring_merges_waiting_buffers_into_one_cast(precision):
+    """MR_OPT_RING_MERGE: a buffer shipped while the GPU is still busy with an earlier cast of the ring is copied at once but
+    cast together with the buffers that follow it -- one ordering pre-pass and one launch over consecutive device buffers.
+    Forced (2: hold until flush or until the ring wraps): 3 full buffers and a partial one become ONE cast; 6.3 buffers
+    through 4 slots become two casts (the wrap sends the first four off) plus the flush.  Off (0): one cast per buffer.
+    Auto (1): anything in between.  Every mode: counters exact, tally within tolerance of the oracle; several producer
+    threads (buffers shipped out of order) included."""
+    import threading
+
+    from paper_1706_07476_b200 import MR_OPT_RING_MERGE
+
+    prob = make_problem(3, nx=68, ny=68, nz=40, n_e=2000)
+    cap = 20_000                                             # above the ordering pre-pass threshold (2^14 rays)
+    rays32 = make_rays(prob, 6 * cap + 6_007)
+    refs = {n: _oracle(prob).cast(rays32[:n], threads=8) for n in (3 * cap + 8_001, len(rays32))}
+
+    def check(m, ref):
+        st = m.get_stats()
+        assert (st.rays_accepted, st.rays_rejected, st.segments) == (ref.rays_accepted, ref.rays_rejected, ref.segments)
+        d = np.abs(m.read_tally() - ref.tally)
+        bound = (1e-4 * np.abs(ref.tally) + 1e-7 * ref.tally.max()) if precision == 0 else (1e-10 * np.abs(ref.tally) + 1e-290)
+        assert np.all(d <= bound)
+
+    with _mr(prob, precision) as m:
+        rays = np.ascontiguousarray(rays32.astype(m.ray_dtype))
+        for mode in (2, 0, 1):
+            m.set_option(MR_OPT_RING_MERGE, mode)
+            assert m.get_option(MR_OPT_RING_MERGE) == mode
+            # 3 full buffers + a partial one, pushed by one thread in ragged pieces
+            n = 3 * cap + 8_001
+            m.clear_tally()
+            m.ring_open(4, cap)
+            for i in range(0, n, 7_777):
+                m.ring_push(rays[i:min(n, i + 7_777)])
+            m.ring_flush()
+            rs = m.ring_stats()
+            assert rs["slots_shipped"] == 4 and rs["rays_pushed"] == n
+            assert rs["casts"] == (1 if mode == 2 else 4 if mode == 0 else rs["casts"]) and 1 <= rs["casts"] <= 4
+            check(m, refs[n])
+            m.ring_close()
+            # 6.3 buffers through 4 slots: the ring wraps while buffers are held back
+            m.clear_tally()
+            m.ring_open(4, cap)
+            m.ring_push(rays)
+            m.ring_flush()
+            rs = m.ring_stats()
+            assert rs["slots_shipped"] == 7
+            if mode == 2:
+                assert rs["casts"] == 2                      # slots 0-3 when slot 0 comes round again, then 0-2 at the flush
+            if mode == 0:
+                assert rs["casts"] == 7
+            assert 2 <= rs["casts"] <= 7
+            check(m, refs[len(rays)])
+            m.ring_close()
+            # four producer threads: buffers are shipped by whoever filled them, not necessarily in ring order
+            m.clear_tally()
+            m.ring_open(3, cap)
+            bounds = np.linspace(0, len(rays), 5).astype(int)
+
+            def produce(lo, hi):
+                for i in range(lo, hi, 3_001):
+                    m.ring_push(rays[i:min(hi, i + 3_001)])
+
+            ts = [threading.Thread(target=produce, args=(bounds[k], bounds[k + 1])) for k in range(4)]
+            for t in ts:
+                t.start()
+            for t in ts:
+                t.join()
+            m.ring_flush()
+            assert m.ring_stats()["slots_shipped"] == 7
+            check(m, refs[len(rays)])
+            m.ring_close()
+        from paper_1706_07476_b200 import MonteRayError
+
+        m.ring_open(2, 4096)
+        with pytest.raises(MonteRayError):
+            m.set_option(MR_OPT_RING_MERGE, 0)               # not while a ring is open
+        m.ring_close()
+
+
 def test_ring_library_side_producers():
     """mr_ring_bench_producers (the bench's producers: C threads inside the library): the union of what 1, 3 and 7 producer
     threads push in ragged pieces equals one mr_cast_rays call (counters exact, tally within tolerance of the oracle); the
