@@ -429,12 +429,8 @@ enum {
                                  shipped while an earlier cast of the ring is still running waits, and consecutive waiting buffers are cast
                                  in one launch by the next ship that finds the GPU free, by a ship that wraps around the ring, or by
                                  mr_ring_flush; 2 = always wait (one cast per ring revolution or flush).  Set before mr_ring_open */
-    MR_OPT_PERSISTENT_LANES = 17, /* the cast kernel with persistent lanes (dictionary / K = 1 / K = 3 pairs / dense-8 record paths, MIXED): the
-                                 grid is as many CTAs as are resident at once and a lane whose ray has left the mesh takes the next ray
-                                 (in the order of the MR_OPT_SORT_RAYS pre-pass) from a counter -- no tail of half-empty CTAs, no ramp per
-                                 launch.  0 (default) = never, 1 = always, 2 = auto (currently never).  Measured slower than one ray per thread on
-                                 every config: after the ordering pre-pass 29-31 of 32 lanes are busy anyway, and
-                                 the refill test, the per-lane "active" predicate and the divergent set-up cost more than the tail */
+    /* 17 was MR_OPT_PERSISTENT_LANES (a cast kernel whose lanes refilled from a counter): measured slower on every config
+        and removed in round 3 */
     MR_OPT_AGGREGATE_FIRST = 9 /* n >= 0: the tally atomics of the first n segments of every ray are warp-aggregated (lanes that score
                                  into the same cell are found with match.any and one of them adds the sum): for batches born in a
                                  region of a few cells, where same-address atomics serialise in L2.  Default 2; 0 = off */

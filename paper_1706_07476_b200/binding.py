@@ -33,7 +33,6 @@ MR_OPT_DEFER_REGION_SHIFT = 13
 MR_OPT_COOP_FLUSH = 14
 MR_OPT_RZ_BLOCK_THREADS = 15
 MR_OPT_TILED_TALLY = 16
-MR_OPT_PERSISTENT_LANES = 17
 MR_OPT_WHOLE_BATCH = 18
 MR_OPT_RING_MERGE = 19
 MR_INFO_RECORD_PATH, MR_INFO_DISTINCT_RECORDS, MR_INFO_COARSE_SHIFT = 100, 101, 102

@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmonteray.so")
 SOURCES = [os.path.join(CSRC, "monteray.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "mr_device.cuh"), os.path.join(CSRC, "mr_sort.cuh"), os.path.join(CSRC, "mr_defer.cuh"), os.path.join(CSRC, "mr_tiled.cuh"), os.path.join(CSRC, "mr_persist.cuh"), os.path.join(CSRC, "mr_microbench.cuh"), os.path.join(ROOT, "include", "monteray.h")]
+DEPS = SOURCES + [os.path.join(CSRC, "mr_device.cuh"), os.path.join(CSRC, "mr_sort.cuh"), os.path.join(CSRC, "mr_defer.cuh"), os.path.join(CSRC, "mr_tiled.cuh"), os.path.join(CSRC, "mr_microbench.cuh"), os.path.join(ROOT, "include", "monteray.h")]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-lineinfo",

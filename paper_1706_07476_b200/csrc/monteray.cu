@@ -26,7 +26,6 @@
 #include "mr_sort.cuh"
 #include "mr_defer.cuh"
 #include "mr_tiled.cuh"
-#include "mr_persist.cuh"
 #include "mr_microbench.cuh"
 
 using namespace mr;
@@ -234,9 +233,7 @@ struct mr_ctx {
     int coop_opt = 2;                // option MR_OPT_COOP_FLUSH: cast_coop_kernel (transposed tally adds) on the paths built for it;
                                      // 2 = auto: when tally + cell records fit in half the L2 (measured: config 5 6.05 -> 5.55 ms, config 2
                                      // 0.590 -> 0.558 ms; config 3, whose slabs stream through L2, 6.38 -> 7.22 ms: off there)
-    long long persist_auto_max = 0;  // auto: batches (chunks) of at most this many rays take the persistent kernel (0: none -- it measured slower
                                      // at every size: config 3 6.72 against 6.10 ms, config 2 0.62 against 0.57 ms, config 5 5.94 against 5.52 ms)
-    int persist_opt = 0;             // option MR_OPT_PERSISTENT_LANES: cast_persist_kernel (lanes refill from a counter); 2 = auto
     int agg_first = 2;               // option MR_OPT_AGGREGATE_FIRST
     int fused_opt = 2;               // option MR_OPT_FUSED_TALLY: 0 off, 1 on, 2 auto (decided by mr_load_materials)
     bool fused = false;              // LAYOUT_K4 records carry the score accumulators (LAYOUT_K4F in the cast kernel)
@@ -667,40 +664,6 @@ int launch_coop_t(mr_ctx *c, const CastParams &P)
     }
 }
 
-// cast_persist_kernel (mr_persist.cuh): persistent lanes that pull rays from a counter
-template <typename Real, typename Rec, int MODE, bool COOP>
-int launch_persist_m(mr_ctx *c, const CastParams &P, int block, size_t smem)
-{
-    if (int rc = set_smem(c, cast_persist_kernel<Real, Rec, MODE, COOP>, smem)) return rc;
-    int sms = 148, per_sm = 1;
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
-    MR_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cast_persist_kernel<Real, Rec, MODE, COOP>, block, smem));
-    const long long grid = std::max<long long>(1, std::min<long long>((P.n + block - 1) / block, (long long)sms * std::max(per_sm, 1)));
-    unsigned long long *work = c->d_counters + 8 + c->lane;
-    MR_CUDA(c, cudaMemsetAsync(work, 0, sizeof(unsigned long long), c->work_stream()));
-    cast_persist_kernel<Real, Rec, MODE, COOP><<<(unsigned)grid, block, smem, c->work_stream()>>>(P, work);
-    c->launches += 1;
-    MR_CUDA(c, cudaGetLastError());
-    return MR_OK;
-}
-
-template <typename Real, typename Rec, bool COOP>
-int launch_persist_t(mr_ctx *c, const CastParams &P)
-{
-    const int block = c->block_threads;
-    const size_t per_block = walker_smem_bytes(block) + (((size_t)(c->M + c->N) * block * sizeof(Real) + 15) & ~(size_t)15) +
-                             (rec_per_entry<Rec>::value ? (size_t)kPerEntryMax * block * sizeof(Real) : 0) +
-                             (Rec::kTiled ? (size_t)c->ndict * sizeof(uint4) : 0) + (COOP ? (size_t)(block / 32) * coop_warp_smem_bytes() : 0);
-    const int mode = edge_mode(c, per_block);
-    const size_t smem = (mode == EDGES_SHARED ? edges_smem_bytes(c) : 0) + per_block;
-    if (smem > 227 * 1024) return COOP ? launch_coop_t<Real, Rec>(c, P) : launch_cast_t<Real, Rec>(c, P);
-    switch (mode) {
-    case EDGES_ARITH: return launch_persist_m<Real, Rec, EDGES_ARITH, COOP>(c, P, block, smem);
-    case EDGES_SHARED: return launch_persist_m<Real, Rec, EDGES_SHARED, COOP>(c, P, block, smem);
-    default: return launch_persist_m<Real, Rec, EDGES_GLOBAL, COOP>(c, P, block, smem);
-    }
-}
-
 template <typename Real, typename Rec>
 int launch_cast_or_coop(mr_ctx *c, const CastParams &P, bool coop_auto_always = false)
 {
@@ -708,8 +671,6 @@ int launch_cast_or_coop(mr_ctx *c, const CastParams &P, bool coop_auto_always = 
     // for its record as well as for its add (config 3 with the dictionary off: 8.42 -> 7.80 ms)
     const bool coop = c->coop_opt == 1 || c->coop_opt == 3 ||
                       (c->coop_opt == 2 && (coop_auto_always || c->resident_bytes() <= c->l2_bytes / 2));
-    const bool persist = c->persist_opt == 1 || (c->persist_opt == 2 && P.n <= c->persist_auto_max);
-    if (persist) return coop ? launch_persist_t<Real, Rec, true>(c, P) : launch_persist_t<Real, Rec, false>(c, P);
     return coop ? launch_coop_t<Real, Rec>(c, P) : launch_cast_t<Real, Rec>(c, P);
 }
 
@@ -1331,7 +1292,7 @@ int mr_create_ex(mr_ctx **out, int device, int precision, const mr_allocator *al
     }
     ok = ok && cudaEventCreate(&c->ev_t0) == cudaSuccess && cudaEventCreate(&c->ev_t1) == cudaSuccess;
     if (ok) {
-        c->d_counters = (unsigned long long *)c->dev_alloc(12 * sizeof(unsigned long long));   // [8], [9]: work counters of the persistent cast kernel, one per compute lane
+        c->d_counters = (unsigned long long *)c->dev_alloc(12 * sizeof(unsigned long long));   // [4..6]: next-event counters; the rest is spare
         ok = c->d_counters && cudaMemset(c->d_counters, 0, 12 * sizeof(unsigned long long)) == cudaSuccess;
     }
     if (!ok) {
@@ -2863,10 +2824,6 @@ int mr_set_option(mr_ctx *c, int option, int64_t value)
         MR_NO_RING(c, "ring-merge option");
         c->ring_merge = (int)value;
         return MR_OK;
-    case MR_OPT_PERSISTENT_LANES:
-        if (value < 0 || value > 2) return c->fail(MR_ERR_INVALID_ARG, "persistent-lanes option is 0 (off), 1 (on) or 2 (auto)");
-        c->persist_opt = (int)value;
-        return MR_OK;
     case MR_OPT_TILED_TALLY:
         if (value != 0 && value != 1) return c->fail(MR_ERR_INVALID_ARG, "tiled-tally option is 0 or 1");
         c->tiled_tally_opt = (int)value;
@@ -2916,7 +2873,6 @@ int mr_get_option(mr_ctx *c, int option, int64_t *value)
     case MR_OPT_COARSE_RECORDS: *value = c->coarse_opt; return MR_OK;
     case MR_OPT_COOP_FLUSH: *value = c->coop_opt; return MR_OK;
     case MR_OPT_TILED_TALLY: *value = c->tiled_tally_opt; return MR_OK;
-    case MR_OPT_PERSISTENT_LANES: *value = c->persist_opt; return MR_OK;
     case MR_OPT_WHOLE_BATCH: *value = c->whole_opt; return MR_OK;
     case MR_OPT_RING_MERGE: *value = c->ring_merge; return MR_OK;
     case MR_INFO_RECORD_PATH: *value = record_path(c); return MR_OK;

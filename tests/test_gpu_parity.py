@@ -542,7 +542,7 @@ def test_cooperative_transposed_tally_adds():
     4 rays per instruction).  Same counters, tallies within tolerance of the oracle, on every record path the kernel is
     built for (dictionary 4/8/16-bit, K = 1, K = 3 pairs, dense 8) and unchanged behaviour on the others; rejected rays,
     rays shorter than a window, a ragged last warp."""
-    from paper_1706_07476_b200 import MR_OPT_COOP_FLUSH, MR_OPT_PERSISTENT_LANES, MR_OPT_TILED_INDEX, MonteRay
+    from paper_1706_07476_b200 import MR_OPT_COOP_FLUSH, MR_OPT_TILED_INDEX, MonteRay
 
     cases = []
     p3 = make_problem(3, nx=68, ny=68, nz=40, n_e=2000)
@@ -563,9 +563,8 @@ def test_cooperative_transposed_tally_adds():
             m.set_option(MR_OPT_TILED_INDEX, tiled)
             m.load_problem(prob)
             assert m.record_path() == path
-            for coop, persist in ((1, 0), (0, 0), (3, 0), (1, 1), (0, 1)):   # 3: pairs by shuffle; persist: cast_persist_kernel
+            for coop in (1, 0, 3):                                            # 3: pairs by shuffle
                 m.set_option(MR_OPT_COOP_FLUSH, coop)
-                m.set_option(MR_OPT_PERSISTENT_LANES, persist)
                 m.clear_tally()
                 m.cast_rays(rays)
                 st = m.get_stats()

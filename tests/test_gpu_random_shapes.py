@@ -24,12 +24,12 @@ def _tol(ref, precision):
 @pytest.mark.parametrize("seed", [11, 12, 13])
 def test_random_shapes_every_cast_variant(seed):
     from oracle.vrc_oracle import Oracle
-    from paper_1706_07476_b200 import (MR_OPT_COARSE_RECORDS, MR_OPT_COOP_FLUSH, MR_OPT_DEFERRED_TALLY, MR_OPT_PERSISTENT_LANES,
+    from paper_1706_07476_b200 import (MR_OPT_COARSE_RECORDS, MR_OPT_COOP_FLUSH, MR_OPT_DEFERRED_TALLY,
                                        MR_OPT_TILED_INDEX, MR_OPT_TILED_TALLY, MonteRay)
 
     g = np.random.default_rng(seed)
     variants = ({}, {MR_OPT_COOP_FLUSH: 1}, {MR_OPT_COOP_FLUSH: 0}, {MR_OPT_COOP_FLUSH: 3}, {MR_OPT_TILED_TALLY: 1, MR_OPT_COOP_FLUSH: 1},
-                {MR_OPT_DEFERRED_TALLY: 1}, {MR_OPT_PERSISTENT_LANES: 1}, {MR_OPT_TILED_INDEX: 0, MR_OPT_COARSE_RECORDS: 0})
+                {MR_OPT_DEFERRED_TALLY: 1}, {MR_OPT_TILED_INDEX: 0, MR_OPT_COARSE_RECORDS: 0})
     before_load = (MR_OPT_TILED_INDEX, MR_OPT_COARSE_RECORDS)
     paths = set()
     for it in range(12):
